@@ -76,7 +76,7 @@ def jacobi_svd(a):
     if m < n:
         v, s, u = jacobi_svd(a.T)
         return u, s, v
-    at = np.ascontiguousarray(a.T)          # row j = column j of a
+    at = np.array(a.T, dtype=np.float64, order="C", copy=True)   # row j = column j of a (always a copy)
     s = np.zeros(n)
     vt = np.zeros((n, n))
     rc = _lib().orc_jacobi_svd(m, n, _ptr(at), _ptr(s), _ptr(vt), JACOBI_TOL, JACOBI_MAX_SWEEPS)

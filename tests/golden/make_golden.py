@@ -1,0 +1,45 @@
+"""Writes tests/golden/oracle_<name>.json from the CPU oracle ONLY (never from the CUDA path).
+
+    python tests/golden/make_golden.py c1 c2 c3 [c4:12]      (name[:steps])
+
+Each file holds, per step: ln Z/V, the bond-swap spectrum sigma/sigma_1 and the T-decomposition spectrum s/s_1
+for one BASELINE.json config (see tests/inputs.py::configs); these take minutes to hours on a CPU, so the GPU
+parity tests read them instead of re-running the oracle.  Expected values are reproducible: rerun this script.
+"""
+import json
+import os
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+sys.path.insert(0, ROOT)
+from oracle import tatrg_oracle as O  # noqa: E402
+
+RUNS = {
+    # name: list of (tag, beta, h, D, p, n_pow, seed, steps)
+    "c1": [("b0.14", 0.14, 0.0, 4, 4, 1, 1234, 16)],
+    "c2": [("b%g_s%d" % (b, s), b, 0.0, 8, 8, 2, s, 40)
+           for b, s in zip((0.140, 0.145, 0.1497, 0.155, 0.160), (1, 2, 3, 4, 5))],
+    "c3": [("h+1e-3", 0.1497, 1e-3, 16, 16, 2, 7, 48), ("h-1e-3", 0.1497, -1e-3, 16, 16, 2, 7, 48)],
+    "c4": [("b0.1497", 0.1497, 0.0, 32, 32, 2, 42, 60)],
+}
+
+if __name__ == "__main__":
+    for arg in sys.argv[1:]:
+        name, _, lim = arg.partition(":")
+        out = {"generator": "tests/golden/make_golden.py (oracle only)", "runs": []}
+        for tag, beta, h, D, p, n_pow, seed, steps in RUNS[name]:
+            steps = min(steps, int(lim)) if lim else steps
+            o = O.TatrgOracle(beta, h, D, p, seed, n_pow=n_pow)
+            rec = dict(tag=tag, beta=beta, h=h, D=D, oversample=p, n_pow=n_pow, seed=seed, lnZ=[], sigma=[], s=[], sec=[])
+            for m in range(steps):
+                t0 = time.time()
+                o.step()
+                rec["lnZ"].append(o.lnZ_per_site())
+                rec["sigma"].append([float(x) for x in o.last["sigma"][:D]])
+                rec["s"].append([float(x) for x in o.last["s"][:D]])
+                rec["sec"].append(round(time.time() - t0, 3))
+                print(name, tag, m + 1, rec["lnZ"][-1], rec["sec"][-1], flush=True)
+                json.dump(out | {"runs": out["runs"] + [rec]}, open(os.path.join(os.path.dirname(__file__), "oracle_%s.json" % name), "w"), indent=0)
+            out["runs"].append(rec)
+        json.dump(out, open(os.path.join(os.path.dirname(__file__), "oracle_%s.json" % name), "w"), indent=0)
