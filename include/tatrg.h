@@ -1,0 +1,131 @@
+/*
+ * tatrg.h -- C ABI of the B200-native Triad-ATRG hot path (arXiv:2507.21909; citations "PAPER.md:<line>").
+ *
+ * One handle = one 4D Ising tensor network being coarse-grained on ONE GPU in FP64.  Every arithmetic step of
+ * the path runs in the library's own sm_100a kernels; the caller (a thin Python binding) only provides device
+ * memory and a CUDA stream.  No entry point throws or aborts; all return a status (0 = TATRG_OK, < 0 = error)
+ * unless stated otherwise; tatrg_last_error() gives the text of the last failure of a handle.
+ *
+ * Pointers are marked  [dev]  (device memory, FP64 unless stated, 16-byte aligned)  or  [host].
+ * The library never frees caller memory and never allocates device memory of its own.
+ */
+#ifndef TATRG_H
+#define TATRG_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tatrg_ctx* tatrg_handle;
+
+enum { TATRG_OK = 0, TATRG_EINVAL = -1, TATRG_ENOMEM = -2, TATRG_ECUDA = -3, TATRG_ENUMERIC = -4, TATRG_ESTATE = -5 };
+
+/* option keys of tatrg_set_option (before the first step only) */
+enum {
+    TATRG_OPT_POWER_ITERS = 1, /* n_pow: RSVD power iterations; passes of Eq. A.4-A.6 (:352-369) = n_pow+1. default 2 */
+    TATRG_OPT_K_TRIAD = 2,     /* internal-line dimension rD of the triad isometries (Eq. 2.9 :135). default D+oversample */
+    TATRG_OPT_TAU = 3,         /* relative gap below which values form one multiplet (R7). default 1e-6 */
+    TATRG_OPT_STAGE_TIMING = 4 /* 1: record CUDA-event times per stage (adds stream syncs). default 0 */
+};
+
+/* which spectrum tatrg_singular_values returns */
+enum { TATRG_SV_SIGMA = 0 /* bond swap, Eq. 2.5 :90 */, TATRG_SV_S = 1 /* decomposition of T, Eq. 2.4 :76 */ };
+
+/* stages of one step (Fig. 5 a-f) for tatrg_stage_ms / tatrg_stage_flops */
+enum { TATRG_ST_DECOMPOSE = 0, TATRG_ST_QR, TATRG_ST_RSVD, TATRG_ST_LIFT, TATRG_ST_TRIAD_ISO, TATRG_ST_TRIAD_TENSORS,
+       TATRG_ST_SQ_GRAMS, TATRG_ST_SQUEEZERS, TATRG_ST_CONTRACT, TATRG_ST_ROTATE, TATRG_NSTAGES };
+
+/* ---- the path: PAPER.md Fig. 5 (a)-(f) :193 ------------------------------------------------------------ */
+
+/* Device bytes a handle with truncation D (Eq. 2.4 :76) and RSVD oversampling p (l = D+p, :371) needs. */
+size_t tatrg_workspace_bytes(int D, int oversample);
+
+/* Builds the initial tensor of the 4D Ising model, Eq. 3.1-3.2 (:241-246), on the device in factored form
+ * T[f,b] = sum_a Phi0[f,a] Psi0[b,a], with site weight exp(beta*h*s_a) (R1).
+ * workspace [dev]: >= tatrg_workspace_bytes(D, oversample) bytes, owned by the caller, must outlive the handle.
+ * seed: Philox4x32-10 key of the RSVD test tensor Omega (:371) and of the gauge reference vectors.
+ * Errors: EINVAL (beta<=0, non-finite, D<2, oversample<0, null pointers), ENOMEM (workspace too small). */
+int tatrg_create(double beta, double h, int D, int oversample, uint64_t seed, void* workspace, size_t workspace_bytes,
+                 tatrg_handle* out);
+
+int tatrg_set_option(tatrg_handle, int key, double value);
+
+/* One coarse-graining step along the current axis 1 (axes cycle x,y,z,t): decomposition (Eq. 2.4), bond swap
+ * by RSVD (Eq. 2.5, App. A), triad isometries and tensors (Eq. 2.9-2.17), squeezers (:171), contraction
+ * (Eq. 2.18-2.19), axis rotation and normalisation.  Work is enqueued on cuda_stream (a cudaStream_t; NULL =
+ * default stream); small spectra are read back inside the call to take the rank decisions.
+ * Errors: ECUDA, ENUMERIC (non-finite or non-positive normalisation), ENOMEM, ESTATE (after an earlier failure). */
+int tatrg_step(tatrg_handle, void* cuda_stream);
+
+/* ln Z / V of the periodic lattice of V = 2^steps sites: sum_j 2^-j ln c_j + 2^-m ln tTr(T^(m)) (R8).
+ * Synchronises the stream of the last step.  NaN on error. */
+double tatrg_lnZ_per_site(tatrg_handle);
+
+/* Copies min(k, available) leading values of the last step's spectrum `which`, normalised to the largest, to
+ * out_host [host].  Returns the number written or < 0. */
+int tatrg_singular_values(tatrg_handle, int which, int k, double* out_host);
+
+int tatrg_steps_done(tatrg_handle);
+const char* tatrg_last_error(tatrg_handle);
+void tatrg_destroy(tatrg_handle); /* frees the host struct only */
+
+/* ---- instrumentation ----------------------------------------------------------------------------------- */
+/* ms[TATRG_NSTAGES] / flops[TATRG_NSTAGES] [host] of the last step (ms only with TATRG_OPT_STAGE_TIMING). flops
+ * are the 2*M*N*K of every GEMM launched in the stage.  launches: kernels launched by the last step. */
+int tatrg_stage_ms(tatrg_handle, double* ms);
+int tatrg_stage_flops(tatrg_handle, double* flops);
+long long tatrg_last_step_launches(tatrg_handle);
+/* device time (ms) and flops spent inside the DGEMM kernel during the last step (needs STAGE_TIMING=2). */
+int tatrg_gemm_profile(tatrg_handle, double* ms, double* flops, long long* calls);
+
+/* Copies a named tensor of the last step to out_host [host] (row-major).  Names: "phi","psi" (state after the
+ * step), "A","Dt","core","X","Y","sigma","E","F","G","H","UA","UX","UY","UD","M2","M3","M4","N2","N3","N4".
+ * dims[8] [host] receives the shape, *ndim its length.  capacity = doubles available in out_host (may be 0 to
+ * query the shape).  Returns the element count or < 0. */
+long long tatrg_get_tensor(tatrg_handle, const char* name, double* out_host, long long capacity, int* ndim, long long* dims);
+
+/* Replaces the state by Phi[d0,d1,d2,d3,g], Psi[d0,d1,d2,d3,g] read from host memory (teacher forcing in tests). */
+int tatrg_set_state(tatrg_handle, const double* phi_host, const double* psi_host, const long long* dims5);
+
+/* ---- primitives (the kernels the path is made of; all on device pointers) ---------------------------------- */
+
+/* C[M,N] (row-major, ldc) = alpha * op(A) op(B) + beta * C, FP64 tensor cores (DMMA).  transa = 0: A is [M,K]
+ * (lda >= K); 1: A is stored [K,M] (lda >= M).  transb = 0: B is [K,N] (ldb >= N); 1: B stored [N,K].
+ * batch >= 1 with element strides between consecutive problems. */
+int tatrg_dgemm(void* cuda_stream, int transa, int transb, long long M, long long N, long long K, double alpha,
+                const double* A, long long lda, const double* B, long long ldb, double beta, double* C, long long ldc,
+                int batch, long long strideA, long long strideB, long long strideC);
+
+/* out = in with legs permuted: out leg i is in leg perm[i]; dims[ndim] are the extents of `in` (row-major). */
+int tatrg_permute(void* cuda_stream, int ndim, const long long* dims, const int* perm, const double* in, double* out);
+
+/* Tensor contraction  "abc,cd->abd"-style (single-letter legs, no repeated output legs) = permutes + one DGEMM.
+ * dimsA/dimsB [host]; scratch [dev] of scratch_bytes for permuted copies (>= 8*(|A|+|B|+|C|) always suffices). */
+int tatrg_contract(void* cuda_stream, const char* spec, const double* A, const long long* dimsA, const double* B,
+                   const long long* dimsB, double* C, void* scratch, size_t scratch_bytes);
+
+/* Philox4x32-10 (R11): raw[4*count] uint32 [dev] for counters e = start..start+count-1, and the
+ * Gaussian z[count] [dev] of the same counters; counter = (e_lo, e_hi, call, stream_id), key = seed. */
+int tatrg_philox_raw(void* cuda_stream, uint64_t seed, uint32_t call, uint32_t stream_id, uint64_t start, long long count,
+                     uint32_t* raw);
+int tatrg_philox_gaussian(void* cuda_stream, uint64_t seed, uint32_t call, uint32_t stream_id, uint64_t start,
+                          long long count, double* z);
+
+/* Symmetric eigen-decomposition by parallel Jacobi: G [dev] n x n (destroyed), lam [dev] n descending,
+ * V [dev] n x n row-major, COLUMNS are eigenvectors.  work [dev] >= tatrg_eigh_work_bytes(n).  Synchronises. */
+size_t tatrg_eigh_work_bytes(int n);
+int tatrg_eigh(void* cuda_stream, int n, double* G, double* lam, double* V, void* work);
+
+/* Thin SVD of A [dev] m x n (m >= n, row-major, preserved) by one-sided Jacobi: U [dev] m x n, s [dev] n
+ * descending, V [dev] n x n (columns = right singular vectors).  work >= tatrg_svd_work_bytes(m,n). */
+size_t tatrg_svd_work_bytes(int m, int n);
+int tatrg_svd(void* cuda_stream, int m, int n, const double* A, double* U, double* s, double* V, void* work);
+
+/* result[0] [dev] = sum_i x[i]*y[i]  (the tensor trace tTr of Eq. 2.1 :48 on the factored tensor). */
+int tatrg_dot(void* cuda_stream, long long n, const double* x, const double* y, double* result);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

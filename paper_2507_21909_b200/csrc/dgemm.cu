@@ -1,0 +1,216 @@
+// dgemm.cu -- FP64 tensor-core GEMM for the Triad-ATRG contractions (Eq. 2.18-2.19 :175, A.4-A.5 :356-361,
+// 2.9-2.13 :135-157 are all permute + GEMM).  sm_100a has no tcgen05 kind for f64; the FP64 tensor path is
+// mma.sync.m8n8k4.f64 (SASS DMMA), fed here by a 4-stage cp.async pipeline of padded shared-memory tiles.
+//
+//   C[M,N] (row-major) = alpha * A(m,k) * B(k,n) + beta * C
+//   A is stored [M][K] (A_KC: k contiguous) or [K][M];  B is stored [K][N] or [N][K] (B_KC: k contiguous).
+//
+// CTA tile 128x128x16, 8 warps as 2(M) x 4(N), warp tile 64x32 = 8x4 DMMA atoms (64 accumulator doubles/thread).
+// Shared-memory row pitches are = 4 (mod 16) doubles, which makes the 8-byte fragment loads of a half-warp hit
+// 16 distinct bank pairs for both storage orders.
+#include "internal.h"
+
+namespace tatrg {
+thread_local LaunchCounter* g_counter = nullptr;
+
+namespace {
+constexpr int BM = 128, BN = 128, BK = 16, NT = 256, STAGES = 4;
+constexpr int PITCH_KC = BK + 4;   // operand stored [row][k]: 20 doubles
+constexpr int PITCH_MC = BM + 4;   // operand stored [k][row]: 132 doubles
+constexpr int TILE_D = BM * PITCH_KC;  // 2560 doubles >= BK*PITCH_MC = 2112
+constexpr int SMEM_BYTES = STAGES * 2 * TILE_D * 8;
+
+__device__ __forceinline__ void cp16(double* dst, const double* src, bool ok) {
+    unsigned d = (unsigned)__cvta_generic_to_shared(dst);
+    int n = ok ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(d), "l"(src), "r"(n));
+}
+__device__ __forceinline__ void cp8(double* dst, const double* src, bool ok) {
+    unsigned d = (unsigned)__cvta_generic_to_shared(dst);
+    int n = ok ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(d), "l"(src), "r"(n));
+}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+__device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+// Load one 128 x 16 operand tile.  KC: global element (r, k) at g[r*ld + k]; else at g[k*ld + r].
+// rows = extent of the non-contracted dimension, K = extent of k; r0/k0 tile origin.
+template <bool KC, bool V16>
+__device__ __forceinline__ void load_tile(double* s, const double* __restrict__ g, int64_t ld, int64_t r0, int64_t k0,
+                                          int64_t rows, int64_t K, int tid) {
+    if (KC) {
+        if (V16) {
+#pragma unroll
+            for (int c = tid; c < BM * BK / 2; c += NT) {
+                int r = c >> 3, kc = (c & 7) * 2;
+                bool ok = (r0 + r < rows) && (k0 + kc < K);
+                const double* src = ok ? g + (r0 + r) * ld + k0 + kc : g;
+                cp16(s + r * PITCH_KC + kc, src, ok);
+            }
+        } else {
+#pragma unroll
+            for (int c = tid; c < BM * BK; c += NT) {
+                int r = c >> 4, kc = c & 15;
+                bool ok = (r0 + r < rows) && (k0 + kc < K);
+                const double* src = ok ? g + (r0 + r) * ld + k0 + kc : g;
+                cp8(s + r * PITCH_KC + kc, src, ok);
+            }
+        }
+    } else {
+        if (V16) {
+#pragma unroll
+            for (int c = tid; c < BM * BK / 2; c += NT) {
+                int k = c >> 6, rc = (c & 63) * 2;
+                bool ok = (k0 + k < K) && (r0 + rc < rows);
+                const double* src = ok ? g + (k0 + k) * ld + r0 + rc : g;
+                cp16(s + k * PITCH_MC + rc, src, ok);
+            }
+        } else {
+#pragma unroll
+            for (int c = tid; c < BM * BK; c += NT) {
+                int k = c >> 7, rc = c & 127;
+                bool ok = (k0 + k < K) && (r0 + rc < rows);
+                const double* src = ok ? g + (k0 + k) * ld + r0 + rc : g;
+                cp8(s + k * PITCH_MC + rc, src, ok);
+            }
+        }
+    }
+}
+
+template <bool A_KC, bool B_KC, bool AV16, bool BV16>
+__global__ void __launch_bounds__(NT, 1)
+dgemm_kernel(int64_t M, int64_t N, int64_t K, double alpha, const double* __restrict__ A, int64_t lda,
+             const double* __restrict__ B, int64_t ldb, double beta, double* __restrict__ C, int64_t ldc, int64_t sA,
+             int64_t sB, int64_t sC, int tiles_m) {
+    extern __shared__ __align__(16) double smem[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int g = lane >> 2, t = lane & 3;
+    const int wm = warp >> 2, wn = warp & 3;
+    // tile order: consecutive CTAs walk down M for a fixed N-panel so that the B panel stays in L2
+    const int64_t tile = blockIdx.x;
+    const int64_t m0 = (tile % tiles_m) * BM, n0 = (tile / tiles_m) * BN;
+    A += (int64_t)blockIdx.z * sA; B += (int64_t)blockIdx.z * sB; C += (int64_t)blockIdx.z * sC;
+
+    double acc[8][4][2];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    const int nk = (int)((K + BK - 1) / BK);
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; ++s) {
+        if (s < nk) {
+            load_tile<A_KC, AV16>(smem + (2 * s) * TILE_D, A, lda, m0, (int64_t)s * BK, M, K, tid);
+            load_tile<B_KC, BV16>(smem + (2 * s + 1) * TILE_D, B, ldb, n0, (int64_t)s * BK, N, K, tid);
+        }
+        cp_commit();
+    }
+    for (int kt = 0; kt < nk; ++kt) {
+        cp_wait<STAGES - 2>();
+        __syncthreads();
+        {
+            int nxt = kt + STAGES - 1;
+            if (nxt < nk) {
+                int s = nxt % STAGES;
+                load_tile<A_KC, AV16>(smem + (2 * s) * TILE_D, A, lda, m0, (int64_t)nxt * BK, M, K, tid);
+                load_tile<B_KC, BV16>(smem + (2 * s + 1) * TILE_D, B, ldb, n0, (int64_t)nxt * BK, N, K, tid);
+            }
+            cp_commit();
+        }
+        const double* As = smem + (2 * (kt % STAGES)) * TILE_D;
+        const double* Bs = As + TILE_D;
+#pragma unroll
+        for (int ks = 0; ks < BK / 4; ++ks) {
+            double a[8], b[4];
+            const int k = ks * 4 + t;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                int m = wm * 64 + i * 8 + g;
+                a[i] = A_KC ? As[m * PITCH_KC + k] : As[k * PITCH_MC + m];
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                int n = wn * 32 + j * 8 + g;
+                b[j] = B_KC ? Bs[n * PITCH_KC + k] : Bs[k * PITCH_MC + n];
+            }
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+    }
+    cp_wait<0>();
+    const bool vec = ((ldc & 1) == 0) && ((((uintptr_t)C) & 15) == 0);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        int64_t m = m0 + wm * 64 + i * 8 + g;
+        if (m >= M) continue;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            int64_t n = n0 + wn * 32 + j * 8 + 2 * t;
+            if (n >= N) continue;
+            double* c = C + m * ldc + n;
+            double v0 = alpha * acc[i][j][0], v1 = alpha * acc[i][j][1];
+            if (n + 1 < N) {
+                if (beta != 0.0) { v0 += beta * c[0]; v1 += beta * c[1]; }
+                if (vec) *reinterpret_cast<double2*>(c) = make_double2(v0, v1);
+                else { c[0] = v0; c[1] = v1; }
+            } else {
+                if (beta != 0.0) v0 += beta * c[0];
+                c[0] = v0;
+            }
+        }
+    }
+}
+
+template <bool A_KC, bool B_KC, bool AV, bool BV>
+cudaError_t launch(cudaStream_t st, int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda, const double* B,
+                   int64_t ldb, double beta, double* C, int64_t ldc, int batch, int64_t sA, int64_t sB, int64_t sC) {
+    auto kern = dgemm_kernel<A_KC, B_KC, AV, BV>;
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    int64_t tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
+    dim3 grid((unsigned)(tm * tn), 1, (unsigned)batch);
+    kern<<<grid, NT, SMEM_BYTES, st>>>(M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC, (int)tm);
+    count_launch();
+    return cudaGetLastError();
+}
+
+template <bool A_KC, bool B_KC>
+cudaError_t pick_vec(bool av, bool bv, cudaStream_t st, int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
+                     const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch, int64_t sA, int64_t sB, int64_t sC) {
+    if (av && bv) return launch<A_KC, B_KC, true, true>(st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+    if (av) return launch<A_KC, B_KC, true, false>(st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+    if (bv) return launch<A_KC, B_KC, false, true>(st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+    return launch<A_KC, B_KC, false, false>(st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+}
+}  // namespace
+
+cudaError_t dgemm(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+                  int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch, int64_t sA,
+                  int64_t sB, int64_t sC) {
+    if (M <= 0 || N <= 0 || batch <= 0) return cudaSuccess;
+    // transa == false: A stored [M][K] -> k contiguous.  transb == false: B stored [K][N] -> n contiguous.
+    const bool a_kc = !transa, b_kc = transb;
+    // 16-byte cp.async needs: even leading dimension, 16B-aligned base and batch stride, even contiguous extent
+    auto v16 = [](const double* p, int64_t ld, int64_t contig_extent, int64_t bs) {
+        return ((uintptr_t)p % 16 == 0) && (ld % 2 == 0) && (contig_extent % 2 == 0) && (bs % 2 == 0);
+    };
+    const bool av = v16(A, lda, a_kc ? K : M, sA), bv = v16(B, ldb, b_kc ? K : N, sB);
+    if (a_kc && b_kc) return pick_vec<true, true>(av, bv, st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+    if (a_kc && !b_kc) return pick_vec<true, false>(av, bv, st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+    if (!a_kc && b_kc) return pick_vec<false, true>(av, bv, st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+    return pick_vec<false, false>(av, bv, st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+}
+
+}  // namespace tatrg
