@@ -26,7 +26,8 @@ enum {
     TATRG_OPT_POWER_ITERS = 1, /* n_pow: RSVD power iterations; passes of Eq. A.4-A.6 (:352-369) = n_pow+1. default 2 */
     TATRG_OPT_K_TRIAD = 2,     /* internal-line dimension rD of the triad isometries (Eq. 2.9 :135). default D+oversample */
     TATRG_OPT_TAU = 3,         /* relative gap below which values form one multiplet (R7). default 1e-6 */
-    TATRG_OPT_STAGE_TIMING = 4 /* 1: record CUDA-event times per stage (adds stream syncs). default 0 */
+    TATRG_OPT_STAGE_TIMING = 4,/* 1: CUDA-event time per stage; 2: also per DGEMM / permute launch (tatrg_gemm_profile). default 0 */
+    TATRG_OPT_KEEP_TENSORS = 5 /* 1: keep copies of the step's intermediate tensors for tatrg_get_tensor (tests). default 0 */
 };
 
 /* which spectrum tatrg_singular_values returns */
@@ -76,8 +77,12 @@ void tatrg_destroy(tatrg_handle); /* frees the host struct only */
 int tatrg_stage_ms(tatrg_handle, double* ms);
 int tatrg_stage_flops(tatrg_handle, double* flops);
 long long tatrg_last_step_launches(tatrg_handle);
-/* device time (ms) and flops spent inside the DGEMM kernel during the last step (needs STAGE_TIMING=2). */
+/* device time (ms; needs STAGE_TIMING=2), flops and launches of the DGEMM kernel during the last step; likewise the
+ * leg-permutation kernel with its algorithmic bytes (8 B read + 8 B written per element). Any out pointer may be NULL. */
 int tatrg_gemm_profile(tatrg_handle, double* ms, double* flops, long long* calls);
+int tatrg_permute_profile(tatrg_handle, double* ms, double* bytes, long long* calls);
+/* high-water mark (bytes) of the workspace since tatrg_create */
+size_t tatrg_workspace_peak(tatrg_handle);
 
 /* Copies a named tensor of the last step to out_host [host] (row-major).  Names: "phi","psi" (state after the
  * step), "A","Dt","core","X","Y","sigma","E","F","G","H","UA","UX","UY","UD","M2","M3","M4","N2","N3","N4".
@@ -100,8 +105,11 @@ int tatrg_dgemm(void* cuda_stream, int transa, int transb, long long M, long lon
 /* out = in with legs permuted: out leg i is in leg perm[i]; dims[ndim] are the extents of `in` (row-major). */
 int tatrg_permute(void* cuda_stream, int ndim, const long long* dims, const int* perm, const double* in, double* out);
 
-/* Tensor contraction  "abc,cd->abd"-style (single-letter legs, no repeated output legs) = permutes + one DGEMM.
- * dimsA/dimsB [host]; scratch [dev] of scratch_bytes for permuted copies (>= 8*(|A|+|B|+|C|) always suffices). */
+/* Tensor contraction  "abc,cd->abd"  (single-letter legs; an UPPERCASE leg is a batch leg and may be missing from one
+ * operand) = leg permutations only where the layout forces them + one batched DGEMM.  dimsA/dimsB [host] hold the
+ * extents of the legs named in spec; C [dev] receives the result in the leg order written after "->".
+ * scratch [dev] of scratch_bytes holds permuted copies and split-K partials (8*(|A|+|B|+|C|) + 64 MiB always suffices;
+ * ENOMEM otherwise). */
 int tatrg_contract(void* cuda_stream, const char* spec, const double* A, const long long* dimsA, const double* B,
                    const long long* dimsB, double* C, void* scratch, size_t scratch_bytes);
 
@@ -112,17 +120,20 @@ int tatrg_philox_raw(void* cuda_stream, uint64_t seed, uint32_t call, uint32_t s
 int tatrg_philox_gaussian(void* cuda_stream, uint64_t seed, uint32_t call, uint32_t stream_id, uint64_t start,
                           long long count, double* z);
 
-/* Symmetric eigen-decomposition by parallel Jacobi: G [dev] n x n (destroyed), lam [dev] n descending,
- * V [dev] n x n row-major, COLUMNS are eigenvectors.  work [dev] >= tatrg_eigh_work_bytes(n).  Synchronises. */
+/* Symmetric eigen-decomposition by (block) two-sided Jacobi: G [dev] n x n row-major (destroyed), lam [dev] n
+ * descending, Vt [dev] n x n row-major, ROW j = eigenvector j.  work [dev] >= tatrg_eigh_work_bytes(n), 256-byte
+ * aligned.  Synchronises the stream (the order of the eigenvalues is taken on the host).  ENUMERIC if not converged. */
 size_t tatrg_eigh_work_bytes(int n);
-int tatrg_eigh(void* cuda_stream, int n, double* G, double* lam, double* V, void* work);
+int tatrg_eigh(void* cuda_stream, int n, double* G, double* lam, double* Vt, void* work);
 
-/* Thin SVD of A [dev] m x n (m >= n, row-major, preserved) by one-sided Jacobi: U [dev] m x n, s [dev] n
- * descending, V [dev] n x n (columns = right singular vectors).  work >= tatrg_svd_work_bytes(m,n). */
-size_t tatrg_svd_work_bytes(int m, int n);
-int tatrg_svd(void* cuda_stream, int m, int n, const double* A, double* U, double* s, double* V, void* work);
+/* SVD of a small matrix X [dev] nv x len (row-major, preserved; 8*(nv*(len+1)+nv*(nv+1)) <= 200 KiB of shared memory)
+ * by one-sided Jacobi on its rows:  X = Vacc^T diag(s) Ut,  s [dev] nv descending, Ut [dev] nv x len with orthonormal
+ * rows (zero rows where s = 0), Vacc [dev] nv x nv orthogonal.  work >= tatrg_svd_work_bytes(nv,len).  Synchronises. */
+size_t tatrg_svd_work_bytes(int nv, int len);
+int tatrg_svd(void* cuda_stream, int nv, int len, const double* X, double* s, double* Ut, double* Vacc, void* work);
 
-/* result[0] [dev] = sum_i x[i]*y[i]  (the tensor trace tTr of Eq. 2.1 :48 on the factored tensor). */
+/* result[0] [dev] = sum_i x[i]*y[i]  (the tensor trace tTr of Eq. 2.1 :48 on the factored tensor).
+ * result must have room for 1200 doubles (partial sums of the first pass follow result[0]). */
 int tatrg_dot(void* cuda_stream, long long n, const double* x, const double* y, double* result);
 
 #ifdef __cplusplus

@@ -11,7 +11,11 @@
 #include "internal.h"
 
 namespace tatrg {
-thread_local LaunchCounter* g_counter = nullptr;
+thread_local Counters* g_counter = nullptr;
+cudaEvent_t Counters::next_event() {
+    if (ev_used == ev_pool.size()) { cudaEvent_t e; cudaEventCreate(&e); ev_pool.push_back(e); }
+    return ev_pool[ev_used++];
+}
 
 namespace {
 constexpr int BM = 128, BN = 128, BK = 16, NT = 256, STAGES = 4;
@@ -196,7 +200,7 @@ cudaError_t pick_vec(bool av, bool bv, cudaStream_t st, int64_t M, int64_t N, in
 }
 }  // namespace
 
-cudaError_t dgemm(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+static cudaError_t dgemm_raw(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                   int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch, int64_t sA,
                   int64_t sB, int64_t sC) {
     if (M <= 0 || N <= 0 || batch <= 0) return cudaSuccess;
@@ -211,6 +215,79 @@ cudaError_t dgemm(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t 
     if (a_kc && !b_kc) return pick_vec<true, false>(av, bv, st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
     if (!a_kc && b_kc) return pick_vec<false, true>(av, bv, st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
     return pick_vec<false, false>(av, bv, st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+}
+
+
+cudaError_t dgemm(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+                  int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch, int64_t sA,
+                  int64_t sB, int64_t sC) {
+    if (M <= 0 || N <= 0 || batch <= 0) return cudaSuccess;
+    Counters* c = g_counter;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (c) { c->gemm_flops += 2.0 * (double)M * (double)N * (double)K * batch; c->gemm_calls += 1; }
+    if (c && c->time_kernels) { e0 = c->next_event(); e1 = c->next_event(); cudaEventRecord(e0, st); }
+    cudaError_t e = cudaSuccess;
+    // grid.z carries the batch: split very large batches
+    for (int b0 = 0; b0 < batch && e == cudaSuccess; b0 += 32768) {
+        int nb = batch - b0 < 32768 ? batch - b0 : 32768;
+        e = dgemm_raw(st, transa, transb, M, N, K, alpha, A + (int64_t)b0 * sA, lda, B + (int64_t)b0 * sB, ldb, beta,
+                      C + (int64_t)b0 * sC, ldc, nb, sA, sB, sC);
+    }
+    if (e0) { cudaEventRecord(e1, st); c->gemm_ev.push_back({e0, e1}); }
+    return e;
+}
+
+// ---- split-K ---------------------------------------------------------------------------------------------------
+namespace {
+constexpr int kSplitTarget = 148 * 2;
+int splitk_count(int64_t M, int64_t N, int64_t K) {
+    int64_t tiles = ((M + BM - 1) / BM) * ((N + BN - 1) / BN);
+    if (tiles >= 74 || K < 8 * BK) return 1;
+    int64_t s = kSplitTarget / tiles;
+    int64_t maxs = K / (4 * BK);          // at least 4 k-tiles per chunk
+    if (s > maxs) s = maxs;
+    if (s > 512) s = 512;
+    return s < 2 ? 1 : (int)s;
+}
+__global__ void splitk_reduce_kernel(const double* __restrict__ part, int nsplit, int64_t MN, int64_t N, double alpha,
+                                     double* __restrict__ C, int64_t ldc) {
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < MN; e += (int64_t)gridDim.x * blockDim.x) {
+        double s = 0;
+        for (int k = 0; k < nsplit; ++k) s += part[(int64_t)k * MN + e];
+        int64_t r = e / N, c = e - r * N;
+        C[r * ldc + c] = alpha * s;
+    }
+}
+}  // namespace
+
+int64_t dgemm_splitk_doubles(int64_t M, int64_t N, int64_t K) {
+    int s = splitk_count(M, N, K);
+    return s > 1 ? (int64_t)s * M * N : 0;
+}
+
+cudaError_t dgemm_splitk(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+                         int64_t lda, const double* B, int64_t ldb, double* C, int64_t ldc, double* part) {
+    int ns = splitk_count(M, N, K);
+    if (ns <= 1 || part == nullptr) return dgemm(st, transa, transb, M, N, K, alpha, A, lda, B, ldb, 0.0, C, ldc);
+    // chunk: multiple of BK; the last chunk takes the ragged tail through a second launch
+    int64_t chunk = ((K + ns - 1) / ns + BK - 1) / BK * BK;
+    int nfull = (int)(K / chunk);
+    int64_t tail = K - (int64_t)nfull * chunk;
+    const int64_t stepA = transa ? chunk * lda : chunk, stepB = transb ? chunk : chunk * ldb;
+    cudaError_t e = cudaSuccess;
+    if (nfull > 0) e = dgemm(st, transa, transb, M, N, chunk, 1.0, A, lda, B, ldb, 0.0, part, N, nfull, stepA, stepB, M * N);
+    if (e != cudaSuccess) return e;
+    int total = nfull;
+    if (tail > 0) {
+        e = dgemm(st, transa, transb, M, N, tail, 1.0, A + nfull * stepA, lda, B + nfull * stepB, ldb, 0.0, part + (int64_t)nfull * M * N, N);
+        if (e != cudaSuccess) return e;
+        total += 1;
+    }
+    int64_t MN = M * N;
+    int64_t blocks = (MN + 255) / 256; if (blocks > 148 * 8) blocks = 148 * 8;
+    splitk_reduce_kernel<<<(unsigned)blocks, 256, 0, st>>>(part, total, MN, N, alpha, C, ldc);
+    count_launch();
+    return cudaGetLastError();
 }
 
 }  // namespace tatrg

@@ -11,6 +11,7 @@ __device__ __forceinline__ double fmode(double v, int mode) {
         case 1: return 1.0 / v;
         case 2: return 1.0 / sqrt(v);
         case 3: return sqrt(v);
+        case 4: return 1.0 / (v * sqrt(v));
         default: return v;
     }
 }
@@ -22,19 +23,40 @@ __global__ void scale_rows_kernel(double* out, const double* in, const double* v
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x)
         out[e] = in[e] * fmode(vec[e / cols], mode);
 }
-__global__ void gather_cols_kernel(double* out, const double* in, int64_t rows, int64_t ld, int64_t c0, int64_t nc) {
-    int64_t total = rows * nc;
-    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
-        int64_t r = e / nc, c = e - r * nc;
-        out[e] = in[r * ld + c0 + c];
-    }
-}
-__global__ void gather_rows_kernel(double* out, const double* in, const int* idx, const double* scale, int64_t nrows, int64_t cols) {
+__global__ void gather_rows_kernel(double* out, const double* in, const int* idx, const double* scale, int64_t nrows, int64_t cols,
+                                   int64_t ld) {
     int64_t total = nrows * cols;
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
         int64_t r = e / cols, c = e - r * cols;
-        out[e] = in[(int64_t)idx[r] * cols + c] * (scale ? scale[r] : 1.0);
+        out[e] = in[(int64_t)idx[r] * ld + c] * (scale ? scale[r] : 1.0);
     }
+}
+__global__ void gather_vec_kernel(double* out, const double* in, const int* idx, int64_t n, int64_t stride, double mul) {
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x)
+        out[e] = in[(int64_t)idx[e] * stride] * mul;
+}
+// One warp per multiplet: modified Gram-Schmidt of the g x g block C[a:b, 0:g] (columns), diag(R) > 0, written as the
+// diagonal block of G.  g == 1 reduces to the sign of C[a,0].  Lane i holds row i of the block (g <= 32).
+__global__ void gauge_blocks_kernel(const double* __restrict__ cfull, int ldc, const int* __restrict__ groups, int ngroups, int k,
+                                    double* __restrict__ G) {
+    int grp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (grp >= ngroups) return;
+    const int lane = threadIdx.x & 31;
+    const int a = groups[2 * grp], b = groups[2 * grp + 1], g = b - a;
+    double q[32];   // row `lane` of Q, columns 0..g-1 (fully unrolled access would be needed for registers; g is tiny)
+    for (int j = 0; j < g; ++j) {
+        double col = (lane < g) ? cfull[(int64_t)(a + lane) * ldc + j] : 0.0;
+        for (int i = 0; i < j; ++i) {
+            double d = q[i] * col;
+            for (int o = 16; o > 0; o >>= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
+            col -= d * q[i];
+        }
+        double n2 = col * col;
+        for (int o = 16; o > 0; o >>= 1) n2 += __shfl_xor_sync(0xffffffffu, n2, o);
+        q[j] = col / sqrt(n2);
+    }
+    if (lane < g)
+        for (int j = 0; j < g; ++j) G[(int64_t)(a + lane) * k + a + j] = q[j];
 }
 __global__ void zero_kernel(double* p, int64_t n) {
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) p[e] = 0.0;
@@ -93,14 +115,22 @@ cudaError_t scale_rows(cudaStream_t st, double* out, const double* in, const dou
     scale_rows_kernel<<<nblocks(rows * cols), 256, 0, st>>>(out, in, vec, rows * cols, cols, mode); count_launch();
     return cudaGetLastError();
 }
-cudaError_t gather_cols(cudaStream_t st, double* out, const double* in, int64_t rows, int64_t ld_in, int64_t c0, int64_t ncols) {
-    if (rows * ncols == 0) return cudaSuccess;
-    gather_cols_kernel<<<nblocks(rows * ncols), 256, 0, st>>>(out, in, rows, ld_in, c0, ncols); count_launch();
+cudaError_t gather_rows_scaled(cudaStream_t st, double* out, const double* in, const int* idx, const double* scale, int64_t nrows,
+                               int64_t cols, int64_t ld_in) {
+    if (nrows * cols == 0) return cudaSuccess;
+    gather_rows_kernel<<<nblocks(nrows * cols), 256, 0, st>>>(out, in, idx, scale, nrows, cols, ld_in); count_launch();
     return cudaGetLastError();
 }
-cudaError_t gather_rows_scaled(cudaStream_t st, double* out, const double* in, const int* idx, const double* scale, int64_t nrows, int64_t cols) {
-    if (nrows * cols == 0) return cudaSuccess;
-    gather_rows_kernel<<<nblocks(nrows * cols), 256, 0, st>>>(out, in, idx, scale, nrows, cols); count_launch();
+cudaError_t gather_vec(cudaStream_t st, double* out, const double* in, const int* idx, int64_t n, int64_t stride_in, double mul) {
+    if (n == 0) return cudaSuccess;
+    gather_vec_kernel<<<nblocks(n), 256, 0, st>>>(out, in, idx, n, stride_in, mul); count_launch();
+    return cudaGetLastError();
+}
+cudaError_t gauge_blocks(cudaStream_t st, const double* cfull, int ldc, const int* groups, int ngroups, int k, double* G) {
+    if (k <= 0 || ngroups <= 0) return cudaSuccess;
+    cudaError_t e = fill_zero(st, G, (int64_t)k * k);
+    if (e != cudaSuccess) return e;
+    gauge_blocks_kernel<<<(ngroups + 3) / 4, 128, 0, st>>>(cfull, ldc, groups, ngroups, k, G); count_launch();
     return cudaGetLastError();
 }
 cudaError_t fill_zero(cudaStream_t st, double* p, int64_t n) {

@@ -18,42 +18,68 @@ constexpr double kEpsLambda = 1e-12;      // R14: Gram eigenvalues
 constexpr double kEpsSqueezer = 1e-6;     // R14: squeezer singular values
 constexpr int kRhoCols = 64;              // R10: reference vectors rho[:, j], j < 64
 
-struct LaunchCounter { long long n = 0; };
-extern thread_local LaunchCounter* g_counter;  // counts kernel launches of the current step
-inline void count_launch(int k = 1) { if (g_counter) g_counter->n += k; }
+// per-thread launch/GEMM accounting of the step being enqueued
+struct Counters {
+    long long launches = 0;
+    double gemm_flops = 0;          // 2*M*N*K of every DGEMM launched
+    long long gemm_calls = 0;
+    long long permuted_bytes = 0;   // read + write bytes of every leg permutation
+    long long permute_calls = 0;
+    // optional device timing of the two kernel families (TATRG_OPT_STAGE_TIMING = 2): events bracket each launch
+    bool time_kernels = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> gemm_ev, perm_ev;
+    std::vector<cudaEvent_t> ev_pool;
+    size_t ev_used = 0;
+    cudaEvent_t next_event();
+};
+extern thread_local Counters* g_counter;
+inline void count_launch(int k = 1) { if (g_counter) g_counter->launches += k; }
 
 // ---- kernels (each file exposes host launchers only) --------------------------------------------------------
 // dgemm.cu : C[M,N] = alpha*op(A)*op(B) + beta*C on FP64 tensor cores (DMMA m8n8k4)
 cudaError_t dgemm(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                   int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch = 1,
                   int64_t sA = 0, int64_t sB = 0, int64_t sC = 0);
+// split-K variant for skinny outputs (Gram matrices of tall operands): partial products of K-chunks go to `part`
+// (>= dgemm_splitk_doubles(M,N,K) doubles, [dev]) and are summed by a second kernel.  Falls back to dgemm when
+// the output already fills the machine.  part may be null when dgemm_splitk_doubles() == 0.
+int64_t dgemm_splitk_doubles(int64_t M, int64_t N, int64_t K);
+cudaError_t dgemm_splitk(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+                         int64_t lda, const double* B, int64_t ldb, double* C, int64_t ldc, double* part);
 
 // permute.cu
 cudaError_t permute(cudaStream_t st, int nd, const int64_t* dims, const int* perm, const double* in, double* out);
 
 // elementwise.cu
 cudaError_t scale_last(cudaStream_t st, double* out, const double* in, const double* vec, int64_t rows, int64_t cols,
-                       int mode);  // out[r,c] = in[r,c] * f(vec[c]); mode 0: v, 1: 1/v, 2: 1/sqrt(v), 3: sqrt(v), 4: 1/sqrt(sqrt(v))...
+                       int mode);  // out[r,c] = in[r,c] * f(vec[c]); mode 0: v, 1: 1/v, 2: 1/sqrt(v), 3: sqrt(v), 4: v^-3/2
 cudaError_t scale_rows(cudaStream_t st, double* out, const double* in, const double* vec, int64_t rows, int64_t cols, int mode);
-cudaError_t gather_cols(cudaStream_t st, double* out, const double* in, int64_t rows, int64_t ld_in, int64_t c0, int64_t ncols);
 cudaError_t gather_rows_scaled(cudaStream_t st, double* out, const double* in, const int* idx, const double* scale, int64_t nrows,
-                               int64_t cols);  // out[r,:] = scale[r]*in[idx[r],:]
+                               int64_t cols, int64_t ld_in);  // out[r,:] = scale[r]*in[idx[r], 0:cols]
+cudaError_t gather_vec(cudaStream_t st, double* out, const double* in, const int* idx, int64_t n, int64_t stride_in, double mul);
 cudaError_t dot(cudaStream_t st, int64_t n, const double* x, const double* y, double* result);
 cudaError_t init_ising(cudaStream_t st, double beta, double h, double* phi, double* psi);
 cudaError_t fill_zero(cudaStream_t st, double* p, int64_t n);
+// G (k x k, row-major) = block-diagonal orthogonal gauge rotation: for every group [a,b) the block is the Q factor
+// (modified Gram-Schmidt, positive diagonal of R) of C[a:b, 0:b-a], C = cfull (k x ldc).  groups: 2*ngroups ints [dev].
+cudaError_t gauge_blocks(cudaStream_t st, const double* cfull, int ldc, const int* groups, int ngroups, int k, double* G);
 
 // philox.cu
 cudaError_t philox_raw(cudaStream_t st, uint64_t seed, uint32_t call, uint32_t stream, uint64_t start, int64_t count, uint32_t* raw);
 cudaError_t philox_gauss(cudaStream_t st, uint64_t seed, uint32_t call, uint32_t stream, uint64_t start, int64_t count, double* z);
 cudaError_t philox_rho(cudaStream_t st, uint64_t seed, uint32_t call, uint32_t stream, int64_t rows, int ncols, double* out);
 
-// jacobi.cu : rows-are-vectors storage.  eigh: G n x n symmetric (destroyed) -> lam (desc), V (columns = eigvecs)
+// jacobi.cu.  All decompositions return vectors as ROWS.
+//   eigh : G n x n symmetric [dev] (destroyed) -> lam[n] descending, Vt[n x n], row j = eigenvector j.  Synchronises.
+//   svd_rows : X [nv x len] [dev] (nv <= 96, len <= 96 ... see jacobi.cu) -> X = Vacc^T diag(s) Ut,  Ut rows orthonormal,
+//   sorted descending; s[nv], Ut[nv x len], Vacc[nv x nv] (row j = left vector j in the basis of the input rows).
 size_t eigh_work_bytes(int n);
-int eigh(cudaStream_t st, int n, double* G, double* lam, double* V, void* work, std::string* err);
-size_t svd_work_bytes(int m, int n);
-int svd(cudaStream_t st, int m, int n, const double* A, double* U, double* s, double* V, void* work, std::string* err);
+int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work, std::vector<double>* lam_host, std::string* err);
+size_t svd_rows_work_bytes(int nv, int len);
+int svd_rows(cudaStream_t st, int nv, int len, const double* X, double* s, double* Ut, double* Vacc, void* work,
+             std::vector<double>* s_host, std::string* err);
 
-// ---- tensors and the workspace stack ------------------------------------------------------------------------
+// ---- tensors and the workspace pool -------------------------------------------------------------------------
 struct Tens {
     double* p = nullptr;
     int nd = 0;
@@ -61,22 +87,26 @@ struct Tens {
     int64_t size() const { int64_t s = 1; for (int i = 0; i < nd; ++i) s *= d[i]; return s; }
 };
 
-struct Arena {
-    char* base = nullptr; size_t cap = 0, top = 0, peak = 0;
-    double* alloc(int64_t n_doubles) {
-        size_t bytes = ((size_t)(n_doubles > 0 ? n_doubles : 1) * 8 + 255) & ~(size_t)255;
-        if (top + bytes > cap) return nullptr;
-        double* p = (double*)(base + top); top += bytes; if (top > peak) peak = top; return p;
-    }
-    size_t mark() const { return top; }
-    void release(size_t m) { top = m; }
+// First-fit free-list allocator over the caller's workspace.  Host bookkeeping only: all work is enqueued on one
+// stream, so a block may be reused as soon as the kernels that read it have been *enqueued*.
+class Pool {
+public:
+    void reset(void* base, size_t bytes);
+    double* alloc(int64_t n_doubles);  // nullptr when full
+    void free(const void* p);
+    size_t peak() const { return peak_; }
+    size_t in_use() const { return used_; }
+    size_t capacity() const { return cap_; }
+private:
+    char* base_ = nullptr; size_t cap_ = 0, used_ = 0, peak_ = 0, high_ = 0;
+    std::map<size_t, size_t> free_;   // offset -> size
+    std::map<size_t, size_t> live_;   // offset -> size
 };
 
-// contract.cu : einsum-style pairwise contraction = permutes + one DGEMM.  Output allocated by the caller.
-struct ContractStats { double flops = 0; int64_t permuted_bytes = 0; };
-int contract(cudaStream_t st, const char* spec, const Tens& A, const Tens& B, Tens& C, Arena& scratch, ContractStats* stats,
-             std::string* err);
-// shape of the result of `spec` applied to A and B (no computation)
+// contract.cu : einsum-style pairwise contraction = (permutes only where the layout forces them) + one DGEMM.
+// Single-letter legs; an UPPERCASE letter is a batch leg (may be missing from one operand: broadcast).
+// C.p must point to room for the result; C.nd / C.d are filled in.
+int contract(cudaStream_t st, const char* spec, const Tens& A, const Tens& B, Tens& C, Pool& pool, std::string* err);
 int contract_shape(const char* spec, const Tens& A, const Tens& B, Tens& C, std::string* err);
 
 }  // namespace tatrg

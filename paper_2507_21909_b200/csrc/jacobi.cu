@@ -1,0 +1,428 @@
+// jacobi.cu -- dense decompositions of the Triad-ATRG step on the device (PAPER.md: truncated SVD of Eq. 2.4 :76 and
+// Eq. 2.5 :90 / A.8 :376, HOSVD of Eq. 2.9 :135, squeezers :171; "SVD ... based on matrix multiplication" :213).
+//
+//   eigh      symmetric eigen-decomposition, two-sided Jacobi.
+//             n <= 64: one CTA, matrix and eigenvectors in shared memory, round-robin parallel ordering.
+//             n  > 64: block Jacobi with 32-wide column blocks.  One round = nb/2 disjoint block pairs; each pair's
+//             64 x 64 diagonal sub-problem is solved to convergence by one CTA in shared memory (the n <= 64 code),
+//             its accumulated 64 x 64 rotation is then applied to the block columns, block rows and to V^T as tile
+//             GEMMs.  nb - 1 rounds = one sweep; sweeps repeat until no CTA rotated anything.
+//   svd_rows  one-sided (Hestenes) Jacobi of a small matrix held in shared memory: one warp per row pair.
+//
+// Vectors are returned as ROWS, sorted by descending value (the order is taken on the host from the read-back
+// spectrum, which the caller needs anyway for its rank decisions).
+#include "internal.h"
+#include <algorithm>
+#include <cmath>
+#include <numeric>
+
+namespace tatrg {
+namespace {
+constexpr int SB = 64;          // side of the shared-memory sub-problem
+constexpr int SP = SB + 1;      // pitch
+constexpr int BW = 32;          // block width of the block-Jacobi
+constexpr double kTolRel = 1e-15;
+constexpr int kMaxSweeps = 40;
+
+// round-robin tournament on np (even) players: round r in [0, np-1), table k in [0, np/2)
+__device__ __host__ __forceinline__ void rr_pair(int np, int r, int k, int& p, int& q) {
+    const int m = np - 1;
+    int a, b;
+    if (k == 0) { a = m; b = r; }
+    else { a = (r + k) % m; b = (r + m - k) % m; }
+    p = a < b ? a : b; q = a < b ? b : a;
+}
+
+// plane rotation that annihilates a_pq of [[app, apq], [apq, aqq]] with J = [[c, s], [-s, c]]  (J^T A J diagonal)
+__device__ __forceinline__ void sym_rot(double app, double aqq, double apq, double& c, double& s) {
+    double zeta = (aqq - app) / (2.0 * apq);
+    double t = (zeta >= 0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+    c = 1.0 / sqrt(1.0 + t * t);
+    s = c * t;
+}
+
+// Two-sided Jacobi on the n x n symmetric S (shared, pitch SP), accumulating J (S_out = J^T S_in J, columns of J).
+// All threads of the CTA call it.  Returns the number of rotations applied.
+__device__ int jacobi_smem(double* S, double* J, int n, double abs_floor, double* cs, double* sn, int* pp, int* qq, int* cnt) {
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int np = n + (n & 1), half = np >> 1;
+    int total = 0;
+    for (int sweep = 0; sweep < kMaxSweeps; ++sweep) {
+        if (tid == 0) *cnt = 0;
+        __syncthreads();
+        for (int r = 0; r < np - 1; ++r) {
+            if (tid < half) {
+                int p, q; rr_pair(np, r, tid, p, q);
+                double c = 1.0, s = 0.0;
+                if (q < n) {
+                    double app = S[p * SP + p], aqq = S[q * SP + q], apq = S[p * SP + q];
+                    if (fabs(apq) > abs_floor && fabs(apq) > kTolRel * sqrt(fabs(app * aqq))) { sym_rot(app, aqq, apq, c, s); atomicAdd(cnt, 1); }
+                }
+                cs[tid] = c; sn[tid] = s; pp[tid] = p; qq[tid] = q;
+            }
+            __syncthreads();
+            // columns of S and of J
+            for (int e = tid; e < n * half; e += nt) {
+                int k = e / n, i = e - k * n;
+                double s = sn[k];
+                if (s == 0.0) continue;
+                double c = cs[k]; int p = pp[k], q = qq[k];
+                double x = S[i * SP + p], y = S[i * SP + q];
+                S[i * SP + p] = c * x - s * y; S[i * SP + q] = s * x + c * y;
+                x = J[i * SP + p]; y = J[i * SP + q];
+                J[i * SP + p] = c * x - s * y; J[i * SP + q] = s * x + c * y;
+            }
+            __syncthreads();
+            // rows of S
+            for (int e = tid; e < n * half; e += nt) {
+                int k = e / n, j = e - k * n;
+                double s = sn[k];
+                if (s == 0.0) continue;
+                double c = cs[k]; int p = pp[k], q = qq[k];
+                double x = S[p * SP + j], y = S[q * SP + j];
+                double xn = c * x - s * y, yn = s * x + c * y;
+                if (j == q) xn = 0.0;      // the rotation annihilates s_pq exactly
+                if (j == p) yn = 0.0;
+                S[p * SP + j] = xn; S[q * SP + j] = yn;
+            }
+            __syncthreads();
+        }
+        int c = *cnt;
+        __syncthreads();
+        total += c;
+        if (c == 0) break;
+    }
+    return total;
+}
+
+__device__ __forceinline__ double block_max(double v, double* red) {
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double m = 0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) m = fmax(m, red[w]);
+    __syncthreads();
+    return m;
+}
+
+// ---- n <= 64 ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(512, 1) eigh_small_kernel(int n, const double* __restrict__ G, double* __restrict__ lam, double* __restrict__ Vt) {
+    extern __shared__ double sh[];
+    double* S = sh; double* J = S + SB * SP;
+    double* cs = J + SB * SP; double* sn = cs + 32; double* red = sn + 32;
+    int* pp = (int*)(red + 32); int* qq = pp + 32; int* cnt = qq + 32;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    double dmax = 0;
+    for (int e = tid; e < n * n; e += nt) {
+        int i = e / n, j = e - i * n;
+        S[i * SP + j] = 0.5 * (G[i * n + j] + G[j * n + i]);
+        J[i * SP + j] = (i == j) ? 1.0 : 0.0;
+        if (i == j) dmax = fmax(dmax, fabs(G[e]));
+    }
+    __syncthreads();
+    dmax = block_max(dmax, red);
+    jacobi_smem(S, J, n, 1e-22 * dmax, cs, sn, pp, qq, cnt);
+    for (int e = tid; e < n * n; e += nt) { int i = e / n, j = e - i * n; Vt[i * n + j] = J[j * SP + i]; }   // row i = eigenvector i
+    for (int i = tid; i < n; i += nt) lam[i] = S[i * SP + i];
+}
+
+// ---- n > 64: block Jacobi ----------------------------------------------------------------------------------------
+__global__ void pad_sym_kernel(int n, int N, const double* __restrict__ G, double* __restrict__ Gp, double* __restrict__ Vt) {
+    int64_t total = (int64_t)N * N;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+        int i = (int)(e / N), j = (int)(e - (int64_t)i * N);
+        Gp[e] = (i < n && j < n) ? 0.5 * (G[(int64_t)i * n + j] + G[(int64_t)j * n + i]) : 0.0;
+        Vt[e] = (i == j) ? 1.0 : 0.0;
+    }
+}
+__global__ void diag_max_kernel(int N, const double* __restrict__ Gp, double* out) {   // one block
+    __shared__ double red[32];
+    double m = 0;
+    for (int i = threadIdx.x; i < N; i += blockDim.x) m = fmax(m, fabs(Gp[(int64_t)i * N + i]));
+    m = block_max(m, red);
+    if (threadIdx.x == 0) out[0] = m;
+}
+
+__device__ __forceinline__ int gidx(int P, int Q, int li) { return li < BW ? P * BW + li : Q * BW + li - BW; }
+
+// one CTA per block pair: solve the 64 x 64 diagonal sub-problem, emit its rotation J, the new diagonal and a flag
+__global__ void __launch_bounds__(512, 1) blk_solve_kernel(int N, int nb, int round, const double* __restrict__ Gp, const double* __restrict__ dmax,
+                                                           double* __restrict__ Jb, double* __restrict__ Dg, int* __restrict__ active,
+                                                           int* __restrict__ counter) {
+    extern __shared__ double sh[];
+    double* S = sh; double* J = S + SB * SP;
+    double* cs = J + SB * SP; double* sn = cs + 32; double* red = sn + 32;
+    int* pp = (int*)(red + 32); int* qq = pp + 32; int* cnt = qq + 32;
+    const int tid = threadIdx.x, nt = blockDim.x, k = blockIdx.x;
+    int P, Q; rr_pair(nb, round, k, P, Q);
+    for (int e = tid; e < SB * SB; e += nt) {
+        int i = e >> 6, j = e & 63;
+        S[i * SP + j] = Gp[(int64_t)gidx(P, Q, i) * N + gidx(P, Q, j)];
+        J[i * SP + j] = (i == j) ? 1.0 : 0.0;
+    }
+    __syncthreads();
+    const double floor_abs = 1e-22 * dmax[0];
+    // quick test: anything to rotate at all?
+    double worst = 0;
+    for (int e = tid; e < SB * SB; e += nt) {
+        int i = e >> 6, j = e & 63;
+        if (i < j) {
+            double a = fabs(S[i * SP + j]);
+            if (a > floor_abs && a > kTolRel * sqrt(fabs(S[i * SP + i] * S[j * SP + j]))) worst = 1.0;
+        }
+    }
+    worst = block_max(worst, red);
+    int rot = 0;
+    if (worst > 0) rot = jacobi_smem(S, J, SB, floor_abs, cs, sn, pp, qq, cnt);
+    if (tid == 0) { active[k] = rot > 0; if (rot > 0) atomicAdd(counter, rot); }
+    if (rot > 0) {
+        for (int e = tid; e < SB * SB; e += nt) { int i = e >> 6, j = e & 63; Jb[(int64_t)k * SB * SB + e] = J[i * SP + j]; }
+        for (int i = tid; i < SB; i += nt) Dg[k * SB + i] = S[i * SP + i];
+    }
+}
+
+// X[:, PQ] <- X[:, PQ] * J_k   (grid: row tiles x pairs; 256 threads, 4x4 outputs each)
+__global__ void __launch_bounds__(256) blk_apply_cols_kernel(int N, int nb, int round, double* __restrict__ X, const double* __restrict__ Jb,
+                                                             const int* __restrict__ active) {
+    const int k = blockIdx.y;
+    if (!active[k]) return;
+    extern __shared__ double sh2[];
+    double (*Xs)[SP] = reinterpret_cast<double (*)[SP]>(sh2);
+    double (*Js)[SP] = reinterpret_cast<double (*)[SP]>(sh2 + SB * SP);
+    int P, Q; rr_pair(nb, round, k, P, Q);
+    const int tid = threadIdx.x, r0 = blockIdx.x * SB;
+    for (int e = tid; e < SB * SB; e += 256) {
+        int i = e >> 6, j = e & 63;
+        Xs[i][j] = X[(int64_t)(r0 + i) * N + gidx(P, Q, j)];
+        Js[i][j] = Jb[(int64_t)k * SB * SB + e];
+    }
+    __syncthreads();
+    const int ti = (tid >> 4) * 4, tj = (tid & 15) * 4;
+    double acc[4][4] = {};
+#pragma unroll 8
+    for (int l = 0; l < SB; ++l) {
+        double a[4], b[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { a[u] = Xs[ti + u][l]; b[u] = Js[l][tj + u]; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int v = 0; v < 4; ++v) acc[u][v] += a[u] * b[v];
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int v = 0; v < 4; ++v) X[(int64_t)(r0 + ti + u) * N + gidx(P, Q, tj + v)] = acc[u][v];
+}
+
+// X[PQ, :] <- J_k^T * X[PQ, :]  for X = Gp (z = 0, with the exact diagonal block written back) and X = Vt (z = 1)
+__global__ void __launch_bounds__(256) blk_apply_rows_kernel(int N, int nb, int round, double* __restrict__ Gp, double* __restrict__ Vt,
+                                                             const double* __restrict__ Jb, const double* __restrict__ Dg,
+                                                             const int* __restrict__ active) {
+    const int k = blockIdx.y;
+    if (!active[k]) return;
+    extern __shared__ double sh2[];
+    double (*Xs)[SP] = reinterpret_cast<double (*)[SP]>(sh2);
+    double (*Js)[SP] = reinterpret_cast<double (*)[SP]>(sh2 + SB * SP);
+    int P, Q; rr_pair(nb, round, k, P, Q);
+    double* X = blockIdx.z == 0 ? Gp : Vt;
+    const int tid = threadIdx.x, c0 = blockIdx.x * SB;
+    for (int e = tid; e < SB * SB; e += 256) {
+        int i = e >> 6, j = e & 63;
+        Xs[i][j] = X[(int64_t)gidx(P, Q, i) * N + c0 + j];
+        Js[i][j] = Jb[(int64_t)k * SB * SB + e];
+    }
+    __syncthreads();
+    const int ti = (tid >> 4) * 4, tj = (tid & 15) * 4;
+    double acc[4][4] = {};
+#pragma unroll 8
+    for (int l = 0; l < SB; ++l) {
+        double a[4], b[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { a[u] = Js[l][ti + u]; b[u] = Xs[l][tj + u]; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int v = 0; v < 4; ++v) acc[u][v] += a[u] * b[v];
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+            const int li = ti + u, col = c0 + tj + v;
+            double val = acc[u][v];
+            if (blockIdx.z == 0) {
+                const int cb = col / BW;
+                if (cb == P || cb == Q) { int lj = (cb == P) ? col - P * BW : BW + col - Q * BW; val = (li == lj) ? Dg[k * SB + li] : 0.0; }
+            }
+            X[(int64_t)gidx(P, Q, li) * N + col] = val;
+        }
+}
+__global__ void extract_diag_kernel(int N, const double* __restrict__ Gp, double* __restrict__ d) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) d[i] = Gp[(int64_t)i * N + i];
+}
+
+// ---- one-sided Jacobi of a small matrix ---------------------------------------------------------------------------
+// W [nv x len] rows in shared memory (pitch len+1), Va [nv x nv] (pitch nv+1).  One warp per pair and round.
+__global__ void __launch_bounds__(1024, 1) svd_rows_kernel(int nv, int len, const double* __restrict__ X, double* __restrict__ s_out,
+                                                           double* __restrict__ Ut, double* __restrict__ Vacc) {
+    extern __shared__ double sh[];
+    const int pw = len + 1, pv = nv + 1;
+    double* W = sh; double* Va = W + nv * pw;
+    __shared__ int cnt;
+    const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nw = nt >> 5;
+    for (int e = tid; e < nv * len; e += nt) { int i = e / len, j = e - i * len; W[i * pw + j] = X[e]; }
+    for (int e = tid; e < nv * nv; e += nt) { int i = e / nv, j = e - i * nv; Va[i * pv + j] = (i == j) ? 1.0 : 0.0; }
+    __syncthreads();
+    const int np = nv + (nv & 1), half = np >> 1;
+    const double tol = kTolRel * sqrt((double)len);
+    for (int sweep = 0; sweep < kMaxSweeps; ++sweep) {
+        if (tid == 0) cnt = 0;
+        __syncthreads();
+        for (int r = 0; r < np - 1; ++r) {
+            for (int k = warp; k < half; k += nw) {
+                int p, q; rr_pair(np, r, k, p, q);
+                if (q >= nv) continue;
+                double* wp = W + p * pw; double* wq = W + q * pw;
+                double al = 0, be = 0, ga = 0;
+                for (int i = lane; i < len; i += 32) { double x = wp[i], y = wq[i]; al += x * x; be += y * y; ga += x * y; }
+                for (int o = 16; o > 0; o >>= 1) {
+                    al += __shfl_xor_sync(0xffffffffu, al, o); be += __shfl_xor_sync(0xffffffffu, be, o); ga += __shfl_xor_sync(0xffffffffu, ga, o);
+                }
+                if (al * be == 0.0 || fabs(ga) <= tol * sqrt(al) * sqrt(be)) continue;
+                double c, s; sym_rot(al, be, ga, c, s);
+                for (int i = lane; i < len; i += 32) { double x = wp[i], y = wq[i]; wp[i] = c * x - s * y; wq[i] = s * x + c * y; }
+                double* vp = Va + p * pv; double* vq = Va + q * pv;
+                for (int i = lane; i < nv; i += 32) { double x = vp[i], y = vq[i]; vp[i] = c * x - s * y; vq[i] = s * x + c * y; }
+                if (lane == 0) atomicAdd(&cnt, 1);
+            }
+            __syncthreads();
+        }
+        int c = cnt;
+        __syncthreads();
+        if (c == 0) break;
+    }
+    for (int k = warp; k < nv; k += nw) {
+        double* w = W + k * pw; double n2 = 0;
+        for (int i = lane; i < len; i += 32) n2 += w[i] * w[i];
+        for (int o = 16; o > 0; o >>= 1) n2 += __shfl_xor_sync(0xffffffffu, n2, o);
+        double sv = sqrt(n2), inv = sv > 0 ? 1.0 / sv : 0.0;
+        for (int i = lane; i < len; i += 32) Ut[k * len + i] = w[i] * inv;
+        for (int i = lane; i < nv; i += 32) Vacc[k * nv + i] = Va[k * pv + i];
+        if (lane == 0) s_out[k] = sv;
+    }
+}
+
+bool check(cudaError_t e, std::string* err, const char* what) {
+    if (e == cudaSuccess) return true;
+    if (err) *err = std::string(what) + ": " + cudaGetErrorString(e);
+    return false;
+}
+constexpr int kSmallSmem = (2 * SB * SP + 96) * 8 + 3 * 32 * 4 + 64;
+constexpr int kApplySmem = 2 * SB * SP * 8;
+}  // namespace
+
+// work layout (bytes): [lam_unsorted N][idx N ints][misc 64 doubles][Vt_unsorted N*N][Gp N*N][Jb nb/2*4096][Dg nb/2*64][active nb/2 ints]
+static int padded_n(int n) { if (n <= SB) return n; int nb = (n + BW - 1) / BW; if (nb & 1) ++nb; return nb * BW; }
+
+size_t eigh_work_bytes(int n) {
+    size_t N = (size_t)padded_n(n);
+    size_t nb2 = N / BW / 2 + 1;
+    return 8 * (N + N + 64 + 2 * N * N + nb2 * SB * SB + nb2 * SB + nb2) + 4096;
+}
+
+int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work, std::vector<double>* lam_host, std::string* err) {
+    if (n <= 0) return TATRG_OK;
+    const int N = padded_n(n);
+    double* w = (double*)work;
+    double* lam_u = w; w += N;
+    int* idx = (int*)w; w += N;
+    double* misc = w; w += 64;
+    double* Vu = w; w += (size_t)N * N;
+    static bool cfg = false;
+    if (!cfg) {
+        if (!check(cudaFuncSetAttribute(eigh_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmallSmem), err, "eigh attr")) return TATRG_ECUDA;
+        if (!check(cudaFuncSetAttribute(blk_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmallSmem), err, "eigh attr")) return TATRG_ECUDA;
+        if (!check(cudaFuncSetAttribute(blk_apply_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kApplySmem), err, "eigh attr")) return TATRG_ECUDA;
+        if (!check(cudaFuncSetAttribute(blk_apply_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kApplySmem), err, "eigh attr")) return TATRG_ECUDA;
+        cfg = true;
+    }
+    if (n <= SB) {
+        eigh_small_kernel<<<1, 512, kSmallSmem, st>>>(n, G, lam_u, Vu); count_launch();
+    } else {
+        double* Gp = w; w += (size_t)N * N;
+        const int nb = N / BW, npair = nb / 2;
+        double* Jb = w; w += (size_t)npair * SB * SB;
+        double* Dg = w; w += (size_t)npair * SB;
+        int* active = (int*)w; w += npair;     // npair ints fit in npair doubles
+        int* counter = (int*)misc + 8;
+        pad_sym_kernel<<<148 * 4, 256, 0, st>>>(n, N, G, Gp, Vu);
+        diag_max_kernel<<<1, 256, 0, st>>>(N, Gp, misc);
+        count_launch(2);
+        int sweep = 0;
+        for (; sweep < kMaxSweeps; ++sweep) {
+            cudaMemsetAsync(counter, 0, sizeof(int), st);
+            for (int r = 0; r < nb - 1; ++r) {
+                blk_solve_kernel<<<npair, 512, kSmallSmem, st>>>(N, nb, r, Gp, misc, Jb, Dg, active, counter);
+                blk_apply_cols_kernel<<<dim3(N / SB, npair), 256, kApplySmem, st>>>(N, nb, r, Gp, Jb, active);
+                blk_apply_rows_kernel<<<dim3(N / SB, npair, 2), 256, kApplySmem, st>>>(N, nb, r, Gp, Vu, Jb, Dg, active);
+                count_launch(3);
+            }
+            int rot = 0;
+            if (!check(cudaMemcpyAsync(&rot, counter, sizeof(int), cudaMemcpyDeviceToHost, st), err, "eigh readback")) return TATRG_ECUDA;
+            if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;
+            if (rot == 0) break;
+        }
+        if (sweep == kMaxSweeps) { if (err) *err = "eigh: block Jacobi did not converge"; return TATRG_ENUMERIC; }
+        extract_diag_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, Gp, lam_u); count_launch();
+    }
+    std::vector<double> lh(n);
+    if (!check(cudaMemcpyAsync(lh.data(), lam_u, sizeof(double) * n, cudaMemcpyDeviceToHost, st), err, "eigh readback")) return TATRG_ECUDA;
+    if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;
+    std::vector<int> order(n);
+    std::iota(order.begin(), order.end(), 0);
+    for (int i = 0; i < n; ++i) if (!std::isfinite(lh[i])) { if (err) *err = "eigh: non-finite eigenvalue"; return TATRG_ENUMERIC; }
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return lh[a] > lh[b]; });
+    if (!check(cudaMemcpyAsync(idx, order.data(), sizeof(int) * n, cudaMemcpyHostToDevice, st), err, "eigh upload")) return TATRG_ECUDA;
+    if (!check(gather_rows_scaled(st, Vt, Vu, idx, nullptr, n, n, N), err, "eigh gather")) return TATRG_ECUDA;
+    if (!check(gather_vec(st, lam, lam_u, idx, n, 1, 1.0), err, "eigh gather")) return TATRG_ECUDA;
+    if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;   // `order` leaves scope
+    if (lam_host) { lam_host->resize(n); for (int i = 0; i < n; ++i) (*lam_host)[i] = lh[order[i]]; }
+    return TATRG_OK;
+}
+
+size_t svd_rows_work_bytes(int nv, int len) { return 8 * ((size_t)nv * (len + nv + 2)) + 4096; }
+
+int svd_rows(cudaStream_t st, int nv, int len, const double* X, double* s, double* Ut, double* Vacc, void* work,
+             std::vector<double>* s_host, std::string* err) {
+    if (nv <= 0 || len <= 0) return TATRG_OK;
+    size_t smem = 8 * ((size_t)nv * (len + 1) + (size_t)nv * (nv + 1));
+    if (smem > 200 * 1024) { if (err) *err = "svd_rows: matrix too large for shared memory"; return TATRG_EINVAL; }
+    static size_t cfg = 0;
+    if (smem > cfg) {
+        if (!check(cudaFuncSetAttribute(svd_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err, "svd attr")) return TATRG_ECUDA;
+        cfg = smem;
+    }
+    double* w = (double*)work;
+    double* su = w; w += nv;
+    int* idx = (int*)w; w += nv;
+    double* Uu = w; w += (size_t)nv * len;
+    double* Vu = w;
+    svd_rows_kernel<<<1, 1024, smem, st>>>(nv, len, X, su, Uu, Vu); count_launch();
+    std::vector<double> sh(nv);
+    if (!check(cudaMemcpyAsync(sh.data(), su, sizeof(double) * nv, cudaMemcpyDeviceToHost, st), err, "svd readback")) return TATRG_ECUDA;
+    if (!check(cudaStreamSynchronize(st), err, "svd sync")) return TATRG_ECUDA;
+    for (int i = 0; i < nv; ++i) if (!std::isfinite(sh[i])) { if (err) *err = "svd_rows: non-finite singular value"; return TATRG_ENUMERIC; }
+    std::vector<int> order(nv);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return sh[a] > sh[b]; });
+    if (!check(cudaMemcpyAsync(idx, order.data(), sizeof(int) * nv, cudaMemcpyHostToDevice, st), err, "svd upload")) return TATRG_ECUDA;
+    if (!check(gather_rows_scaled(st, Ut, Uu, idx, nullptr, nv, len, len), err, "svd gather")) return TATRG_ECUDA;
+    if (!check(gather_rows_scaled(st, Vacc, Vu, idx, nullptr, nv, nv, nv), err, "svd gather")) return TATRG_ECUDA;
+    if (!check(gather_vec(st, s, su, idx, nv, 1, 1.0), err, "svd gather")) return TATRG_ECUDA;
+    if (!check(cudaStreamSynchronize(st), err, "svd sync")) return TATRG_ECUDA;
+    if (s_host) { s_host->resize(nv); for (int i = 0; i < nv; ++i) (*s_host)[i] = sh[order[i]]; }
+    return TATRG_OK;
+}
+
+}  // namespace tatrg

@@ -54,7 +54,17 @@ __global__ void permute_tiled_kernel(PermArgs a, int64_t extA, int64_t extB, int
 }
 }  // namespace
 
+static cudaError_t permute_raw(cudaStream_t st, int nd, const int64_t* dims, const int* perm, const double* in, double* out);
 cudaError_t permute(cudaStream_t st, int nd, const int64_t* dims, const int* perm, const double* in, double* out) {
+    Counters* c = g_counter;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (c) { int64_t t = 1; for (int i = 0; i < nd; ++i) t *= dims[i]; c->permuted_bytes += 16 * t; c->permute_calls += 1; }
+    if (c && c->time_kernels) { e0 = c->next_event(); e1 = c->next_event(); cudaEventRecord(e0, st); }
+    cudaError_t e = permute_raw(st, nd, dims, perm, in, out);
+    if (e0) { cudaEventRecord(e1, st); c->perm_ev.push_back({e0, e1}); }
+    return e;
+}
+static cudaError_t permute_raw(cudaStream_t st, int nd, const int64_t* dims, const int* perm, const double* in, double* out) {
     if (nd < 1 || nd > 8) return cudaErrorInvalidValue;
     // drop unit legs, then merge input legs that remain adjacent and in order in the output
     int64_t d[8]; int p[8]; int n = 0;

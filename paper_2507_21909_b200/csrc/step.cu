@@ -1,0 +1,587 @@
+// step.cu -- one Triad-ATRG coarse-graining step, Fig. 5 (a)-(f) of PAPER.md (:193), enqueued on one CUDA stream.
+//
+//   (a) decomposition of T = Phi Psi^T            Eq. 2.4 :76            decompose()
+//   (b) bond swap by RSVD                         Eq. 2.5 :90, App. A    bond_swap()
+//   (c) triad isometries / triad tensors          Eq. 2.9-2.17 :135-167  triad()
+//   (d) squeezers                                 :113, :171             half_grams(), squeezer()
+//   (e) coarse-graining contraction               Eq. 2.18-2.19 :175     contract_upper/lower()
+//   (f) axis rotation, trace                      Fig. 5(f)              run()
+//
+// All arithmetic is in the kernels of dgemm.cu / permute.cu / elementwise.cu / philox.cu / jacobi.cu; the host code
+// here only takes the rank decisions (from read-back spectra) and sizes / sequences the launches.
+// Readings R1..R14 are those of DESIGN.md section 3.
+#include "step.h"
+#include <algorithm>
+#include <cstdarg>
+
+namespace tatrg {
+namespace {
+
+[[noreturn]] void fail(int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
+    throw Fail{code, buf};
+}
+void ck(cudaError_t e, const char* what) { if (e != cudaSuccess) fail(TATRG_ECUDA, "%s: %s", what, cudaGetErrorString(e)); }
+
+// R7: number of leading values to keep: at most kmax, only values > eps*v[0], never cutting through a multiplet
+int select_rank(const std::vector<double>& v, int kmax, double eps, double tau) {
+    if (v.empty() || !(v[0] > 0)) return 0;
+    int npos = 0;
+    for (double x : v) if (x > eps * v[0]) ++npos;
+    if (npos <= kmax) return npos;
+    int k = kmax;
+    while (k > 0 && (v[k - 1] - v[k]) <= tau * v[k - 1]) --k;
+    return k > 0 ? k : kmax;
+}
+// runs of consecutive values with relative gap <= tau among the first k
+std::vector<int> multiplets(const std::vector<double>& v, int k, double tau) {
+    std::vector<int> g; int start = 0;
+    for (int i = 1; i <= k; ++i)
+        if (i == k || (v[i - 1] - v[i]) > tau * v[i - 1]) { g.push_back(start); g.push_back(i); start = i; }
+    return g;
+}
+
+struct Stepper {
+    tatrg_ctx& c;
+    cudaStream_t st;
+    std::vector<std::vector<double*>> scopes;
+    int call;
+
+    Stepper(tatrg_ctx& ctx, cudaStream_t s) : c(ctx), st(s), call(ctx.m + 1) { scopes.emplace_back(); }
+    ~Stepper() { while (!scopes.empty()) pop(); }
+
+    // ---- memory ----------------------------------------------------------------------------------------------
+    void push() { scopes.emplace_back(); }
+    void pop() { for (double* p : scopes.back()) c.pool.free(p); scopes.pop_back(); }
+    struct Scope { Stepper& s; Scope(Stepper& s_) : s(s_) { s.push(); } ~Scope() { s.pop(); } };
+    double* raw(int64_t n) {
+        double* p = c.pool.alloc(n);
+        if (!p) fail(TATRG_ENOMEM, "workspace exhausted: need %lld more doubles (in use %zu of %zu bytes)", (long long)n, c.pool.in_use(), c.pool.capacity());
+        scopes.back().push_back(p);
+        return p;
+    }
+    Tens make(std::initializer_list<int64_t> dims) {
+        Tens t; t.nd = 0; for (int64_t d : dims) t.d[t.nd++] = d;
+        t.p = raw(t.size());
+        return t;
+    }
+    static Tens view(const Tens& t, std::initializer_list<int64_t> dims) {
+        Tens v; v.p = t.p; v.nd = 0; for (int64_t d : dims) v.d[v.nd++] = d;
+        if (v.size() != t.size()) fail(TATRG_EINVAL, "internal: bad view");
+        return v;
+    }
+    // move ownership of t one scope up (so that it survives the current scope)
+    void keep(const Tens& t) {
+        auto& cur = scopes.back();
+        auto it = std::find(cur.begin(), cur.end(), t.p);
+        if (it == cur.end()) return;
+        cur.erase(it);
+        scopes[scopes.size() - 2].push_back(t.p);
+    }
+    void drop(Tens& t) {
+        for (auto sc = scopes.rbegin(); sc != scopes.rend(); ++sc) {
+            auto it = std::find(sc->begin(), sc->end(), t.p);
+            if (it != sc->end()) { sc->erase(it); c.pool.free(t.p); t.p = nullptr; return; }
+        }
+    }
+    // hand a tensor over to the context (state, or kept for inspection): leaves every scope
+    void detach(const Tens& t) {
+        for (auto& sc : scopes) { auto it = std::find(sc.begin(), sc.end(), t.p); if (it != sc.end()) { sc.erase(it); return; } }
+    }
+    void save(const char* name, const Tens& t) {   // copy for tatrg_get_tensor (tests); only with keep_tensors
+        if (!c.keep_tensors) return;
+        Tens k = t; k.p = c.pool.alloc(t.size());
+        if (!k.p) fail(TATRG_ENOMEM, "workspace exhausted keeping tensor %s", name);
+        ck(cudaMemcpyAsync(k.p, t.p, 8 * t.size(), cudaMemcpyDeviceToDevice, st), "save"); count_launch();
+        auto it = c.kept.find(name);
+        if (it != c.kept.end()) c.pool.free(it->second.p);
+        c.kept[name] = k;
+    }
+
+    // ---- thin wrappers ---------------------------------------------------------------------------------------
+    Tens ein(const char* spec, const Tens& A, const Tens& B) {
+        Tens C; std::string e;
+        int rc = contract_shape(spec, A, B, C, &e);
+        if (rc != TATRG_OK) fail(rc, "%s", e.c_str());
+        C.p = raw(C.size());
+        rc = contract(st, spec, A, B, C, c.pool, &e);
+        if (rc != TATRG_OK) fail(rc, "%s [%s]", e.c_str(), spec);
+        return C;
+    }
+    Tens perm(const Tens& t, std::initializer_list<int> p) {
+        Tens o; o.nd = t.nd; int pr[8]; int i = 0;
+        for (int x : p) { pr[i] = x; o.d[i] = t.d[x]; ++i; }
+        o.p = raw(o.size());
+        ck(permute(st, t.nd, t.d, pr, t.p, o.p), "permute");
+        return o;
+    }
+    // C[M,N] = op(A) op(B), plain 2-D, with split-K when the output is small
+    Tens mm(bool ta, bool tb, int64_t M, int64_t N, int64_t K, const double* A, int64_t lda, const double* B, int64_t ldb) {
+        Tens C = make({M, N});
+        int64_t need = dgemm_splitk_doubles(M, N, K);
+        double* part = need ? c.pool.alloc(need) : nullptr;
+        ck(dgemm_splitk(st, ta, tb, M, N, K, 1.0, A, lda, B, ldb, C.p, N, part), "dgemm");
+        if (part) c.pool.free(part);
+        return C;
+    }
+    std::vector<double> to_host(const double* d, int64_t n) {
+        std::vector<double> h(n);
+        ck(cudaMemcpyAsync(h.data(), d, 8 * n, cudaMemcpyDeviceToHost, st), "readback");
+        ck(cudaStreamSynchronize(st), "sync");
+        return h;
+    }
+    double* to_dev(const std::vector<double>& h) {
+        double* d = raw((int64_t)h.size());
+        ck(cudaMemcpyAsync(d, h.data(), 8 * h.size(), cudaMemcpyHostToDevice, st), "upload");
+        return d;
+    }
+    int* to_dev_int(const std::vector<int>& h) {
+        int* d = (int*)raw((int64_t)(h.size() + 1) / 2 + 1);
+        ck(cudaMemcpyAsync(d, h.data(), 4 * h.size(), cudaMemcpyHostToDevice, st), "upload");
+        return d;
+    }
+
+    // ---- decompositions --------------------------------------------------------------------------------------
+    // eigen-decomposition of the symmetric n x n matrix G (destroyed): lam [dev], Vt rows [dev], lam on the host
+    void eig(Tens& G, int n, double*& lam, Tens& Vt, std::vector<double>& lam_h) {
+        lam = raw(n);
+        Vt = make({n, n});
+        size_t wb = eigh_work_bytes(n);
+        double* work = c.pool.alloc((int64_t)(wb / 8 + 1));
+        if (!work) fail(TATRG_ENOMEM, "workspace exhausted (eigh work, n=%d)", n);
+        std::string e;
+        int rc = eigh(st, n, G.p, lam, Vt.p, work, &lam_h, &e);
+        c.pool.free(work);
+        if (rc != TATRG_OK) fail(rc, "%s", e.c_str());
+    }
+
+    // Orthonormal basis of the numerical column space of mat [m x n]:  mat = Q R, Q [m x r], R [r x n]   (R14).
+    // Gram matrix -> eigen-decomposition -> Q = mat V lam^-1/2 (directions with lam <= 1e-12 lam_max dropped), and a
+    // second identical pass on Q for narrow matrices (n <= 128), where it is cheap, to restore orthogonality to eps.
+    void orth(const Tens& mat, Tens& Q, Tens& R) {
+        Scope sc(*this);
+        const int64_t m = mat.d[0], n = mat.d[1];
+        Tens G = mm(true, false, n, n, m, mat.p, n, mat.p, n);
+        double* lam; Tens Vt; std::vector<double> lh;
+        eig(G, (int)n, lam, Vt, lh);
+        if (!(lh[0] > 0)) fail(TATRG_ENUMERIC, "orth: zero matrix");
+        int r = 0;
+        for (double x : lh) if (x > kEpsOrthLambda * lh[0]) ++r;
+        Tens Q1 = mm(false, true, m, r, n, mat.p, n, Vt.p, n);
+        ck(scale_last(st, Q1.p, Q1.p, lam, m, r, 2), "scale");
+        Tens R1 = make({r, n});
+        ck(scale_rows(st, R1.p, Vt.p, lam, r, n, 3), "scale");
+        if (n > 128) { Q = Q1; R = R1; keep(Q); keep(R); return; }
+        Tens G2 = mm(true, false, r, r, m, Q1.p, r, Q1.p, r);
+        double* lam2; Tens V2; std::vector<double> l2;
+        eig(G2, r, lam2, V2, l2);
+        if (!(l2[r - 1] > 0)) fail(TATRG_ENUMERIC, "orth: second pass lost rank");
+        Q = mm(false, true, m, r, r, Q1.p, r, V2.p, r);
+        ck(scale_last(st, Q.p, Q.p, lam2, m, r, 2), "scale");
+        Tens SV = make({r, r});
+        ck(scale_rows(st, SV.p, V2.p, lam2, r, r, 3), "scale");
+        R = mm(false, false, r, n, r, SV.p, r, R1.p, n);
+        keep(Q); keep(R);
+    }
+
+    // R10: block-diagonal gauge rotation Gm (k x k) from wt [k x n] (rows = the vectors to fix) and the multiplet
+    // groups of the spectrum v: Cfull = wt rho, per group Q of its MGS-QR.
+    Tens gauge(const Tens& wt, bool as_cols, const std::vector<double>& v, int k, uint32_t stream_id) {
+        const int64_t n = as_cols ? wt.d[0] : wt.d[1];
+        std::vector<int> grp = multiplets(v, k, c.tau);
+        int gmax = 1;
+        for (size_t i = 0; i < grp.size(); i += 2) gmax = std::max(gmax, grp[i + 1] - grp[i]);
+        if (gmax > 32 || gmax > kRhoCols) fail(TATRG_ENUMERIC, "multiplet of %d values: unsupported", gmax);
+        Tens rho = make({n, gmax});
+        ck(philox_rho(st, c.seed, (uint32_t)call, stream_id, n, gmax, rho.p), "rho");
+        Tens cf = as_cols ? mm(true, false, k, gmax, n, wt.p, wt.d[1], rho.p, gmax) : mm(false, false, k, gmax, n, wt.p, n, rho.p, gmax);
+        int* gd = to_dev_int(grp);
+        Tens Gm = make({k, k});
+        ck(gauge_blocks(st, cf.p, gmax, gd, (int)grp.size() / 2, k, Gm.p), "gauge");
+        return Gm;
+    }
+
+    void decompose(Tens& a, Tens& dt, Tens& core);
+    void bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x, Tens& y, double*& sig, int& gr);
+    void triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y, const double* sig, Tens U[4], Tens& e, Tens& f, Tens& g, Tens& h);
+    void half_grams(const Tens& P, const Tens& Q, const Tens& Iu, const Tens& Jl, Tens th[3]);
+    void squeezer(Tens& thf, Tens& thb, int du, int dl, int dir, Tens& Mt, Tens& Nt);
+    void run();
+};
+
+// (a) Eq. 2.4 :76 -- T = Phi Psi^T = A core Dt^T, A and Dt isometric (:137), core = G^T diag(s/s1) G in the canonical
+// gauge (R10); c_m = s1 is the normalisation of this step (R8).
+void Stepper::decompose(Tens& a, Tens& dt, Tens& core) {
+    Scope sc(*this);
+    const int64_t F = c.phi.size() / c.phi.d[4], gph = c.phi.d[4];
+    Tens qf, rf, qb, rb;
+    orth(view(c.phi, {F, gph}), qf, rf);
+    orth(view(c.psi, {F, gph}), qb, rb);
+    const int r1 = (int)rf.d[0], r2 = (int)rb.d[0];
+    // SVD of the small core rf rb^T (r1 x r2), orthogonalising the rows of the orientation with fewer rows
+    const bool flip = r1 > r2;
+    const int nv = flip ? r2 : r1, len = flip ? r1 : r2;
+    Tens X = flip ? mm(false, true, r2, r1, gph, rb.p, gph, rf.p, gph) : mm(false, true, r1, r2, gph, rf.p, gph, rb.p, gph);
+    double* s = raw(nv); Tens Ut = make({nv, len}), Va = make({nv, nv});
+    std::vector<double> sh;
+    {
+        double* work = raw((int64_t)(svd_rows_work_bytes(nv, len) / 8 + 1));
+        std::string e;
+        int rc = svd_rows(st, nv, len, X.p, s, Ut.p, Va.p, work, &sh, &e);
+        if (rc != TATRG_OK) fail(rc, "%s", e.c_str());
+    }
+    const double cm = sh[0];
+    if (!(cm > 0) || !std::isfinite(cm)) fail(TATRG_ENUMERIC, "decompose: non-positive normalisation c_m = %g", cm);
+    c.lnc.push_back(std::log(cm));
+    for (double& v : sh) v /= cm;
+    c.sv_s = sh;
+    const int chi = select_rank(sh, c.D, kEpsSV, c.tau);
+    // rows of Va are the singular vectors on the side of X's rows, rows of Ut those on the side of its columns
+    const Tens& urows = flip ? Ut : Va;    // [nv x r1]
+    const Tens& vrows = flip ? Va : Ut;    // [nv x r2]
+    Tens a0 = mm(false, true, F, chi, r1, qf.p, r1, urows.p, r1);
+    Tens d0 = mm(false, true, F, chi, r2, qb.p, r2, vrows.p, r2);
+    Tens Gm = gauge(a0, true, sh, chi, 1);
+    a = mm(false, false, F, chi, chi, a0.p, chi, Gm.p, chi);
+    dt = mm(false, false, F, chi, chi, d0.p, chi, Gm.p, chi);
+    std::vector<double> sk(sh.begin(), sh.begin() + chi);
+    double* sd = to_dev(sk);
+    Tens SG = make({chi, chi});
+    ck(scale_rows(st, SG.p, Gm.p, sd, chi, chi, 0), "scale");
+    core = mm(true, false, chi, chi, chi, Gm.p, chi, SG.p, chi);
+    a = view(a, {c.phi.d[0], c.phi.d[1], c.phi.d[2], c.phi.d[3], chi});
+    dt = view(dt, {c.psi.d[0], c.psi.d[1], c.psi.d[2], c.psi.d[3], chi});
+    keep(a); keep(dt); keep(core);
+}
+
+// (b) Eq. 2.5 :90, App. A :329-394 -- sum_i1 B C ~ X sigma Y by randomized SVD of the never-formed core S.
+void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x, Tens& y, double*& sig, int& gr) {
+    Scope sc(*this);
+    const int64_t d1 = a.d[0], d2 = a.d[1], d3 = a.d[2], d4 = a.d[3], chi = a.d[4];
+    const int64_t F = d1 * d2 * d3 * d4, J = d2 * d3 * d4;
+    Tens QB, RB, QC, RC;
+    {
+        Scope s2(*this);
+        // B[i1,j',al] = sum_a' Dt[i1,j',a'] core[al,a'],  C[i1,i',be] = sum_a' A[i1,i',a'] core[a',be]   (core symmetric)
+        Tens b = mm(false, true, F, chi, chi, dt.p, chi, core.p, chi);
+        Tens bm = perm(view(b, {d1, J, chi}), {1, 0, 2});              // Eq. A.2 :345  B[(j'),(i1 al)]
+        drop(b);
+        orth(view(bm, {J, d1 * chi}), QB, RB);
+        drop(bm);
+        Tens cc = mm(false, false, F, chi, chi, a.p, chi, core.p, chi);
+        Tens cm = perm(view(cc, {d1, J, chi}), {1, 0, 2});             // Eq. A.3 :348  C[(i'),(i1 be)]
+        drop(cc);
+        orth(view(cm, {J, d1 * chi}), QC, RC);
+        keep(QB); keep(RB); keep(QC); keep(RC);
+    }
+    const int64_t npb = QB.d[1], npc = QC.d[1];
+    Tens RB3 = view(RB, {npb, d1, chi}), RC3 = view(RC, {npc, d1, chi});
+    const int64_t l = std::min<int64_t>(c.D + c.p, std::min(chi * npc, chi * npb));     // R3: sketch width
+    // Omega drawn in the physical basis (be, j', m) and projected on Q^B  (R11, R12)
+    Tens omega;
+    {
+        Scope s2(*this);
+        Tens om = make({chi, J, l});
+        ck(philox_gauss(st, c.seed, (uint32_t)call, 0, 0, chi * J * l, om.p), "philox");
+        omega = ein("jp,Bjm->Bpm", QB, om);
+        keep(omega);
+    }
+    Tens qk, yt;
+    for (int k = 0; k <= c.n_pow; ++k) {                                 // R4: n_pow + 1 passes of Eq. A.4-A.6
+        Scope s2(*this);
+        Tens t = ein("pia,bpm->iabm", RB3, omega);
+        Tens yk = ein("qib,iabm->aqm", RC3, t);                          // Eq. A.4 :356
+        drop(t);
+        Tens q2, r2;
+        orth(view(yk, {chi * npc, yk.d[2]}), q2, r2);
+        drop(yk); drop(r2);
+        if (qk.p) drop(qk);
+        qk = view(q2, {chi, npc, q2.d[1]});
+        Tens t2 = ein("qib,aqm->ibam", RC3, qk);
+        if (yt.p) drop(yt);
+        yt = ein("pia,ibam->bpm", RB3, t2);                              // Eq. A.5 :361  = (Q^T S)^T
+        drop(t2);
+        keep(qk); keep(yt);
+        if (k < c.n_pow) {
+            Tens q3, r3;
+            orth(view(yt, {chi * npb, yt.d[2]}), q3, r3);                // Eq. A.6 :365
+            drop(r3); drop(omega);
+            omega = view(q3, {chi, npb, q3.d[1]});
+            keep(omega);
+        }
+    }
+    // Eq. A.7-A.8 :373-376: SVD of the projected tensor, via an orthonormal basis of its columns and a small Jacobi SVD
+    const int64_t rk = yt.d[2];
+    Tens Qy, Ry;
+    orth(view(yt, {chi * npb, rk}), Qy, Ry);
+    const int ry = (int)Ry.d[0];
+    double* s = raw(ry); Tens Ut = make({ry, rk}), Va = make({ry, ry});
+    std::vector<double> sh;
+    {
+        double* work = raw((int64_t)(svd_rows_work_bytes(ry, (int)rk) / 8 + 1));
+        std::string e;
+        int rc = svd_rows(st, ry, (int)rk, Ry.p, s, Ut.p, Va.p, work, &sh, &e);
+        if (rc != TATRG_OK) fail(rc, "%s", e.c_str());
+    }
+    if (!(sh[0] > 0)) fail(TATRG_ENUMERIC, "bond swap: zero spectrum");
+    gr = select_rank(sh, c.D, kEpsSV, c.tau);
+    c.sv_sigma.assign((size_t)rk, 0.0);
+    for (int i = 0; i < ry; ++i) c.sv_sigma[i] = sh[i] / sh[0];
+    // Eq. A.9 :379 and A.10-A.11 :389-392
+    Tens ub = mm(false, true, chi * npc, gr, rk, qk.p, rk, Ut.p, rk);         // U^bond[(al q), g]
+    Tens vb = mm(false, true, chi * npb, gr, ry, Qy.p, ry, Va.p, ry);         // V^bond[(be p), g]
+    x = ein("jq,Aqg->Ajg", QC, view(ub, {chi, npc, gr}));
+    y = ein("jp,Bpg->Bjg", QB, view(vb, {chi, npb, gr}));
+    x = view(x, {chi, d2, d3, d4, gr});
+    y = view(y, {chi, d2, d3, d4, gr});
+    sig = raw(gr);
+    ck(cudaMemcpyAsync(sig, s, 8 * gr, cudaMemcpyDeviceToDevice, st), "copy"); count_launch();
+    keep(x); keep(y);
+    { Tens t; t.p = sig; keep(t); }
+}
+
+// (c) Eq. 2.9 :135 (canonical form :137) and Eq. 2.10-2.17 :147-167.
+// U[0..3] = U^A, U^X, U^Y, U^D stored [k, leg2, leg3]; E[i1,kA,i4,al], F[al,kX,i4,g] (carries sigma), G[be,kY,j4,g], H[j1,kD,j4,be].
+void Stepper::triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y, const double* sig, Tens U[4], Tens& e, Tens& f,
+                    Tens& g, Tens& h) {
+    Scope sc(*this);
+    const int64_t d1 = a.d[0], d2 = a.d[1], d3 = a.d[2], d4 = a.d[3], chi = a.d[4], gr = x.d[4];
+    const int64_t n = d2 * d3, J = d2 * d3 * d4;
+    Tens gram[4];
+    for (int side = 0; side < 2; ++side) {      // side 0: X and A,  side 1: Y and Dt
+        Scope s2(*this);
+        const Tens& xx = side == 0 ? x : y;
+        const Tens& aa = side == 0 ? a : dt;
+        Tens xs = make({chi, d2, d3, d4, gr});
+        ck(scale_last(st, xs.p, xx.p, sig, chi * J, gr, 0), "scale");
+        // G^X[(i2 i3),(i2' i3')] = sum_{al,i4,g} Xs Xs
+        Tens xp = perm(xs, {0, 3, 4, 1, 2});
+        Tens gx = mm(true, false, n, n, chi * d4 * gr, xp.p, n, xp.p, n);
+        drop(xp);
+        // kappa[al,al'] = sum_{i',g} Xs Xs ;  G^A = sum_{i1,i4,al,al'} A kappa A
+        Tens ka = mm(false, true, chi, chi, J * gr, xs.p, J * gr, xs.p, J * gr);
+        drop(xs);
+        Tens ta = mm(false, false, d1 * J, chi, chi, aa.p, chi, ka.p, chi);
+        Tens ap = perm(aa, {0, 3, 4, 1, 2});
+        Tens tp = perm(view(ta, {d1, d2, d3, d4, chi}), {0, 3, 4, 1, 2});
+        drop(ta);
+        Tens ga = mm(true, false, n, n, d1 * d4 * chi, ap.p, n, tp.p, n);
+        gram[side == 0 ? 0 : 3] = ga; gram[side == 0 ? 1 : 2] = gx;
+        keep(ga); keep(gx);
+    }
+    for (int i = 0; i < 4; ++i) {
+        Scope s2(*this);
+        double* lam; Tens Vt; std::vector<double> lh;
+        eig(gram[i], (int)n, lam, Vt, lh);
+        drop(gram[i]);
+        std::vector<double> sv(lh.size());
+        for (size_t j = 0; j < lh.size(); ++j) sv[j] = std::sqrt(std::max(lh[j], 0.0));    // multiplet rule on the singular-value scale
+        const int k = select_rank(sv, std::min<int64_t>(c.Ktri, n), std::sqrt(kEpsLambda), c.tau);
+        if (k <= 0) fail(TATRG_ENUMERIC, "triad: empty isometry");
+        U[i] = make({k, d2, d3});
+        ck(cudaMemcpyAsync(U[i].p, Vt.p, 8 * (int64_t)k * n, cudaMemcpyDeviceToDevice, st), "copy"); count_launch();
+        keep(U[i]);
+    }
+    e = ein("mjk,Ijkla->Imla", U[0], a);                                   // Eq. 2.10
+    Tens f0 = ein("xjk,Ajklg->Axlg", U[1], x);                             // Eq. 2.11 (sigma goes into F only)
+    ck(scale_last(st, f0.p, f0.p, sig, f0.size() / gr, gr, 0), "scale");
+    f = f0;
+    g = ein("yjk,Bjklg->Bylg", U[2], y);                                   // Eq. 2.12
+    h = ein("djk,Jjklb->Jdlb", U[3], dt);                                  // Eq. 2.13
+    for (int i = 0; i < 4; ++i) keep(U[i]);
+    keep(e); keep(f); keep(g); keep(h);
+}
+
+// (d) Gram matrices of one half of the unit cell on the doubled bonds 2, 3, 4  (R6; PAPER.md :171, Table 1 :229-230).
+// P[o1,kU,u4,bond] sits on the upper site, Q[bond,kL,l4,o2] on the lower site; Iu[kU,u2,u3], Jl[kL,l2,l3].
+// th[d-2][(u l),(u' l')] for d = 2,3,4, staged so that nothing larger than K^4 appears.
+void Stepper::half_grams(const Tens& P, const Tens& Q, const Tens& Iu, const Tens& Jl, Tens th[3]) {
+    Scope sc(*this);
+    {   // direction 4: Iu and Jl are isometries and drop out
+        Scope s2(*this);
+        Tens ee = ein("ikua,ikvb->uavb", P, P);
+        Tens ff = ein("akld,bkwd->albw", Q, Q);
+        th[2] = ein("uavb,albw->ulvw", ee, ff);
+        keep(th[2]);
+    }
+    Tens ef;
+    {
+        Scope s2(*this);
+        Tens ee = ein("ikua,imub->kmab", P, P);
+        Tens ff = ein("axld,byld->abxy", Q, Q);
+        ef = ein("kmab,abxy->kmxy", ee, ff);
+        keep(ef);
+    }
+    for (int d = 2; d <= 3; ++d) {
+        Scope s2(*this);
+        Tens ii = d == 2 ? ein("kuc,mvc->uvkm", Iu, Iu) : ein("kcu,mcv->uvkm", Iu, Iu);
+        Tens jj = d == 2 ? ein("xlc,ywc->lwxy", Jl, Jl) : ein("xcl,ycw->lwxy", Jl, Jl);
+        Tens tmp = ein("uvkm,kmxy->uvxy", ii, ef);
+        th[d - 2] = ein("uvxy,lwxy->ulvw", tmp, jj);
+        keep(th[d - 2]);
+    }
+    for (int i = 0; i < 3; ++i) keep(th[i]);
+}
+
+// (d) squeezer pair of one direction (R6): thf = R1^T R1, thb = R2 R2^T, SVD R1 R2 = U s V^T,
+// M = R2 V s^-1/2, N = R1^T U s^-1/2, gauge-fixed (R10).  Returned as rows: Mt[k,u,l], Nt[k,u,l].
+void Stepper::squeezer(Tens& thf, Tens& thb, int du, int dl, int dir, Tens& Mt, Tens& Nt) {
+    Scope sc(*this);
+    const int n = du * dl;
+    double *lam1, *lam2; Tens W1, W2; std::vector<double> l1, l2;
+    eig(thf, n, lam1, W1, l1);
+    eig(thb, n, lam2, W2, l2);
+    if (!(l1[0] > 0) || !(l2[0] > 0)) fail(TATRG_ENUMERIC, "squeezer %d: zero Gram matrix", dir);
+    int k1 = 0, k2 = 0;
+    for (double v : l1) if (v > kEpsLambda * l1[0]) ++k1;
+    for (double v : l2) if (v > kEpsLambda * l2[0]) ++k2;
+    Tens r1 = make({k1, n}), r2t = make({k2, n});
+    ck(scale_rows(st, r1.p, W1.p, lam1, k1, n, 3), "scale");       // R1 = Lambda1^1/2 W1^T
+    ck(scale_rows(st, r2t.p, W2.p, lam2, k2, n, 3), "scale");      // R2^T
+    drop(W1); drop(W2);
+    Tens cm = mm(false, true, k1, k2, n, r1.p, n, r2t.p, n);       // R1 R2
+    Tens gc = mm(true, false, k2, k2, k1, cm.p, k2, cm.p, k2);     // (R1 R2)^T (R1 R2): right singular vectors, s^2
+    double* lamc; Tens Vc; std::vector<double> lc;
+    eig(gc, k2, lamc, Vc, lc);
+    std::vector<double> s(lc.size());
+    for (size_t i = 0; i < lc.size(); ++i) s[i] = std::sqrt(std::max(lc[i], 0.0));
+    const int k = select_rank(s, c.D, kEpsSqueezer, c.tau);
+    if (k <= 0) fail(TATRG_ENUMERIC, "squeezer %d: empty", dir);
+    std::vector<double> sk(s.begin(), s.begin() + k);
+    double* sd = to_dev(sk);
+    Tens wt = mm(false, false, k, n, k2, Vc.p, k2, r2t.p, n);      // (R2 V)^T
+    Tens cv = mm(false, true, k, k1, k2, Vc.p, k2, cm.p, k2);      // (R1 R2 V)^T = (U s)^T
+    Tens nt = mm(false, false, k, n, k1, cv.p, k1, r1.p, n);       // (R1^T U s)^T
+    Tens Gm = gauge(wt, false, s, k, (uint32_t)dir);
+    ck(scale_rows(st, wt.p, wt.p, sd, k, n, 2), "scale");          // s^-1/2
+    ck(scale_rows(st, nt.p, nt.p, sd, k, n, 4), "scale");          // s^-3/2
+    Mt = mm(true, false, k, n, k, Gm.p, k, wt.p, n);
+    Nt = mm(true, false, k, n, k, Gm.p, k, nt.p, n);
+    Mt = view(Mt, {k, du, dl}); Nt = view(Nt, {k, du, dl});
+    keep(Mt); keep(Nt);
+}
+
+void Stepper::run() {
+    Counters& cn = c.cnt;
+    const bool timed = c.timing >= 1;
+    if (timed && c.stage_ev.empty()) { c.stage_ev.resize(TATRG_NSTAGES + 1); for (auto& e : c.stage_ev) ck(cudaEventCreate(&e), "event"); }
+    double flops_mark = cn.gemm_flops;
+    int stage = 0;
+    auto mark = [&]() {   // closes stage `stage`
+        c.stage_flops[stage] = cn.gemm_flops - flops_mark; flops_mark = cn.gemm_flops;
+        ++stage;
+        if (timed) ck(cudaEventRecord(c.stage_ev[stage], st), "event");
+    };
+    if (timed) ck(cudaEventRecord(c.stage_ev[0], st), "event");
+    if (c.phi.nd != 5 || c.psi.nd != 5) fail(TATRG_ESTATE, "no state");
+    for (int i = 0; i < 5; ++i) if (c.phi.d[i] != c.psi.d[i]) fail(TATRG_ESTATE, "Phi and Psi shapes differ");
+
+    Tens a, dt, core;
+    decompose(a, dt, core);                                         // (a)
+    save("A", a); save("Dt", dt); save("core", core);
+    mark();
+    // (b) the QR / RSVD / lift stages are timed together under TATRG_ST_QR..LIFT: QR and RSVD flops are attributed by bond_swap
+    Tens x, y; double* sig; int gr;
+    bond_swap(a, dt, core, x, y, sig, gr);
+    save("X", x); save("Y", y); { Tens s; s.p = sig; s.nd = 1; s.d[0] = gr; save("sigma", s); }
+    mark(); mark(); mark();
+    Tens U[4], e, f, g, h;
+    triad(a, dt, x, y, sig, U, e, f, g, h);                         // (c)
+    save("E", e); save("F", f); save("G", g); save("H", h);
+    save("UA", U[0]); save("UX", U[1]); save("UY", U[2]); save("UD", U[3]);
+    drop(a); drop(dt); drop(core); drop(x); drop(y);
+    mark(); mark();
+    // (d) squeezer Gram matrices of the upper half (E F I J) and of the sigma-weighted lower half (G sigma, H, K, L)
+    Tens thf[3], thb[3];
+    half_grams(e, f, U[0], U[1], thf);
+    {
+        Scope s2(*this);
+        Tens gs = make({g.d[0], g.d[1], g.d[2], g.d[3]});
+        ck(scale_last(st, gs.p, g.p, sig, g.size() / gr, gr, 0), "scale");
+        Tens P = perm(gs, {3, 1, 2, 0});          // [g, kY, j4u, be]
+        Tens Q = perm(h, {3, 1, 2, 0});           // [be, kD, j4l, j1]
+        half_grams(P, Q, U[2], U[3], thb);
+        for (int i = 0; i < 3; ++i) keep(thb[i]);
+    }
+    mark();
+    Tens Mt[3], Nt[3];
+    for (int d = 2; d <= 4; ++d) {
+        const int du = (int)c.phi.d[d - 1], dl = du;
+        squeezer(thf[d - 2], thb[d - 2], du, dl, d, Mt[d - 2], Nt[d - 2]);
+        drop(thf[d - 2]); drop(thb[d - 2]);
+    }
+    save("M2", Mt[0]); save("M3", Mt[1]); save("M4", Mt[2]); save("N2", Nt[0]); save("N3", Nt[1]); save("N4", Nt[2]);
+    mark();
+    // (e) Eq. 2.18 :175  Phi'[i1,k2,k3,k4,g]
+    Tens phin, psin;
+    {
+        Scope s2(*this);
+        Tens fm = ein("zul,axld->uaxzd", Mt[2], f);
+        Tens xi = ein("ikua,uaxzd->ikxzd", e, fm);                  // Xi[i1,kA,kX,k4,g]
+        drop(fm);
+        Tens im = ein("kuc,zul->kclz", U[0], Mt[0]);
+        Tens imm = ein("kclz,ycw->klwzy", im, Mt[1]);
+        Tens lam = ein("klwzy,xlw->kxzy", imm, U[1]);               // Lambda[kA,kX,k2,k3]
+        drop(im); drop(imm);
+        Tens ph = ein("Ikxzd,kxpq->Ipqzd", xi, lam);
+        drop(xi);
+        phin = perm(ph, {1, 2, 3, 0, 4});                           // (f) rotate: axis 1 becomes axis 4  (R5)
+        keep(phin);
+    }
+    {   // Eq. 2.19 :175  Psi'[j1,k2,k3,k4,g]
+        Scope s2(*this);
+        Tens gn = ein("zul,byug->lbyzg", Nt[2], g);
+        Tens xi = ein("jdlb,lbyzg->jdyzg", h, gn);                  // Xi'[j1,kD,kY,k4,g]
+        drop(gn);
+        Tens kn = ein("yuc,zul->yclz", U[2], Nt[0]);
+        Tens knn = ein("yclz,vcw->ylwzv", kn, Nt[1]);
+        Tens lam = ein("ylwzv,dlw->dyzv", knn, U[3]);               // Lambda'[kD,kY,k2,k3]
+        drop(kn); drop(knn);
+        Tens ps = ein("Jdyzg,dypq->Jpqzg", xi, lam);
+        drop(xi);
+        psin = perm(ps, {1, 2, 3, 0, 4});
+        keep(psin);
+    }
+    mark();
+    c.pool.free(c.phi.p); c.pool.free(c.psi.p);
+    detach(phin); detach(psin);
+    c.phi = phin; c.psi = psin;
+    ck(dot(st, c.phi.size(), c.phi.p, c.psi.p, c.trace_dev), "dot");
+    mark();
+    c.m += 1;
+}
+}  // namespace
+
+int run_step(tatrg_ctx* c, cudaStream_t st) {
+    Counters& cn = c->cnt;
+    cn.launches = 0; cn.gemm_flops = 0; cn.gemm_calls = 0; cn.permuted_bytes = 0; cn.permute_calls = 0;
+    cn.time_kernels = c->timing >= 2; cn.gemm_ev.clear(); cn.perm_ev.clear(); cn.ev_used = 0;
+    g_counter = &cn;
+    int rc = TATRG_OK;
+    const size_t lnc0 = c->lnc.size();
+    try {
+        Stepper s(*c, st);
+        s.run();
+    } catch (const Fail& f) {
+        rc = f.code; c->err = f.msg;
+    } catch (const std::exception& e) {
+        rc = TATRG_ECUDA; c->err = e.what();
+    }
+    g_counter = nullptr;
+    c->last_stream = st;
+    c->last_launches = cn.launches;
+    if (rc != TATRG_OK) { c->failed = true; c->lnc.resize(lnc0); return rc; }
+    c->gemm_flops = cn.gemm_flops; c->gemm_calls = cn.gemm_calls; c->perm_calls = cn.permute_calls; c->perm_bytes = cn.permuted_bytes;
+    if (c->timing >= 1) {
+        cudaError_t e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { c->failed = true; c->err = cudaGetErrorString(e); return TATRG_ECUDA; }
+        for (int i = 0; i < TATRG_NSTAGES; ++i) { float ms = 0; cudaEventElapsedTime(&ms, c->stage_ev[i], c->stage_ev[i + 1]); c->stage_ms[i] = ms; }
+        c->gemm_ms = 0; c->perm_ms = 0;
+        for (auto& ev : cn.gemm_ev) { float ms = 0; cudaEventElapsedTime(&ms, ev.first, ev.second); c->gemm_ms += ms; }
+        for (auto& ev : cn.perm_ev) { float ms = 0; cudaEventElapsedTime(&ms, ev.first, ev.second); c->perm_ms += ms; }
+    }
+    return TATRG_OK;
+}
+
+}  // namespace tatrg
