@@ -23,6 +23,9 @@ constexpr int SP = SB + 1;      // pitch
 constexpr int BW = 32;          // block width of the block-Jacobi
 constexpr double kTolRel = 1e-15;
 constexpr int kMaxSweeps = 40;
+// off-diagonal entries below kFloorRel * max|diag| are not rotated: two orders below the rounding of the GEMM that
+// produced the matrix
+constexpr double kFloorRel = 1e-18;
 
 // round-robin tournament on np (even) players: round r in [0, np-1), table k in [0, np/2)
 __device__ __host__ __forceinline__ void rr_pair(int np, int r, int k, int& p, int& q) {
@@ -121,7 +124,7 @@ __global__ void __launch_bounds__(512, 1) eigh_small_kernel(int n, const double*
     }
     __syncthreads();
     dmax = block_max(dmax, red);
-    jacobi_smem(S, J, n, 1e-22 * dmax, cs, sn, pp, qq, cnt);
+    jacobi_smem(S, J, n, kFloorRel * dmax, cs, sn, pp, qq, cnt);
     for (int e = tid; e < n * n; e += nt) { int i = e / n, j = e - i * n; Vt[i * n + j] = J[j * SP + i]; }   // row i = eigenvector i
     for (int i = tid; i < n; i += nt) lam[i] = S[i * SP + i];
 }
@@ -135,127 +138,225 @@ __global__ void pad_sym_kernel(int n, int N, const double* __restrict__ G, doubl
         Vt[e] = (i == j) ? 1.0 : 0.0;
     }
 }
-__global__ void diag_max_kernel(int N, const double* __restrict__ Gp, double* out) {   // one block
+__global__ void diag_max_kernel(int N, const double* __restrict__ Gp, double* out, double floor_rel) {   // one block
     __shared__ double red[32];
     double m = 0;
     for (int i = threadIdx.x; i < N; i += blockDim.x) m = fmax(m, fabs(Gp[(int64_t)i * N + i]));
     m = block_max(m, red);
-    if (threadIdx.x == 0) out[0] = m;
+    if (threadIdx.x == 0) { out[0] = m; out[1] = floor_rel * m; }
 }
 
 __device__ __forceinline__ int gidx(int P, int Q, int li) { return li < BW ? P * BW + li : Q * BW + li - BW; }
 
-// one CTA per block pair: solve the 64 x 64 diagonal sub-problem, emit its rotation J, the new diagonal and a flag
-__global__ void __launch_bounds__(512, 1) blk_solve_kernel(int N, int nb, int round, const double* __restrict__ Gp, const double* __restrict__ dmax,
-                                                           double* __restrict__ Jb, double* __restrict__ Dg, int* __restrict__ active,
-                                                           int* __restrict__ counter) {
+// ---- block pair solver, v2: 1024 threads, two barriers per round --------------------------------------------------
+// Pair schedule of the 64 local indices.  mode 0 (FULL): round-robin over all 64 (63 rounds): every pair once.
+// mode 1 (CROSS): p = k, q = 32 + (k + r) mod 32 (32 rounds): only pairs across the two 32-blocks, whose diagonal
+// blocks were diagonalised earlier in the sweep.
+__device__ __forceinline__ void sched(int mode, int r, int k, int& p, int& q) {
+    if (mode == 0) rr_pair(SB, r, k, p, q);
+    else { p = k; q = BW + ((k + r) & (BW - 1)); }
+}
+struct Rot { double c, s; int p, q; };
+
+// S value after the row phase of the current round, computed from the column-updated buffer (read-only here)
+__device__ __forceinline__ double row_updated(const double* S, const Rot* cur, const int* pair_of, int a, int b) {
+    const Rot rt = cur[pair_of[a]];
+    if (rt.s == 0.0) return S[a * SP + b];
+    if ((a == rt.p && b == rt.q) || (a == rt.q && b == rt.p)) return 0.0;
+    const double x = S[rt.p * SP + b], y = S[rt.q * SP + b];
+    return a == rt.p ? rt.c * x - rt.s * y : rt.s * x + rt.c * y;
+}
+
+__global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int round, int mode, const double* __restrict__ Gp,
+                                                             const double* __restrict__ misc, double* __restrict__ Jb,
+                                                             double* __restrict__ Dg, int* __restrict__ active, int* __restrict__ counter) {
     extern __shared__ double sh[];
-    double* S = sh; double* J = S + SB * SP;
-    double* cs = J + SB * SP; double* sn = cs + 32; double* red = sn + 32;
-    int* pp = (int*)(red + 32); int* qq = pp + 32; int* cnt = qq + 32;
-    const int tid = threadIdx.x, nt = blockDim.x, k = blockIdx.x;
+    double* Sa = sh; double* Sb = Sa + SB * SP; double* J = Sb + SB * SP;
+    Rot* rots = reinterpret_cast<Rot*>(J + SB * SP);          // 2 x 32
+    double* red = reinterpret_cast<double*>(rots + 64);       // 32
+    int* pair_of = reinterpret_cast<int*>(red + 32);          // 2 x 64
+    int* cnt = pair_of + 128;
+    const int tid = threadIdx.x, k = blockIdx.x;
     int P, Q; rr_pair(nb, round, k, P, Q);
-    for (int e = tid; e < SB * SB; e += nt) {
+    for (int e = tid; e < SB * SB; e += 1024) {
         int i = e >> 6, j = e & 63;
-        S[i * SP + j] = Gp[(int64_t)gidx(P, Q, i) * N + gidx(P, Q, j)];
+        Sa[i * SP + j] = Gp[(int64_t)gidx(P, Q, i) * N + gidx(P, Q, j)];
         J[i * SP + j] = (i == j) ? 1.0 : 0.0;
     }
+    if (tid == 0) *cnt = 0;
     __syncthreads();
-    const double floor_abs = 1e-22 * dmax[0];
-    // quick test: anything to rotate at all?
+    const double floor_abs = misc[1];
+    // quick test: anything to rotate among the pairs this mode visits?
     double worst = 0;
-    for (int e = tid; e < SB * SB; e += nt) {
+    for (int e = tid; e < SB * SB; e += 1024) {
         int i = e >> 6, j = e & 63;
-        if (i < j) {
-            double a = fabs(S[i * SP + j]);
-            if (a > floor_abs && a > kTolRel * sqrt(fabs(S[i * SP + i] * S[j * SP + j]))) worst = 1.0;
+        if (i < j && (mode == 0 || (i < BW && j >= BW))) {
+            double a = fabs(Sa[i * SP + j]);
+            if (a > floor_abs && a > kTolRel * sqrt(fabs(Sa[i * SP + i] * Sa[j * SP + j]))) worst = 1.0;
         }
     }
     worst = block_max(worst, red);
-    int rot = 0;
-    if (worst > 0) rot = jacobi_smem(S, J, SB, floor_abs, cs, sn, pp, qq, cnt);
-    if (tid == 0) { active[k] = rot > 0; if (rot > 0) atomicAdd(counter, rot); }
-    if (rot > 0) {
-        for (int e = tid; e < SB * SB; e += nt) { int i = e >> 6, j = e & 63; Jb[(int64_t)k * SB * SB + e] = J[i * SP + j]; }
-        for (int i = tid; i < SB; i += nt) Dg[k * SB + i] = S[i * SP + i];
+    if (worst == 0.0) { if (tid == 0) active[k] = 0; return; }
+    const int nrounds = mode == 0 ? SB - 1 : BW;
+    const int max_sweeps = mode == 0 ? 12 : 1;
+    double* S = Sa; double* T = Sb;
+    int total = 0;
+    for (int sweep = 0; sweep < max_sweeps; ++sweep) {
+        // rotations of round 0 from the current S
+        if (tid < 32) {
+            int p, q; sched(mode, 0, tid, p, q);
+            Rot rt; rt.c = 1.0; rt.s = 0.0; rt.p = p; rt.q = q;
+            double app = S[p * SP + p], aqq = S[q * SP + q], apq = S[p * SP + q];
+            if (fabs(apq) > floor_abs && fabs(apq) > kTolRel * sqrt(fabs(app * aqq))) { sym_rot(app, aqq, apq, rt.c, rt.s); atomicAdd(cnt, 1); }
+            rots[tid] = rt; pair_of[p] = tid; pair_of[q] = tid;
+        }
+        __syncthreads();
+        for (int r = 0; r < nrounds; ++r) {
+            const Rot* cur = rots + (r & 1) * 32; Rot* nxt = rots + ((r + 1) & 1) * 32;
+            const int* pof = pair_of + (r & 1) * 64; int* pof_n = pair_of + ((r + 1) & 1) * 64;
+            // columns of S and J, in place
+#pragma unroll
+            for (int it = 0; it < 2; ++it) {
+                const int e = tid + it * 1024, kk = e >> 6, i = e & 63;
+                const Rot rt = cur[kk];
+                if (rt.s != 0.0) {
+                    double x = S[i * SP + rt.p], y = S[i * SP + rt.q];
+                    S[i * SP + rt.p] = rt.c * x - rt.s * y; S[i * SP + rt.q] = rt.s * x + rt.c * y;
+                    x = J[i * SP + rt.p]; y = J[i * SP + rt.q];
+                    J[i * SP + rt.p] = rt.c * x - rt.s * y; J[i * SP + rt.q] = rt.s * x + rt.c * y;
+                }
+            }
+            __syncthreads();
+            // rows: S -> T (every row belongs to exactly one pair, so T is written completely)
+#pragma unroll
+            for (int it = 0; it < 2; ++it) {
+                const int e = tid + it * 1024, kk = e >> 6, j = e & 63;
+                const Rot rt = cur[kk];
+                double x = S[rt.p * SP + j], y = S[rt.q * SP + j];
+                double xn = x, yn = y;
+                if (rt.s != 0.0) { xn = rt.c * x - rt.s * y; yn = rt.s * x + rt.c * y; if (j == rt.q) xn = 0.0; if (j == rt.p) yn = 0.0; }
+                T[rt.p * SP + j] = xn; T[rt.q * SP + j] = yn;
+            }
+            // meanwhile the first warp prepares the next round from the row-updated values it derives itself
+            if (tid < 32 && r + 1 < nrounds) {
+                int p, q; sched(mode, r + 1, tid, p, q);
+                Rot rt; rt.c = 1.0; rt.s = 0.0; rt.p = p; rt.q = q;
+                double app = row_updated(S, cur, pof, p, p), aqq = row_updated(S, cur, pof, q, q), apq = row_updated(S, cur, pof, p, q);
+                if (fabs(apq) > floor_abs && fabs(apq) > kTolRel * sqrt(fabs(app * aqq))) { sym_rot(app, aqq, apq, rt.c, rt.s); atomicAdd(cnt, 1); }
+                nxt[tid] = rt; pof_n[p] = tid; pof_n[q] = tid;
+            }
+            __syncthreads();
+            double* tmp = S; S = T; T = tmp;
+        }
+        // the Rot/pair_of buffers of round 0 of the next sweep are rewritten above: parity of nrounds does not matter
+        const int c = *cnt;
+        __syncthreads();
+        if (tid == 0) *cnt = 0;
+        total += c;
+        if (c == 0) break;
+        __syncthreads();
+    }
+    if (tid == 0) { active[k] = total > 0; if (total > 0) atomicAdd(counter, total); }
+    if (total > 0) {
+        for (int e = tid; e < SB * SB; e += 1024) { int i = e >> 6, j = e & 63; Jb[(int64_t)k * SB * SB + e] = J[i * SP + j]; }
+        for (int e = tid; e < SB * SB; e += 1024) { int i = e >> 6, j = e & 63; Dg[(int64_t)k * SB * SB + e] = S[i * SP + j]; }
     }
 }
 
-// X[:, PQ] <- X[:, PQ] * J_k   (grid: row tiles x pairs; 256 threads, 4x4 outputs each)
-__global__ void __launch_bounds__(256) blk_apply_cols_kernel(int N, int nb, int round, double* __restrict__ X, const double* __restrict__ Jb,
-                                                             const int* __restrict__ active) {
-    const int k = blockIdx.y;
-    if (!active[k]) return;
-    extern __shared__ double sh2[];
-    double (*Xs)[SP] = reinterpret_cast<double (*)[SP]>(sh2);
-    double (*Js)[SP] = reinterpret_cast<double (*)[SP]>(sh2 + SB * SP);
-    int P, Q; rr_pair(nb, round, k, P, Q);
-    const int tid = threadIdx.x, r0 = blockIdx.x * SB;
-    for (int e = tid; e < SB * SB; e += 256) {
-        int i = e >> 6, j = e & 63;
-        Xs[i][j] = X[(int64_t)(r0 + i) * N + gidx(P, Q, j)];
-        Js[i][j] = Jb[(int64_t)k * SB * SB + e];
-    }
-    __syncthreads();
-    const int ti = (tid >> 4) * 4, tj = (tid & 15) * 4;
-    double acc[4][4] = {};
+// 64x64x64 product helpers on shared tiles (256 threads, 4x4 outputs each):  acc = A^T B  or  acc = A B
+__device__ __forceinline__ void tile_atb(const double (*A)[SP], const double (*B)[SP], double acc[4][4], int ti, int tj) {
 #pragma unroll 8
     for (int l = 0; l < SB; ++l) {
         double a[4], b[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { a[u] = Xs[ti + u][l]; b[u] = Js[l][tj + u]; }
+        for (int u = 0; u < 4; ++u) { a[u] = A[l][ti + u]; b[u] = B[l][tj + u]; }
 #pragma unroll
         for (int u = 0; u < 4; ++u)
 #pragma unroll
             for (int v = 0; v < 4; ++v) acc[u][v] += a[u] * b[v];
     }
+}
+__device__ __forceinline__ void tile_ab(const double (*A)[SP], const double (*B)[SP], double acc[4][4], int ti, int tj) {
+#pragma unroll 8
+    for (int l = 0; l < SB; ++l) {
+        double a[4], b[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { a[u] = A[ti + u][l]; b[u] = B[l][tj + u]; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int v = 0; v < 4; ++v) acc[u][v] += a[u] * b[v];
+    }
+}
+
+// One launch applies the round's rotations to G (both sides, tile by tile, using the symmetry) and to V^T:
+//   blockIdx.y <  npair : tile (k = blockIdx.y, l = blockIdx.x), k <= l:  G[PQ_k,PQ_l] <- J_k^T G[PQ_k,PQ_l] J_l  (+ mirror)
+//   blockIdx.y >= npair : V^T[PQ_k, 64-column tile blockIdx.x] <- J_k^T V^T[...]
+__global__ void __launch_bounds__(256) blk_apply2_kernel(int N, int nb, int round, double* __restrict__ Gp, double* __restrict__ Vt,
+                                                         const double* __restrict__ Jb, const double* __restrict__ Dg,
+                                                         const int* __restrict__ active) {
+    extern __shared__ double sh2[];
+    double (*Xs)[SP] = reinterpret_cast<double (*)[SP]>(sh2);
+    double (*Ja)[SP] = reinterpret_cast<double (*)[SP]>(sh2 + SB * SP);
+    double (*Jc)[SP] = reinterpret_cast<double (*)[SP]>(sh2 + 2 * SB * SP);
+    const int npair = nb >> 1, tid = threadIdx.x;
+    const int ti = (tid >> 4) * 4, tj = (tid & 15) * 4;
+    if ((int)blockIdx.y >= npair) {
+        const int k = blockIdx.y - npair;
+        if (!active[k]) return;
+        int P, Q; rr_pair(nb, round, k, P, Q);
+        const int c0 = blockIdx.x * SB;
+        if (c0 >= N) return;
+        for (int e = tid; e < SB * SB; e += 256) {
+            int i = e >> 6, j = e & 63;
+            Xs[i][j] = Vt[(int64_t)gidx(P, Q, i) * N + c0 + j];
+            Ja[i][j] = Jb[(int64_t)k * SB * SB + e];
+        }
+        __syncthreads();
+        double acc[4][4] = {};
+        tile_atb(Ja, Xs, acc, ti, tj);
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int v = 0; v < 4; ++v) Vt[(int64_t)gidx(P, Q, ti + u) * N + c0 + tj + v] = acc[u][v];
+        return;
+    }
+    const int k = blockIdx.y, l = blockIdx.x;
+    if (l >= npair || k > l) return;
+    const bool ak = active[k] != 0, al = active[l] != 0;
+    if (!ak && !al) return;
+    int P, Q, R, S2; rr_pair(nb, round, k, P, Q); rr_pair(nb, round, l, R, S2);
+    if (k == l) {   // the solved diagonal block: exactly what the solver left (annihilated entries are exact zeros)
+        for (int e = tid; e < SB * SB; e += 256) {
+            int i = e >> 6, j = e & 63;
+            Gp[(int64_t)gidx(P, Q, i) * N + gidx(P, Q, j)] = Dg[(int64_t)k * SB * SB + e];
+        }
+        return;
+    }
+    for (int e = tid; e < SB * SB; e += 256) {
+        int i = e >> 6, j = e & 63;
+        Xs[i][j] = Gp[(int64_t)gidx(P, Q, i) * N + gidx(R, S2, j)];
+        Ja[i][j] = ak ? Jb[(int64_t)k * SB * SB + e] : (i == j ? 1.0 : 0.0);
+        Jc[i][j] = al ? Jb[(int64_t)l * SB * SB + e] : (i == j ? 1.0 : 0.0);
+    }
+    __syncthreads();
+    double acc[4][4] = {};
+    tile_atb(Ja, Xs, acc, ti, tj);        // J_k^T X
+    __syncthreads();
 #pragma unroll
     for (int u = 0; u < 4; ++u)
 #pragma unroll
-        for (int v = 0; v < 4; ++v) X[(int64_t)(r0 + ti + u) * N + gidx(P, Q, tj + v)] = acc[u][v];
-}
-
-// X[PQ, :] <- J_k^T * X[PQ, :]  for X = Gp (z = 0, with the exact diagonal block written back) and X = Vt (z = 1)
-__global__ void __launch_bounds__(256) blk_apply_rows_kernel(int N, int nb, int round, double* __restrict__ Gp, double* __restrict__ Vt,
-                                                             const double* __restrict__ Jb, const double* __restrict__ Dg,
-                                                             const int* __restrict__ active) {
-    const int k = blockIdx.y;
-    if (!active[k]) return;
-    extern __shared__ double sh2[];
-    double (*Xs)[SP] = reinterpret_cast<double (*)[SP]>(sh2);
-    double (*Js)[SP] = reinterpret_cast<double (*)[SP]>(sh2 + SB * SP);
-    int P, Q; rr_pair(nb, round, k, P, Q);
-    double* X = blockIdx.z == 0 ? Gp : Vt;
-    const int tid = threadIdx.x, c0 = blockIdx.x * SB;
-    for (int e = tid; e < SB * SB; e += 256) {
-        int i = e >> 6, j = e & 63;
-        Xs[i][j] = X[(int64_t)gidx(P, Q, i) * N + c0 + j];
-        Js[i][j] = Jb[(int64_t)k * SB * SB + e];
-    }
+        for (int v = 0; v < 4; ++v) Xs[ti + u][tj + v] = acc[u][v];
     __syncthreads();
-    const int ti = (tid >> 4) * 4, tj = (tid & 15) * 4;
-    double acc[4][4] = {};
-#pragma unroll 8
-    for (int l = 0; l < SB; ++l) {
-        double a[4], b[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) { a[u] = Js[l][ti + u]; b[u] = Xs[l][tj + u]; }
-#pragma unroll
-        for (int u = 0; u < 4; ++u)
-#pragma unroll
-            for (int v = 0; v < 4; ++v) acc[u][v] += a[u] * b[v];
-    }
+    double acc2[4][4] = {};
+    tile_ab(Xs, Jc, acc2, ti, tj);        // (J_k^T X) J_l
 #pragma unroll
     for (int u = 0; u < 4; ++u)
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
-            const int li = ti + u, col = c0 + tj + v;
-            double val = acc[u][v];
-            if (blockIdx.z == 0) {
-                const int cb = col / BW;
-                if (cb == P || cb == Q) { int lj = (cb == P) ? col - P * BW : BW + col - Q * BW; val = (li == lj) ? Dg[k * SB + li] : 0.0; }
-            }
-            X[(int64_t)gidx(P, Q, li) * N + col] = val;
+            const int gi = gidx(P, Q, ti + u), gj = gidx(R, S2, tj + v);
+            Gp[(int64_t)gi * N + gj] = acc2[u][v];
+            Gp[(int64_t)gj * N + gi] = acc2[u][v];
         }
 }
 __global__ void extract_diag_kernel(int N, const double* __restrict__ Gp, double* __restrict__ d) {
@@ -319,7 +420,8 @@ bool check(cudaError_t e, std::string* err, const char* what) {
     return false;
 }
 constexpr int kSmallSmem = (2 * SB * SP + 96) * 8 + 3 * 32 * 4 + 64;
-constexpr int kApplySmem = 2 * SB * SP * 8;
+constexpr int kApplySmem = 3 * SB * SP * 8;
+constexpr int kSolve2Smem = 3 * SB * SP * 8 + 64 * 24 + 32 * 8 + 128 * 4 + 64;
 }  // namespace
 
 // work layout (bytes): [lam_unsorted N][idx N ints][misc 64 doubles][Vt_unsorted N*N][Gp N*N][Jb nb/2*4096][Dg nb/2*64][active nb/2 ints]
@@ -328,7 +430,7 @@ static int padded_n(int n) { if (n <= SB) return n; int nb = (n + BW - 1) / BW; 
 size_t eigh_work_bytes(int n) {
     size_t N = (size_t)padded_n(n);
     size_t nb2 = N / BW / 2 + 1;
-    return 8 * (N + N + 64 + 2 * N * N + nb2 * SB * SB + nb2 * SB + nb2) + 4096;
+    return 8 * (N + N + 64 + 2 * N * N + 2 * nb2 * SB * SB + nb2) + 4096;
 }
 
 int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work, std::vector<double>* lam_host, std::string* err) {
@@ -342,9 +444,8 @@ int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work,
     static bool cfg = false;
     if (!cfg) {
         if (!check(cudaFuncSetAttribute(eigh_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmallSmem), err, "eigh attr")) return TATRG_ECUDA;
-        if (!check(cudaFuncSetAttribute(blk_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmallSmem), err, "eigh attr")) return TATRG_ECUDA;
-        if (!check(cudaFuncSetAttribute(blk_apply_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kApplySmem), err, "eigh attr")) return TATRG_ECUDA;
-        if (!check(cudaFuncSetAttribute(blk_apply_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kApplySmem), err, "eigh attr")) return TATRG_ECUDA;
+        if (!check(cudaFuncSetAttribute(blk_solve2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSolve2Smem), err, "eigh attr")) return TATRG_ECUDA;
+        if (!check(cudaFuncSetAttribute(blk_apply2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kApplySmem), err, "eigh attr")) return TATRG_ECUDA;
         cfg = true;
     }
     if (n <= SB) {
@@ -353,20 +454,19 @@ int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work,
         double* Gp = w; w += (size_t)N * N;
         const int nb = N / BW, npair = nb / 2;
         double* Jb = w; w += (size_t)npair * SB * SB;
-        double* Dg = w; w += (size_t)npair * SB;
+        double* Dg = w; w += (size_t)npair * SB * SB;
         int* active = (int*)w; w += npair;     // npair ints fit in npair doubles
         int* counter = (int*)misc + 8;
         pad_sym_kernel<<<148 * 4, 256, 0, st>>>(n, N, G, Gp, Vu);
-        diag_max_kernel<<<1, 256, 0, st>>>(N, Gp, misc);
+        diag_max_kernel<<<1, 256, 0, st>>>(N, Gp, misc, kFloorRel);
         count_launch(2);
         int sweep = 0;
         for (; sweep < kMaxSweeps; ++sweep) {
             cudaMemsetAsync(counter, 0, sizeof(int), st);
             for (int r = 0; r < nb - 1; ++r) {
-                blk_solve_kernel<<<npair, 512, kSmallSmem, st>>>(N, nb, r, Gp, misc, Jb, Dg, active, counter);
-                blk_apply_cols_kernel<<<dim3(N / SB, npair), 256, kApplySmem, st>>>(N, nb, r, Gp, Jb, active);
-                blk_apply_rows_kernel<<<dim3(N / SB, npair, 2), 256, kApplySmem, st>>>(N, nb, r, Gp, Vu, Jb, Dg, active);
-                count_launch(3);
+                blk_solve2_kernel<<<npair, 1024, kSolve2Smem, st>>>(N, nb, r, r == 0 ? 0 : 1, Gp, misc, Jb, Dg, active, counter);
+                blk_apply2_kernel<<<dim3(N / SB, 2 * npair), 256, kApplySmem, st>>>(N, nb, r, Gp, Vu, Jb, Dg, active);
+                count_launch(2);
             }
             int rot = 0;
             if (!check(cudaMemcpyAsync(&rot, counter, sizeof(int), cudaMemcpyDeviceToHost, st), err, "eigh readback")) return TATRG_ECUDA;
