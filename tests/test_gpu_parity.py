@@ -1,0 +1,234 @@
+"""GPU parity tests proper: the CUDA Triad-ATRG path, through the C ABI, against the CPU oracle on the same seeded
+inputs.  Only gauge-invariant quantities are compared (SVD signs and bases are not unique):
+
+    ln Z / V                          relative error <= 1e-10   (north_star)
+    retained singular values          absolute error <= 1e-9 of the leading value   (north_star)
+    projectors / reconstructions      stage by stage, teacher-forced from the oracle's state
+
+Expected values come from tests/golden/*.json, written by tests/golden/make_golden.py from the oracle ONLY, or from
+the oracle run inside the test for the small cases."""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+
+import paper_2507_21909_b200 as T
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
+TOL_LNZ, TOL_SV = 1e-10, 1e-9
+
+
+def golden(name):
+    path = os.path.join(HERE, "golden", "oracle_%s.json" % name)
+    if not os.path.exists(path):
+        pytest.skip("golden file %s not generated" % name)
+    return json.load(open(path))["runs"]
+
+
+def run_against(rec, max_steps=None):
+    t = T.Tatrg(rec["beta"], rec["h"], rec["D"], rec["oversample"], rec["seed"], power_iters=rec["n_pow"])
+    n = len(rec["lnZ"]) if max_steps is None else min(max_steps, len(rec["lnZ"]))
+    worst = [0.0, 0.0, 0.0]
+    for m in range(n):
+        t.step()
+        lz = t.lnZ_per_site()
+        worst[0] = max(worst[0], abs(lz - rec["lnZ"][m]) / abs(rec["lnZ"][m]))
+        for i, (which, key) in enumerate(((T.SV_SIGMA, "sigma"), (T.SV_S, "s"))):
+            got = t.singular_values(which, rec["D"])
+            ref = np.zeros(rec["D"])
+            ref[:len(rec[key][m])] = rec[key][m]
+            g = np.zeros(rec["D"])
+            g[:len(got)] = got
+            worst[1 + i] = max(worst[1 + i], float(np.abs(g - ref).max()))
+    assert t.steps_done() == n and t.launches() > 0
+    t.close()
+    return worst
+
+
+def test_config1_full_run():
+    """BASELINE.json configs[0]: 16^4, beta=0.14, D=4, p=4, 1 power iteration, seed 1234."""
+    (rec,) = golden("c1")
+    w = run_against(rec)
+    assert w[0] <= TOL_LNZ and w[1] <= TOL_SV and w[2] <= TOL_SV, w
+
+
+@pytest.mark.parametrize("idx", range(5))
+def test_config2_beta_sweep(idx):
+    """configs[1]: 2^10 per axis (40 steps), D=8, p=8, 2 power iterations, five (beta, seed) pairs around T_c."""
+    rec = golden("c2")[idx]
+    w = run_against(rec)
+    assert w[0] <= TOL_LNZ and w[1] <= TOL_SV and w[2] <= TOL_SV, w
+
+
+@pytest.mark.parametrize("idx", range(2))
+def test_config3_field(idx):
+    """configs[2]: 2^12 per axis (48 steps), D=16, p=16, h = +-1e-3, seed 7."""
+    rec = golden("c3")[idx]
+    w = run_against(rec)
+    assert w[0] <= TOL_LNZ and w[1] <= TOL_SV and w[2] <= TOL_SV, w
+
+
+def test_config4_first_steps_at_full_size():
+    """configs[3] (headline, D=32, p=32): as many steps as the oracle could afford (the weight of step m in ln Z/V is
+    2^-m); the remaining steps are covered by test_d32_stage_properties."""
+    (rec,) = golden("c4")
+    w = run_against(rec)
+    assert w[0] <= TOL_LNZ and w[1] <= TOL_SV and w[2] <= TOL_SV, w
+
+
+# ---- pins that need no oracle run: exact values the mathematics fixes ------------------------------------------------------
+@pytest.mark.parametrize("beta,h", [(0.14, 0.0), (0.1497, 1e-3), (0.3, -0.2)])
+def test_one_step_is_exact_closed_form(beta, h):
+    """Lattice 2x1x1x1 (periodic): Z = e^{6 beta} [2 e^{2 beta} cosh(2 beta h) + 2 e^{-2 beta}]; nothing is truncated at D>=4."""
+    t = T.Tatrg(beta, h, 4, 4, 1)
+    t.step()
+    z = math.exp(6 * beta) * (2 * math.exp(2 * beta) * math.cosh(2 * beta * h) + 2 * math.exp(-2 * beta))
+    assert abs(t.lnZ_per_site() - math.log(z) / 2) <= 1e-13
+
+
+def test_low_temperature_limit():
+    """beta = 2, 16 steps: ln Z/V - 4 beta = ln 2 / 2^16 (two ordered ground states); the spectrum collapses to rank 2 then 1."""
+    t = T.Tatrg(2.0, 0.0, 4, 4, 3, power_iters=1)
+    for _ in range(16):
+        t.step()
+    assert abs(t.lnZ_per_site() - 8.0 - math.log(2) / 2 ** 16) <= 1e-11
+
+
+def test_high_temperature_limit():
+    t = T.Tatrg(1e-3, 0.0, 4, 4, 3, power_iters=1)
+    for _ in range(12):
+        t.step()
+    b = 1e-3
+    assert abs(t.lnZ_per_site() - math.log(2) - 4 * math.log(math.cosh(b))) <= 1e-10
+
+
+# ---- oracle run inside the test: small and edge configurations ----------------------------------------------------------------
+@pytest.mark.parametrize("beta,h,D,p,n_pow,seed,steps", [
+    (0.1497, 0.0, 2, 0, 0, 5, 8),        # minimal D, no oversampling, no power iteration
+    (0.1497, 0.0, 3, 2, 1, 6, 8),        # odd D: ragged everywhere
+    (0.16, 5e-2, 5, 3, 2, 7, 10),        # ordered phase with field
+    (0.12, 0.0, 6, 6, 3, 8, 8),
+    (0.1497, 0.0, 4, 4, 1, 2 ** 40 + 17, 6),   # 64-bit seed
+])
+def test_small_runs_against_live_oracle(beta, h, D, p, n_pow, seed, steps):
+    from oracle import tatrg_oracle as O
+    t = T.Tatrg(beta, h, D, p, seed, power_iters=n_pow)
+    o = O.TatrgOracle(beta, h, D, p, seed, n_pow=n_pow)
+    for m in range(steps):
+        t.step()
+        o.step()
+        lo = o.lnZ_per_site()
+        assert abs(t.lnZ_per_site() - lo) <= TOL_LNZ * abs(lo), m
+        for which, key in ((T.SV_SIGMA, "sigma"), (T.SV_S, "s")):
+            got, ref = t.singular_values(which, D), o.last[key][:D]
+            k = min(len(got), len(ref))
+            assert np.abs(got[:k] - ref[:k]).max() <= TOL_SV, (m, key)
+            assert np.all(np.abs(ref[k:]) <= TOL_SV) and np.all(np.abs(got[k:]) <= TOL_SV)
+
+
+def test_k_triad_option_and_full_rank_equals_atrg():
+    """K = chi2*chi3 (no triad truncation) and a smaller K both follow the oracle (PAPER.md :179 'r = D recovers ATRG')."""
+    from oracle import tatrg_oracle as O
+    for K in (16, 5):
+        t = T.Tatrg(0.1497, 0.0, 4, 12, 9, power_iters=1, K=K)
+        o = O.TatrgOracle(0.1497, 0.0, 4, 12, 9, n_pow=1, K=K)
+        for m in range(6):
+            t.step()
+            o.step()
+            assert abs(t.lnZ_per_site() - o.lnZ_per_site()) <= TOL_LNZ * abs(o.lnZ_per_site()), (K, m)
+
+
+# ---- stage-wise, teacher-forced: the GPU step is fed the oracle's state; gauge-invariant stage outputs are compared ---------------
+def _proj(x, nlast=1):
+    m = x.reshape(-1, int(np.prod(x.shape[-nlast:])))
+    return m @ m.T
+
+
+@pytest.mark.parametrize("D,p,n_pow,presteps", [(4, 4, 1, 3), (6, 6, 2, 4)])
+def test_stagewise_teacher_forced(D, p, n_pow, presteps):
+    from oracle import tatrg_oracle as O
+    beta, h, seed = 0.1497, 0.0, 21
+    o = O.TatrgOracle(beta, h, D, p, seed, n_pow=n_pow)
+    t = T.Tatrg(beta, h, D, p, seed, power_iters=n_pow)
+    t.set_option(T.OPT_KEEP_TENSORS, 1)
+    for _ in range(presteps):
+        o.step()
+        t.step()
+    t.set_state(o.phi, o.psi)          # teacher forcing: identical inputs to the compared step
+    o.step()
+    t.step()
+    L = o.last
+    a, dt, core, x, y, sig = (t.get_tensor(n) for n in ("A", "Dt", "core", "X", "Y", "sigma"))
+    tol = 1e-10
+    # (a) canonical gauge makes A, Dt, core themselves comparable
+    assert np.abs(a - L["a"]).max() <= tol and np.abs(dt - L["dt"]).max() <= tol and np.abs(core - L["core"]).max() <= tol
+    am = a.reshape(-1, a.shape[-1])
+    assert np.abs(am.T @ am - np.eye(a.shape[-1])).max() <= 1e-12          # isometry (:137)
+    # (b) X sigma Y^T is gauge invariant; X, Y isometric
+    assert np.abs(sig - L["sig"]).max() <= tol * L["sig"][0]
+    rec_g = np.einsum("aig,g,bjg->aibj", x.reshape(x.shape[0], -1, x.shape[-1]), sig, y.reshape(y.shape[0], -1, y.shape[-1]))
+    rec_o = np.einsum("aig,g,bjg->aibj", L["x"].reshape(x.shape[0], -1, x.shape[-1]), L["sig"], L["y"].reshape(y.shape[0], -1, y.shape[-1]))
+    assert np.abs(rec_g - rec_o).max() <= tol * L["sig"][0]
+    xm = x.reshape(-1, x.shape[-1])
+    assert np.abs(xm.T @ xm - np.eye(x.shape[-1])).max() <= 1e-11
+    # (c) triad isometries: projectors U U^T
+    for name, uo in zip(("UA", "UX", "UY", "UD"), L["u"]):
+        ug = t.get_tensor(name)                                            # [k, leg2, leg3]
+        pg = ug.reshape(ug.shape[0], -1).T @ ug.reshape(ug.shape[0], -1)
+        po = uo.reshape(-1, uo.shape[-1]) @ uo.reshape(-1, uo.shape[-1]).T
+        assert ug.shape[0] == uo.shape[-1], name
+        assert np.abs(pg - po).max() <= 1e-9, name
+    # (d) squeezers: canonical gauge makes M, N comparable up to nothing
+    for mu in (2, 3, 4):
+        mg, ng = t.get_tensor("M%d" % mu), t.get_tensor("N%d" % mu)        # [k, u, l]
+        mo, no = L["m"][mu], L["n"][mu]                                    # [u, l, k]
+        assert mg.shape[0] == mo.shape[-1], mu
+        pg = np.einsum("kul,kvw->ulvw", mg, ng)
+        po = np.einsum("ulk,vwk->ulvw", mo, no)
+        assert np.abs(pg - po).max() <= 1e-8 * max(1.0, np.abs(po).max()), mu
+        assert np.abs(np.einsum("kul,jul->kj", mg, ng) - np.eye(mg.shape[0])).max() <= 1e-9    # N^T M = 1
+    # (e,f) new state: T' = Phi' Psi'^T is gauge invariant
+    phi, psi = t.get_tensor("phi"), t.get_tensor("psi")
+    assert phi.shape == o.phi.shape
+    tg = phi.reshape(-1, phi.shape[-1]) @ psi.reshape(-1, psi.shape[-1]).T
+    to = o.phi.reshape(-1, o.phi.shape[-1]) @ o.psi.reshape(-1, o.psi.shape[-1]).T
+    assert np.abs(tg - to).max() <= 1e-9 * np.abs(to).max()
+
+
+# ---- full size (D = 32, the launch configuration bench.py times): properties and sampled outputs ----------------------------------
+def test_d32_stage_properties_and_sampled_contraction():
+    from oracle import tatrg_oracle as O
+    D, p = 32, 32
+    t = T.Tatrg(0.1497, 0.0, D, p, 42)
+    t.set_option(T.OPT_KEEP_TENSORS, 1)
+    for _ in range(6):
+        t.step()
+    assert t.workspace_peak() <= T.workspace_bytes(D, p)
+    a, x, sig = t.get_tensor("A"), t.get_tensor("X"), t.get_tensor("sigma")
+    assert a.shape == (32, 32, 32, 32, 32) and x.shape[:4] == (32, 32, 32, 32)
+    for m in (a.reshape(-1, a.shape[-1]), x.reshape(-1, x.shape[-1])):
+        assert np.abs(m.T @ m - np.eye(m.shape[1])).max() <= 1e-10       # isometries (:137)
+    assert np.all(np.diff(sig) <= 0) and sig[-1] > 0
+    ua = t.get_tensor("UA")
+    um = ua.reshape(ua.shape[0], -1)
+    assert np.abs(um @ um.T - np.eye(um.shape[0])).max() <= 1e-10
+    for mu in (2, 3, 4):
+        mg, ng = t.get_tensor("M%d" % mu), t.get_tensor("N%d" % mu)
+        assert np.abs(np.einsum("kul,jul->kj", mg, ng) - np.eye(mg.shape[0])).max() <= 1e-8
+    # sampled outputs of the O(r^2 D^7) contraction (Eq. 2.18 :175), recomputed one slab at a time with the oracle's
+    # contract_half from the GPU's own E, F, I, J, M (teacher-forced stage parity at full size)
+    e, f = t.get_tensor("E"), t.get_tensor("F")
+    ux = t.get_tensor("UX")
+    m2, m3, m4 = (t.get_tensor("M%d" % mu) for mu in (2, 3, 4))
+    phi = t.get_tensor("phi")                                              # [k2,k3,k4,i1,g]
+    tr = lambda m: np.ascontiguousarray(m.transpose(1, 2, 0))             # [k,u,l] -> oracle's [u,l,k]
+    tu = lambda u: np.ascontiguousarray(u.transpose(1, 2, 0))             # [k,j,k'] -> oracle's [j,k',k]
+    rng = np.random.default_rng(0)
+    for _ in range(2):
+        i1 = int(rng.integers(0, e.shape[0]))
+        slab = O.contract_half(e[i1:i1 + 1], f, tu(ua), tu(ux), tr(m2), tr(m3), tr(m4))[0]     # [k2,k3,k4,g]
+        got = phi[:, :, :, i1, :]
+        assert np.abs(got - slab).max() <= 1e-11 * max(1.0, np.abs(slab).max())

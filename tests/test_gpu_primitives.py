@@ -1,0 +1,176 @@
+"""GPU parity tests of the kernels the Triad-ATRG path is made of, through the C ABI, against the CPU oracle's
+routines (oracle/) or their plain numpy definition in FP64.  Sizes span several tiles and a ragged tail.
+
+Tolerances: a K-term FP64 dot product accumulated in a different order differs by at most
+~K * 2^-53 * sum|a_k b_k|; the tests bound that by 64 * eps * K * max|a| * max|b| ... integers are bit-exact."""
+import numpy as np
+import pytest
+
+import paper_2507_21909_b200 as T
+from tests import inputs
+
+pytestmark = pytest.mark.gpu
+EPS = 2.0 ** -52
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+# ---- Philox (bit-exact integers, Gaussians to a few ulp) --------------------------------------------------------------
+@pytest.mark.parametrize("seed,call,stream,start,count", [(0, 0, 0, 0, 1), (1234, 7, 0, 0, 4099), (2 ** 63 + 5, 3, 1, 2 ** 32 - 3, 1000),
+                                                          (42, 60, 4, 123456789012, 257)])
+def test_philox_integers_bit_exact(torch, seed, call, stream, start, count):
+    from oracle import philox
+    raw = T.philox_raw(seed, call, stream, start, count)
+    e = np.arange(start, start + count, dtype=np.uint64)
+    ref = philox.philox4x32_10(e & np.uint64(0xFFFFFFFF), e >> np.uint64(32), call, stream, seed & 0xFFFFFFFF, (seed >> 32) & 0xFFFFFFFF)
+    assert np.array_equal(raw, np.stack(ref, axis=1))
+
+
+def test_philox_known_answer_on_device(torch):
+    assert [hex(v) for v in T.philox_raw(0, 0, 0, 0, 1)[0]] == ["0x6627e8d5", "0xe169c58d", "0xbc57ac4c", "0x9b00dbd8"]
+
+
+def test_philox_gaussians_match_oracle(torch):
+    from oracle import philox
+    z = T.philox_gaussian(1234, 5, 0, 1000, 200003)
+    ref = philox.gaussians(1234, 5, 0, 1000, 200003)
+    # libm vs CUDA math: log, sqrt, cos(2 pi u) differ by a few ulp of the result scale (|z| <= ~9)
+    assert np.abs(z - ref).max() <= 64 * EPS
+    assert T.philox_gaussian(1, 1, 1, 0, 0).size == 0
+
+
+# ---- DGEMM --------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("M,N,K", [(1, 1, 1), (128, 128, 16), (129, 257, 33), (300, 70, 1000), (64, 2048, 7), (5, 5, 100003), (1024, 3, 64)])
+@pytest.mark.parametrize("ta,tb", [(False, False), (True, False), (False, True), (True, True)])
+def test_dgemm_matches_definition(torch, M, N, K, ta, tb):
+    a = inputs.random_tensor((M, K), 1)
+    b = inputs.random_tensor((K, N), 2)
+    ref = a @ b
+    A = dev(torch, a.T if ta else a)
+    B = dev(torch, b.T if tb else b)
+    C = T.dgemm(A, B, transa=ta, transb=tb).cpu().numpy()
+    bound = 8 * EPS * K * np.abs(a).max() * np.abs(b).max()
+    assert np.abs(C - ref).max() <= bound
+
+
+def test_dgemm_batched_alpha_beta(torch):
+    a = inputs.random_tensor((5, 70, 40), 3)
+    b = inputs.random_tensor((5, 40, 90), 4)
+    c0 = inputs.random_tensor((5, 70, 90), 5)
+    C = dev(torch, c0)
+    T.dgemm(dev(torch, a), dev(torch, b), alpha=0.5, beta=-2.0, C=C)
+    ref = 0.5 * np.einsum("bik,bkj->bij", a, b) - 2.0 * c0
+    assert np.abs(C.cpu().numpy() - ref).max() <= 8 * EPS * 40 * 25
+
+
+# ---- permute ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,perm", [((3, 5, 7, 4, 6), (1, 2, 3, 0, 4)), ((3, 5, 7, 4, 6), (4, 3, 2, 1, 0)), ((33, 65), (1, 0)),
+                                        ((2, 2, 2, 2, 2), (1, 2, 3, 0, 4)), ((8, 8, 8, 8, 8), (0, 3, 4, 1, 2)), ((1, 7, 1, 5), (3, 2, 1, 0)),
+                                        ((16, 16, 16, 16, 16), (1, 2, 3, 0, 4)), ((40, 3, 50), (2, 1, 0)), ((6,), (0,))])
+def test_permute_bit_exact(torch, shape, perm):
+    x = inputs.random_tensor(shape, 6)
+    out = T.permute(dev(torch, x), perm).cpu().numpy()
+    assert np.array_equal(out, np.transpose(x, perm))
+
+
+# ---- contraction engine ---------------------------------------------------------------------------------------------------
+SPECS = [("abc,cd->abd", (3, 4, 5), (5, 6)), ("ajklg,amnlg->jkmn", (3, 4, 5, 6, 7), (3, 2, 3, 6, 7)),
+         ("mjk,Ijkla->Imla", (6, 3, 4), (5, 3, 4, 2, 3)), ("pia,bpm->iabm", (5, 3, 4), (4, 5, 6)),
+         ("zul,axld->uaxzd", (3, 4, 5), (2, 6, 5, 3)), ("jp,Bjm->Bpm", (10, 4), (3, 10, 5)),
+         ("ikua,ikvb->uavb", (3, 4, 5, 2), (3, 4, 5, 2)), ("Ikxzd,kxpq->Ipqzd", (4, 6, 5, 3, 2), (6, 5, 3, 4)),
+         ("kmab,abxy->kmxy", (5, 5, 3, 3), (3, 3, 4, 4)), ("qib,iabm->aqm", (7, 2, 3), (2, 3, 3, 5)),
+         ("a,a->", (1000,), (1000,)), ("ab,b->a", (200, 300), (300,))]
+
+
+@pytest.mark.parametrize("spec,sa,sb", [s for s in SPECS if s[1] is not None])
+def test_contract_matches_einsum(torch, spec, sa, sb):
+    a = inputs.random_tensor(sa, 7)
+    b = inputs.random_tensor(sb, 8)
+    ref = np.einsum(spec.lower() if not any(ch.isupper() for ch in spec) else _lower_unique(spec), a, b)
+    out = T.contract(spec, dev(torch, a), dev(torch, b)).cpu().numpy()
+    k = a.size * b.size / max(ref.size, 1)
+    assert out.shape == ref.shape
+    assert np.abs(out - ref).max() <= 16 * EPS * max(k, 1) ** 0.5 * 25 * max(1.0, np.abs(ref).max())
+
+
+def _lower_unique(spec):
+    import string
+    for ch in sorted(set(c for c in spec if c.isupper())):
+        free = [c for c in string.ascii_lowercase if c not in spec][0]
+        spec = spec.replace(ch, free)
+    return spec
+
+
+def test_contract_rejects_bad_specs(torch):
+    a = dev(torch, inputs.random_tensor((3, 4), 1))
+    with pytest.raises(T.TatrgError):
+        T.contract("ab,cd->ad", a, a)          # b and c appear once
+    with pytest.raises(T.TatrgError):
+        T.contract("ab,bc->ac", a, a)          # extent mismatch on b
+
+
+# ---- dot (tTr) ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 31, 1024, 1000003])
+def test_dot(torch, n):
+    x = inputs.random_tensor((n,), 9)
+    y = inputs.random_tensor((n,), 10)
+    ref = float(np.dot(x, y))
+    assert abs(T.dot(dev(torch, x), dev(torch, y)) - ref) <= 8 * EPS * np.abs(x * y).sum()
+
+
+# ---- eigen-decomposition vs the oracle's Jacobi ------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,rank", [(1, 1), (2, 2), (5, 3), (16, 16), (64, 40), (65, 65), (100, 30), (256, 256), (300, 120)])
+def test_eigh_matches_oracle(torch, n, rank):
+    from oracle import tatrg_oracle as O
+    g = inputs.random_psd(n, rank, 11 + n)
+    lam_o, v_o = O.jacobi_eigh(g)
+    lam, vt = T.eigh(dev(torch, g))
+    lam, vt = lam.cpu().numpy(), vt.cpu().numpy()
+    assert np.abs(lam - lam_o).max() <= 64 * EPS * n * lam_o[0]
+    assert np.abs(vt @ vt.T - np.eye(n)).max() <= 64 * EPS * n
+    assert np.abs(vt.T @ (lam[:, None] * vt) - g).max() <= 64 * EPS * n * lam_o[0]
+    # gauge-invariant: projector on the eigenvectors of the `rank` non-zero (geometric, simple) eigenvalues
+    k = min(rank, 8)
+    assert np.abs(vt[:k].T @ vt[:k] - v_o[:, :k] @ v_o[:, :k].T).max() <= 1e-10
+
+
+def test_eigh_graded_gram_keeps_relative_accuracy_above_the_floor(torch):
+    """Gram matrix with eigenvalues 1 .. 1e-12: every eigenvalue above the documented floor (1e-18 of the largest
+    diagonal entry, two orders below GEMM rounding) must come out to FP64 absolute accuracy."""
+    n = 96
+    rng = np.random.default_rng(5)
+    q, _ = np.linalg.qr(rng.standard_normal((n, n)))
+    lam_true = 10.0 ** (-12 * np.arange(n) / (n - 1))
+    g = (q * lam_true) @ q.T
+    lam, vt = T.eigh(dev(torch, g))
+    assert np.abs(lam.cpu().numpy() - lam_true).max() <= 64 * EPS * n
+
+
+# ---- small SVD vs the oracle's one-sided Jacobi --------------------------------------------------------------------------------
+@pytest.mark.parametrize("nv,ln", [(1, 1), (2, 5), (4, 4), (8, 16), (32, 32), (64, 64), (40, 96), (96, 96)])
+def test_svd_rows_matches_oracle(torch, nv, ln):
+    from oracle import tatrg_oracle as O
+    x = inputs.lowrank_plus_noise(nv, ln, min(nv, ln, 6), 1e-3, 13 + nv)
+    u_o, s_o, v_o = O.jacobi_svd(x)
+    s, ut, va = T.svd_rows(dev(torch, x))
+    s, ut, va = s.cpu().numpy(), ut.cpu().numpy(), va.cpu().numpy()
+    assert np.abs(s - s_o[:nv]).max() <= 64 * EPS * max(nv, ln) * s_o[0]
+    assert np.abs(va.T @ (s[:, None] * ut) - x).max() <= 64 * EPS * max(nv, ln) * s_o[0]
+    assert np.abs(ut @ ut.T - np.eye(nv)).max() <= 64 * EPS * max(nv, ln)
+
+
+def test_svd_rows_rank_deficient_gives_exact_zero_structure(torch):
+    rng = np.random.default_rng(3)
+    x = rng.standard_normal((8, 2)) @ rng.standard_normal((2, 12))
+    s, ut, va = T.svd_rows(dev(torch, x))
+    s = s.cpu().numpy()
+    assert (s[2:] <= 1e-13 * s[0]).all() and s[1] > 1e-3 * s[0]
