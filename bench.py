@@ -1,0 +1,259 @@
+"""bench.py -- sec/step and FP64 TFLOP/s of the Triad-ATRG hot path at D = 32 on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+Workload: BASELINE.json configs[3] -- 4D Ising, beta = 0.1497, h = 0, Triad-ATRG D = 32, p = 32 (K = l = 64), 2 power
+iterations, Philox seed 42.  A "step" is one coarse-graining step of the whole hot path (Fig. 5 a-f) in the
+saturated regime (all legs = D, reached after 5 steps; those 5 unsaturated steps are run before the warm-up).
+`value` = seconds per step with the state resident in HBM; `e2e` = the same through the C ABI with HOST buffers
+(state uploaded from pinned memory before, and downloaded after, every step, inside the timed region).
+Replicas only for N > 1: every rank coarse-grains its own network, no collective in the path.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+BETA, H, D, P, N_POW, SEED = 0.1497, 0.0, 32, 32, 2, 42
+PRE_STEPS = 5                      # legs grow 2 -> 4 -> 16 -> 32: saturated from step 6 on
+METRIC = "sec_per_coarse_graining_step_D32"
+UNIT = "s/step"
+WORKLOAD = "configs[3]: 4D Ising beta=0.1497 h=0, Triad-ATRG D=32 p=32 (K=l=64), 2 power iterations, Philox seed 42, saturated steps"
+# model FLOPs of one saturated step in the 2*M*N*K convention: counted live by the library
+FP64_TO_BF16_NOMINAL = 45.0 / 2250.0   # guide's nominal B200 FP64-tensor : dense bf16 ratio (blackwell_cuda_programming.md)
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(hbm=p["hbm_gbs"], bf16=p["bf16_tflops"], bf16_sus=p.get("bf16_tflops_sustained", p["bf16_tflops"]), src="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sus=1400.0, src="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag = index, [], set(), False
+        self.max_mhz = None
+
+    def run(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q, "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip().split(",")
+                self.samples.append(float(out[0]))
+                self.max_mhz = float(out[1])
+                for n, v in zip(names, out[2:]):
+                    if v.strip().lower().startswith("active"):
+                        self.reasons.add(n)
+            except Exception:
+                pass
+            time.sleep(0.2)
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+
+
+# ---- the oracle on a bounded sample (cpu_baseline leg and --impl reference) -------------------------------------------
+MODEL_FLOPS_PER_STEP = 2.385e12    # 2*M*N*K of every contraction of one saturated D=32 step (counted by the library)
+
+
+def oracle_sample(n_slabs=4, seed=0):
+    """Times oracle.contract_half -- the O(r^2 D^7) contraction of Eq. 2.18, the FLOP-dominant stage -- on `n_slabs`
+    of the 32 i1-slabs of synthetic triad tensors of the saturated D=32 shapes, and extrapolates to a whole step by
+    the model-FLOP ratio.  Returns (seconds per step extrapolated, seconds measured, flops of the sample, threads)."""
+    import numpy as np
+    import __graft_entry__ as G
+    G.build_oracle()
+    from oracle import tatrg_oracle as O
+    K = D + P
+    rng = np.random.default_rng(seed)
+    e = rng.standard_normal((n_slabs, K, D, D))
+    f = rng.standard_normal((D, K, D, D))
+    i_, j_ = rng.standard_normal((D, D, K)), rng.standard_normal((D, D, K))
+    m2, m3, m4 = (rng.standard_normal((D, D, D)) for _ in range(3))
+    flops = (2.0 * n_slabs * K * D ** 4 + 2.0 * n_slabs * K * D * K * D * D * D       # E M4, (E M4) F
+             + 2.0 * K * D ** 4 + 2.0 * K * D ** 5 + 2.0 * K * K * D ** 4              # I M2, (I M2) M3, ... J
+             + 2.0 * n_slabs * D ** 4 * K * K)                                          # Xi Lambda
+    t0 = time.perf_counter()
+    out = O.contract_half(e, f, i_, j_, m2, m3, m4)
+    dt = time.perf_counter() - t0
+    assert out.shape == (n_slabs, D, D, D, D)
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        threads = os.cpu_count() or 1
+    return dt * MODEL_FLOPS_PER_STEP / flops, dt, flops, threads
+
+
+def run_reference(args):
+    """The reference arm of this tier = the oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    for _ in range(args.warmup):
+        oracle_sample(1)
+    vals, meas, threads = [], [], 1
+    for _ in range(args.steps):
+        v, dt, fl, threads = oracle_sample(16)
+        vals.append(v)
+        meas.append(dt)
+    value = sum(vals) / len(vals)
+    sample = ("oracle.contract_half (Eq. 2.18, numpy einsum) on 16 of 32 i1-slabs of synthetic saturated D=32 triad tensors "
+              "(%.2e flop, %.2f s measured per step-sample), extrapolated by the model-FLOP ratio %.3e/step" % (fl, sum(meas) / len(meas), MODEL_FLOPS_PER_STEP))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": value * 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD, "l2": "inputs_exceed_l2"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ---- the CUDA path ---------------------------------------------------------------------------------------------------
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2507_21909_b200 as T
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    T.lib()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    t = T.Tatrg(BETA, H, D, P, SEED + rank, power_iters=N_POW, device="cuda:%d" % local)
+    for _ in range(PRE_STEPS):
+        t.step()
+    for _ in range(args.warmup):
+        t.step()
+    sampler = ClockSampler(local)
+    sampler.start()
+    # ---- timed region 1: K steps, state resident in HBM ----
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches = 0
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        t.step()
+        launches += t.launches()
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    lnz = t.lnZ_per_site()
+    # ---- timed region 2: end to end through the C ABI with host buffers ----
+    n5 = D ** 5
+    host = [torch.empty(n5, dtype=torch.float64).pin_memory() for _ in range(2)]
+    shape = t.get_tensor_into("phi", host[0])
+    t.get_tensor_into("psi", host[1])
+    k_e2e = max(1, min(args.steps, 3))
+    barrier()
+    ev0.record()
+    for _ in range(k_e2e):
+        t.set_state_host(host[0].view(shape), host[1].view(shape))      # H2D: 2 * D^5 doubles
+        t.step()
+        _ = t.lnZ_per_site()                                            # D2H: the step's result
+        _ = t.singular_values(T.SV_SIGMA, D)
+        t.get_tensor_into("phi", host[0])                               # D2H: 2 * D^5 doubles (state for the next call)
+        t.get_tensor_into("psi", host[1])
+    ev1.record()
+    barrier()
+    ms_e2e = ev0.elapsed_time(ev1)
+    sampler.stop_flag = True
+    sampler.join(timeout=2)
+    # ---- profiling pass (not part of `value`): per-launch CUDA events on the library's stream around every DGEMM / permute ----
+    t.set_option(T.OPT_STAGE_TIMING, 2)
+    g_ms = g_fl = p_ms = p_by = 0.0
+    g_n = p_n = 0
+    stage = None
+    n_prof = max(1, min(args.steps, 3))
+    step_ms_prof = 0.0
+    for _ in range(n_prof):
+        t.step()
+        a, b, c = t.gemm_profile()
+        g_ms, g_fl, g_n = g_ms + a, g_fl + b, g_n + c
+        a, b, c = t.permute_profile()
+        p_ms, p_by, p_n = p_ms + a, p_by + b, p_n + c
+        sm = t.stage_ms()
+        stage = sm if stage is None else stage + sm
+        step_ms_prof += float(sm.sum())
+    t.set_option(T.OPT_STAGE_TIMING, 0)
+    dmma = T.dmma_issue_rate(20000, 2)
+    # ---- max over ranks ----
+    tm = torch.tensor([ms, ms_e2e], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+    ms, ms_e2e = float(tm[0]), float(tm[1])
+    if rank == 0:
+        pk = peaks()
+        sec = ms * 1e-3 / (args.steps * world)            # whole-job: `world` replicas advance one step each per step time
+        sec_e2e = ms_e2e * 1e-3 / (k_e2e * world)
+        peak_tf = pk["bf16_sus"] * FP64_TO_BF16_NOMINAL   # kernel timed inside a long step -> sustained figure
+        ach_tf = g_fl / (g_ms * 1e-3) / 1e12
+        line = {
+            "metric": METRIC, "value": sec, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": WORKLOAD, "parallelism": "replicas" if world > 1 else "single",
+                                            "l2": "inputs_exceed_l2 (state 2 x 268 MB, Xi 1.07 GB vs 126 MB L2)", "pre_steps": PRE_STEPS},
+            "e2e": {"value": sec_e2e, "unit": UNIT, "h2d_bytes_per_step": 16 * n5, "d2h_bytes_per_step": 16 * n5 + 8 * (1 + D), "steps": k_e2e},
+            "gpu_launches": launches, "lnZ_per_site": lnz, "clocks": sampler.summary(),
+            "model_tflops": g_fl / n_prof / (ms / args.steps * 1e-3) / 1e12,
+            "roofline": {"bound": "tensor", "kernel": "dgemm_kernel (DMMA m8n8k4, all %d launches of a step)" % (g_n // n_prof),
+                         "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": None,
+                         "peak_source": "MEASURED_PEAKS.json bf16_tflops_sustained (%s) x nominal FP64:bf16 ratio 45/2250" % pk["src"],
+                         "dmma_issue_rate_tflops": dmma, "time_share_of_step": g_ms / step_ms_prof},
+            "permute": {"bound": "hbm", "achieved": p_by / (p_ms * 1e-3) / 1e9, "peak": pk["hbm"], "unit": "GB/s",
+                        "frac": p_by / (p_ms * 1e-3) / 1e9 / pk["hbm"], "launches_per_step": p_n // n_prof,
+                        "time_share_of_step": p_ms / step_ms_prof},
+            "stage_ms": {k: round(float(v) / n_prof, 2) for k, v in zip(T.STAGES, stage) if not k.startswith("_")},
+        }
+        if world == 1:
+            v, dt, fl, threads = oracle_sample(16)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                    "sample": "oracle.contract_half (Eq. 2.18) on 16 of 32 i1-slabs of synthetic saturated D=32 triad tensors: "
+                                              "%.2e flop in %.2f s, extrapolated by the model-FLOP ratio (%.3e flop/step); the oracle's Jacobi "
+                                              "decompositions are not in the sample" % (fl, dt, MODEL_FLOPS_PER_STEP)}
+        print(json.dumps(line))
+    t.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

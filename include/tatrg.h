@@ -136,6 +136,10 @@ int tatrg_svd(void* cuda_stream, int nv, int len, const double* X, double* s, do
  * result must have room for 1200 doubles (partial sums of the first pass follow result[0]). */
 int tatrg_dot(void* cuda_stream, long long n, const double* x, const double* y, double* result);
 
+/* Calibration: FP64 tensor-core (DMMA m8n8k4) issue rate of the whole device with register-resident operands, in
+ * TFLOP/s, timed with CUDA events inside the call (synchronises).  ctas_per_sm in 1..8; scratch_dev [dev] >= 8 bytes. */
+int tatrg_dmma_issue_rate(void* cuda_stream, int iters, int ctas_per_sm, double* tflops_out, double* scratch_dev);
+
 #ifdef __cplusplus
 }
 #endif

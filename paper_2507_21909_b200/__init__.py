@@ -59,6 +59,7 @@ _SIGNATURES = {
     "tatrg_svd": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_void_p,
                              _c.c_void_p]),
     "tatrg_dot": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
+    "tatrg_dmma_issue_rate": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_int, _dp, _c.c_void_p]),
 }
 
 
@@ -196,6 +197,22 @@ class Tatrg:
         dims = (ctypes.c_longlong * 5)(*phi.shape)
         _check(lib().tatrg_set_state(self._h, phi.ctypes.data_as(_dp), psi.ctypes.data_as(_dp), dims), "tatrg_set_state", self._h)
 
+    def set_state_host(self, phi_t, psi_t):
+        """Same as set_state, from (pinned) torch CPU float64 tensors, without a numpy copy."""
+        dims = (ctypes.c_longlong * 5)(*phi_t.shape)
+        _check(lib().tatrg_set_state(self._h, ctypes.cast(phi_t.data_ptr(), _dp), ctypes.cast(psi_t.data_ptr(), _dp), dims),
+               "tatrg_set_state", self._h)
+
+    def get_tensor_into(self, name, out_t):
+        """Copies tensor `name` into the (pinned) torch CPU float64 tensor out_t; returns its shape."""
+        nd = ctypes.c_int()
+        dims = (ctypes.c_longlong * 8)()
+        n = _check(lib().tatrg_get_tensor(self._h, name.encode(), ctypes.cast(out_t.data_ptr(), _dp), out_t.numel(),
+                                          ctypes.byref(nd), dims), "tatrg_get_tensor", self._h)
+        if n > out_t.numel():
+            raise TatrgError("get_tensor_into: buffer too small")
+        return [dims[i] for i in range(nd.value)]
+
     def close(self):
         if getattr(self, "_h", None):
             lib().tatrg_destroy(self._h)
@@ -300,3 +317,12 @@ def dot(x, y):
     res = torch.empty(1200, dtype=torch.float64, device=x.device)
     _check(lib().tatrg_dot(_stream_ptr(), x.numel(), _p(x), _p(y), _p(res)), "tatrg_dot")
     return float(res[0].item())
+
+
+def dmma_issue_rate(iters=20000, ctas_per_sm=2):
+    """Register-resident DMMA issue rate of the device in TFLOP/s (calibration of the FP64 tensor ceiling)."""
+    torch = _torch_cuda()
+    scratch = torch.zeros(8, dtype=torch.float64, device="cuda")
+    out = ctypes.c_double()
+    _check(lib().tatrg_dmma_issue_rate(_stream_ptr(), iters, ctas_per_sm, ctypes.byref(out), _p(scratch)), "tatrg_dmma_issue_rate")
+    return out.value

@@ -15,6 +15,8 @@
 #include <algorithm>
 #include <cmath>
 #include <numeric>
+#include <cstdio>
+#include <cstdlib>
 
 namespace tatrg {
 namespace {
@@ -23,9 +25,9 @@ constexpr int SP = SB + 1;      // pitch
 constexpr int BW = 32;          // block width of the block-Jacobi
 constexpr double kTolRel = 1e-15;
 constexpr int kMaxSweeps = 40;
-// off-diagonal entries below kFloorRel * max|diag| are not rotated: two orders below the rounding of the GEMM that
+// off-diagonal entries below kFloorRel * max|diag| are not rotated: one order below the rounding of the GEMM that
 // produced the matrix
-constexpr double kFloorRel = 1e-18;
+constexpr double kFloorRel = 1e-17;
 
 // round-robin tournament on np (even) players: round r in [0, np-1), table k in [0, np/2)
 __device__ __host__ __forceinline__ void rr_pair(int np, int r, int k, int& p, int& q) {
@@ -36,12 +38,19 @@ __device__ __host__ __forceinline__ void rr_pair(int np, int r, int k, int& p, i
     p = a < b ? a : b; q = a < b ? b : a;
 }
 
-// plane rotation that annihilates a_pq of [[app, apq], [apq, aqq]] with J = [[c, s], [-s, c]]  (J^T A J diagonal)
+// plane rotation that annihilates a_pq of [[app, apq], [apq, aqq]] with J = [[c, s], [-s, c]]  (J^T A J diagonal):
+// t = tan(theta) is the smaller root of t^2 + 2 zeta t - 1 = 0, zeta = (aqq - app) / (2 apq), written with one sqrt,
+// one division and one rsqrt (FP64 div / sqrt are long software sequences and sit on the critical path of a round).
 __device__ __forceinline__ void sym_rot(double app, double aqq, double apq, double& c, double& s) {
-    double zeta = (aqq - app) / (2.0 * apq);
-    double t = (zeta >= 0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-    c = 1.0 / sqrt(1.0 + t * t);
+    const double d = aqq - app;
+    const double r = sqrt(fma(d, d, 4.0 * apq * apq));
+    const double t = (d >= 0 ? 2.0 * apq : -2.0 * apq) / (fabs(d) + r);
+    c = rsqrt(fma(t, t, 1.0));
     s = c * t;
+}
+// rotate only above the relative threshold (no sqrt: compare squares) and above the absolute floor
+__device__ __forceinline__ bool needs_rot(double app, double aqq, double apq, double floor_abs) {
+    return fabs(apq) > floor_abs && apq * apq > (kTolRel * kTolRel) * fabs(app * aqq);
 }
 
 // Two-sided Jacobi on the n x n symmetric S (shared, pitch SP), accumulating J (S_out = J^T S_in J, columns of J).
@@ -59,7 +68,7 @@ __device__ int jacobi_smem(double* S, double* J, int n, double abs_floor, double
                 double c = 1.0, s = 0.0;
                 if (q < n) {
                     double app = S[p * SP + p], aqq = S[q * SP + q], apq = S[p * SP + q];
-                    if (fabs(apq) > abs_floor && fabs(apq) > kTolRel * sqrt(fabs(app * aqq))) { sym_rot(app, aqq, apq, c, s); atomicAdd(cnt, 1); }
+                    if (needs_rot(app, aqq, apq, abs_floor)) { sym_rot(app, aqq, apq, c, s); atomicAdd(cnt, 1); }
                 }
                 cs[tid] = c; sn[tid] = s; pp[tid] = p; qq[tid] = q;
             }
@@ -192,13 +201,13 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
         int i = e >> 6, j = e & 63;
         if (i < j && (mode == 0 || (i < BW && j >= BW))) {
             double a = fabs(Sa[i * SP + j]);
-            if (a > floor_abs && a > kTolRel * sqrt(fabs(Sa[i * SP + i] * Sa[j * SP + j]))) worst = 1.0;
+            if (needs_rot(Sa[i * SP + i], Sa[j * SP + j], a, floor_abs)) worst = 1.0;
         }
     }
     worst = block_max(worst, red);
     if (worst == 0.0) { if (tid == 0) active[k] = 0; return; }
     const int nrounds = mode == 0 ? SB - 1 : BW;
-    const int max_sweeps = mode == 0 ? 12 : 1;
+    const int max_sweeps = mode == 0 ? 2 : 1;
     double* S = Sa; double* T = Sb;
     int total = 0;
     for (int sweep = 0; sweep < max_sweeps; ++sweep) {
@@ -207,7 +216,7 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
             int p, q; sched(mode, 0, tid, p, q);
             Rot rt; rt.c = 1.0; rt.s = 0.0; rt.p = p; rt.q = q;
             double app = S[p * SP + p], aqq = S[q * SP + q], apq = S[p * SP + q];
-            if (fabs(apq) > floor_abs && fabs(apq) > kTolRel * sqrt(fabs(app * aqq))) { sym_rot(app, aqq, apq, rt.c, rt.s); atomicAdd(cnt, 1); }
+            if (needs_rot(app, aqq, apq, floor_abs)) { sym_rot(app, aqq, apq, rt.c, rt.s); atomicAdd(cnt, 1); }
             rots[tid] = rt; pair_of[p] = tid; pair_of[q] = tid;
         }
         __syncthreads();
@@ -242,7 +251,7 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
                 int p, q; sched(mode, r + 1, tid, p, q);
                 Rot rt; rt.c = 1.0; rt.s = 0.0; rt.p = p; rt.q = q;
                 double app = row_updated(S, cur, pof, p, p), aqq = row_updated(S, cur, pof, q, q), apq = row_updated(S, cur, pof, p, q);
-                if (fabs(apq) > floor_abs && fabs(apq) > kTolRel * sqrt(fabs(app * aqq))) { sym_rot(app, aqq, apq, rt.c, rt.s); atomicAdd(cnt, 1); }
+                if (needs_rot(app, aqq, apq, floor_abs)) { sym_rot(app, aqq, apq, rt.c, rt.s); atomicAdd(cnt, 1); }
                 nxt[tid] = rt; pof_n[p] = tid; pof_n[q] = tid;
             }
             __syncthreads();
@@ -390,7 +399,7 @@ __global__ void __launch_bounds__(1024, 1) svd_rows_kernel(int nv, int len, cons
                 for (int o = 16; o > 0; o >>= 1) {
                     al += __shfl_xor_sync(0xffffffffu, al, o); be += __shfl_xor_sync(0xffffffffu, be, o); ga += __shfl_xor_sync(0xffffffffu, ga, o);
                 }
-                if (al * be == 0.0 || fabs(ga) <= tol * sqrt(al) * sqrt(be)) continue;
+                if (al * be == 0.0 || ga * ga <= (tol * tol) * al * be) continue;
                 double c, s; sym_rot(al, be, ga, c, s);
                 for (int i = lane; i < len; i += 32) { double x = wp[i], y = wq[i]; wp[i] = c * x - s * y; wq[i] = s * x + c * y; }
                 double* vp = Va + p * pv; double* vq = Va + q * pv;
@@ -460,6 +469,7 @@ int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work,
         pad_sym_kernel<<<148 * 4, 256, 0, st>>>(n, N, G, Gp, Vu);
         diag_max_kernel<<<1, 256, 0, st>>>(N, Gp, misc, kFloorRel);
         count_launch(2);
+        static const bool verbose = getenv("TATRG_EIGH_VERBOSE") != nullptr;   // debugging aid only
         int sweep = 0;
         for (; sweep < kMaxSweeps; ++sweep) {
             cudaMemsetAsync(counter, 0, sizeof(int), st);
@@ -471,6 +481,7 @@ int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work,
             int rot = 0;
             if (!check(cudaMemcpyAsync(&rot, counter, sizeof(int), cudaMemcpyDeviceToHost, st), err, "eigh readback")) return TATRG_ECUDA;
             if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;
+            if (verbose) fprintf(stderr, "[tatrg eigh n=%d] sweep %d rotations %d\n", n, sweep, rot);
             if (rot == 0) break;
         }
         if (sweep == kMaxSweeps) { if (err) *err = "eigh: block Jacobi did not converge"; return TATRG_ENUMERIC; }
