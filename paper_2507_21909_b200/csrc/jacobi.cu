@@ -39,14 +39,18 @@ __device__ __host__ __forceinline__ void rr_pair(int np, int r, int k, int& p, i
 }
 
 // plane rotation that annihilates a_pq of [[app, apq], [apq, aqq]] with J = [[c, s], [-s, c]]  (J^T A J diagonal):
-// t = tan(theta) is the smaller root of t^2 + 2 zeta t - 1 = 0, zeta = (aqq - app) / (2 apq), written with one sqrt,
-// one division and one rsqrt (FP64 div / sqrt are long software sequences and sit on the critical path of a round).
+// t = tan(theta) is the smaller root of t^2 + 2 zeta t - 1 = 0, zeta = (aqq - app) / (2 apq), evaluated without
+// division or sqrt (FP64 div / sqrt are long software sequences and sit on the critical path of a round).
 __device__ __forceinline__ void sym_rot(double app, double aqq, double apq, double& c, double& s) {
-    const double d = aqq - app;
-    const double r = sqrt(fma(d, d, 4.0 * apq * apq));
-    const double t = (d >= 0 ? 2.0 * apq : -2.0 * apq) / (fabs(d) + r);
-    c = rsqrt(fma(t, t, 1.0));
-    s = c * t;
+    // With d = aqq - app, r = sqrt(d^2 + 4 apq^2), w = r (r + |d|) / 2:  c = (r + |d|) / (2 sqrt(w)),  s = +-apq / sqrt(w)
+    // (tan = s / c = +-2 apq / (|d| + r), the smaller root, and c^2 + s^2 = 1 identically).  Two rsqrt, no division.
+    const double d = aqq - app, ad = fabs(d);
+    const double q2 = fma(d, d, 4.0 * apq * apq);
+    const double r = q2 * rsqrt(q2);
+    const double h = 0.5 * (r + ad);
+    const double inv = rsqrt(r * h);
+    c = h * inv;
+    s = (d >= 0 ? apq : -apq) * inv;
 }
 // rotate only above the relative threshold (no sqrt: compare squares) and above the absolute floor
 __device__ __forceinline__ bool needs_rot(double app, double aqq, double apq, double floor_abs) {
@@ -272,62 +276,62 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
     }
 }
 
-// 64x64x64 product helpers on shared tiles (256 threads, 4x4 outputs each):  acc = A^T B  or  acc = A B
-__device__ __forceinline__ void tile_atb(const double (*A)[SP], const double (*B)[SP], double acc[4][4], int ti, int tj) {
-#pragma unroll 8
-    for (int l = 0; l < SB; ++l) {
-        double a[4], b[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) { a[u] = A[l][ti + u]; b[u] = B[l][tj + u]; }
-#pragma unroll
-        for (int u = 0; u < 4; ++u)
-#pragma unroll
-            for (int v = 0; v < 4; ++v) acc[u][v] += a[u] * b[v];
-    }
+// 64x64x64 tile products on FP64 tensor cores (mma.sync.m8n8k4).  256 threads = 8 warps as 4 (M) x 2 (N); a warp owns
+// a 16 x 32 block = 2 x 4 atoms.  Shared tiles have pitch AP = 68 doubles (= 4 mod 16): the 8-byte fragment loads of a
+// half-warp then hit 16 distinct banks whether the fragment index runs along a row or down a column.
+constexpr int AP = 68;
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
-__device__ __forceinline__ void tile_ab(const double (*A)[SP], const double (*B)[SP], double acc[4][4], int ti, int tj) {
-#pragma unroll 8
-    for (int l = 0; l < SB; ++l) {
-        double a[4], b[4];
+// acc = A^T B (TRANS_A) or A B, for the warp's block at (m0, n0)
+template <bool TRANS_A>
+__device__ __forceinline__ void tile_mma(const double* __restrict__ A, const double* __restrict__ B, double acc[2][4][2], int m0, int n0, int g, int t) {
+#pragma unroll 4
+    for (int k0 = 0; k0 < SB; k0 += 4) {
+        double a[2], b[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { a[u] = A[ti + u][l]; b[u] = B[l][tj + u]; }
+        for (int i = 0; i < 2; ++i) a[i] = TRANS_A ? A[(k0 + t) * AP + m0 + 8 * i + g] : A[(m0 + 8 * i + g) * AP + k0 + t];
 #pragma unroll
-        for (int u = 0; u < 4; ++u)
+        for (int j = 0; j < 4; ++j) b[j] = B[(k0 + t) * AP + n0 + 8 * j + g];
 #pragma unroll
-            for (int v = 0; v < 4; ++v) acc[u][v] += a[u] * b[v];
+        for (int i = 0; i < 2; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
     }
 }
 
 // One launch applies the round's rotations to G (both sides, tile by tile, using the symmetry) and to V^T:
 //   blockIdx.y <  npair : tile (k = blockIdx.y, l = blockIdx.x), k <= l:  G[PQ_k,PQ_l] <- J_k^T G[PQ_k,PQ_l] J_l  (+ mirror)
 //   blockIdx.y >= npair : V^T[PQ_k, 64-column tile blockIdx.x] <- J_k^T V^T[...]
-__global__ void __launch_bounds__(256) blk_apply2_kernel(int N, int nb, int round, double* __restrict__ Gp, double* __restrict__ Vt,
-                                                         const double* __restrict__ Jb, const double* __restrict__ Dg,
-                                                         const int* __restrict__ active) {
+__global__ void __launch_bounds__(256, 2) blk_apply2_kernel(int N, int nb, int round, double* __restrict__ Gp, double* __restrict__ Vt,
+                                                            const double* __restrict__ Jb, const double* __restrict__ Dg,
+                                                            const int* __restrict__ active) {
     extern __shared__ double sh2[];
-    double (*Xs)[SP] = reinterpret_cast<double (*)[SP]>(sh2);
-    double (*Ja)[SP] = reinterpret_cast<double (*)[SP]>(sh2 + SB * SP);
-    double (*Jc)[SP] = reinterpret_cast<double (*)[SP]>(sh2 + 2 * SB * SP);
-    const int npair = nb >> 1, tid = threadIdx.x;
-    const int ti = (tid >> 4) * 4, tj = (tid & 15) * 4;
+    double* Xs = sh2; double* Ja = sh2 + SB * AP; double* Jc = sh2 + 2 * SB * AP;
+    const int npair = nb >> 1, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, t = lane & 3, m0 = (warp >> 1) * 16, n0 = (warp & 1) * 32;
+    double acc[2][4][2];
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
     if ((int)blockIdx.y >= npair) {
         const int k = blockIdx.y - npair;
         if (!active[k]) return;
         int P, Q; rr_pair(nb, round, k, P, Q);
         const int c0 = blockIdx.x * SB;
-        if (c0 >= N) return;
-        for (int e = tid; e < SB * SB; e += 256) {
-            int i = e >> 6, j = e & 63;
-            Xs[i][j] = Vt[(int64_t)gidx(P, Q, i) * N + c0 + j];
-            Ja[i][j] = Jb[(int64_t)k * SB * SB + e];
+        for (int e = tid; e < SB * SB / 2; e += 256) {
+            int i = e >> 5, j = (e & 31) * 2;
+            *reinterpret_cast<double2*>(Xs + i * AP + j) = *reinterpret_cast<const double2*>(Vt + (int64_t)gidx(P, Q, i) * N + c0 + j);
+            *reinterpret_cast<double2*>(Ja + i * AP + j) = *reinterpret_cast<const double2*>(Jb + (int64_t)k * SB * SB + i * SB + j);
         }
         __syncthreads();
-        double acc[4][4] = {};
-        tile_atb(Ja, Xs, acc, ti, tj);
+        tile_mma<true>(Ja, Xs, acc, m0, n0, g, t);
 #pragma unroll
-        for (int u = 0; u < 4; ++u)
+        for (int i = 0; i < 2; ++i)
 #pragma unroll
-            for (int v = 0; v < 4; ++v) Vt[(int64_t)gidx(P, Q, ti + u) * N + c0 + tj + v] = acc[u][v];
+            for (int j = 0; j < 4; ++j)
+                *reinterpret_cast<double2*>(Vt + (int64_t)gidx(P, Q, m0 + 8 * i + g) * N + c0 + n0 + 8 * j + 2 * t) = make_double2(acc[i][j][0], acc[i][j][1]);
         return;
     }
     const int k = blockIdx.y, l = blockIdx.x;
@@ -342,31 +346,46 @@ __global__ void __launch_bounds__(256) blk_apply2_kernel(int N, int nb, int roun
         }
         return;
     }
-    for (int e = tid; e < SB * SB; e += 256) {
-        int i = e >> 6, j = e & 63;
-        Xs[i][j] = Gp[(int64_t)gidx(P, Q, i) * N + gidx(R, S2, j)];
-        Ja[i][j] = ak ? Jb[(int64_t)k * SB * SB + e] : (i == j ? 1.0 : 0.0);
-        Jc[i][j] = al ? Jb[(int64_t)l * SB * SB + e] : (i == j ? 1.0 : 0.0);
+    for (int e = tid; e < SB * SB / 2; e += 256) {
+        int i = e >> 5, j = (e & 31) * 2;      // j, j+1 lie in the same 32-wide block
+        *reinterpret_cast<double2*>(Xs + i * AP + j) = *reinterpret_cast<const double2*>(Gp + (int64_t)gidx(P, Q, i) * N + gidx(R, S2, j));
+        double2 ja = make_double2(i == j ? 1.0 : 0.0, i == j + 1 ? 1.0 : 0.0), jc = ja;
+        if (ak) ja = *reinterpret_cast<const double2*>(Jb + (int64_t)k * SB * SB + i * SB + j);
+        if (al) jc = *reinterpret_cast<const double2*>(Jb + (int64_t)l * SB * SB + i * SB + j);
+        *reinterpret_cast<double2*>(Ja + i * AP + j) = ja;
+        *reinterpret_cast<double2*>(Jc + i * AP + j) = jc;
     }
     __syncthreads();
-    double acc[4][4] = {};
-    tile_atb(Ja, Xs, acc, ti, tj);        // J_k^T X
+    tile_mma<true>(Ja, Xs, acc, m0, n0, g, t);        // J_k^T X
     __syncthreads();
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
+    for (int i = 0; i < 2; ++i)
 #pragma unroll
-        for (int v = 0; v < 4; ++v) Xs[ti + u][tj + v] = acc[u][v];
-    __syncthreads();
-    double acc2[4][4] = {};
-    tile_ab(Xs, Jc, acc2, ti, tj);        // (J_k^T X) J_l
-#pragma unroll
-    for (int u = 0; u < 4; ++u)
-#pragma unroll
-        for (int v = 0; v < 4; ++v) {
-            const int gi = gidx(P, Q, ti + u), gj = gidx(R, S2, tj + v);
-            Gp[(int64_t)gi * N + gj] = acc2[u][v];
-            Gp[(int64_t)gj * N + gi] = acc2[u][v];
+        for (int j = 0; j < 4; ++j) {
+            *reinterpret_cast<double2*>(Xs + (m0 + 8 * i + g) * AP + n0 + 8 * j + 2 * t) = make_double2(acc[i][j][0], acc[i][j][1]);
+            acc[i][j][0] = acc[i][j][1] = 0.0;
         }
+    __syncthreads();
+    tile_mma<false>(Xs, Jc, acc, m0, n0, g, t);       // (J_k^T X) J_l
+    // write the tile, then its mirror through shared memory so that both stores are row-contiguous
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            *reinterpret_cast<double2*>(Gp + (int64_t)gidx(P, Q, m0 + 8 * i + g) * N + gidx(R, S2, n0 + 8 * j + 2 * t)) = make_double2(acc[i][j][0], acc[i][j][1]);
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            Ja[(n0 + 8 * j + 2 * t) * AP + m0 + 8 * i + g] = acc[i][j][0];         // transposed
+            Ja[(n0 + 8 * j + 2 * t + 1) * AP + m0 + 8 * i + g] = acc[i][j][1];
+        }
+    __syncthreads();
+    for (int e = tid; e < SB * SB / 2; e += 256) {
+        int i = e >> 5, j = (e & 31) * 2;
+        *reinterpret_cast<double2*>(Gp + (int64_t)gidx(R, S2, i) * N + gidx(P, Q, j)) = *reinterpret_cast<const double2*>(Ja + i * AP + j);
+    }
 }
 __global__ void extract_diag_kernel(int N, const double* __restrict__ Gp, double* __restrict__ d) {
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) d[i] = Gp[(int64_t)i * N + i];
@@ -429,7 +448,7 @@ bool check(cudaError_t e, std::string* err, const char* what) {
     return false;
 }
 constexpr int kSmallSmem = (2 * SB * SP + 96) * 8 + 3 * 32 * 4 + 64;
-constexpr int kApplySmem = 3 * SB * SP * 8;
+constexpr int kApplySmem = 3 * SB * 68 * 8;
 constexpr int kSolve2Smem = 3 * SB * SP * 8 + 64 * 24 + 32 * 8 + 128 * 4 + 64;
 }  // namespace
 
