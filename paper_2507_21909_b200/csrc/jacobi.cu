@@ -518,6 +518,12 @@ int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work,
     if (!check(gather_vec(st, lam, lam_u, idx, n, 1, 1.0), err, "eigh gather")) return TATRG_ECUDA;
     if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;   // `order` leaves scope
     if (lam_host) { lam_host->resize(n); for (int i = 0; i < n; ++i) (*lam_host)[i] = lh[order[i]]; }
+    if (getenv("TATRG_EIGH_VERBOSE")) {
+        int c[5] = {0, 0, 0, 0, 0}; const double l0 = lh[order[0]]; const double th[5] = {1e-4, 1e-8, 1e-12, 1e-14, 1e-16};
+        for (int i = 0; i < n; ++i) for (int j = 0; j < 5; ++j) if (lh[i] > th[j] * l0) ++c[j];
+        fprintf(stderr, "[tatrg eigh n=%d] spectrum: >1e-4:%d >1e-8:%d >1e-12:%d >1e-14:%d >1e-16:%d  lam[32]/lam0=%.2e lam[64]/lam0=%.2e lam[128]/lam0=%.2e\n", n, c[0], c[1], c[2], c[3], c[4],
+                n > 32 ? lh[order[32]] / l0 : 0.0, n > 64 ? lh[order[64]] / l0 : 0.0, n > 128 ? lh[order[128]] / l0 : 0.0);
+    }
     return TATRG_OK;
 }
 
