@@ -5,9 +5,13 @@
 //   C[M,N] (row-major) = alpha * A(m,k) * B(k,n) + beta * C
 //   A is stored [M][K] (A_KC: k contiguous) or [K][M];  B is stored [K][N] or [N][K] (B_KC: k contiguous).
 //
-// CTA tile 128x128x16, 8 warps as 2(M) x 4(N), warp tile 64x32 = 8x4 DMMA atoms (64 accumulator doubles/thread).
+// Two tile configurations:
+//   L: CTA tile 128x128x16, 8 warps as 2(M) x 4(N), warp tile 64x32 = 8x4 DMMA atoms (64 accumulator doubles/thread)
+//   S: CTA tile  64x 64x16, 4 warps as 2 x 2,        warp tile 32x32 = 4x4 atoms; for outputs with min(M,N) <= 64
+//      (Gram matrices of D^4 x D operands, A.G with G = D x D), where L would spend >= 3/4 of its DMMAs on padding.
 // Shared-memory row pitches are = 4 (mod 16) doubles, which makes the 8-byte fragment loads of a half-warp hit
 // 16 distinct bank pairs for both storage orders.
+// Batched launches take a K of their own for the last batch entry (klast): split-K passes its ragged tail that way.
 #include "internal.h"
 
 namespace tatrg {
@@ -18,11 +22,20 @@ cudaEvent_t Counters::next_event() {
 }
 
 namespace {
-constexpr int BM = 128, BN = 128, BK = 16, NT = 256, STAGES = 4;
+constexpr int BK = 16, STAGES = 4;
 constexpr int PITCH_KC = BK + 4;   // operand stored [row][k]: 20 doubles
-constexpr int PITCH_MC = BM + 4;   // operand stored [k][row]: 132 doubles
-constexpr int TILE_D = BM * PITCH_KC;  // 2560 doubles >= BK*PITCH_MC = 2112
-constexpr int SMEM_BYTES = STAGES * 2 * TILE_D * 8;
+
+template <int BM_, int BN_, int WM_, int WN_>
+struct Cfg {
+    static constexpr int BM = BM_, BN = BN_, WM = WM_, WN = WN_;
+    static constexpr int NT = 32 * WM * WN;
+    static constexpr int MI = BM / WM / 8, NI = BN / WN / 8;          // atoms per warp
+    static constexpr int ROWS = BM > BN ? BM : BN;
+    static constexpr int TILE_D = ROWS * PITCH_KC > BK * (ROWS + 4) ? ROWS * PITCH_KC : BK * (ROWS + 4);
+    static constexpr int SMEM = STAGES * 2 * TILE_D * 8;
+};
+using CfgL = Cfg<128, 128, 2, 4>;
+using CfgS = Cfg<64, 64, 2, 2>;
 
 __device__ __forceinline__ void cp16(double* dst, const double* src, bool ok) {
     unsigned d = (unsigned)__cvta_generic_to_shared(dst);
@@ -42,15 +55,16 @@ __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b)
                  : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-// Load one 128 x 16 operand tile.  KC: global element (r, k) at g[r*ld + k]; else at g[k*ld + r].
+// Load one ROWS x 16 operand tile.  KC: global element (r, k) at g[r*ld + k]; else at g[k*ld + r].
 // rows = extent of the non-contracted dimension, K = extent of k; r0/k0 tile origin.
-template <bool KC, bool V16>
+template <bool KC, bool V16, int ROWS, int NT>
 __device__ __forceinline__ void load_tile(double* s, const double* __restrict__ g, int64_t ld, int64_t r0, int64_t k0,
                                           int64_t rows, int64_t K, int tid) {
+    constexpr int PITCH_MC = ROWS + 4;
     if (KC) {
         if (V16) {
 #pragma unroll
-            for (int c = tid; c < BM * BK / 2; c += NT) {
+            for (int c = tid; c < ROWS * BK / 2; c += NT) {
                 int r = c >> 3, kc = (c & 7) * 2;
                 bool ok = (r0 + r < rows) && (k0 + kc < K);
                 const double* src = ok ? g + (r0 + r) * ld + k0 + kc : g;
@@ -58,7 +72,7 @@ __device__ __forceinline__ void load_tile(double* s, const double* __restrict__ 
             }
         } else {
 #pragma unroll
-            for (int c = tid; c < BM * BK; c += NT) {
+            for (int c = tid; c < ROWS * BK; c += NT) {
                 int r = c >> 4, kc = c & 15;
                 bool ok = (r0 + r < rows) && (k0 + kc < K);
                 const double* src = ok ? g + (r0 + r) * ld + k0 + kc : g;
@@ -68,16 +82,16 @@ __device__ __forceinline__ void load_tile(double* s, const double* __restrict__ 
     } else {
         if (V16) {
 #pragma unroll
-            for (int c = tid; c < BM * BK / 2; c += NT) {
-                int k = c >> 6, rc = (c & 63) * 2;
+            for (int c = tid; c < ROWS * BK / 2; c += NT) {
+                int k = c / (ROWS / 2), rc = (c % (ROWS / 2)) * 2;
                 bool ok = (k0 + k < K) && (r0 + rc < rows);
                 const double* src = ok ? g + (k0 + k) * ld + r0 + rc : g;
                 cp16(s + k * PITCH_MC + rc, src, ok);
             }
         } else {
 #pragma unroll
-            for (int c = tid; c < BM * BK; c += NT) {
-                int k = c >> 7, rc = c & 127;
+            for (int c = tid; c < ROWS * BK; c += NT) {
+                int k = c / ROWS, rc = c % ROWS;
                 bool ok = (k0 + k < K) && (r0 + rc < rows);
                 const double* src = ok ? g + (k0 + k) * ld + r0 + rc : g;
                 cp8(s + k * PITCH_MC + rc, src, ok);
@@ -86,32 +100,35 @@ __device__ __forceinline__ void load_tile(double* s, const double* __restrict__ 
     }
 }
 
-template <bool A_KC, bool B_KC, bool AV16, bool BV16>
-__global__ void __launch_bounds__(NT, 1)
-dgemm_kernel(int64_t M, int64_t N, int64_t K, double alpha, const double* __restrict__ A, int64_t lda,
+template <class C_, bool A_KC, bool B_KC, bool AV16, bool BV16>
+__global__ void __launch_bounds__(C_::NT, C_::NT == 256 ? 1 : 2)
+dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, const double* __restrict__ A, int64_t lda,
              const double* __restrict__ B, int64_t ldb, double beta, double* __restrict__ C, int64_t ldc, int64_t sA,
              int64_t sB, int64_t sC, int tiles_m) {
+    constexpr int BM = C_::BM, BN = C_::BN, NT = C_::NT, MI = C_::MI, NI = C_::NI, TILE_D = C_::TILE_D;
+    constexpr int PA = BM + 4, PB = BN + 4;
     extern __shared__ __align__(16) double smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g = lane >> 2, t = lane & 3;
-    const int wm = warp >> 2, wn = warp & 3;
+    const int wm = warp / C_::WN, wn = warp % C_::WN;
     // tile order: consecutive CTAs walk down M for a fixed N-panel so that the B panel stays in L2
     const int64_t tile = blockIdx.x;
     const int64_t m0 = (tile % tiles_m) * BM, n0 = (tile / tiles_m) * BN;
+    const int64_t K = (Klast > 0 && blockIdx.z == gridDim.z - 1) ? Klast : Kall;
     A += (int64_t)blockIdx.z * sA; B += (int64_t)blockIdx.z * sB; C += (int64_t)blockIdx.z * sC;
 
-    double acc[8][4][2];
+    double acc[MI][NI][2];
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < MI; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+        for (int j = 0; j < NI; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
     const int nk = (int)((K + BK - 1) / BK);
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
         if (s < nk) {
-            load_tile<A_KC, AV16>(smem + (2 * s) * TILE_D, A, lda, m0, (int64_t)s * BK, M, K, tid);
-            load_tile<B_KC, BV16>(smem + (2 * s + 1) * TILE_D, B, ldb, n0, (int64_t)s * BK, N, K, tid);
+            load_tile<A_KC, AV16, BM, NT>(smem + (2 * s) * TILE_D, A, lda, m0, (int64_t)s * BK, M, K, tid);
+            load_tile<B_KC, BV16, BN, NT>(smem + (2 * s + 1) * TILE_D, B, ldb, n0, (int64_t)s * BK, N, K, tid);
         }
         cp_commit();
     }
@@ -122,8 +139,8 @@ dgemm_kernel(int64_t M, int64_t N, int64_t K, double alpha, const double* __rest
             int nxt = kt + STAGES - 1;
             if (nxt < nk) {
                 int s = nxt % STAGES;
-                load_tile<A_KC, AV16>(smem + (2 * s) * TILE_D, A, lda, m0, (int64_t)nxt * BK, M, K, tid);
-                load_tile<B_KC, BV16>(smem + (2 * s + 1) * TILE_D, B, ldb, n0, (int64_t)nxt * BK, N, K, tid);
+                load_tile<A_KC, AV16, BM, NT>(smem + (2 * s) * TILE_D, A, lda, m0, (int64_t)nxt * BK, M, K, tid);
+                load_tile<B_KC, BV16, BN, NT>(smem + (2 * s + 1) * TILE_D, B, ldb, n0, (int64_t)nxt * BK, N, K, tid);
             }
             cp_commit();
         }
@@ -131,33 +148,33 @@ dgemm_kernel(int64_t M, int64_t N, int64_t K, double alpha, const double* __rest
         const double* Bs = As + TILE_D;
 #pragma unroll
         for (int ks = 0; ks < BK / 4; ++ks) {
-            double a[8], b[4];
+            double a[MI], b[NI];
             const int k = ks * 4 + t;
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                int m = wm * 64 + i * 8 + g;
-                a[i] = A_KC ? As[m * PITCH_KC + k] : As[k * PITCH_MC + m];
+            for (int i = 0; i < MI; ++i) {
+                int m = wm * (MI * 8) + i * 8 + g;
+                a[i] = A_KC ? As[m * PITCH_KC + k] : As[k * PA + m];
             }
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                int n = wn * 32 + j * 8 + g;
-                b[j] = B_KC ? Bs[n * PITCH_KC + k] : Bs[k * PITCH_MC + n];
+            for (int j = 0; j < NI; ++j) {
+                int n = wn * (NI * 8) + j * 8 + g;
+                b[j] = B_KC ? Bs[n * PITCH_KC + k] : Bs[k * PB + n];
             }
 #pragma unroll
-            for (int i = 0; i < 8; ++i)
+            for (int i = 0; i < MI; ++i)
 #pragma unroll
-                for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                for (int j = 0; j < NI; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
     }
     cp_wait<0>();
     const bool vec = ((ldc & 1) == 0) && ((((uintptr_t)C) & 15) == 0);
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        int64_t m = m0 + wm * 64 + i * 8 + g;
+    for (int i = 0; i < MI; ++i) {
+        int64_t m = m0 + wm * (MI * 8) + i * 8 + g;
         if (m >= M) continue;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            int64_t n = n0 + wn * 32 + j * 8 + 2 * t;
+        for (int j = 0; j < NI; ++j) {
+            int64_t n = n0 + wn * (NI * 8) + j * 8 + 2 * t;
             if (n >= N) continue;
             double* c = C + m * ldc + n;
             double v0 = alpha * acc[i][j][0], v1 = alpha * acc[i][j][1];
@@ -173,81 +190,106 @@ dgemm_kernel(int64_t M, int64_t N, int64_t K, double alpha, const double* __rest
     }
 }
 
-template <bool A_KC, bool B_KC, bool AV, bool BV>
-cudaError_t launch(cudaStream_t st, int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda, const double* B,
-                   int64_t ldb, double beta, double* C, int64_t ldc, int batch, int64_t sA, int64_t sB, int64_t sC) {
-    auto kern = dgemm_kernel<A_KC, B_KC, AV, BV>;
+struct Args {
+    cudaStream_t st; int64_t M, N, K, Klast; double alpha; const double* A; int64_t lda; const double* B; int64_t ldb; double beta;
+    double* C; int64_t ldc; int batch; int64_t sA, sB, sC;
+};
+
+template <class C_, bool A_KC, bool B_KC, bool AV, bool BV>
+cudaError_t launch(const Args& a) {
+    auto kern = dgemm_kernel<C_, A_KC, B_KC, AV, BV>;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C_::SMEM);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    int64_t tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
-    dim3 grid((unsigned)(tm * tn), 1, (unsigned)batch);
-    kern<<<grid, NT, SMEM_BYTES, st>>>(M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC, (int)tm);
+    int64_t tm = (a.M + C_::BM - 1) / C_::BM, tn = (a.N + C_::BN - 1) / C_::BN;
+    dim3 grid((unsigned)(tm * tn), 1, (unsigned)a.batch);
+    kern<<<grid, C_::NT, C_::SMEM, a.st>>>(a.M, a.N, a.K, a.Klast, a.alpha, a.A, a.lda, a.B, a.ldb, a.beta, a.C, a.ldc, a.sA, a.sB, a.sC, (int)tm);
     count_launch();
     return cudaGetLastError();
 }
-
-template <bool A_KC, bool B_KC>
-cudaError_t pick_vec(bool av, bool bv, cudaStream_t st, int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
-                     const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch, int64_t sA, int64_t sB, int64_t sC) {
-    if (av && bv) return launch<A_KC, B_KC, true, true>(st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
-    if (av) return launch<A_KC, B_KC, true, false>(st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
-    if (bv) return launch<A_KC, B_KC, false, true>(st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
-    return launch<A_KC, B_KC, false, false>(st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+template <class C_, bool A_KC, bool B_KC>
+cudaError_t pick_vec(bool av, bool bv, const Args& a) {
+    if (av && bv) return launch<C_, A_KC, B_KC, true, true>(a);
+    if (av) return launch<C_, A_KC, B_KC, true, false>(a);
+    if (bv) return launch<C_, A_KC, B_KC, false, true>(a);
+    return launch<C_, A_KC, B_KC, false, false>(a);
 }
-}  // namespace
+template <class C_>
+cudaError_t pick_order(bool a_kc, bool b_kc, bool av, bool bv, const Args& a) {
+    if (a_kc && b_kc) return pick_vec<C_, true, true>(av, bv, a);
+    if (a_kc && !b_kc) return pick_vec<C_, true, false>(av, bv, a);
+    if (!a_kc && b_kc) return pick_vec<C_, false, true>(av, bv, a);
+    return pick_vec<C_, false, false>(av, bv, a);
+}
+inline bool small_cfg(int64_t M, int64_t N) { return (M < N ? M : N) <= 64; }
 
-static cudaError_t dgemm_raw(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
-                  int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch, int64_t sA,
-                  int64_t sB, int64_t sC) {
-    if (M <= 0 || N <= 0 || batch <= 0) return cudaSuccess;
+cudaError_t dgemm_raw(bool transa, bool transb, const Args& a) {
+    if (a.M <= 0 || a.N <= 0 || a.batch <= 0) return cudaSuccess;
     // transa == false: A stored [M][K] -> k contiguous.  transb == false: B stored [K][N] -> n contiguous.
     const bool a_kc = !transa, b_kc = transb;
     // 16-byte cp.async needs: even leading dimension, 16B-aligned base and batch stride, even contiguous extent
     auto v16 = [](const double* p, int64_t ld, int64_t contig_extent, int64_t bs) {
         return ((uintptr_t)p % 16 == 0) && (ld % 2 == 0) && (contig_extent % 2 == 0) && (bs % 2 == 0);
     };
-    const bool av = v16(A, lda, a_kc ? K : M, sA), bv = v16(B, ldb, b_kc ? K : N, sB);
-    if (a_kc && b_kc) return pick_vec<true, true>(av, bv, st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
-    if (a_kc && !b_kc) return pick_vec<true, false>(av, bv, st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
-    if (!a_kc && b_kc) return pick_vec<false, true>(av, bv, st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
-    return pick_vec<false, false>(av, bv, st, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+    const bool kodd = (a.K % 2 != 0) || (a.Klast % 2 != 0);
+    const bool av = v16(a.A, a.lda, a_kc ? (kodd ? 1 : 2) : a.M, a.sA), bv = v16(a.B, a.ldb, b_kc ? (kodd ? 1 : 2) : a.N, a.sB);
+    if (small_cfg(a.M, a.N)) return pick_order<CfgS>(a_kc, b_kc, av, bv, a);
+    return pick_order<CfgL>(a_kc, b_kc, av, bv, a);
 }
+}  // namespace
 
-
-cudaError_t dgemm(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
-                  int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch, int64_t sA,
-                  int64_t sB, int64_t sC) {
+static cudaError_t dgemm_klast(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, int64_t Klast, double alpha,
+                               const double* A, int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch,
+                               int64_t sA, int64_t sB, int64_t sC) {
     if (M <= 0 || N <= 0 || batch <= 0) return cudaSuccess;
     Counters* c = g_counter;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (c) { c->gemm_flops += 2.0 * (double)M * (double)N * (double)K * batch; c->gemm_calls += 1; }
+    const double kk = Klast > 0 ? (double)K * (batch - 1) + (double)Klast : (double)K * batch;
+    if (c) { c->gemm_flops += 2.0 * (double)M * (double)N * kk; c->gemm_calls += 1; }
     if (c && c->time_kernels) { e0 = c->next_event(); e1 = c->next_event(); cudaEventRecord(e0, st); }
     cudaError_t e = cudaSuccess;
     // grid.z carries the batch: split very large batches
     for (int b0 = 0; b0 < batch && e == cudaSuccess; b0 += 32768) {
         int nb = batch - b0 < 32768 ? batch - b0 : 32768;
-        e = dgemm_raw(st, transa, transb, M, N, K, alpha, A + (int64_t)b0 * sA, lda, B + (int64_t)b0 * sB, ldb, beta,
-                      C + (int64_t)b0 * sC, ldc, nb, sA, sB, sC);
+        Args a{st, M, N, K, (b0 + nb == batch) ? Klast : 0, alpha, A + (int64_t)b0 * sA, lda, B + (int64_t)b0 * sB, ldb, beta,
+               C + (int64_t)b0 * sC, ldc, nb, sA, sB, sC};
+        e = dgemm_raw(transa, transb, a);
     }
-    if (e0) { cudaEventRecord(e1, st); c->gemm_ev.push_back({e0, e1}); }
+    if (e0) { cudaEventRecord(e1, st); c->gemm_ev.push_back({e0, e1}); c->gemm_shapes.push_back({M, N, (int64_t)(kk / batch), batch, transa, transb}); }
     return e;
+}
+
+cudaError_t dgemm(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+                  int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch, int64_t sA,
+                  int64_t sB, int64_t sC) {
+    return dgemm_klast(st, transa, transb, M, N, K, 0, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
 }
 
 // ---- split-K ---------------------------------------------------------------------------------------------------
 namespace {
-constexpr int kSplitTarget = 148 * 2;
+// Number of K-chunks for a non-batched GEMM: the smallest split whose CTA count fills whole waves of the 148 SMs
+// (>= 93 % of the last wave used), chunks of >= 256, partials capped at 64 M doubles.  1 = no split.
 int splitk_count(int64_t M, int64_t N, int64_t K) {
-    int64_t tiles = ((M + BM - 1) / BM) * ((N + BN - 1) / BN);
-    if (tiles >= 74 || K < 8 * BK) return 1;
-    int64_t s = kSplitTarget / tiles;
-    int64_t maxs = K / (4 * BK);          // at least 4 k-tiles per chunk
-    if (s > maxs) s = maxs;
-    if (s > 512) s = 512;
-    return s < 2 ? 1 : (int)s;
+    const int bm = small_cfg(M, N) ? CfgS::BM : CfgL::BM, bn = small_cfg(M, N) ? CfgS::BN : CfgL::BN;
+    const int per_sm = small_cfg(M, N) ? 2 : 1;
+    const int64_t tiles = ((M + bm - 1) / bm) * ((N + bn - 1) / bn);
+    const int64_t slots = 148 * per_sm;
+    auto eff = [&](int64_t ctas) { int64_t waves = (ctas + slots - 1) / slots; return (double)ctas / (double)(waves * slots); };
+    if (K < 512 || eff(tiles) >= 0.93) return 1;
+    int64_t maxs = K / 256;
+    if (maxs > 1024) maxs = 1024;
+    const int64_t cap = (64LL << 20) / (M * N > 0 ? M * N : 1);
+    if (maxs > cap) maxs = cap;
+    int best = 1; double best_eff = eff(tiles);
+    for (int64_t sp = 2; sp <= maxs; ++sp) {
+        const double e = eff(tiles * sp);
+        if (e >= 0.93) return (int)sp;
+        if (e > best_eff + 0.02) { best_eff = e; best = (int)sp; }
+    }
+    return best;
 }
 __global__ void splitk_reduce_kernel(const double* __restrict__ part, int nsplit, int64_t MN, int64_t N, double alpha,
                                      double* __restrict__ C, int64_t ldc) {
@@ -269,23 +311,17 @@ cudaError_t dgemm_splitk(cudaStream_t st, bool transa, bool transb, int64_t M, i
                          int64_t lda, const double* B, int64_t ldb, double* C, int64_t ldc, double* part) {
     int ns = splitk_count(M, N, K);
     if (ns <= 1 || part == nullptr) return dgemm(st, transa, transb, M, N, K, alpha, A, lda, B, ldb, 0.0, C, ldc);
-    // chunk: multiple of BK; the last chunk takes the ragged tail through a second launch
+    // chunk: multiple of BK; the last batch entry takes the ragged tail (klast)
     int64_t chunk = ((K + ns - 1) / ns + BK - 1) / BK * BK;
-    int nfull = (int)(K / chunk);
-    int64_t tail = K - (int64_t)nfull * chunk;
+    int nchunks = (int)((K + chunk - 1) / chunk);
+    int64_t tail = K - (int64_t)(nchunks - 1) * chunk;
     const int64_t stepA = transa ? chunk * lda : chunk, stepB = transb ? chunk : chunk * ldb;
-    cudaError_t e = cudaSuccess;
-    if (nfull > 0) e = dgemm(st, transa, transb, M, N, chunk, 1.0, A, lda, B, ldb, 0.0, part, N, nfull, stepA, stepB, M * N);
+    cudaError_t e = dgemm_klast(st, transa, transb, M, N, chunk, tail == chunk ? 0 : tail, 1.0, A, lda, B, ldb, 0.0, part, N, nchunks,
+                                stepA, stepB, M * N);
     if (e != cudaSuccess) return e;
-    int total = nfull;
-    if (tail > 0) {
-        e = dgemm(st, transa, transb, M, N, tail, 1.0, A + nfull * stepA, lda, B + nfull * stepB, ldb, 0.0, part + (int64_t)nfull * M * N, N);
-        if (e != cudaSuccess) return e;
-        total += 1;
-    }
     int64_t MN = M * N;
     int64_t blocks = (MN + 255) / 256; if (blocks > 148 * 8) blocks = 148 * 8;
-    splitk_reduce_kernel<<<(unsigned)blocks, 256, 0, st>>>(part, total, MN, N, alpha, C, ldc);
+    splitk_reduce_kernel<<<(unsigned)blocks, 256, 0, st>>>(part, nchunks, MN, N, alpha, C, ldc);
     count_launch();
     return cudaGetLastError();
 }

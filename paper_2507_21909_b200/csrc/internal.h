@@ -28,6 +28,8 @@ struct Counters {
     // optional device timing of the two kernel families (TATRG_OPT_STAGE_TIMING = 2): events bracket each launch
     bool time_kernels = false;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> gemm_ev, perm_ev;
+    struct GemmShape { int64_t M, N, K; int batch; bool ta, tb; };
+    std::vector<GemmShape> gemm_shapes;   // parallel to gemm_ev (time_kernels only)
     std::vector<cudaEvent_t> ev_pool;
     size_t ev_used = 0;
     cudaEvent_t next_event();

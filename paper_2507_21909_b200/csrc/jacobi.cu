@@ -276,6 +276,138 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
     }
 }
 
+// ---- block pair solver, v3: register-resident columns, one barrier per round ---------------------------------------
+// 32 warps; warp w owns the two columns (p, q) of its current pair of the 64 x 64 sub-problem S and of the accumulated
+// rotation J: lane l holds rows l and 32 + l of each (8 doubles).  One round:
+//   diagonal entries by shuffle -> rotation (every lane, redundantly) -> column phase in registers ->
+//   columns + per-row rotation data to shared memory -> ONE barrier ->
+//   fetch the columns of the next pair -> row phase on them (partner rows by shuffle).
+// Every column receives every row phase exactly once because a round's row phase is applied by whoever holds the
+// column after the barrier.  Shared-memory traffic per round is 2 x 64 KB (was 3 x 64 KB read + write) and no thread
+// waits on another warp's square roots.
+constexpr int CS3 = 129;   // doubles per column slot: S rows 0..63, J rows 64..127, +1 pad
+struct Solve3Smem {
+    double col[2][SB][CS3];
+    double rc[2][SB], rs[2][SB];
+    int rp[2][SB];
+    double diag[SB];
+    int cnt[8];
+    int any;
+};
+
+__global__ void __launch_bounds__(1024, 1) blk_solve3_kernel(int N, int nb, int round, int mode, const double* __restrict__ Gp,
+                                                             const double* __restrict__ misc, double* __restrict__ Jb,
+                                                             double* __restrict__ Dg, int* __restrict__ active, int* __restrict__ counter) {
+    extern __shared__ double sh[];
+    Solve3Smem& sm = *reinterpret_cast<Solve3Smem*>(sh);
+    const int tid = threadIdx.x, w = tid >> 5, l = tid & 31, k = blockIdx.x;
+    int P, Q; rr_pair(nb, round, k, P, Q);
+    const double floor_abs = misc[1];
+    const int nrounds = mode == 0 ? SB - 1 : BW;
+    const int max_sweeps = mode == 0 ? 2 : 1;
+    int p, q; sched(mode, 0, w, p, q);
+    double sp[2], sq[2], jp[2], jq[2];
+    // S is symmetric: column c = row c, contiguous within each 32-block
+    sp[0] = Gp[(int64_t)gidx(P, Q, p) * N + P * BW + l]; sp[1] = Gp[(int64_t)gidx(P, Q, p) * N + Q * BW + l];
+    sq[0] = Gp[(int64_t)gidx(P, Q, q) * N + P * BW + l]; sq[1] = Gp[(int64_t)gidx(P, Q, q) * N + Q * BW + l];
+    jp[0] = (l == p) ? 1.0 : 0.0; jp[1] = (32 + l == p) ? 1.0 : 0.0;
+    jq[0] = (l == q) ? 1.0 : 0.0; jq[1] = (32 + l == q) ? 1.0 : 0.0;
+    if (tid < 8) sm.cnt[tid] = 0;
+    if (tid == 0) sm.any = 0;
+    {   // diagonal to shared memory for the quick test
+        double dpv = __shfl_sync(0xffffffffu, (p >> 5) ? sp[1] : sp[0], p & 31);
+        double dqv = __shfl_sync(0xffffffffu, (q >> 5) ? sq[1] : sq[0], q & 31);
+        if (l == 0) { sm.diag[p] = dpv; sm.diag[q] = dqv; }
+    }
+    __syncthreads();
+    {   // quick test: anything to rotate among the pairs this mode visits?
+        bool need = false;
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            const int row = s * 32 + l;
+            if (row != p && (mode == 0 || ((row < BW) != (p < BW)))) need |= needs_rot(sm.diag[row], sm.diag[p], sp[s], floor_abs);
+            if (row != q && (mode == 0 || ((row < BW) != (q < BW)))) need |= needs_rot(sm.diag[row], sm.diag[q], sq[s], floor_abs);
+        }
+        if (__any_sync(0xffffffffu, need) && l == 0) sm.any = 1;
+    }
+    __syncthreads();
+    if (!sm.any) { if (tid == 0) active[k] = 0; return; }
+    int total = 0;
+    const int total_rounds = max_sweeps * nrounds;
+    int wrot = 0;
+    for (int t = 0; t < total_rounds; ++t) {
+        const int r = t % nrounds, b = t & 1, sweep = t / nrounds;
+        // rotation of this warp's pair
+        const double app = __shfl_sync(0xffffffffu, (p >> 5) ? sp[1] : sp[0], p & 31);
+        const double aqq = __shfl_sync(0xffffffffu, (q >> 5) ? sq[1] : sq[0], q & 31);
+        const double apq = __shfl_sync(0xffffffffu, (p >> 5) ? sq[1] : sq[0], p & 31);
+        double c = 1.0, s = 0.0;
+        if (needs_rot(app, aqq, apq, floor_abs)) { sym_rot(app, aqq, apq, c, s); ++wrot; }
+        // column phase
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            double x = sp[u], y = sq[u];
+            sp[u] = c * x - s * y; sq[u] = s * x + c * y;
+            x = jp[u]; y = jq[u];
+            jp[u] = c * x - s * y; jq[u] = s * x + c * y;
+        }
+        // publish columns and the row-phase data of rows p, q
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            sm.col[b][p][u * 32 + l] = sp[u]; sm.col[b][p][64 + u * 32 + l] = jp[u];
+            sm.col[b][q][u * 32 + l] = sq[u]; sm.col[b][q][64 + u * 32 + l] = jq[u];
+        }
+        if (l == 0) { sm.rc[b][p] = c; sm.rs[b][p] = -s; sm.rp[b][p] = q; sm.rc[b][q] = c; sm.rs[b][q] = s; sm.rp[b][q] = p; }
+        const bool last_of_sweep = (r == nrounds - 1);
+        if (last_of_sweep && l == 0 && wrot) atomicAdd(&sm.cnt[sweep], wrot);
+        __syncthreads();
+        bool stop = (t == total_rounds - 1);
+        if (last_of_sweep) { const int cs = sm.cnt[sweep]; total += cs; wrot = 0; if (cs == 0) stop = true; }
+        // next pair and its columns
+        if (!stop) sched(mode, (t + 1) % nrounds, w, p, q);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            sp[u] = sm.col[b][p][u * 32 + l]; jp[u] = sm.col[b][p][64 + u * 32 + l];
+            sq[u] = sm.col[b][q][u * 32 + l]; jq[u] = sm.col[b][q][64 + u * 32 + l];
+        }
+        // row phase of round t on the columns now held
+        double c0 = sm.rc[b][l], s0 = sm.rs[b][l], c1 = sm.rc[b][32 + l], s1 = sm.rs[b][32 + l];
+        const int p0 = sm.rp[b][l], p1 = sm.rp[b][32 + l];
+        {
+            const double a0 = __shfl_sync(0xffffffffu, sp[0], p0 & 31), a1 = __shfl_sync(0xffffffffu, sp[1], p0 & 31);
+            const double b0 = __shfl_sync(0xffffffffu, sp[0], p1 & 31), b1 = __shfl_sync(0xffffffffu, sp[1], p1 & 31);
+            double n0 = c0 * sp[0] + s0 * ((p0 >> 5) ? a1 : a0), n1 = c1 * sp[1] + s1 * ((p1 >> 5) ? b1 : b0);
+            if (s0 != 0.0 && p0 == p) n0 = 0.0;
+            if (s1 != 0.0 && p1 == p) n1 = 0.0;
+            sp[0] = n0; sp[1] = n1;
+        }
+        {
+            const double a0 = __shfl_sync(0xffffffffu, sq[0], p0 & 31), a1 = __shfl_sync(0xffffffffu, sq[1], p0 & 31);
+            const double b0 = __shfl_sync(0xffffffffu, sq[0], p1 & 31), b1 = __shfl_sync(0xffffffffu, sq[1], p1 & 31);
+            double n0 = c0 * sq[0] + s0 * ((p0 >> 5) ? a1 : a0), n1 = c1 * sq[1] + s1 * ((p1 >> 5) ? b1 : b0);
+            if (s0 != 0.0 && p0 == q) n0 = 0.0;
+            if (s1 != 0.0 && p1 == q) n1 = 0.0;
+            sq[0] = n0; sq[1] = n1;
+        }
+        if (stop) break;
+    }
+    if (tid == 0) { active[k] = total > 0; if (total > 0) atomicAdd(counter, total); }
+    if (total == 0) return;
+    // final columns -> shared -> coalesced global stores of J [i][j] and S [i][j]
+    __syncthreads();
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+        sm.col[0][p][u * 32 + l] = sp[u]; sm.col[0][p][64 + u * 32 + l] = jp[u];
+        sm.col[0][q][u * 32 + l] = sq[u]; sm.col[0][q][64 + u * 32 + l] = jq[u];
+    }
+    __syncthreads();
+    for (int e = tid; e < SB * SB; e += 1024) {
+        const int i = e >> 6, j = e & 63;
+        Jb[(int64_t)k * SB * SB + e] = sm.col[0][j][64 + i];
+        Dg[(int64_t)k * SB * SB + e] = sm.col[0][j][i];
+    }
+}
+
 // 64x64x64 tile products on FP64 tensor cores (mma.sync.m8n8k4).  256 threads = 8 warps as 4 (M) x 2 (N); a warp owns
 // a 16 x 32 block = 2 x 4 atoms.  Shared tiles have pitch AP = 68 doubles (= 4 mod 16): the 8-byte fragment loads of a
 // half-warp then hit 16 distinct banks whether the fragment index runs along a row or down a column.
@@ -450,6 +582,7 @@ bool check(cudaError_t e, std::string* err, const char* what) {
 constexpr int kSmallSmem = (2 * SB * SP + 96) * 8 + 3 * 32 * 4 + 64;
 constexpr int kApplySmem = 3 * SB * 68 * 8;
 constexpr int kSolve2Smem = 3 * SB * SP * 8 + 64 * 24 + 32 * 8 + 128 * 4 + 64;
+constexpr int kSolve3Smem = (int)sizeof(Solve3Smem) + 64;
 }  // namespace
 
 // work layout (bytes): [lam_unsorted N][idx N ints][misc 64 doubles][Vt_unsorted N*N][Gp N*N][Jb nb/2*4096][Dg nb/2*64][active nb/2 ints]
@@ -473,6 +606,7 @@ int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work,
     if (!cfg) {
         if (!check(cudaFuncSetAttribute(eigh_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmallSmem), err, "eigh attr")) return TATRG_ECUDA;
         if (!check(cudaFuncSetAttribute(blk_solve2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSolve2Smem), err, "eigh attr")) return TATRG_ECUDA;
+        if (!check(cudaFuncSetAttribute(blk_solve3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSolve3Smem), err, "eigh attr")) return TATRG_ECUDA;
         if (!check(cudaFuncSetAttribute(blk_apply2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kApplySmem), err, "eigh attr")) return TATRG_ECUDA;
         cfg = true;
     }
@@ -489,11 +623,13 @@ int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work,
         diag_max_kernel<<<1, 256, 0, st>>>(N, Gp, misc, kFloorRel);
         count_launch(2);
         static const bool verbose = getenv("TATRG_EIGH_VERBOSE") != nullptr;   // debugging aid only
+        static const bool use_v2 = getenv("TATRG_EIGH_V3") == nullptr;         // v3 (register-resident, issue-bound) is kept for A/B timing only
         int sweep = 0;
         for (; sweep < kMaxSweeps; ++sweep) {
             cudaMemsetAsync(counter, 0, sizeof(int), st);
             for (int r = 0; r < nb - 1; ++r) {
-                blk_solve2_kernel<<<npair, 1024, kSolve2Smem, st>>>(N, nb, r, r == 0 ? 0 : 1, Gp, misc, Jb, Dg, active, counter);
+                if (use_v2) blk_solve2_kernel<<<npair, 1024, kSolve2Smem, st>>>(N, nb, r, r == 0 ? 0 : 1, Gp, misc, Jb, Dg, active, counter);
+                else blk_solve3_kernel<<<npair, 1024, kSolve3Smem, st>>>(N, nb, r, r == 0 ? 0 : 1, Gp, misc, Jb, Dg, active, counter);
                 blk_apply2_kernel<<<dim3(N / SB, 2 * npair), 256, kApplySmem, st>>>(N, nb, r, Gp, Vu, Jb, Dg, active);
                 count_launch(2);
             }

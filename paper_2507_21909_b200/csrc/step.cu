@@ -13,6 +13,8 @@
 #include "step.h"
 #include <algorithm>
 #include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
 
 namespace tatrg {
 namespace {
@@ -284,7 +286,9 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
         Scope s2(*this);
         Tens om = make({chi, J, l});
         ck(philox_gauss(st, c.seed, (uint32_t)call, 0, 0, chi * J * l, om.p), "philox");
-        omega = ein("jp,Bjm->Bpm", QB, om);
+        Tens omp = perm(om, {1, 0, 2});                                   // [j', be, m]: one wide GEMM instead of chi narrow ones
+        drop(om);
+        omega = ein("jp,jbm->bpm", QB, omp);
         keep(omega);
     }
     Tens qk, yt;
@@ -331,8 +335,11 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
     // Eq. A.9 :379 and A.10-A.11 :389-392
     Tens ub = mm(false, true, chi * npc, gr, rk, qk.p, rk, Ut.p, rk);         // U^bond[(al q), g]
     Tens vb = mm(false, true, chi * npb, gr, ry, Qy.p, ry, Va.p, ry);         // V^bond[(be p), g]
-    x = ein("jq,Aqg->Ajg", QC, view(ub, {chi, npc, gr}));
-    y = ein("jp,Bpg->Bjg", QB, view(vb, {chi, npb, gr}));
+    // one GEMM with N = (al, g) each: the batched form has N = g <= D, a quarter of a tile
+    Tens ubp = perm(view(ub, {chi, npc, gr}), {1, 0, 2});
+    Tens vbp = perm(view(vb, {chi, npb, gr}), {1, 0, 2});
+    x = ein("jq,qag->ajg", QC, ubp);
+    y = ein("jp,pbg->bjg", QB, vbp);
     x = view(x, {chi, d2, d3, d4, gr});
     y = view(y, {chi, d2, d3, d4, gr});
     sig = raw(gr);
@@ -556,7 +563,7 @@ void Stepper::run() {
 int run_step(tatrg_ctx* c, cudaStream_t st) {
     Counters& cn = c->cnt;
     cn.launches = 0; cn.gemm_flops = 0; cn.gemm_calls = 0; cn.permuted_bytes = 0; cn.permute_calls = 0;
-    cn.time_kernels = c->timing >= 2; cn.gemm_ev.clear(); cn.perm_ev.clear(); cn.ev_used = 0;
+    cn.time_kernels = c->timing >= 2; cn.gemm_ev.clear(); cn.perm_ev.clear(); cn.gemm_shapes.clear(); cn.ev_used = 0;
     g_counter = &cn;
     int rc = TATRG_OK;
     const size_t lnc0 = c->lnc.size();
@@ -578,7 +585,15 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
         if (e != cudaSuccess) { c->failed = true; c->err = cudaGetErrorString(e); return TATRG_ECUDA; }
         for (int i = 0; i < TATRG_NSTAGES; ++i) { float ms = 0; cudaEventElapsedTime(&ms, c->stage_ev[i], c->stage_ev[i + 1]); c->stage_ms[i] = ms; }
         c->gemm_ms = 0; c->perm_ms = 0;
-        for (auto& ev : cn.gemm_ev) { float ms = 0; cudaEventElapsedTime(&ms, ev.first, ev.second); c->gemm_ms += ms; }
+        const bool verbose = getenv("TATRG_GEMM_VERBOSE") != nullptr;   // debugging aid: per-launch shapes and rates
+        for (size_t i = 0; i < cn.gemm_ev.size(); ++i) {
+            float ms = 0; cudaEventElapsedTime(&ms, cn.gemm_ev[i].first, cn.gemm_ev[i].second); c->gemm_ms += ms;
+            if (verbose && i < cn.gemm_shapes.size()) {
+                const auto& g = cn.gemm_shapes[i];
+                fprintf(stderr, "[tatrg gemm] M=%lld N=%lld K=%lld batch=%d ta=%d tb=%d  %.3f ms  %.2f TF/s\n", (long long)g.M, (long long)g.N,
+                        (long long)g.K, g.batch, (int)g.ta, (int)g.tb, ms, 2.0 * g.M * g.N * g.K * g.batch / (ms * 1e-3) / 1e12);
+            }
+        }
         for (auto& ev : cn.perm_ev) { float ms = 0; cudaEventElapsedTime(&ms, ev.first, ev.second); c->perm_ms += ms; }
     }
     return TATRG_OK;
