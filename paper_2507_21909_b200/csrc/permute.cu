@@ -4,6 +4,7 @@
 // is preserved the copy is coalesced on both sides directly, otherwise a 32x32 (or 64x64) tile goes through
 // padded shared memory so that reads run along the input's innermost leg and writes along the output's.
 #include "internal.h"
+#include <cstdlib>
 
 namespace tatrg {
 namespace {
@@ -52,6 +53,66 @@ __global__ void permute_tiled_kernel(PermArgs a, int64_t extA, int64_t extB, int
         if (ia < extA && ib < extB) out[off_out + ia * soutA + ib] = tile[tx][j];
     }
 }
+
+// innermost leg preserved, vectorised: one warp per "run" = all rows that share every outer index but the last one.
+// A run is ext_last rows of `inner` contiguous doubles, contiguous in the output and strided (sin_last) in the input;
+// the outer index is decoded once per run, lanes then walk the run in 16-byte units.
+__global__ void __launch_bounds__(256) permute_runs_kernel(PermArgs a, int64_t ext_last, int64_t sin_last, int64_t inner, int64_t nruns,
+                                                           int64_t chunk_rows, int64_t chunks, const double* __restrict__ in, double* __restrict__ out) {
+    const int lane = threadIdx.x & 31;
+    const int64_t warps = (int64_t)gridDim.x * (blockDim.x >> 5);
+    const int h = (int)(inner >> 1);                      // 16-byte units per row
+    const int64_t rstride = sin_last >> 1;
+    const int drow = 32 / h, dcol = 32 - drow * h;
+    for (int64_t w = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); w < nruns * chunks; w += warps) {
+        const int64_t run = w / chunks, ch = w - run * chunks;
+        int64_t off_in = 0, r = run;
+#pragma unroll 1
+        for (int d = a.nd - 1; d >= 0; --d) { int64_t q = r / a.ext[d]; int64_t i = r - q * a.ext[d]; r = q; off_in += i * a.sin[d]; }
+        const int64_t row0 = ch * chunk_rows;
+        const int64_t nrows = (ext_last - row0 < chunk_rows) ? ext_last - row0 : chunk_rows;
+        const double2* src = reinterpret_cast<const double2*>(in + off_in + row0 * sin_last);
+        double2* dst = reinterpret_cast<double2*>(out + (run * ext_last + row0) * inner);
+        const int64_t units = nrows * h;
+        int row = lane / h, col = lane - row * h;         // position of unit `lane`
+#pragma unroll 4
+        for (int64_t u = lane; u < units; u += 32) {
+            dst[u] = src[(int64_t)row * rstride + col];
+            row += drow; col += dcol;
+            if (col >= h) { col -= h; ++row; }
+        }
+    }
+}
+
+// general case, vectorised: 64 x 64 tile over (A = input-innermost leg, B = output-innermost leg), 16-byte global
+// accesses on both sides, 8-byte shared-memory accesses with pitch 65.
+__global__ void __launch_bounds__(256) permute_tiled64_kernel(PermArgs a, int64_t extA, int64_t extB, int64_t sinB, int64_t soutA, int64_t tilesA,
+                                                              int64_t tilesB, const double* __restrict__ in, double* __restrict__ out) {
+    __shared__ double tile[64][65];                       // tile[b][a]
+    int64_t blk = blockIdx.x;
+    int64_t ta = blk % tilesA; blk /= tilesA;
+    int64_t tb = blk % tilesB; blk /= tilesB;
+    int64_t off_in = 0, off_out = 0, r = blk;
+#pragma unroll 1
+    for (int d = a.nd - 1; d >= 0; --d) { int64_t q = r / a.ext[d]; int64_t i = r - q * a.ext[d]; r = q; off_in += i * a.sin[d]; off_out += i * a.sout[d]; }
+    const int tid = threadIdx.x, c2 = (tid & 31) * 2, r0 = tid >> 5;       // 32 lanes x 16 B = one 64-double row; 8 rows per pass
+    const int64_t a0 = ta * 64, b0 = tb * 64;
+#pragma unroll
+    for (int j = r0; j < 64; j += 8) {
+        const int64_t ia = a0 + c2, ib = b0 + j;
+        if (ia < extA && ib < extB) {                     // extA even: ia + 1 < extA too
+            const double2 v = *reinterpret_cast<const double2*>(in + off_in + ib * sinB + ia);
+            tile[j][c2] = v.x; tile[j][c2 + 1] = v.y;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = r0; j < 64; j += 8) {
+        const int64_t ia = a0 + j, ib = b0 + c2;
+        if (ia < extA && ib < extB)
+            *reinterpret_cast<double2*>(out + off_out + ia * soutA + ib) = make_double2(tile[c2][j], tile[c2 + 1][j]);
+    }
+}
 }  // namespace
 
 static cudaError_t permute_raw(cudaStream_t st, int nd, const int64_t* dims, const int* perm, const double* in, double* out);
@@ -92,6 +153,20 @@ static cudaError_t permute_raw(cudaStream_t st, int nd, const int64_t* dims, con
         a.nd = m - 1;
         for (int i = 0; i < m - 1; ++i) { a.ext[i] = od[i]; a.sin[i] = sin_o[i]; a.sout[i] = sout_o[i]; }
         int64_t inner = od[m - 1], rows = total / inner;
+        static const int variant = getenv("TATRG_PERMUTE_VARIANT") ? atoi(getenv("TATRG_PERMUTE_VARIANT")) : 3;   // A/B aid: bit 0 runs kernel, bit 1 tiled64
+        const bool al16 = (variant & 1) && (((uintptr_t)in | (uintptr_t)out) & 15) == 0;
+        if (al16 && inner % 2 == 0 && inner / 2 <= 32 * 1024 && m >= 2) {
+            // vectorised: runs over the last outer leg (all input strides are multiples of `inner`, hence even)
+            PermArgs b; b.nd = m - 2;
+            for (int i = 0; i < m - 2; ++i) { b.ext[i] = od[i]; b.sin[i] = sin_o[i]; b.sout[i] = sout_o[i]; }
+            const int64_t ext_last = od[m - 2], nruns = rows / ext_last;
+            int64_t chunk_rows = 1024 / (inner / 2); if (chunk_rows < 1) chunk_rows = 1;      // ~16 KB per warp visit
+            const int64_t chunks = (ext_last + chunk_rows - 1) / chunk_rows;
+            int64_t nb = (nruns * chunks + 7) / 8; if (nb > 148 * 64) nb = 148 * 64;
+            permute_runs_kernel<<<(unsigned)nb, 256, 0, st>>>(b, ext_last, sin_o[m - 2], inner, nruns, chunk_rows, chunks, in, out);
+            count_launch();
+            return cudaGetLastError();
+        }
         int64_t blocks = (total + 255) / 256; if (blocks > 148 * 32) blocks = 148 * 32;
         permute_rows_kernel<<<(unsigned)blocks, 256, 0, st>>>(a, inner, rows, in, out);
         count_launch();
@@ -105,6 +180,18 @@ static cudaError_t permute_raw(cudaStream_t st, int nd, const int64_t* dims, con
     for (int i = 0; i < m; ++i) if (i != ia && i != ib) { a.ext[a.nd] = od[i]; a.sin[a.nd] = sin_o[i]; a.sout[a.nd] = sout_o[i]; ++a.nd; }
     int64_t extA = od[ia], extB = od[ib];
     int64_t outer = total / (extA * extB);
+    {
+        static const int variant2 = getenv("TATRG_PERMUTE_VARIANT") ? atoi(getenv("TATRG_PERMUTE_VARIANT")) : 3;
+        bool even = (variant2 & 2) && (extA % 2 == 0) && (extB % 2 == 0) && (sin_o[ib] % 2 == 0) && (sout_o[ia] % 2 == 0) && ((((uintptr_t)in | (uintptr_t)out) & 15) == 0);
+        for (int i = 0; i < a.nd; ++i) even = even && (a.sin[i] % 2 == 0) && (a.sout[i] % 2 == 0);
+        if (even && extA >= 64 && extB >= 64) {
+            int64_t tA = (extA + 63) / 64, tB = (extB + 63) / 64, nb = tA * tB * outer;
+            if (nb > 0x7fffffffLL) return cudaErrorInvalidValue;
+            permute_tiled64_kernel<<<(unsigned)nb, 256, 0, st>>>(a, extA, extB, sin_o[ib], sout_o[ia], tA, tB, in, out);
+            count_launch();
+            return cudaGetLastError();
+        }
+    }
     const int T = 32;
     int64_t tilesA = (extA + T - 1) / T, tilesB = (extB + T - 1) / T;
     int64_t blocks = tilesA * tilesB * outer;
