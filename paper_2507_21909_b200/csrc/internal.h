@@ -77,6 +77,9 @@ cudaError_t philox_rho(cudaStream_t st, uint64_t seed, uint32_t call, uint32_t s
 //   sorted descending; s[nv], Ut[nv x len], Vacc[nv x nv] (row j = left vector j in the basis of the input rows).
 size_t eigh_work_bytes(int n);
 int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work, std::vector<double>* lam_host, std::string* err);
+struct EighItem { int n; double* G; double* lam; double* Vt; std::vector<double>* lam_host; };
+size_t eigh_batched_work_bytes(int nmax, int count);
+int eigh_batched(cudaStream_t st, int count, const EighItem* items, void* work, std::string* err);
 size_t svd_rows_work_bytes(int nv, int len);
 int svd_rows(cudaStream_t st, int nv, int len, const double* X, double* s, double* Ut, double* Vacc, void* work,
              std::vector<double>* s_host, std::string* err);

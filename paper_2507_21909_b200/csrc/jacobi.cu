@@ -143,7 +143,13 @@ __global__ void __launch_bounds__(512, 1) eigh_small_kernel(int n, const double*
 }
 
 // ---- n > 64: block Jacobi ----------------------------------------------------------------------------------------
-__global__ void pad_sym_kernel(int n, int N, const double* __restrict__ G, double* __restrict__ Gp, double* __restrict__ Vt) {
+constexpr int kMaxBatch = 8;
+struct BatchIn { int n[kMaxBatch]; const double* G[kMaxBatch]; };
+// blockIdx.y = matrix of the batch; every per-matrix array sits at (base + blockIdx.y * wstride)
+__global__ void pad_sym_kernel(BatchIn bin, int N, double* __restrict__ Gp, double* __restrict__ Vt, int64_t wstride) {
+    const int n = bin.n[blockIdx.y];
+    const double* __restrict__ G = bin.G[blockIdx.y];
+    Gp += blockIdx.y * wstride; Vt += blockIdx.y * wstride;
     int64_t total = (int64_t)N * N;
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
         int i = (int)(e / N), j = (int)(e - (int64_t)i * N);
@@ -151,8 +157,9 @@ __global__ void pad_sym_kernel(int n, int N, const double* __restrict__ G, doubl
         Vt[e] = (i == j) ? 1.0 : 0.0;
     }
 }
-__global__ void diag_max_kernel(int N, const double* __restrict__ Gp, double* out, double floor_rel) {   // one block
+__global__ void diag_max_kernel(int N, const double* __restrict__ Gp, double* out, double floor_rel, int64_t wstride) {   // one block per matrix
     __shared__ double red[32];
+    Gp += blockIdx.x * wstride; out += blockIdx.x * wstride;
     double m = 0;
     for (int i = threadIdx.x; i < N; i += blockDim.x) m = fmax(m, fabs(Gp[(int64_t)i * N + i]));
     m = block_max(m, red);
@@ -182,7 +189,10 @@ __device__ __forceinline__ double row_updated(const double* S, const Rot* cur, c
 
 __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int round, int mode, const double* __restrict__ Gp,
                                                              const double* __restrict__ misc, double* __restrict__ Jb,
-                                                             double* __restrict__ Dg, int* __restrict__ active, int* __restrict__ counter) {
+                                                             double* __restrict__ Dg, int* __restrict__ active, int* __restrict__ counter,
+                                                             int64_t wstride) {
+    Gp += blockIdx.y * wstride; misc += blockIdx.y * wstride; Jb += blockIdx.y * wstride; Dg += blockIdx.y * wstride;
+    active += blockIdx.y * wstride * 2;      // wstride counts doubles
     extern __shared__ double sh[];
     double* Sa = sh; double* Sb = Sa + SB * SP; double* J = Sb + SB * SP;
     Rot* rots = reinterpret_cast<Rot*>(J + SB * SP);          // 2 x 32
@@ -276,138 +286,6 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
     }
 }
 
-// ---- block pair solver, v3: register-resident columns, one barrier per round ---------------------------------------
-// 32 warps; warp w owns the two columns (p, q) of its current pair of the 64 x 64 sub-problem S and of the accumulated
-// rotation J: lane l holds rows l and 32 + l of each (8 doubles).  One round:
-//   diagonal entries by shuffle -> rotation (every lane, redundantly) -> column phase in registers ->
-//   columns + per-row rotation data to shared memory -> ONE barrier ->
-//   fetch the columns of the next pair -> row phase on them (partner rows by shuffle).
-// Every column receives every row phase exactly once because a round's row phase is applied by whoever holds the
-// column after the barrier.  Shared-memory traffic per round is 2 x 64 KB (was 3 x 64 KB read + write) and no thread
-// waits on another warp's square roots.
-constexpr int CS3 = 129;   // doubles per column slot: S rows 0..63, J rows 64..127, +1 pad
-struct Solve3Smem {
-    double col[2][SB][CS3];
-    double rc[2][SB], rs[2][SB];
-    int rp[2][SB];
-    double diag[SB];
-    int cnt[8];
-    int any;
-};
-
-__global__ void __launch_bounds__(1024, 1) blk_solve3_kernel(int N, int nb, int round, int mode, const double* __restrict__ Gp,
-                                                             const double* __restrict__ misc, double* __restrict__ Jb,
-                                                             double* __restrict__ Dg, int* __restrict__ active, int* __restrict__ counter) {
-    extern __shared__ double sh[];
-    Solve3Smem& sm = *reinterpret_cast<Solve3Smem*>(sh);
-    const int tid = threadIdx.x, w = tid >> 5, l = tid & 31, k = blockIdx.x;
-    int P, Q; rr_pair(nb, round, k, P, Q);
-    const double floor_abs = misc[1];
-    const int nrounds = mode == 0 ? SB - 1 : BW;
-    const int max_sweeps = mode == 0 ? 2 : 1;
-    int p, q; sched(mode, 0, w, p, q);
-    double sp[2], sq[2], jp[2], jq[2];
-    // S is symmetric: column c = row c, contiguous within each 32-block
-    sp[0] = Gp[(int64_t)gidx(P, Q, p) * N + P * BW + l]; sp[1] = Gp[(int64_t)gidx(P, Q, p) * N + Q * BW + l];
-    sq[0] = Gp[(int64_t)gidx(P, Q, q) * N + P * BW + l]; sq[1] = Gp[(int64_t)gidx(P, Q, q) * N + Q * BW + l];
-    jp[0] = (l == p) ? 1.0 : 0.0; jp[1] = (32 + l == p) ? 1.0 : 0.0;
-    jq[0] = (l == q) ? 1.0 : 0.0; jq[1] = (32 + l == q) ? 1.0 : 0.0;
-    if (tid < 8) sm.cnt[tid] = 0;
-    if (tid == 0) sm.any = 0;
-    {   // diagonal to shared memory for the quick test
-        double dpv = __shfl_sync(0xffffffffu, (p >> 5) ? sp[1] : sp[0], p & 31);
-        double dqv = __shfl_sync(0xffffffffu, (q >> 5) ? sq[1] : sq[0], q & 31);
-        if (l == 0) { sm.diag[p] = dpv; sm.diag[q] = dqv; }
-    }
-    __syncthreads();
-    {   // quick test: anything to rotate among the pairs this mode visits?
-        bool need = false;
-#pragma unroll
-        for (int s = 0; s < 2; ++s) {
-            const int row = s * 32 + l;
-            if (row != p && (mode == 0 || ((row < BW) != (p < BW)))) need |= needs_rot(sm.diag[row], sm.diag[p], sp[s], floor_abs);
-            if (row != q && (mode == 0 || ((row < BW) != (q < BW)))) need |= needs_rot(sm.diag[row], sm.diag[q], sq[s], floor_abs);
-        }
-        if (__any_sync(0xffffffffu, need) && l == 0) sm.any = 1;
-    }
-    __syncthreads();
-    if (!sm.any) { if (tid == 0) active[k] = 0; return; }
-    int total = 0;
-    const int total_rounds = max_sweeps * nrounds;
-    int wrot = 0;
-    for (int t = 0; t < total_rounds; ++t) {
-        const int r = t % nrounds, b = t & 1, sweep = t / nrounds;
-        // rotation of this warp's pair
-        const double app = __shfl_sync(0xffffffffu, (p >> 5) ? sp[1] : sp[0], p & 31);
-        const double aqq = __shfl_sync(0xffffffffu, (q >> 5) ? sq[1] : sq[0], q & 31);
-        const double apq = __shfl_sync(0xffffffffu, (p >> 5) ? sq[1] : sq[0], p & 31);
-        double c = 1.0, s = 0.0;
-        if (needs_rot(app, aqq, apq, floor_abs)) { sym_rot(app, aqq, apq, c, s); ++wrot; }
-        // column phase
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            double x = sp[u], y = sq[u];
-            sp[u] = c * x - s * y; sq[u] = s * x + c * y;
-            x = jp[u]; y = jq[u];
-            jp[u] = c * x - s * y; jq[u] = s * x + c * y;
-        }
-        // publish columns and the row-phase data of rows p, q
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            sm.col[b][p][u * 32 + l] = sp[u]; sm.col[b][p][64 + u * 32 + l] = jp[u];
-            sm.col[b][q][u * 32 + l] = sq[u]; sm.col[b][q][64 + u * 32 + l] = jq[u];
-        }
-        if (l == 0) { sm.rc[b][p] = c; sm.rs[b][p] = -s; sm.rp[b][p] = q; sm.rc[b][q] = c; sm.rs[b][q] = s; sm.rp[b][q] = p; }
-        const bool last_of_sweep = (r == nrounds - 1);
-        if (last_of_sweep && l == 0 && wrot) atomicAdd(&sm.cnt[sweep], wrot);
-        __syncthreads();
-        bool stop = (t == total_rounds - 1);
-        if (last_of_sweep) { const int cs = sm.cnt[sweep]; total += cs; wrot = 0; if (cs == 0) stop = true; }
-        // next pair and its columns
-        if (!stop) sched(mode, (t + 1) % nrounds, w, p, q);
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            sp[u] = sm.col[b][p][u * 32 + l]; jp[u] = sm.col[b][p][64 + u * 32 + l];
-            sq[u] = sm.col[b][q][u * 32 + l]; jq[u] = sm.col[b][q][64 + u * 32 + l];
-        }
-        // row phase of round t on the columns now held
-        double c0 = sm.rc[b][l], s0 = sm.rs[b][l], c1 = sm.rc[b][32 + l], s1 = sm.rs[b][32 + l];
-        const int p0 = sm.rp[b][l], p1 = sm.rp[b][32 + l];
-        {
-            const double a0 = __shfl_sync(0xffffffffu, sp[0], p0 & 31), a1 = __shfl_sync(0xffffffffu, sp[1], p0 & 31);
-            const double b0 = __shfl_sync(0xffffffffu, sp[0], p1 & 31), b1 = __shfl_sync(0xffffffffu, sp[1], p1 & 31);
-            double n0 = c0 * sp[0] + s0 * ((p0 >> 5) ? a1 : a0), n1 = c1 * sp[1] + s1 * ((p1 >> 5) ? b1 : b0);
-            if (s0 != 0.0 && p0 == p) n0 = 0.0;
-            if (s1 != 0.0 && p1 == p) n1 = 0.0;
-            sp[0] = n0; sp[1] = n1;
-        }
-        {
-            const double a0 = __shfl_sync(0xffffffffu, sq[0], p0 & 31), a1 = __shfl_sync(0xffffffffu, sq[1], p0 & 31);
-            const double b0 = __shfl_sync(0xffffffffu, sq[0], p1 & 31), b1 = __shfl_sync(0xffffffffu, sq[1], p1 & 31);
-            double n0 = c0 * sq[0] + s0 * ((p0 >> 5) ? a1 : a0), n1 = c1 * sq[1] + s1 * ((p1 >> 5) ? b1 : b0);
-            if (s0 != 0.0 && p0 == q) n0 = 0.0;
-            if (s1 != 0.0 && p1 == q) n1 = 0.0;
-            sq[0] = n0; sq[1] = n1;
-        }
-        if (stop) break;
-    }
-    if (tid == 0) { active[k] = total > 0; if (total > 0) atomicAdd(counter, total); }
-    if (total == 0) return;
-    // final columns -> shared -> coalesced global stores of J [i][j] and S [i][j]
-    __syncthreads();
-#pragma unroll
-    for (int u = 0; u < 2; ++u) {
-        sm.col[0][p][u * 32 + l] = sp[u]; sm.col[0][p][64 + u * 32 + l] = jp[u];
-        sm.col[0][q][u * 32 + l] = sq[u]; sm.col[0][q][64 + u * 32 + l] = jq[u];
-    }
-    __syncthreads();
-    for (int e = tid; e < SB * SB; e += 1024) {
-        const int i = e >> 6, j = e & 63;
-        Jb[(int64_t)k * SB * SB + e] = sm.col[0][j][64 + i];
-        Dg[(int64_t)k * SB * SB + e] = sm.col[0][j][i];
-    }
-}
-
 // 64x64x64 tile products on FP64 tensor cores (mma.sync.m8n8k4).  256 threads = 8 warps as 4 (M) x 2 (N); a warp owns
 // a 16 x 32 block = 2 x 4 atoms.  Shared tiles have pitch AP = 68 doubles (= 4 mod 16): the 8-byte fragment loads of a
 // half-warp then hit 16 distinct banks whether the fragment index runs along a row or down a column.
@@ -437,7 +315,9 @@ __device__ __forceinline__ void tile_mma(const double* __restrict__ A, const dou
 //   blockIdx.y >= npair : V^T[PQ_k, 64-column tile blockIdx.x] <- J_k^T V^T[...]
 __global__ void __launch_bounds__(256, 2) blk_apply2_kernel(int N, int nb, int round, double* __restrict__ Gp, double* __restrict__ Vt,
                                                             const double* __restrict__ Jb, const double* __restrict__ Dg,
-                                                            const int* __restrict__ active) {
+                                                            const int* __restrict__ active, int64_t wstride) {
+    Gp += blockIdx.z * wstride; Vt += blockIdx.z * wstride; Jb += blockIdx.z * wstride; Dg += blockIdx.z * wstride;
+    active += blockIdx.z * wstride * 2;
     extern __shared__ double sh2[];
     double* Xs = sh2; double* Ja = sh2 + SB * AP; double* Jc = sh2 + 2 * SB * AP;
     const int npair = nb >> 1, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -582,66 +462,22 @@ bool check(cudaError_t e, std::string* err, const char* what) {
 constexpr int kSmallSmem = (2 * SB * SP + 96) * 8 + 3 * 32 * 4 + 64;
 constexpr int kApplySmem = 3 * SB * 68 * 8;
 constexpr int kSolve2Smem = 3 * SB * SP * 8 + 64 * 24 + 32 * 8 + 128 * 4 + 64;
-constexpr int kSolve3Smem = (int)sizeof(Solve3Smem) + 64;
 }  // namespace
 
-// work layout (bytes): [lam_unsorted N][idx N ints][misc 64 doubles][Vt_unsorted N*N][Gp N*N][Jb nb/2*4096][Dg nb/2*64][active nb/2 ints]
 static int padded_n(int n) { if (n <= SB) return n; int nb = (n + BW - 1) / BW; if (nb & 1) ++nb; return nb * BW; }
 
-size_t eigh_work_bytes(int n) {
-    size_t N = (size_t)padded_n(n);
-    size_t nb2 = N / BW / 2 + 1;
-    return 8 * (N + N + 64 + 2 * N * N + 2 * nb2 * SB * SB + nb2) + 4096;
+// per-matrix work layout (doubles): [lam_u N][idx N][misc 64][Vt_unsorted N*N][Gp N*N][Jb npair*4096][Dg npair*4096][active npair]
+static size_t work_doubles(int N) {
+    size_t nb2 = (size_t)N / BW / 2 + 1;
+    size_t d = 2 * (size_t)N + 64 + 2 * (size_t)N * N + 2 * nb2 * SB * SB + nb2;
+    return (d + 63) & ~(size_t)63;
 }
+size_t eigh_work_bytes(int n) { return 8 * work_doubles(padded_n(n)) + 4096; }
+size_t eigh_batched_work_bytes(int nmax, int count) { return 8 * work_doubles(padded_n(nmax)) * (size_t)(count > 0 ? count : 1) + 4096; }
 
-int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work, std::vector<double>* lam_host, std::string* err) {
-    if (n <= 0) return TATRG_OK;
-    const int N = padded_n(n);
-    double* w = (double*)work;
-    double* lam_u = w; w += N;
-    int* idx = (int*)w; w += N;
-    double* misc = w; w += 64;
-    double* Vu = w; w += (size_t)N * N;
-    static bool cfg = false;
-    if (!cfg) {
-        if (!check(cudaFuncSetAttribute(eigh_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmallSmem), err, "eigh attr")) return TATRG_ECUDA;
-        if (!check(cudaFuncSetAttribute(blk_solve2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSolve2Smem), err, "eigh attr")) return TATRG_ECUDA;
-        if (!check(cudaFuncSetAttribute(blk_solve3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSolve3Smem), err, "eigh attr")) return TATRG_ECUDA;
-        if (!check(cudaFuncSetAttribute(blk_apply2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kApplySmem), err, "eigh attr")) return TATRG_ECUDA;
-        cfg = true;
-    }
-    if (n <= SB) {
-        eigh_small_kernel<<<1, 512, kSmallSmem, st>>>(n, G, lam_u, Vu); count_launch();
-    } else {
-        double* Gp = w; w += (size_t)N * N;
-        const int nb = N / BW, npair = nb / 2;
-        double* Jb = w; w += (size_t)npair * SB * SB;
-        double* Dg = w; w += (size_t)npair * SB * SB;
-        int* active = (int*)w; w += npair;     // npair ints fit in npair doubles
-        int* counter = (int*)misc + 8;
-        pad_sym_kernel<<<148 * 4, 256, 0, st>>>(n, N, G, Gp, Vu);
-        diag_max_kernel<<<1, 256, 0, st>>>(N, Gp, misc, kFloorRel);
-        count_launch(2);
-        static const bool verbose = getenv("TATRG_EIGH_VERBOSE") != nullptr;   // debugging aid only
-        static const bool use_v2 = getenv("TATRG_EIGH_V3") == nullptr;         // v3 (register-resident, issue-bound) is kept for A/B timing only
-        int sweep = 0;
-        for (; sweep < kMaxSweeps; ++sweep) {
-            cudaMemsetAsync(counter, 0, sizeof(int), st);
-            for (int r = 0; r < nb - 1; ++r) {
-                if (use_v2) blk_solve2_kernel<<<npair, 1024, kSolve2Smem, st>>>(N, nb, r, r == 0 ? 0 : 1, Gp, misc, Jb, Dg, active, counter);
-                else blk_solve3_kernel<<<npair, 1024, kSolve3Smem, st>>>(N, nb, r, r == 0 ? 0 : 1, Gp, misc, Jb, Dg, active, counter);
-                blk_apply2_kernel<<<dim3(N / SB, 2 * npair), 256, kApplySmem, st>>>(N, nb, r, Gp, Vu, Jb, Dg, active);
-                count_launch(2);
-            }
-            int rot = 0;
-            if (!check(cudaMemcpyAsync(&rot, counter, sizeof(int), cudaMemcpyDeviceToHost, st), err, "eigh readback")) return TATRG_ECUDA;
-            if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;
-            if (verbose) fprintf(stderr, "[tatrg eigh n=%d] sweep %d rotations %d\n", n, sweep, rot);
-            if (rot == 0) break;
-        }
-        if (sweep == kMaxSweeps) { if (err) *err = "eigh: block Jacobi did not converge"; return TATRG_ENUMERIC; }
-        extract_diag_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, Gp, lam_u); count_launch();
-    }
+// sorts one matrix' spectrum on the host and gathers its eigenvectors
+static int finish_one(cudaStream_t st, int n, int N, double* lam_u, int* idx, double* Vu, double* lam, double* Vt, std::vector<double>* lam_host,
+                      std::string* err) {
     std::vector<double> lh(n);
     if (!check(cudaMemcpyAsync(lh.data(), lam_u, sizeof(double) * n, cudaMemcpyDeviceToHost, st), err, "eigh readback")) return TATRG_ECUDA;
     if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;
@@ -657,10 +493,85 @@ int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work,
     if (getenv("TATRG_EIGH_VERBOSE")) {
         int c[5] = {0, 0, 0, 0, 0}; const double l0 = lh[order[0]]; const double th[5] = {1e-4, 1e-8, 1e-12, 1e-14, 1e-16};
         for (int i = 0; i < n; ++i) for (int j = 0; j < 5; ++j) if (lh[i] > th[j] * l0) ++c[j];
-        fprintf(stderr, "[tatrg eigh n=%d] spectrum: >1e-4:%d >1e-8:%d >1e-12:%d >1e-14:%d >1e-16:%d  lam[32]/lam0=%.2e lam[64]/lam0=%.2e lam[128]/lam0=%.2e\n", n, c[0], c[1], c[2], c[3], c[4],
-                n > 32 ? lh[order[32]] / l0 : 0.0, n > 64 ? lh[order[64]] / l0 : 0.0, n > 128 ? lh[order[128]] / l0 : 0.0);
+        fprintf(stderr, "[tatrg eigh n=%d] spectrum: >1e-4:%d >1e-8:%d >1e-12:%d >1e-14:%d >1e-16:%d\n", n, c[0], c[1], c[2], c[3], c[4]);
     }
     return TATRG_OK;
+}
+
+// Eigen-decompositions of up to kMaxBatch independent symmetric matrices in the same launches: the pair solver runs
+// on n/64 CTAs per matrix only, so a batch fills the SMs that a single decomposition leaves idle, and the barrier /
+// launch latency of a round is paid once for the whole batch.  All matrices are padded to the largest one.
+int eigh_batched(cudaStream_t st, int count, const EighItem* items, void* work, std::string* err) {
+    if (count <= 0) return TATRG_OK;
+    static bool cfg = false;
+    if (!cfg) {
+        if (!check(cudaFuncSetAttribute(eigh_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmallSmem), err, "eigh attr")) return TATRG_ECUDA;
+        if (!check(cudaFuncSetAttribute(blk_solve2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSolve2Smem), err, "eigh attr")) return TATRG_ECUDA;
+        if (!check(cudaFuncSetAttribute(blk_apply2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kApplySmem), err, "eigh attr")) return TATRG_ECUDA;
+        cfg = true;
+    }
+    int nmax = 0;
+    for (int i = 0; i < count; ++i) { if (items[i].n <= 0) { if (err) *err = "eigh: empty matrix"; return TATRG_EINVAL; } nmax = std::max(nmax, items[i].n); }
+    const int N = padded_n(nmax);
+    const int64_t ws = (int64_t)work_doubles(N);
+    double* base = (double*)work;
+    auto lam_u = [&](int z) { return base + z * ws; };
+    auto idx = [&](int z) { return (int*)(base + z * ws + N); };
+    auto misc = [&](int z) { return base + z * ws + 2 * (int64_t)N; };
+    auto Vu = [&](int z) { return base + z * ws + 2 * (int64_t)N + 64; };
+    if (nmax <= SB) {
+        for (int z = 0; z < count; ++z) {
+            eigh_small_kernel<<<1, 512, kSmallSmem, st>>>(items[z].n, items[z].G, lam_u(z), Vu(z)); count_launch();
+        }
+        for (int z = 0; z < count; ++z) {
+            int rc = finish_one(st, items[z].n, items[z].n, lam_u(z), idx(z), Vu(z), items[z].lam, items[z].Vt, items[z].lam_host, err);
+            if (rc != TATRG_OK) return rc;
+        }
+        return TATRG_OK;
+    }
+    static const bool verbose = getenv("TATRG_EIGH_VERBOSE") != nullptr;   // debugging aid only
+    const int nb = N / BW, npair = nb / 2;
+    for (int z0 = 0; z0 < count; z0 += kMaxBatch) {
+        const int bc = std::min(kMaxBatch, count - z0);
+        BatchIn bin;
+        for (int z = 0; z < bc; ++z) { bin.n[z] = items[z0 + z].n; bin.G[z] = items[z0 + z].G; }
+        double* Vu0 = Vu(z0); double* Gp0 = Vu0 + (int64_t)N * N;
+        double* Jb0 = Gp0 + (int64_t)N * N; double* Dg0 = Jb0 + (int64_t)npair * SB * SB;
+        int* active0 = (int*)(Dg0 + (int64_t)npair * SB * SB);
+        double* misc0 = misc(z0);
+        int* counter = (int*)misc0 + 8;
+        pad_sym_kernel<<<dim3(148 * 2, bc), 256, 0, st>>>(bin, N, Gp0, Vu0, ws);
+        diag_max_kernel<<<bc, 256, 0, st>>>(N, Gp0, misc0, kFloorRel, ws);
+        count_launch(2);
+        int sweep = 0;
+        for (; sweep < kMaxSweeps; ++sweep) {
+            cudaMemsetAsync(counter, 0, sizeof(int), st);
+            for (int r = 0; r < nb - 1; ++r) {
+                blk_solve2_kernel<<<dim3(npair, bc), 1024, kSolve2Smem, st>>>(N, nb, r, r == 0 ? 0 : 1, Gp0, misc0, Jb0, Dg0, active0, counter, ws);
+                blk_apply2_kernel<<<dim3(N / SB, 2 * npair, bc), 256, kApplySmem, st>>>(N, nb, r, Gp0, Vu0, Jb0, Dg0, active0, ws);
+                count_launch(2);
+            }
+            int rot = 0;
+            if (!check(cudaMemcpyAsync(&rot, counter, sizeof(int), cudaMemcpyDeviceToHost, st), err, "eigh readback")) return TATRG_ECUDA;
+            if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;
+            if (verbose) fprintf(stderr, "[tatrg eigh batch=%d N=%d] sweep %d rotations %d\n", bc, N, sweep, rot);
+            if (rot == 0) break;
+        }
+        if (sweep == kMaxSweeps) { if (err) *err = "eigh: block Jacobi did not converge"; return TATRG_ENUMERIC; }
+        for (int z = 0; z < bc; ++z) { extract_diag_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, Gp0 + z * ws, lam_u(z0 + z)); count_launch(); }
+        for (int z = 0; z < bc; ++z) {
+            const EighItem& it = items[z0 + z];
+            int rc = finish_one(st, it.n, N, lam_u(z0 + z), idx(z0 + z), Vu(z0 + z), it.lam, it.Vt, it.lam_host, err);
+            if (rc != TATRG_OK) return rc;
+        }
+    }
+    return TATRG_OK;
+}
+
+int eigh(cudaStream_t st, int n, double* G, double* lam, double* Vt, void* work, std::vector<double>* lam_host, std::string* err) {
+    if (n <= 0) return TATRG_OK;
+    EighItem it{n, G, lam, Vt, lam_host};
+    return eigh_batched(st, 1, &it, work, err);
 }
 
 size_t svd_rows_work_bytes(int nv, int len) { return 8 * ((size_t)nv * (len + nv + 2)) + 4096; }

@@ -158,6 +158,28 @@ struct Stepper {
         if (rc != TATRG_OK) fail(rc, "%s", e.c_str());
     }
 
+    // the same for several independent matrices in the same launches (jacobi.cu: eigh_batched)
+    struct EigOut { double* lam; Tens Vt; std::vector<double> lh; };
+    void eig_batch(const std::vector<Tens*>& G, const std::vector<int>& n, std::vector<EigOut>& out) {
+        const int cnt = (int)G.size();
+        out.resize(cnt);
+        int nmax = 0;
+        std::vector<EighItem> items(cnt);
+        for (int i = 0; i < cnt; ++i) {
+            out[i].lam = raw(n[i]);
+            out[i].Vt = make({n[i], n[i]});
+            items[i] = EighItem{n[i], G[i]->p, out[i].lam, out[i].Vt.p, &out[i].lh};
+            nmax = std::max(nmax, n[i]);
+        }
+        size_t wb = eigh_batched_work_bytes(nmax, cnt);
+        double* work = c.pool.alloc((int64_t)(wb / 8 + 1));
+        if (!work) fail(TATRG_ENOMEM, "workspace exhausted (batched eigh work, n=%d x %d)", nmax, cnt);
+        std::string e;
+        int rc = eigh_batched(st, cnt, items.data(), work, &e);
+        c.pool.free(work);
+        if (rc != TATRG_OK) fail(rc, "%s", e.c_str());
+    }
+
     // Orthonormal basis of the numerical column space of mat [m x n]:  mat = Q R, Q [m x r], R [r x n]   (R14).
     // Gram matrix -> eigen-decomposition -> Q = mat V lam^-1/2 (directions with lam <= 1e-12 lam_max dropped), and a
     // second identical pass on Q for narrow matrices (n <= 128), where it is cheap, to restore orthogonality to eps.
@@ -187,6 +209,29 @@ struct Stepper {
         keep(Q); keep(R);
     }
 
+    // orth() of two matrices of the same shape with n > 128 (single pass): the two Gram matrices are decomposed together
+    void orth_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2]) {
+        const int64_t m = m0.d[0], n = m0.d[1];
+        if (n <= 128 || m1.d[0] != m || m1.d[1] != n) { orth(m0, Q[0], R[0]); orth(m1, Q[1], R[1]); return; }
+        Scope sc(*this);
+        const Tens* mats[2] = {&m0, &m1};
+        Tens G[2];
+        for (int i = 0; i < 2; ++i) G[i] = mm(true, false, n, n, m, mats[i]->p, n, mats[i]->p, n);
+        std::vector<EigOut> eo;
+        eig_batch({&G[0], &G[1]}, {(int)n, (int)n}, eo);
+        for (int i = 0; i < 2; ++i) {
+            const std::vector<double>& lh = eo[i].lh;
+            if (!(lh[0] > 0)) fail(TATRG_ENUMERIC, "orth: zero matrix");
+            int r = 0;
+            for (double x : lh) if (x > kEpsOrthLambda * lh[0]) ++r;
+            Q[i] = mm(false, true, m, r, n, mats[i]->p, n, eo[i].Vt.p, n);
+            ck(scale_last(st, Q[i].p, Q[i].p, eo[i].lam, m, r, 2), "scale");
+            R[i] = make({r, n});
+            ck(scale_rows(st, R[i].p, eo[i].Vt.p, eo[i].lam, r, n, 3), "scale");
+            keep(Q[i]); keep(R[i]);
+        }
+    }
+
     // R10: block-diagonal gauge rotation Gm (k x k) from wt [k x n] (rows = the vectors to fix) and the multiplet
     // groups of the spectrum v: Cfull = wt rho, per group Q of its MGS-QR.
     Tens gauge(const Tens& wt, bool as_cols, const std::vector<double>& v, int k, uint32_t stream_id) {
@@ -208,7 +253,7 @@ struct Stepper {
     void bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x, Tens& y, double*& sig, int& gr);
     void triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y, const double* sig, Tens U[4], Tens& e, Tens& f, Tens& g, Tens& h);
     void half_grams(const Tens& P, const Tens& Q, const Tens& Iu, const Tens& Jl, Tens th[3]);
-    void squeezer(Tens& thf, Tens& thb, int du, int dl, int dir, Tens& Mt, Tens& Nt);
+    void squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], Tens Nt[3]);
     void run();
 };
 
@@ -269,12 +314,12 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
         Tens b = mm(false, true, F, chi, chi, dt.p, chi, core.p, chi);
         Tens bm = perm(view(b, {d1, J, chi}), {1, 0, 2});              // Eq. A.2 :345  B[(j'),(i1 al)]
         drop(b);
-        orth(view(bm, {J, d1 * chi}), QB, RB);
-        drop(bm);
         Tens cc = mm(false, false, F, chi, chi, a.p, chi, core.p, chi);
         Tens cm = perm(view(cc, {d1, J, chi}), {1, 0, 2});             // Eq. A.3 :348  C[(i'),(i1 be)]
         drop(cc);
-        orth(view(cm, {J, d1 * chi}), QC, RC);
+        Tens Qs[2], Rs[2];
+        orth_pair(view(bm, {J, d1 * chi}), view(cm, {J, d1 * chi}), Qs, Rs);
+        QB = Qs[0]; RB = Rs[0]; QC = Qs[1]; RC = Rs[1];
         keep(QB); keep(RB); keep(QC); keep(RC);
     }
     const int64_t npb = QB.d[1], npc = QC.d[1];
@@ -377,18 +422,21 @@ void Stepper::triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y,
         gram[side == 0 ? 0 : 3] = ga; gram[side == 0 ? 1 : 2] = gx;
         keep(ga); keep(gx);
     }
-    for (int i = 0; i < 4; ++i) {
+    {
         Scope s2(*this);
-        double* lam; Tens Vt; std::vector<double> lh;
-        eig(gram[i], (int)n, lam, Vt, lh);
-        drop(gram[i]);
-        std::vector<double> sv(lh.size());
-        for (size_t j = 0; j < lh.size(); ++j) sv[j] = std::sqrt(std::max(lh[j], 0.0));    // multiplet rule on the singular-value scale
-        const int k = select_rank(sv, std::min<int64_t>(c.Ktri, n), std::sqrt(kEpsLambda), c.tau);
-        if (k <= 0) fail(TATRG_ENUMERIC, "triad: empty isometry");
-        U[i] = make({k, d2, d3});
-        ck(cudaMemcpyAsync(U[i].p, Vt.p, 8 * (int64_t)k * n, cudaMemcpyDeviceToDevice, st), "copy"); count_launch();
-        keep(U[i]);
+        std::vector<EigOut> eo;
+        eig_batch({&gram[0], &gram[1], &gram[2], &gram[3]}, {(int)n, (int)n, (int)n, (int)n}, eo);
+        for (int i = 0; i < 4; ++i) {
+            drop(gram[i]);
+            const std::vector<double>& lh = eo[i].lh;
+            std::vector<double> sv(lh.size());
+            for (size_t j = 0; j < lh.size(); ++j) sv[j] = std::sqrt(std::max(lh[j], 0.0));    // multiplet rule on the singular-value scale
+            const int k = select_rank(sv, std::min<int64_t>(c.Ktri, n), std::sqrt(kEpsLambda), c.tau);
+            if (k <= 0) fail(TATRG_ENUMERIC, "triad: empty isometry");
+            U[i] = make({k, d2, d3});
+            ck(cudaMemcpyAsync(U[i].p, eo[i].Vt.p, 8 * (int64_t)k * n, cudaMemcpyDeviceToDevice, st), "copy"); count_launch();
+            keep(U[i]);
+        }
     }
     e = ein("mjk,Ijkla->Imla", U[0], a);                                   // Eq. 2.10
     Tens f0 = ein("xjk,Ajklg->Axlg", U[1], x);                             // Eq. 2.11 (sigma goes into F only)
@@ -431,42 +479,58 @@ void Stepper::half_grams(const Tens& P, const Tens& Q, const Tens& Iu, const Ten
     for (int i = 0; i < 3; ++i) keep(th[i]);
 }
 
-// (d) squeezer pair of one direction (R6): thf = R1^T R1, thb = R2 R2^T, SVD R1 R2 = U s V^T,
+// (d) squeezer pairs of the three directions (R6): thf = R1^T R1, thb = R2 R2^T, SVD R1 R2 = U s V^T,
 // M = R2 V s^-1/2, N = R1^T U s^-1/2, gauge-fixed (R10).  Returned as rows: Mt[k,u,l], Nt[k,u,l].
-void Stepper::squeezer(Tens& thf, Tens& thb, int du, int dl, int dir, Tens& Mt, Tens& Nt) {
+// The six Gram matrices are eigen-decomposed in one batch, then the three (R1 R2)^T (R1 R2) in another.
+void Stepper::squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], Tens Nt[3]) {
     Scope sc(*this);
-    const int n = du * dl;
-    double *lam1, *lam2; Tens W1, W2; std::vector<double> l1, l2;
-    eig(thf, n, lam1, W1, l1);
-    eig(thb, n, lam2, W2, l2);
-    if (!(l1[0] > 0) || !(l2[0] > 0)) fail(TATRG_ENUMERIC, "squeezer %d: zero Gram matrix", dir);
-    int k1 = 0, k2 = 0;
-    for (double v : l1) if (v > kEpsLambda * l1[0]) ++k1;
-    for (double v : l2) if (v > kEpsLambda * l2[0]) ++k2;
-    Tens r1 = make({k1, n}), r2t = make({k2, n});
-    ck(scale_rows(st, r1.p, W1.p, lam1, k1, n, 3), "scale");       // R1 = Lambda1^1/2 W1^T
-    ck(scale_rows(st, r2t.p, W2.p, lam2, k2, n, 3), "scale");      // R2^T
-    drop(W1); drop(W2);
-    Tens cm = mm(false, true, k1, k2, n, r1.p, n, r2t.p, n);       // R1 R2
-    Tens gc = mm(true, false, k2, k2, k1, cm.p, k2, cm.p, k2);     // (R1 R2)^T (R1 R2): right singular vectors, s^2
-    double* lamc; Tens Vc; std::vector<double> lc;
-    eig(gc, k2, lamc, Vc, lc);
-    std::vector<double> s(lc.size());
-    for (size_t i = 0; i < lc.size(); ++i) s[i] = std::sqrt(std::max(lc[i], 0.0));
-    const int k = select_rank(s, c.D, kEpsSqueezer, c.tau);
-    if (k <= 0) fail(TATRG_ENUMERIC, "squeezer %d: empty", dir);
-    std::vector<double> sk(s.begin(), s.begin() + k);
-    double* sd = to_dev(sk);
-    Tens wt = mm(false, false, k, n, k2, Vc.p, k2, r2t.p, n);      // (R2 V)^T
-    Tens cv = mm(false, true, k, k1, k2, Vc.p, k2, cm.p, k2);      // (R1 R2 V)^T = (U s)^T
-    Tens nt = mm(false, false, k, n, k1, cv.p, k1, r1.p, n);       // (R1^T U s)^T
-    Tens Gm = gauge(wt, false, s, k, (uint32_t)dir);
-    ck(scale_rows(st, wt.p, wt.p, sd, k, n, 2), "scale");          // s^-1/2
-    ck(scale_rows(st, nt.p, nt.p, sd, k, n, 4), "scale");          // s^-3/2
-    Mt = mm(true, false, k, n, k, Gm.p, k, wt.p, n);
-    Nt = mm(true, false, k, n, k, Gm.p, k, nt.p, n);
-    Mt = view(Mt, {k, du, dl}); Nt = view(Nt, {k, du, dl});
-    keep(Mt); keep(Nt);
+    std::vector<EigOut> eo;
+    {
+        std::vector<Tens*> gs; std::vector<int> ns;
+        for (int d = 0; d < 3; ++d) { gs.push_back(&thf[d]); ns.push_back(du[d] * du[d]); gs.push_back(&thb[d]); ns.push_back(du[d] * du[d]); }
+        eig_batch(gs, ns, eo);
+        for (int d = 0; d < 3; ++d) { drop(thf[d]); drop(thb[d]); }
+    }
+    Tens r1[3], r2t[3], cm[3], gc[3];
+    int k1[3], k2[3];
+    for (int d = 0; d < 3; ++d) {
+        const int n = du[d] * du[d];
+        const std::vector<double>&l1 = eo[2 * d].lh, &l2 = eo[2 * d + 1].lh;
+        if (!(l1[0] > 0) || !(l2[0] > 0)) fail(TATRG_ENUMERIC, "squeezer %d: zero Gram matrix", d + 2);
+        k1[d] = k2[d] = 0;
+        for (double v : l1) if (v > kEpsLambda * l1[0]) ++k1[d];
+        for (double v : l2) if (v > kEpsLambda * l2[0]) ++k2[d];
+        r1[d] = make({k1[d], n}); r2t[d] = make({k2[d], n});
+        ck(scale_rows(st, r1[d].p, eo[2 * d].Vt.p, eo[2 * d].lam, k1[d], n, 3), "scale");          // R1 = Lambda1^1/2 W1^T
+        ck(scale_rows(st, r2t[d].p, eo[2 * d + 1].Vt.p, eo[2 * d + 1].lam, k2[d], n, 3), "scale");  // R2^T
+        drop(eo[2 * d].Vt); drop(eo[2 * d + 1].Vt);
+        cm[d] = mm(false, true, k1[d], k2[d], n, r1[d].p, n, r2t[d].p, n);                            // R1 R2
+        gc[d] = mm(true, false, k2[d], k2[d], k1[d], cm[d].p, k2[d], cm[d].p, k2[d]);                 // (R1 R2)^T (R1 R2): V, s^2
+    }
+    std::vector<EigOut> ec;
+    eig_batch({&gc[0], &gc[1], &gc[2]}, {k2[0], k2[1], k2[2]}, ec);
+    for (int d = 0; d < 3; ++d) {
+        const int n = du[d] * du[d], dir = d + 2;
+        drop(gc[d]);
+        const std::vector<double>& lc = ec[d].lh;
+        std::vector<double> s(lc.size());
+        for (size_t i = 0; i < lc.size(); ++i) s[i] = std::sqrt(std::max(lc[i], 0.0));
+        const int k = select_rank(s, c.D, kEpsSqueezer, c.tau);
+        if (k <= 0) fail(TATRG_ENUMERIC, "squeezer %d: empty", dir);
+        std::vector<double> sk(s.begin(), s.begin() + k);
+        double* sd = to_dev(sk);
+        const Tens& Vc = ec[d].Vt;
+        Tens wt = mm(false, false, k, n, k2[d], Vc.p, k2[d], r2t[d].p, n);       // (R2 V)^T
+        Tens cv = mm(false, true, k, k1[d], k2[d], Vc.p, k2[d], cm[d].p, k2[d]); // (R1 R2 V)^T = (U s)^T
+        Tens nt = mm(false, false, k, n, k1[d], cv.p, k1[d], r1[d].p, n);        // (R1^T U s)^T
+        Tens Gm = gauge(wt, false, s, k, (uint32_t)dir);
+        ck(scale_rows(st, wt.p, wt.p, sd, k, n, 2), "scale");                    // s^-1/2
+        ck(scale_rows(st, nt.p, nt.p, sd, k, n, 4), "scale");                    // s^-3/2
+        Mt[d] = mm(true, false, k, n, k, Gm.p, k, wt.p, n);
+        Nt[d] = mm(true, false, k, n, k, Gm.p, k, nt.p, n);
+        Mt[d] = view(Mt[d], {k, du[d], du[d]}); Nt[d] = view(Nt[d], {k, du[d], du[d]});
+        keep(Mt[d]); keep(Nt[d]);
+    }
 }
 
 void Stepper::run() {
@@ -513,10 +577,9 @@ void Stepper::run() {
     }
     mark();
     Tens Mt[3], Nt[3];
-    for (int d = 2; d <= 4; ++d) {
-        const int du = (int)c.phi.d[d - 1], dl = du;
-        squeezer(thf[d - 2], thb[d - 2], du, dl, d, Mt[d - 2], Nt[d - 2]);
-        drop(thf[d - 2]); drop(thb[d - 2]);
+    {
+        const int du[3] = {(int)c.phi.d[1], (int)c.phi.d[2], (int)c.phi.d[3]};
+        squeezers(thf, thb, du, Mt, Nt);
     }
     save("M2", Mt[0]); save("M3", Mt[1]); save("M4", Mt[2]); save("N2", Nt[0]); save("N3", Nt[1]); save("N4", Nt[2]);
     mark();
