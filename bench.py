@@ -135,6 +135,22 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+# ---- replicas-only aggregation -------------------------------------------------------------------
+def max_over_ranks(values, device):
+    """Element-wise maximum of a list of floats over all ranks (identity without a process group)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(values, dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def aggregate_seconds_per_step(ms_max, steps, world):
+    """`world` independent replicas each advance `steps` steps in ms_max milliseconds: whole-job seconds per step."""
+    return ms_max * 1e-3 / (steps * world)
+
+
 # ---- the CUDA path ---------------------------------------------------------------------------------------------------
 def run_cuda(args):
     import torch
@@ -212,14 +228,11 @@ def run_cuda(args):
     t.set_option(T.OPT_STAGE_TIMING, 0)
     dmma = T.dmma_issue_rate(20000, 2)
     # ---- max over ranks ----
-    tm = torch.tensor([ms, ms_e2e], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-    ms, ms_e2e = float(tm[0]), float(tm[1])
+    ms, ms_e2e = max_over_ranks([ms, ms_e2e], "cuda")
     if rank == 0:
         pk = peaks()
-        sec = ms * 1e-3 / (args.steps * world)            # whole-job: `world` replicas advance one step each per step time
-        sec_e2e = ms_e2e * 1e-3 / (k_e2e * world)
+        sec = aggregate_seconds_per_step(ms, args.steps, world)
+        sec_e2e = aggregate_seconds_per_step(ms_e2e, k_e2e, world)
         derived_tf = pk["bf16_sus"] * FP64_TO_BF16_NOMINAL   # kernel timed inside a long step -> sustained figure
         peak_tf = max(derived_tf, dmma)                      # the stricter denominator
         ach_tf = g_fl / (g_ms * 1e-3) / 1e12
