@@ -178,15 +178,22 @@ __device__ __forceinline__ void sched(int mode, int r, int k, int& p, int& q) {
 }
 struct Rot { double c, s; int p, q; };
 
-// S value after the row phase of the current round, computed from the column-updated buffer (read-only here)
-__device__ __forceinline__ double row_updated(const double* S, const Rot* cur, const int* pair_of, int a, int b) {
-    const Rot rt = cur[pair_of[a]];
-    if (rt.s == 0.0) return S[a * SP + b];
-    if ((a == rt.p && b == rt.q) || (a == rt.q && b == rt.p)) return 0.0;
-    const double x = S[rt.p * SP + b], y = S[rt.q * SP + b];
-    return a == rt.p ? rt.c * x - rt.s * y : rt.s * x + rt.c * y;
+// entry (a, b) of R^T S R for the round's direct sum of plane rotations R, from the un-rotated S (read-only here)
+__device__ __forceinline__ double rotated_entry(const double* S, const Rot* cur, const int* pair_of, int a, int b) {
+    const Rot ra = cur[pair_of[a]], rb = cur[pair_of[b]];
+    if (ra.s != 0.0 && ra.p == rb.p && a != b) return 0.0;            // the annihilated pair entry
+    const double wap = (a == ra.p) ? ra.c : ra.s, waq = (a == ra.p) ? -ra.s : ra.c;
+    const double wbp = (b == rb.p) ? rb.c : rb.s, wbq = (b == rb.p) ? -rb.s : rb.c;
+    const double top = wbp * S[ra.p * SP + rb.p] + wbq * S[ra.p * SP + rb.q];
+    const double bot = wbp * S[ra.q * SP + rb.p] + wbq * S[ra.q * SP + rb.q];
+    return wap * top + waq * bot;
 }
 
+// One CTA (1024 threads) per block pair.  A round costs ONE barrier:
+//   every thread owns one 2x2 block (row pair k1 = warp, column pair k2 = lane) and writes R_k1^T S_block R_k2 into the
+//   second buffer (both sides of the two-sided update in one pass over S);
+//   then warp 0 derives the next round's rotations from the OLD buffer (rotated_entry) while warps 1..31 rotate the
+//   columns of the accumulated J in place.  None of the three touches data another one writes.
 __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int round, int mode, const double* __restrict__ Gp,
                                                              const double* __restrict__ misc, double* __restrict__ Jb,
                                                              double* __restrict__ Dg, int* __restrict__ active, int* __restrict__ counter,
@@ -199,7 +206,7 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
     double* red = reinterpret_cast<double*>(rots + 64);       // 32
     int* pair_of = reinterpret_cast<int*>(red + 32);          // 2 x 64
     int* cnt = pair_of + 128;
-    const int tid = threadIdx.x, k = blockIdx.x;
+    const int tid = threadIdx.x, k = blockIdx.x, warp = tid >> 5, lane = tid & 31;
     int P, Q; rr_pair(nb, round, k, P, Q);
     for (int e = tid; e < SB * SB; e += 1024) {
         int i = e >> 6, j = e & 63;
@@ -230,48 +237,48 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
             int p, q; sched(mode, 0, tid, p, q);
             Rot rt; rt.c = 1.0; rt.s = 0.0; rt.p = p; rt.q = q;
             double app = S[p * SP + p], aqq = S[q * SP + q], apq = S[p * SP + q];
-            if (needs_rot(app, aqq, apq, floor_abs)) { sym_rot(app, aqq, apq, rt.c, rt.s); atomicAdd(cnt, 1); }
+            const bool need = needs_rot(app, aqq, apq, floor_abs);
+            if (need) sym_rot(app, aqq, apq, rt.c, rt.s);
+            const int nrot = __popc(__ballot_sync(0xffffffffu, need));
+            if (tid == 0) *cnt += nrot;
             rots[tid] = rt; pair_of[p] = tid; pair_of[q] = tid;
         }
         __syncthreads();
         for (int r = 0; r < nrounds; ++r) {
             const Rot* cur = rots + (r & 1) * 32; Rot* nxt = rots + ((r + 1) & 1) * 32;
             const int* pof = pair_of + (r & 1) * 64; int* pof_n = pair_of + ((r + 1) & 1) * 64;
-            // columns of S and J, in place
-#pragma unroll
-            for (int it = 0; it < 2; ++it) {
-                const int e = tid + it * 1024, kk = e >> 6, i = e & 63;
-                const Rot rt = cur[kk];
-                if (rt.s != 0.0) {
-                    double x = S[i * SP + rt.p], y = S[i * SP + rt.q];
-                    S[i * SP + rt.p] = rt.c * x - rt.s * y; S[i * SP + rt.q] = rt.s * x + rt.c * y;
-                    x = J[i * SP + rt.p]; y = J[i * SP + rt.q];
-                    J[i * SP + rt.p] = rt.c * x - rt.s * y; J[i * SP + rt.q] = rt.s * x + rt.c * y;
+            {   // two-sided update of the 2x2 block (row pair = warp, column pair = lane): S -> T
+                const Rot r1 = cur[warp], r2 = cur[lane];
+                const double a = S[r1.p * SP + r2.p], b = S[r1.p * SP + r2.q], c_ = S[r1.q * SP + r2.p], d = S[r1.q * SP + r2.q];
+                const double a1 = r2.c * a - r2.s * b, b1 = r2.s * a + r2.c * b, c1 = r2.c * c_ - r2.s * d, d1 = r2.s * c_ + r2.c * d;
+                double A = r1.c * a1 - r1.s * c1, C = r1.s * a1 + r1.c * c1, B = r1.c * b1 - r1.s * d1, D = r1.s * b1 + r1.c * d1;
+                if (warp == lane && r1.s != 0.0) { B = 0.0; C = 0.0; }      // the rotation annihilates s_pq exactly
+                T[r1.p * SP + r2.p] = A; T[r1.p * SP + r2.q] = B; T[r1.q * SP + r2.p] = C; T[r1.q * SP + r2.q] = D;
+            }
+            if (warp == 0) {
+                if (r + 1 < nrounds) {      // next round's rotations, from the old buffer
+                    int p, q; sched(mode, r + 1, lane, p, q);
+                    Rot rt; rt.c = 1.0; rt.s = 0.0; rt.p = p; rt.q = q;
+                    const double app = rotated_entry(S, cur, pof, p, p), aqq = rotated_entry(S, cur, pof, q, q), apq = rotated_entry(S, cur, pof, p, q);
+                    const bool need = needs_rot(app, aqq, apq, floor_abs);
+                    if (need) sym_rot(app, aqq, apq, rt.c, rt.s);
+                    const int nrot = __popc(__ballot_sync(0xffffffffu, need));
+                    if (lane == 0) *cnt += nrot;
+                    nxt[lane] = rt; pof_n[p] = lane; pof_n[q] = lane;
                 }
-            }
-            __syncthreads();
-            // rows: S -> T (every row belongs to exactly one pair, so T is written completely)
-#pragma unroll
-            for (int it = 0; it < 2; ++it) {
-                const int e = tid + it * 1024, kk = e >> 6, j = e & 63;
-                const Rot rt = cur[kk];
-                double x = S[rt.p * SP + j], y = S[rt.q * SP + j];
-                double xn = x, yn = y;
-                if (rt.s != 0.0) { xn = rt.c * x - rt.s * y; yn = rt.s * x + rt.c * y; if (j == rt.q) xn = 0.0; if (j == rt.p) yn = 0.0; }
-                T[rt.p * SP + j] = xn; T[rt.q * SP + j] = yn;
-            }
-            // meanwhile the first warp prepares the next round from the row-updated values it derives itself
-            if (tid < 32 && r + 1 < nrounds) {
-                int p, q; sched(mode, r + 1, tid, p, q);
-                Rot rt; rt.c = 1.0; rt.s = 0.0; rt.p = p; rt.q = q;
-                double app = row_updated(S, cur, pof, p, p), aqq = row_updated(S, cur, pof, q, q), apq = row_updated(S, cur, pof, p, q);
-                if (needs_rot(app, aqq, apq, floor_abs)) { sym_rot(app, aqq, apq, rt.c, rt.s); atomicAdd(cnt, 1); }
-                nxt[tid] = rt; pof_n[p] = tid; pof_n[q] = tid;
+            } else {                        // columns of J, in place
+                for (int e = tid - 32; e < SB * 32; e += 1024 - 32) {
+                    const int kk = e >> 6, i = e & 63;
+                    const Rot rt = cur[kk];
+                    if (rt.s != 0.0) {
+                        const double x = J[i * SP + rt.p], y = J[i * SP + rt.q];
+                        J[i * SP + rt.p] = rt.c * x - rt.s * y; J[i * SP + rt.q] = rt.s * x + rt.c * y;
+                    }
+                }
             }
             __syncthreads();
             double* tmp = S; S = T; T = tmp;
         }
-        // the Rot/pair_of buffers of round 0 of the next sweep are rewritten above: parity of nrounds does not matter
         const int c = *cnt;
         __syncthreads();
         if (tid == 0) *cnt = 0;
