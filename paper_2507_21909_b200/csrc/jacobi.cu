@@ -190,10 +190,10 @@ __device__ __forceinline__ double rotated_entry(const double* S, const Rot* cur,
 }
 
 // One CTA (1024 threads) per block pair.  A round costs ONE barrier:
-//   every thread owns one 2x2 block (row pair k1 = warp, column pair k2 = lane) and writes R_k1^T S_block R_k2 into the
-//   second buffer (both sides of the two-sided update in one pass over S);
-//   then warp 0 derives the next round's rotations from the OLD buffer (rotated_entry) while warps 1..31 rotate the
-//   columns of the accumulated J in place.  None of the three touches data another one writes.
+//   warps 1..31 write R_k1^T S_block R_k2 for the 32 x 32 blocks of 2 x 2 entries (row pair k1, column pair k2) into the
+//   second buffer (both sides of the two-sided update in one pass over S) and then rotate the columns of the
+//   accumulated J in place, while warp 0 derives the next round's rotations from the OLD buffer (rotated_entry).
+//   None of the three touches data another one writes.
 __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int round, int mode, const double* __restrict__ Gp,
                                                              const double* __restrict__ misc, double* __restrict__ Jb,
                                                              double* __restrict__ Dg, int* __restrict__ active, int* __restrict__ counter,
@@ -247,13 +247,18 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
         for (int r = 0; r < nrounds; ++r) {
             const Rot* cur = rots + (r & 1) * 32; Rot* nxt = rots + ((r + 1) & 1) * 32;
             const int* pof = pair_of + (r & 1) * 64; int* pof_n = pair_of + ((r + 1) & 1) * 64;
-            {   // two-sided update of the 2x2 block (row pair = warp, column pair = lane): S -> T
-                const Rot r1 = cur[warp], r2 = cur[lane];
-                const double a = S[r1.p * SP + r2.p], b = S[r1.p * SP + r2.q], c_ = S[r1.q * SP + r2.p], d = S[r1.q * SP + r2.q];
-                const double a1 = r2.c * a - r2.s * b, b1 = r2.s * a + r2.c * b, c1 = r2.c * c_ - r2.s * d, d1 = r2.s * c_ + r2.c * d;
-                double A = r1.c * a1 - r1.s * c1, C = r1.s * a1 + r1.c * c1, B = r1.c * b1 - r1.s * d1, D = r1.s * b1 + r1.c * d1;
-                if (warp == lane && r1.s != 0.0) { B = 0.0; C = 0.0; }      // the rotation annihilates s_pq exactly
-                T[r1.p * SP + r2.p] = A; T[r1.p * SP + r2.q] = B; T[r1.q * SP + r2.p] = C; T[r1.q * SP + r2.q] = D;
+            // two-sided update of the 2x2 blocks (row pair k1, column pair k2): S -> T.  Warp 0 is kept free for the
+            // rotation arithmetic (the longest dependent chain of a round); its 32 blocks go to the first 32 other threads.
+            if (warp != 0) {
+                for (int bidx = tid - 32; bidx < 32 * 32; bidx += 1024 - 32) {
+                    const int k1 = bidx >> 5, k2 = bidx & 31;
+                    const Rot r1 = cur[k1], r2 = cur[k2];
+                    const double a = S[r1.p * SP + r2.p], b = S[r1.p * SP + r2.q], c_ = S[r1.q * SP + r2.p], d = S[r1.q * SP + r2.q];
+                    const double a1 = r2.c * a - r2.s * b, b1 = r2.s * a + r2.c * b, c1 = r2.c * c_ - r2.s * d, d1 = r2.s * c_ + r2.c * d;
+                    double A = r1.c * a1 - r1.s * c1, C = r1.s * a1 + r1.c * c1, B = r1.c * b1 - r1.s * d1, D = r1.s * b1 + r1.c * d1;
+                    if (k1 == k2 && r1.s != 0.0) { B = 0.0; C = 0.0; }      // the rotation annihilates s_pq exactly
+                    T[r1.p * SP + r2.p] = A; T[r1.p * SP + r2.q] = B; T[r1.q * SP + r2.p] = C; T[r1.q * SP + r2.q] = D;
+                }
             }
             if (warp == 0) {
                 if (r + 1 < nrounds) {      // next round's rotations, from the old buffer
