@@ -56,6 +56,12 @@ __device__ __forceinline__ void sym_rot(double app, double aqq, double apq, doub
 __device__ __forceinline__ bool needs_rot(double app, double aqq, double apq, double floor_abs) {
     return fabs(apq) > floor_abs && apq * apq > (kTolRel * kTolRel) * fabs(app * aqq);
 }
+// A rotation counts against convergence of the block method only above 10 x that threshold: the 64-term tile products
+// that apply the rotations leave rounding of a few ulp of sqrt(a_pp a_qq) in a_pq, which inside a cluster of nearly equal
+// eigenvalues keeps triggering (harmless, 45-degree) rotations at 1e-15 for ever (seen at n = 2304).
+__device__ __forceinline__ bool significant_rot(double app, double aqq, double apq, double floor_abs) {
+    return fabs(apq) > floor_abs && apq * apq > (100.0 * kTolRel * kTolRel) * fabs(app * aqq);
+}
 
 // Two-sided Jacobi on the n x n symmetric S (shared, pitch SP), accumulating J (S_out = J^T S_in J, columns of J).
 // All threads of the CTA call it.  Returns the number of rotations applied.
@@ -213,7 +219,7 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
         Sa[i * SP + j] = Gp[(int64_t)gidx(P, Q, i) * N + gidx(P, Q, j)];
         J[i * SP + j] = (i == j) ? 1.0 : 0.0;
     }
-    if (tid == 0) *cnt = 0;
+    if (tid == 0) { cnt[0] = 0; cnt[1] = 0; }
     __syncthreads();
     const double floor_abs = misc[1];
     // quick test: anything to rotate among the pairs this mode visits?
@@ -230,7 +236,7 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
     const int nrounds = mode == 0 ? SB - 1 : BW;
     const int max_sweeps = mode == 0 ? 2 : 1;
     double* S = Sa; double* T = Sb;
-    int total = 0;
+    int total = 0, total_sig = 0;
     for (int sweep = 0; sweep < max_sweeps; ++sweep) {
         // rotations of round 0 from the current S
         if (tid < 32) {
@@ -240,7 +246,8 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
             const bool need = needs_rot(app, aqq, apq, floor_abs);
             if (need) sym_rot(app, aqq, apq, rt.c, rt.s);
             const int nrot = __popc(__ballot_sync(0xffffffffu, need));
-            if (tid == 0) *cnt += nrot;
+            const int nsig = __popc(__ballot_sync(0xffffffffu, need && significant_rot(app, aqq, apq, floor_abs)));
+            if (tid == 0) { cnt[0] += nrot; cnt[1] += nsig; }
             rots[tid] = rt; pair_of[p] = tid; pair_of[q] = tid;
         }
         __syncthreads();
@@ -268,7 +275,8 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
                     const bool need = needs_rot(app, aqq, apq, floor_abs);
                     if (need) sym_rot(app, aqq, apq, rt.c, rt.s);
                     const int nrot = __popc(__ballot_sync(0xffffffffu, need));
-                    if (lane == 0) *cnt += nrot;
+                    const int nsig = __popc(__ballot_sync(0xffffffffu, need && significant_rot(app, aqq, apq, floor_abs)));
+                    if (lane == 0) { cnt[0] += nrot; cnt[1] += nsig; }
                     nxt[lane] = rt; pof_n[p] = lane; pof_n[q] = lane;
                 }
             } else {                        // columns of J, in place
@@ -284,14 +292,14 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
             __syncthreads();
             double* tmp = S; S = T; T = tmp;
         }
-        const int c = *cnt;
+        const int c = cnt[0], cs = cnt[1];
         __syncthreads();
-        if (tid == 0) *cnt = 0;
-        total += c;
+        if (tid == 0) { cnt[0] = 0; cnt[1] = 0; }
+        total += c; total_sig += cs;
         if (c == 0) break;
         __syncthreads();
     }
-    if (tid == 0) { active[k] = total > 0; if (total > 0) atomicAdd(counter, total); }
+    if (tid == 0) { active[k] = total > 0; if (total_sig > 0) atomicAdd(counter, total_sig); }
     if (total > 0) {
         for (int e = tid; e < SB * SB; e += 1024) { int i = e >> 6, j = e & 63; Jb[(int64_t)k * SB * SB + e] = J[i * SP + j]; }
         for (int e = tid; e < SB * SB; e += 1024) { int i = e >> 6, j = e & 63; Dg[(int64_t)k * SB * SB + e] = S[i * SP + j]; }

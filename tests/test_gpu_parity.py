@@ -232,3 +232,25 @@ def test_d32_stage_properties_and_sampled_contraction():
         slab = O.contract_half(e[i1:i1 + 1], f, tu(ua), tu(ux), tr(m2), tr(m3), tr(m4))[0]     # [k2,k3,k4,g]
         got = phi[:, :, :, i1, :]
         assert np.abs(got - slab).max() <= 1e-11 * max(1.0, np.abs(slab).max())
+
+
+def test_config5_d48_runs_and_improves_on_d32():
+    """BASELINE.json configs[4], Triad half (D=48, p=48, K=96, seed 99): the largest size; n = 2304 eigen-problems.
+    No oracle value exists at this size (a saturated oracle step would take hours): properties only --
+    workspace bound, isometry of A, ordered positive spectrum, and ln Z/V above the D=32 value after the same number
+    of steps (the free energy decreases monotonically with D, Fig. 9 :286-288)."""
+    t48 = T.Tatrg(0.1497, 0.0, 48, 48, 99)
+    t48.set_option(T.OPT_KEEP_TENSORS, 1)
+    t32 = T.Tatrg(0.1497, 0.0, 32, 32, 99)
+    for _ in range(6):
+        t48.step()
+        t32.step()
+    assert t48.workspace_peak() <= T.workspace_bytes(48, 48)
+    a = t48.get_tensor("A")
+    assert a.shape == (48, 48, 48, 48, 48)
+    am = a.reshape(-1, 48)
+    assert np.abs(am.T @ am - np.eye(48)).max() <= 1e-10
+    sig = t48.singular_values(T.SV_SIGMA, 48)
+    assert len(sig) == 48 and np.all(np.diff(sig) <= 0) and sig[-1] > 0
+    z48, z32 = t48.lnZ_per_site(), t32.lnZ_per_site()
+    assert np.isfinite(z48) and z48 > z32 and z48 - z32 < 5e-3
