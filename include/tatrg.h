@@ -67,6 +67,10 @@ double tatrg_lnZ_per_site(tatrg_handle);
  * out_host [host].  Returns the number written or < 0. */
 int tatrg_singular_values(tatrg_handle, int which, int k, double* out_host);
 
+/* X ratio of the current tensor, Eq. 3.3 (:298-303): X = (Tr A)^2 / Tr A^2, A[k,l] = sum T[i1 i2 i3 k, i1 i2 i3 l]; 2 in the
+ * ordered phase, 1 in the disordered one.  One contraction on cuda_stream, synchronises.  x_out [host]. */
+int tatrg_x_ratio(tatrg_handle, void* cuda_stream, double* x_out);
+
 int tatrg_steps_done(tatrg_handle);
 const char* tatrg_last_error(tatrg_handle);
 void tatrg_destroy(tatrg_handle); /* frees the host struct only */

@@ -420,6 +420,16 @@ class TatrgOracle:
     def singular_values(self, which="sigma"):
         return self.last[which]
 
+    def x_ratio(self):
+        return x_ratio(self.phi, self.psi)
+
+
+def x_ratio(phi, psi):
+    """Eq. 3.3 :298-303 (Gu-Wen ratio): X = (Tr A)^2 / Tr A^2 with A[k,l] = sum T[i1 i2 i3 k, i1 i2 i3 l], written on the
+    factored tensor T[f,b] = sum_g Phi[f,g] Psi[b,g].  X counts the ground-state degeneracy: 2 ordered, 1 disordered."""
+    a = _es("ijkag,ijkbg->ab", phi, psi)
+    return float(np.trace(a) ** 2 / np.trace(a @ a))
+
 
 def squeezer_grams_lower(gs, h, k_, l_, direction):
     """Gram of the lower half  L[g,j1,(j2u j2l),(j3u j3l),(j4u j4l)] =

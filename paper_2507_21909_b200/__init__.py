@@ -30,6 +30,7 @@ _SIGNATURES = {
     "tatrg_step": (_c.c_int, [_c.c_void_p, _c.c_void_p]),
     "tatrg_lnZ_per_site": (_c.c_double, [_c.c_void_p]),
     "tatrg_singular_values": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_int, _dp]),
+    "tatrg_x_ratio": (_c.c_int, [_c.c_void_p, _c.c_void_p, _dp]),
     "tatrg_steps_done": (_c.c_int, [_c.c_void_p]),
     "tatrg_last_error": (_c.c_char_p, [_c.c_void_p]),
     "tatrg_destroy": (None, [_c.c_void_p]),
@@ -153,6 +154,13 @@ class Tatrg:
         out = np.zeros(k)
         n = _check(lib().tatrg_singular_values(self._h, which, k, out.ctypes.data_as(_dp)), "tatrg_singular_values", self._h)
         return out[:n]
+
+    def x_ratio(self, stream=None):
+        torch = _torch_cuda()
+        x = ctypes.c_double()
+        with torch.cuda.device(self.device):
+            _check(lib().tatrg_x_ratio(self._h, _stream_ptr(stream), ctypes.byref(x)), "tatrg_x_ratio", self._h)
+        return x.value
 
     def steps_done(self):
         return lib().tatrg_steps_done(self._h)

@@ -74,6 +74,26 @@ double tatrg_lnZ_per_site(tatrg_handle c) {
     return v + w * std::log(tr);
 }
 
+int tatrg_x_ratio(tatrg_handle c, void* cuda_stream, double* x_out) {
+    if (!c || !x_out) return TATRG_EINVAL;
+    if (c->failed) return TATRG_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int n = (int)c->phi.d[3];
+    Tens a; a.p = c->pool.alloc((int64_t)n * n + 2);
+    if (!a.p) return TATRG_ENOMEM;
+    std::string err;
+    int rc = contract(st, "ijkag,ijkbg->ab", c->phi, c->psi, a, c->pool, &err);      // A[k,l] = sum T[i1 i2 i3 k, i1 i2 i3 l]
+    double tr[2] = {0, 0};
+    if (rc == TATRG_OK && traces(st, a.p, n, a.p + (int64_t)n * n) != cudaSuccess) rc = TATRG_ECUDA;
+    if (rc == TATRG_OK && cudaMemcpyAsync(tr, a.p + (int64_t)n * n, 16, cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = TATRG_ECUDA;
+    if (rc == TATRG_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = TATRG_ECUDA;
+    c->pool.free(a.p);
+    if (rc != TATRG_OK) { c->err = err; return rc; }
+    if (!(tr[1] > 0)) { c->err = "x_ratio: non-positive Tr A^2"; return TATRG_ENUMERIC; }
+    *x_out = tr[0] * tr[0] / tr[1];
+    return TATRG_OK;
+}
+
 int tatrg_singular_values(tatrg_handle c, int which, int k, double* out_host) {
     if (!c || !out_host || k < 0) return TATRG_EINVAL;
     if (c->m == 0) return TATRG_ESTATE;

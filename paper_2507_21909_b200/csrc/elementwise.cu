@@ -102,6 +102,20 @@ __global__ void init_ising_kernel(double beta, double h, double* phi, double* ps
     psi[e] = v;
     phi[e] = v * exp(beta * h * sgn);
 }
+// out[0] = Tr A, out[1] = Tr A^2 of a small n x n matrix (one block): the two reductions of the X ratio, Eq. 3.3 :301
+__global__ void traces_kernel(const double* __restrict__ A, int n, double* out) {
+    double t1 = 0, t2 = 0;
+    for (int e = threadIdx.x; e < n * n; e += blockDim.x) { int i = e / n, j = e - i * n; if (i == j) t1 += A[e]; t2 += A[e] * A[j * n + i]; }
+    __shared__ double sh[2][32];
+    for (int o = 16; o > 0; o >>= 1) { t1 += __shfl_down_sync(0xffffffffu, t1, o); t2 += __shfl_down_sync(0xffffffffu, t2, o); }
+    if ((threadIdx.x & 31) == 0) { sh[0][threadIdx.x >> 5] = t1; sh[1][threadIdx.x >> 5] = t2; }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        t1 = (threadIdx.x < (blockDim.x >> 5)) ? sh[0][threadIdx.x] : 0.0; t2 = (threadIdx.x < (blockDim.x >> 5)) ? sh[1][threadIdx.x] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) { t1 += __shfl_down_sync(0xffffffffu, t1, o); t2 += __shfl_down_sync(0xffffffffu, t2, o); }
+        if (threadIdx.x == 0) { out[0] = t1; out[1] = t2; }
+    }
+}
 inline unsigned nblocks(int64_t total) { int64_t b = (total + 255) / 256; if (b > 148 * 16) b = 148 * 16; if (b < 1) b = 1; return (unsigned)b; }
 }  // namespace
 
@@ -143,6 +157,10 @@ cudaError_t dot(cudaStream_t st, int64_t n, const double* x, const double* y, do
     int np = (int)nblocks(n); if (np > 148 * 8) np = 148 * 8;
     dot_partial_kernel<<<np, 256, 0, st>>>(x, y, n, result + 1);
     dot_final_kernel<<<1, 256, 0, st>>>(result + 1, np, result); count_launch(2);
+    return cudaGetLastError();
+}
+cudaError_t traces(cudaStream_t st, const double* A, int n, double* out) {
+    traces_kernel<<<1, 256, 0, st>>>(A, n, out); count_launch();
     return cudaGetLastError();
 }
 cudaError_t init_ising(cudaStream_t st, double beta, double h, double* phi, double* psi) {

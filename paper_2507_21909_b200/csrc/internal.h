@@ -61,6 +61,7 @@ cudaError_t gather_rows_scaled(cudaStream_t st, double* out, const double* in, c
 cudaError_t gather_vec(cudaStream_t st, double* out, const double* in, const int* idx, int64_t n, int64_t stride_in, double mul);
 cudaError_t dot(cudaStream_t st, int64_t n, const double* x, const double* y, double* result);
 cudaError_t init_ising(cudaStream_t st, double beta, double h, double* phi, double* psi);
+cudaError_t traces(cudaStream_t st, const double* A, int n, double* out);   // out[0] = Tr A, out[1] = Tr A^2
 cudaError_t fill_zero(cudaStream_t st, double* p, int64_t n);
 // G (k x k, row-major) = block-diagonal orthogonal gauge rotation: for every group [a,b) the block is the Q factor
 // (modified Gram-Schmidt, positive diagonal of R) of C[a:b, 0:b-a], C = cfull (k x ldc).  groups: 2*ngroups ints [dev].

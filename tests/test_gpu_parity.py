@@ -254,3 +254,20 @@ def test_config5_d48_runs_and_improves_on_d32():
     assert len(sig) == 48 and np.all(np.diff(sig) <= 0) and sig[-1] > 0
     z48, z32 = t48.lnZ_per_site(), t32.lnZ_per_site()
     assert np.isfinite(z48) and z48 > z32 and z48 - z32 < 5e-3
+
+
+def test_x_ratio_matches_oracle_and_closed_form():
+    """Eq. 3.3 :298-303.  Initial tensor: X = e^{2 beta} / cosh 2 beta; then step by step against the oracle."""
+    from oracle import tatrg_oracle as O
+    beta = 0.1497
+    t = T.Tatrg(beta, 0.0, 6, 6, 5, power_iters=2)
+    o = O.TatrgOracle(beta, 0.0, 6, 6, 5, n_pow=2)
+    assert abs(t.x_ratio() - math.exp(2 * beta) / math.cosh(2 * beta)) <= 1e-13
+    for m in range(8):
+        t.step()
+        o.step()
+        assert abs(t.x_ratio() - o.x_ratio()) <= 1e-9 * o.x_ratio(), m
+    lo = T.Tatrg(1.0, 0.0, 4, 4, 3, power_iters=1)
+    for _ in range(8):
+        lo.step()
+    assert abs(lo.x_ratio() - 2.0) <= 1e-6

@@ -455,3 +455,33 @@ def test_noise_stability_of_the_gauge_fixing():
             o.step()
         return o.lnZ_per_site()
     assert abs(go(0.0) - go(1e-13)) < 5e-12
+
+
+# ---- X ratio, Eq. 3.3 :298-303 ---------------------------------------------------------------------------------
+@pytest.mark.parametrize("beta", [0.14, 0.1497, 0.7])
+def test_x_ratio_of_the_initial_tensor_closed_form(beta):
+    """A[k,l] = e^{3 beta} sum_a w_a[k] w_a[l] with w_a = (sqrt cosh, +-sqrt sinh):  X = e^{2 beta} / cosh(2 beta)."""
+    phi, psi = O.init_tensor(beta, 0.0)
+    assert abs(O.x_ratio(phi, psi) - math.exp(2 * beta) / math.cosh(2 * beta)) <= 1e-14
+
+
+@pytest.mark.parametrize("beta,h", [(0.14, 0.0), (0.3, 0.05)])
+def test_x_ratio_after_one_exact_step_is_a_ratio_of_partition_functions(beta, h):
+    """After one (exact, D >= 4) step the open axis is the coarse-grained one: Tr A = Z(2x1x1x1) and
+    Tr A^2 = Z(4x1x1x1) up to the same normalisation squared, both by brute-force enumeration."""
+    o = O.TatrgOracle(beta, h, 4, 4, 1, n_pow=1)
+    o.step()
+    z2 = math.exp(2 * enumerate_lnz_per_site((2, 1, 1, 1), beta, h))
+    z4 = math.exp(4 * enumerate_lnz_per_site((4, 1, 1, 1), beta, h))
+    assert abs(o.x_ratio() - z2 * z2 / z4) <= 1e-12 * (z2 * z2 / z4)
+
+
+def test_x_ratio_counts_the_ground_state_degeneracy():
+    """X -> 2 in the ordered phase, X -> 1 in the disordered phase (:303)."""
+    lo = O.TatrgOracle(1.0, 0.0, 4, 4, 3, n_pow=1)
+    hi = O.TatrgOracle(0.05, 0.0, 4, 4, 3, n_pow=1)
+    for m in range(16):
+        hi.step()
+        if m < 8:
+            lo.step()
+    assert abs(lo.x_ratio() - 2.0) <= 1e-6 and abs(hi.x_ratio() - 1.0) <= 1e-2
