@@ -27,7 +27,10 @@ enum {
     TATRG_OPT_K_TRIAD = 2,     /* internal-line dimension rD of the triad isometries (Eq. 2.9 :135). default D+oversample */
     TATRG_OPT_TAU = 3,         /* relative gap below which values form one multiplet (R7). default 1e-6 */
     TATRG_OPT_STAGE_TIMING = 4,/* 1: CUDA-event time per stage; 2: also per DGEMM / permute launch (tatrg_gemm_profile). default 0 */
-    TATRG_OPT_KEEP_TENSORS = 5 /* 1: keep copies of the step's intermediate tensors for tatrg_get_tensor (tests). default 0 */
+    TATRG_OPT_KEEP_TENSORS = 5,/* 1: keep copies of the step's intermediate tensors for tatrg_get_tensor (tests). default 0 */
+    TATRG_OPT_METHOD = 6       /* 0: Triad-ATRG (default).  1: plain ATRG, Eq. 2.7-2.8 (:104-113): no triad split, squeezers from
+                                  Gamma^ATRG, O(D^9) contraction sliced so that no D^7 tensor is stored (fn 6 :205).  Before the first
+                                  step only; ENOMEM unless the workspace holds tatrg_workspace_bytes_atrg(D, oversample). */
 };
 
 /* which spectrum tatrg_singular_values returns */
@@ -41,6 +44,8 @@ enum { TATRG_ST_DECOMPOSE = 0, TATRG_ST_QR, TATRG_ST_RSVD, TATRG_ST_LIFT, TATRG_
 
 /* Device bytes a handle with truncation D (Eq. 2.4 :76) and RSVD oversampling p (l = D+p, :371) needs. */
 size_t tatrg_workspace_bytes(int D, int oversample);
+/* The same for TATRG_OPT_METHOD = 1 (plain ATRG keeps three D^6 slabs). */
+size_t tatrg_workspace_bytes_atrg(int D, int oversample);
 
 /* Builds the initial tensor of the 4D Ising model, Eq. 3.1-3.2 (:241-246), on the device in factored form
  * T[f,b] = sum_a Phi0[f,a] Psi0[b,a], with site weight exp(beta*h*s_a) (R1).

@@ -376,8 +376,9 @@ def contract_psi(g, h, k_, l_, n2, n3, n4):
 class TatrgOracle:
     """State = (Phi, Psi, [ln c_m], step counter).  step() = Fig. 5 (a)-(f) :193."""
 
-    def __init__(self, beta, h, D, oversample, seed, n_pow=2, K=None, tau=TAU_MULTIPLET, exact_swap=False):
+    def __init__(self, beta, h, D, oversample, seed, n_pow=2, K=None, tau=TAU_MULTIPLET, exact_swap=False, method="triad"):
         self.beta, self.h, self.D, self.p, self.seed = beta, h, D, oversample, seed
+        self.method = method                                   # "triad" (Eq. 2.9-2.19) or "atrg" (Eq. 2.7-2.8)
         self.n_pow, self.tau, self.exact_swap = n_pow, tau, exact_swap
         self.K = K if K is not None else D + oversample        # R3: triad internal-line dimension rD = D + p
         self.phi, self.psi = init_tensor(beta, h)
@@ -390,6 +391,8 @@ class TatrgOracle:
         a, dt, core, s_all, lnc = decompose(self.phi, self.psi, D, self.seed, call, tau)          # (a)
         x, y, sig, sig_all = bond_swap(a, dt, core, D, self.p, self.n_pow, self.seed, call, tau,
                                        exact=self.exact_swap)                                        # (b)
+        if self.method == "atrg":
+            return self._finish_atrg(a, dt, core, s_all, lnc, x, y, sig, sig_all, call)
         (ua, ux, uy, ud), tri_spec = triad_isometries(a, dt, x, y, sig, self.K, tau)               # (c)
         e, f, g, h = triad_tensors(a, dt, x, y, sig, ua, ux, uy, ud)
         ms, ns, sq_spec = {}, {}, {}
@@ -408,6 +411,25 @@ class TatrgOracle:
                          efgh=(e, f, g, h), m=ms, n=ns, triad_spectra=tri_spec, squeezer_spectra=sq_spec)
         return self
 
+    def _finish_atrg(self, a, dt, core, s_all, lnc, x, y, sig, sig_all, call):
+        """Steps (d)-(f) of plain ATRG: squeezers from Gamma^ATRG = A (X sigma) | (sigma Y) Dt, contraction by Eq. 2.7-2.8."""
+        D, tau = self.D, self.tau
+        xs, ys = x * sig, y * sig
+        yp, ysp, dp = (t.transpose(4, 1, 2, 3, 0) for t in (y, ys, dt))          # lower half: upper site Y, lower site Dt
+        ms, ns, sq_spec = {}, {}, {}
+        for mu in (2, 3, 4):
+            th_f = atrg_grams(a, xs, mu)
+            th_b = atrg_grams(ysp, dp, mu)
+            ms[mu], ns[mu], sq_spec[mu] = squeezer_pair(th_f, th_b, D, self.seed, call, mu, tau)
+        phi_new = contract_atrg(a, xs, ms[2], ms[3], ms[4])                       # [i1,k2,k3,k4,g]
+        psi_new = contract_atrg(yp, dp, ns[2], ns[3], ns[4])                      # [g,k2,k3,k4,j1]
+        self.phi = np.ascontiguousarray(phi_new.transpose(1, 2, 3, 0, 4))
+        self.psi = np.ascontiguousarray(psi_new.transpose(1, 2, 3, 4, 0))
+        self.lnc.append(lnc)
+        self.m += 1
+        self.last = dict(s=s_all, sigma=sig_all, a=a, dt=dt, core=core, x=x, y=y, sig=sig, m=ms, n=ns, squeezer_spectra=sq_spec)
+        return self
+
     def trace(self):
         """tTr of one tensor with itself on every axis: sum_{f,g} Phi[f,g] Psi[f,g]  (Eq. 2.1 :48, V = 2^m)."""
         return float(_es("ijklg,ijklg->", self.phi, self.psi))
@@ -422,6 +444,24 @@ class TatrgOracle:
 
     def x_ratio(self):
         return x_ratio(self.phi, self.psi)
+
+
+# --------------------------------------------------------------------------------------------------------
+# plain ATRG (no triad split), Eq. 2.7-2.8 :104-113  -- SURVEY A9, config 5's second half
+# --------------------------------------------------------------------------------------------------------
+_ATRG_GRAM = {2: "iucda,alefg,ivcdb,bwefg->ulvw", 3: "icuda,aelfg,icvdb,bewfg->ulvw", 4: "icdua,aeflg,icdvb,befwg->ulvw"}
+
+
+def atrg_grams(p, q, direction):
+    """Gram matrix of one half of Gamma^ATRG on the doubled bond `direction`: the half is
+    P[o1,u2,u3,u4,b] (upper site) . Q[b,l2,l3,l4,o2] (lower site); every index but the pair (u_d, l_d) is contracted
+    with a second copy.  One einsum = the definition (reading R6)."""
+    return _es(_ATRG_GRAM[direction], p, q, p, q)
+
+
+def contract_atrg(p, q, s2, s3, s4):
+    """Eq. 2.7 :106 (and 2.8 with the other half): R[o1,k2,k3,k4,o2] = sum P Q S2 S3 S4, squeezers S[u,l,k]."""
+    return _es("iuvda,amnlg,umx,vny,dlz->ixyzg", p, q, s2, s3, s4)
 
 
 def x_ratio(phi, psi):

@@ -15,7 +15,8 @@ _LIB_PATH = os.path.join(_HERE, "libtatrg.so")
 _lib = None
 
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC, ESTATE = 0, -1, -2, -3, -4, -5
-OPT_POWER_ITERS, OPT_K_TRIAD, OPT_TAU, OPT_STAGE_TIMING, OPT_KEEP_TENSORS = 1, 2, 3, 4, 5
+OPT_POWER_ITERS, OPT_K_TRIAD, OPT_TAU, OPT_STAGE_TIMING, OPT_KEEP_TENSORS, OPT_METHOD = 1, 2, 3, 4, 5, 6
+METHOD_TRIAD, METHOD_ATRG = 0, 1
 SV_SIGMA, SV_S = 0, 1
 STAGES = ["decompose", "bond_swap", "_rsvd", "_lift", "triad", "_triad_tensors", "squeezer_grams", "squeezers", "contract",
           "rotate_trace"]
@@ -24,6 +25,7 @@ _c = ctypes
 _dp = _c.POINTER(_c.c_double)
 _SIGNATURES = {
     "tatrg_workspace_bytes": (_c.c_size_t, [_c.c_int, _c.c_int]),
+    "tatrg_workspace_bytes_atrg": (_c.c_size_t, [_c.c_int, _c.c_int]),
     "tatrg_create": (_c.c_int, [_c.c_double, _c.c_double, _c.c_int, _c.c_int, _c.c_uint64, _c.c_void_p, _c.c_size_t,
                                 _c.POINTER(_c.c_void_p)]),
     "tatrg_set_option": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_double]),
@@ -112,10 +114,11 @@ def workspace_bytes(D, oversample):
 class Tatrg:
     """One 4D Ising tensor network being coarse-grained on one GPU (tatrg_create .. tatrg_destroy)."""
 
-    def __init__(self, beta, h, D, oversample, seed, power_iters=2, K=None, tau=None, device="cuda:0", workspace=None):
+    def __init__(self, beta, h, D, oversample, seed, power_iters=2, K=None, tau=None, device="cuda:0", workspace=None,
+                 method=METHOD_TRIAD):
         torch = _torch_cuda()
         L = lib()
-        need = L.tatrg_workspace_bytes(D, oversample)
+        need = L.tatrg_workspace_bytes_atrg(D, oversample) if method == METHOD_ATRG else L.tatrg_workspace_bytes(D, oversample)
         if need == 0:
             raise TatrgError("unsupported (D, oversample) = (%d, %d)" % (D, oversample))
         self.device = torch.device(device)
@@ -133,6 +136,8 @@ class Tatrg:
             self.set_option(OPT_K_TRIAD, K)
         if tau is not None:
             self.set_option(OPT_TAU, tau)
+        if method != METHOD_TRIAD:
+            self.set_option(OPT_METHOD, method)
 
     def set_option(self, key, value):
         _check(lib().tatrg_set_option(self._h, key, float(value)), "tatrg_set_option", self._h)

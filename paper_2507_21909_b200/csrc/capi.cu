@@ -22,6 +22,13 @@ size_t tatrg_workspace_bytes(int D, int oversample) {
     return (size_t)workspace_doubles(D, oversample) * 8;
 }
 
+size_t tatrg_workspace_bytes_atrg(int D, int oversample) {
+    const size_t base = tatrg_workspace_bytes(D, oversample);
+    if (base == 0) return 0;
+    const double d = D;
+    return base + (size_t)(8.0 * (4.0 * std::pow(d, 6) + 8.0 * std::pow(d, 5)));
+}
+
 int tatrg_create(double beta, double h, int D, int oversample, uint64_t seed, void* workspace, size_t workspace_bytes, tatrg_handle* out) {
     if (!out) return TATRG_EINVAL;
     *out = nullptr;
@@ -53,6 +60,11 @@ int tatrg_set_option(tatrg_handle c, int key, double value) {
         case TATRG_OPT_TAU: if (c->m > 0) return TATRG_ESTATE; if (!(value >= 0) || value > 0.1) return TATRG_EINVAL; c->tau = value; return TATRG_OK;
         case TATRG_OPT_STAGE_TIMING: c->timing = (int)value; return TATRG_OK;
         case TATRG_OPT_KEEP_TENSORS: c->keep_tensors = value != 0; return TATRG_OK;
+        case TATRG_OPT_METHOD:
+            if (c->m > 0) return TATRG_ESTATE;
+            if (value != 0 && value != 1) return TATRG_EINVAL;
+            if (value == 1 && c->pool.capacity() < (tatrg_workspace_bytes_atrg(c->D, c->p) & ~(size_t)255)) return TATRG_ENOMEM;
+            c->method = (int)value; return TATRG_OK;
         default: return TATRG_EINVAL;
     }
 }

@@ -254,6 +254,8 @@ struct Stepper {
     void triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y, const double* sig, Tens U[4], Tens& e, Tens& f, Tens& g, Tens& h);
     void half_grams(const Tens& P, const Tens& Q, const Tens& Iu, const Tens& Jl, Tens th[3]);
     void squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], Tens Nt[3]);
+    void atrg_grams(const Tens& P, const Tens& Q, Tens th[3]);
+    Tens atrg_contract(const Tens& P, const Tens& Q, Tens S[3]);
     void run();
 };
 
@@ -533,6 +535,48 @@ void Stepper::squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], T
     }
 }
 
+// ---- plain ATRG (Eq. 2.7-2.8 :104-113): no triad split -------------------------------------------
+// One half of the unit cell is P[o1,u2,u3,u4,b] (upper site) . Q[b,l2,l3,l4,o2] (lower site).
+// Gram matrices on the doubled bonds, th[d-2][(u l),(u' l')]: sum_b,b' PP_d[u,b,u',b'] QQ_d[b,l,b',l'] with every other
+// leg of P (resp. Q) traced against its copy -- nothing larger than D^5 is formed.
+void Stepper::atrg_grams(const Tens& P, const Tens& Q, Tens th[3]) {
+    Scope sc(*this);
+    static const char* pp[3] = {"iucda,ivcdb->uavb", "icuda,icvdb->uavb", "icdua,icdvb->uavb"};
+    static const char* qq[3] = {"alcdg,bwcdg->albw", "acldg,bcwdg->albw", "acdlg,bcdwg->albw"};
+    for (int d = 0; d < 3; ++d) {
+        Scope s2(*this);
+        Tens a = ein(pp[d], P, P);
+        Tens b = ein(qq[d], Q, Q);
+        th[d] = ein("uavb,albw->ulvw", a, b);
+        keep(th[d]);
+    }
+    for (int d = 0; d < 3; ++d) keep(th[d]);
+}
+
+// R[o1,k2,k3,k4,o2] = sum P[o1,u2,u3,u4,b] Q[b,l2,l3,l4,o2] S2[k2,u2,l2] S3[k3,u3,l3] S4[k4,u4,l4]   (Eq. 2.7 :106, O(D^9)).
+// The D^7 intermediate of the paper (fn 6 :205: "memory blocking") is never materialised: the contraction is sliced over
+// o1, one D^6 slab at a time.
+Tens Stepper::atrg_contract(const Tens& P, const Tens& Q, Tens S[3]) {
+    Scope sc(*this);
+    const int64_t o1 = P.d[0], o2 = Q.d[4], k2 = S[0].d[0], k3 = S[1].d[0], k4 = S[2].d[0];
+    Tens R = make({o1, k2, k3, k4, o2});
+    Tens pm = ein("iuvda,zdl->iuvalz", P, S[2]);                    // [o1,u2,u3,b,l4,k4]
+    const int64_t slab = pm.size() / o1;
+    for (int64_t i = 0; i < o1; ++i) {
+        Scope s2(*this);
+        Tens pi; pi.p = pm.p + i * slab; pi.nd = 5; for (int d = 0; d < 5; ++d) pi.d[d] = pm.d[d + 1];
+        Tens big = ein("uvalz,amnlg->uvzmng", pi, Q);               // [u2,u3,k4,l2,l3,o2]: 2 D^8 flop per slab
+        Tens t2 = ein("uvzmng,pum->vzngp", big, S[0]);
+        drop(big);
+        Tens ri; ri.p = R.p + i * (k2 * k3 * k4 * o2);
+        std::string e;
+        int rc = contract(st, "vzngp,qvn->pqzg", t2, S[1], ri, c.pool, &e);
+        if (rc != TATRG_OK) fail(rc, "%s", e.c_str());
+    }
+    keep(R);
+    return R;
+}
+
 void Stepper::run() {
     Counters& cn = c.cnt;
     const bool timed = c.timing >= 1;
@@ -557,63 +601,103 @@ void Stepper::run() {
     bond_swap(a, dt, core, x, y, sig, gr);
     save("X", x); save("Y", y); { Tens s; s.p = sig; s.nd = 1; s.d[0] = gr; save("sigma", s); }
     mark(); mark(); mark();
-    Tens U[4], e, f, g, h;
-    triad(a, dt, x, y, sig, U, e, f, g, h);                         // (c)
-    save("E", e); save("F", f); save("G", g); save("H", h);
-    save("UA", U[0]); save("UX", U[1]); save("UY", U[2]); save("UD", U[3]);
-    drop(a); drop(dt); drop(core); drop(x); drop(y);
-    mark(); mark();
-    // (d) squeezer Gram matrices of the upper half (E F I J) and of the sigma-weighted lower half (G sigma, H, K, L)
-    Tens thf[3], thb[3];
-    half_grams(e, f, U[0], U[1], thf);
-    {
-        Scope s2(*this);
-        Tens gs = make({g.d[0], g.d[1], g.d[2], g.d[3]});
-        ck(scale_last(st, gs.p, g.p, sig, g.size() / gr, gr, 0), "scale");
-        Tens P = perm(gs, {3, 1, 2, 0});          // [g, kY, j4u, be]
-        Tens Q = perm(h, {3, 1, 2, 0});           // [be, kD, j4l, j1]
-        half_grams(P, Q, U[2], U[3], thb);
-        for (int i = 0; i < 3; ++i) keep(thb[i]);
-    }
-    mark();
-    Tens Mt[3], Nt[3];
-    {
-        const int du[3] = {(int)c.phi.d[1], (int)c.phi.d[2], (int)c.phi.d[3]};
-        squeezers(thf, thb, du, Mt, Nt);
-    }
-    save("M2", Mt[0]); save("M3", Mt[1]); save("M4", Mt[2]); save("N2", Nt[0]); save("N3", Nt[1]); save("N4", Nt[2]);
-    mark();
-    // (e) Eq. 2.18 :175  Phi'[i1,k2,k3,k4,g]
     Tens phin, psin;
-    {
-        Scope s2(*this);
-        Tens fm = ein("zul,axld->uaxzd", Mt[2], f);
-        Tens xi = ein("ikua,uaxzd->ikxzd", e, fm);                  // Xi[i1,kA,kX,k4,g]
-        drop(fm);
-        Tens im = ein("kuc,zul->kclz", U[0], Mt[0]);
-        Tens imm = ein("kclz,ycw->klwzy", im, Mt[1]);
-        Tens lam = ein("klwzy,xlw->kxzy", imm, U[1]);               // Lambda[kA,kX,k2,k3]
-        drop(im); drop(imm);
-        Tens ph = ein("Ikxzd,kxpq->Ipqzd", xi, lam);
-        drop(xi);
-        phin = perm(ph, {1, 2, 3, 0, 4});                           // (f) rotate: axis 1 becomes axis 4  (R5)
-        keep(phin);
+    if (c.method == 1) {
+        // ---- plain ATRG: squeezers from Gamma^ATRG = A (X sigma) | (sigma Y) Dt, contraction by Eq. 2.7-2.8 ----
+        const int64_t gq = x.d[4];
+        Tens xs = make({x.d[0], x.d[1], x.d[2], x.d[3], gq}), ys = make({y.d[0], y.d[1], y.d[2], y.d[3], gq});
+        ck(scale_last(st, xs.p, x.p, sig, x.size() / gq, gq, 0), "scale");
+        ck(scale_last(st, ys.p, y.p, sig, y.size() / gq, gq, 0), "scale");
+        Tens yp = perm(y, {4, 1, 2, 3, 0});          // [g, u2,u3,u4, be]   (upper site of the lower half)
+        Tens ysp = perm(ys, {4, 1, 2, 3, 0});
+        Tens dp = perm(dt, {4, 1, 2, 3, 0});         // [be, l2,l3,l4, j1]  (lower site of the lower half)
+        drop(ys); drop(y); drop(x); drop(core);
+        mark(); mark();
+        Tens thf[3], thb[3];
+        atrg_grams(a, xs, thf);
+        atrg_grams(ysp, dp, thb);
+        drop(ysp);
+        mark();
+        Tens Mt[3], Nt[3];
+        {
+            const int du[3] = {(int)c.phi.d[1], (int)c.phi.d[2], (int)c.phi.d[3]};
+            squeezers(thf, thb, du, Mt, Nt);
+        }
+        save("M2", Mt[0]); save("M3", Mt[1]); save("M4", Mt[2]); save("N2", Nt[0]); save("N3", Nt[1]); save("N4", Nt[2]);
+        mark();
+        {
+            Scope s2(*this);
+            Tens ph = atrg_contract(a, xs, Mt);                       // Phi'[i1,k2,k3,k4,g]
+            phin = perm(ph, {1, 2, 3, 0, 4});
+            keep(phin);
+        }
+        drop(a); drop(xs);
+        {
+            Scope s2(*this);
+            Tens ps = atrg_contract(yp, dp, Nt);                      // [g,k2,k3,k4,j1]
+            psin = perm(ps, {1, 2, 3, 4, 0});                         // -> Psi[k2,k3,k4,j1,g]
+            keep(psin);
+        }
+        drop(dt);
+        mark();
+    } else {
+        Tens U[4], e, f, g, h;
+        triad(a, dt, x, y, sig, U, e, f, g, h);                         // (c)
+        save("E", e); save("F", f); save("G", g); save("H", h);
+        save("UA", U[0]); save("UX", U[1]); save("UY", U[2]); save("UD", U[3]);
+        drop(a); drop(dt); drop(core); drop(x); drop(y);
+        mark(); mark();
+        // (d) squeezer Gram matrices of the upper half (E F I J) and of the sigma-weighted lower half (G sigma, H, K, L)
+        Tens thf[3], thb[3];
+        half_grams(e, f, U[0], U[1], thf);
+        {
+            Scope s2(*this);
+            Tens gs = make({g.d[0], g.d[1], g.d[2], g.d[3]});
+            ck(scale_last(st, gs.p, g.p, sig, g.size() / gr, gr, 0), "scale");
+            Tens P = perm(gs, {3, 1, 2, 0});          // [g, kY, j4u, be]
+            Tens Q = perm(h, {3, 1, 2, 0});           // [be, kD, j4l, j1]
+            half_grams(P, Q, U[2], U[3], thb);
+            for (int i = 0; i < 3; ++i) keep(thb[i]);
+        }
+        mark();
+        Tens Mt[3], Nt[3];
+        {
+            const int du[3] = {(int)c.phi.d[1], (int)c.phi.d[2], (int)c.phi.d[3]};
+            squeezers(thf, thb, du, Mt, Nt);
+        }
+        save("M2", Mt[0]); save("M3", Mt[1]); save("M4", Mt[2]); save("N2", Nt[0]); save("N3", Nt[1]); save("N4", Nt[2]);
+        mark();
+        // (e) Eq. 2.18 :175  Phi'[i1,k2,k3,k4,g]
+        {
+            Scope s2(*this);
+            Tens fm = ein("zul,axld->uaxzd", Mt[2], f);
+            Tens xi = ein("ikua,uaxzd->ikxzd", e, fm);                  // Xi[i1,kA,kX,k4,g]
+            drop(fm);
+            Tens im = ein("kuc,zul->kclz", U[0], Mt[0]);
+            Tens imm = ein("kclz,ycw->klwzy", im, Mt[1]);
+            Tens lam = ein("klwzy,xlw->kxzy", imm, U[1]);               // Lambda[kA,kX,k2,k3]
+            drop(im); drop(imm);
+            Tens ph = ein("Ikxzd,kxpq->Ipqzd", xi, lam);
+            drop(xi);
+            phin = perm(ph, {1, 2, 3, 0, 4});                           // (f) rotate: axis 1 becomes axis 4  (R5)
+            keep(phin);
+        }
+        {   // Eq. 2.19 :175  Psi'[j1,k2,k3,k4,g]
+            Scope s2(*this);
+            Tens gn = ein("zul,byug->lbyzg", Nt[2], g);
+            Tens xi = ein("jdlb,lbyzg->jdyzg", h, gn);                  // Xi'[j1,kD,kY,k4,g]
+            drop(gn);
+            Tens kn = ein("yuc,zul->yclz", U[2], Nt[0]);
+            Tens knn = ein("yclz,vcw->ylwzv", kn, Nt[1]);
+            Tens lam = ein("ylwzv,dlw->dyzv", knn, U[3]);               // Lambda'[kD,kY,k2,k3]
+            drop(kn); drop(knn);
+            Tens ps = ein("Jdyzg,dypq->Jpqzg", xi, lam);
+            drop(xi);
+            psin = perm(ps, {1, 2, 3, 0, 4});
+            keep(psin);
+        }
+        mark();
     }
-    {   // Eq. 2.19 :175  Psi'[j1,k2,k3,k4,g]
-        Scope s2(*this);
-        Tens gn = ein("zul,byug->lbyzg", Nt[2], g);
-        Tens xi = ein("jdlb,lbyzg->jdyzg", h, gn);                  // Xi'[j1,kD,kY,k4,g]
-        drop(gn);
-        Tens kn = ein("yuc,zul->yclz", U[2], Nt[0]);
-        Tens knn = ein("yclz,vcw->ylwzv", kn, Nt[1]);
-        Tens lam = ein("ylwzv,dlw->dyzv", knn, U[3]);               // Lambda'[kD,kY,k2,k3]
-        drop(kn); drop(knn);
-        Tens ps = ein("Jdyzg,dypq->Jpqzg", xi, lam);
-        drop(xi);
-        psin = perm(ps, {1, 2, 3, 0, 4});
-        keep(psin);
-    }
-    mark();
     c.pool.free(c.phi.p); c.pool.free(c.psi.p);
     detach(phin); detach(psin);
     c.phi = phin; c.psi = psin;

@@ -17,6 +17,7 @@ struct tatrg_ctx {
     int D = 0, p = 0;
     uint64_t seed = 0;
     int n_pow = 2, Ktri = 0;
+    int method = 0;                  // 0: Triad-ATRG, 1: plain ATRG
     double tau = tatrg::kTauDefault;
     int timing = 0;
     bool keep_tensors = false;

@@ -271,3 +271,29 @@ def test_x_ratio_matches_oracle_and_closed_form():
     for _ in range(8):
         lo.step()
     assert abs(lo.x_ratio() - 2.0) <= 1e-6
+
+
+@pytest.mark.parametrize("D,p,n_pow,steps", [(3, 3, 1, 8), (4, 4, 2, 10), (5, 3, 1, 6)])
+def test_plain_atrg_method_matches_untriaded_oracle(D, p, n_pow, steps):
+    """SURVEY A9 / PAPER.md Eq. 2.7-2.8 :104-113: the plain-ATRG path (no triad isometries, squeezers from Gamma^ATRG,
+    sliced O(D^9) contraction) against the oracle's plain-ATRG method (one einsum per equation)."""
+    from oracle import tatrg_oracle as O
+    beta, seed = 0.1497, 31
+    t = T.Tatrg(beta, 0.0, D, p, seed, power_iters=n_pow, method=T.METHOD_ATRG)
+    o = O.TatrgOracle(beta, 0.0, D, p, seed, n_pow=n_pow, method="atrg")
+    for m in range(steps):
+        t.step()
+        o.step()
+        lo = o.lnZ_per_site()
+        assert abs(t.lnZ_per_site() - lo) <= TOL_LNZ * abs(lo), m
+        got, ref = t.singular_values(T.SV_SIGMA, D), o.last["sigma"][:D]
+        k = min(len(got), len(ref))
+        assert np.abs(got[:k] - ref[:k]).max() <= TOL_SV, m
+    # and it differs from the truncated triad run (K = D + p < D^2 at D = 4), i.e. the option does something
+    if D == 4:
+        tt = T.Tatrg(beta, 0.0, D, 1, seed, power_iters=n_pow, K=5)
+        ta = T.Tatrg(beta, 0.0, D, 1, seed, power_iters=n_pow, method=T.METHOD_ATRG)
+        for _ in range(steps):
+            tt.step()
+            ta.step()
+        assert abs(tt.lnZ_per_site() - ta.lnZ_per_site()) > 1e-8

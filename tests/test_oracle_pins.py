@@ -485,3 +485,34 @@ def test_x_ratio_counts_the_ground_state_degeneracy():
         if m < 8:
             lo.step()
     assert abs(lo.x_ratio() - 2.0) <= 1e-6 and abs(hi.x_ratio() - 1.0) <= 1e-2
+
+
+# ---- plain ATRG (Eq. 2.7-2.8 :104-113) -----------------------------------------------------------------------------------
+@pytest.mark.parametrize("beta,h", [(0.14, 0.0), (0.1497, 1e-3)])
+def test_atrg_one_and_two_steps_are_exact(beta, h):
+    """Same enumeration pins as the triad method: nothing is truncated in step 1 at D >= 4 and in step 2 at D >= 16."""
+    o = O.TatrgOracle(beta, h, 16, 0, 1, n_pow=1, method="atrg")
+    o.step()
+    assert abs(o.lnZ_per_site() - enumerate_lnz_per_site((2, 1, 1, 1), beta, h)) <= 1e-13
+    o.step()
+    assert abs(o.lnZ_per_site() - enumerate_lnz_per_site((2, 2, 1, 1), beta, h)) <= 1e-12
+
+
+def test_triad_with_full_internal_dimension_recovers_atrg():
+    """PAPER.md :179 "r = D recovers ATRG": the triad run with K = chi2*chi3 and the plain ATRG run agree (up to the
+    1e-6 numerical-rank cut of the triad isometries, reading R14)."""
+    t = O.TatrgOracle(0.1497, 0.0, 4, 4, 9, n_pow=1, K=16)
+    a = O.TatrgOracle(0.1497, 0.0, 4, 4, 9, n_pow=1, method="atrg")
+    for _ in range(6):
+        t.step()
+        a.step()
+        assert abs(t.lnZ_per_site() - a.lnZ_per_site()) <= 1e-8
+
+
+def test_atrg_staged_gram_equals_definition_on_random_tensors():
+    """atrg_grams is one einsum of four operands; check it against the explicit half-cell tensor."""
+    p = inputs.random_tensor((2, 3, 2, 3, 2), 1)
+    q = inputs.random_tensor((2, 2, 3, 2, 3), 2)
+    half = np.einsum("iucda,alefg->iuclefdg", p, q)               # [o1,u2,u3,l2,l3,l4,u4,o2]
+    th2 = np.einsum("iuclefdg,ivcwefdg->ulvw", half, half)
+    assert np.abs(O.atrg_grams(p, q, 2) - th2).max() <= 1e-12
