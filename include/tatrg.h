@@ -7,7 +7,9 @@
  * unless stated otherwise; tatrg_last_error() gives the text of the last failure of a handle.
  *
  * Pointers are marked  [dev]  (device memory, FP64 unless stated, 16-byte aligned)  or  [host].
- * The library never frees caller memory and never allocates device memory of its own.
+ * The library never frees caller memory and never allocates device memory of its own.  All work of a call is ordered on
+ * the caller's stream; the eigen-decompositions additionally use ONE auxiliary high-priority stream and a few events that
+ * the library creates on first use (forked from and joined back into the caller's stream inside the call).
  */
 #ifndef TATRG_H
 #define TATRG_H

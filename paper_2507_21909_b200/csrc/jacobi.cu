@@ -24,7 +24,8 @@ constexpr int SB = 64;          // side of the shared-memory sub-problem
 constexpr int SP = SB + 1;      // pitch
 constexpr int BW = 32;          // block width of the block-Jacobi
 constexpr double kTolRel = 1e-15;
-constexpr int kMaxSweeps = 40;
+constexpr int kMaxSweeps = 40;        // sweeps of the in-CTA solvers
+constexpr int kMaxBlockSweeps = 120;  // sweeps of the block method (n = 2304 Gram matrices with wide noise-level clusters take ~40)
 // off-diagonal entries below kFloorRel * max|diag| are not rotated: one order below the rounding of the GEMM that
 // produced the matrix
 constexpr double kFloorRel = 1e-17;
@@ -200,11 +201,13 @@ __device__ __forceinline__ double rotated_entry(const double* S, const Rot* cur,
 //   second buffer (both sides of the two-sided update in one pass over S) and then rotate the columns of the
 //   accumulated J in place, while warp 0 derives the next round's rotations from the OLD buffer (rotated_entry).
 //   None of the three touches data another one writes.
-__global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int round, int mode, const double* __restrict__ Gp,
-                                                             const double* __restrict__ misc, double* __restrict__ Jb,
+__global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int round, int prev_round, int mode, const double* __restrict__ Gp,
+                                                             const double* __restrict__ misc, const double* __restrict__ Jprev,
+                                                             const double* __restrict__ Dprev, double* __restrict__ Jb,
                                                              double* __restrict__ Dg, int* __restrict__ active, int* __restrict__ counter,
                                                              int64_t wstride) {
     Gp += blockIdx.y * wstride; misc += blockIdx.y * wstride; Jb += blockIdx.y * wstride; Dg += blockIdx.y * wstride;
+    Jprev += blockIdx.y * wstride; Dprev += blockIdx.y * wstride;
     active += blockIdx.y * wstride * 2;      // wstride counts doubles
     extern __shared__ double sh[];
     double* Sa = sh; double* Sb = Sa + SB * SP; double* J = Sb + SB * SP;
@@ -214,11 +217,62 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
     int* cnt = pair_of + 128;
     const int tid = threadIdx.x, k = blockIdx.x, warp = tid >> 5, lane = tid & 31;
     int P, Q; rr_pair(nb, round, k, P, Q);
-    for (int e = tid; e < SB * SB; e += 1024) {
-        int i = e >> 6, j = e & 63;
-        Sa[i * SP + j] = Gp[(int64_t)gidx(P, Q, i) * N + gidx(P, Q, j)];
-        J[i * SP + j] = (i == j) ? 1.0 : 0.0;
+    if (prev_round < 0) {
+        // the matrix in Gp is up to date: take the diagonal sub-problem from it
+        for (int e = tid; e < SB * SB; e += 1024) {
+            int i = e >> 6, j = e & 63;
+            Sa[i * SP + j] = Gp[(int64_t)gidx(P, Q, i) * N + gidx(P, Q, j)];
+        }
+    } else {
+        // Gp is the matrix BEFORE the previous round's rotations were applied (that apply runs concurrently on another
+        // stream and writes a different buffer).  The sub-problem of this pair is assembled from the previous round's
+        // solver outputs: diagonal 32-blocks from the solved sub-problems (Dprev), the cross block as the needed
+        // 32 x 32 corner of J_a^T G[PQ_a, PQ_b] J_b.
+        int* loc = cnt + 4;                                   // a, hP, b, hQ, Pa, Qa, Pb, Qb
+        if (tid == 0) {
+            for (int kk = 0; kk < (nb >> 1); ++kk) {
+                int A, B; rr_pair(nb, prev_round, kk, A, B);
+                if (A == P) { loc[0] = kk; loc[1] = 0; loc[4] = A; loc[5] = B; }
+                if (B == P) { loc[0] = kk; loc[1] = 1; loc[4] = A; loc[5] = B; }
+                if (A == Q) { loc[2] = kk; loc[3] = 0; loc[6] = A; loc[7] = B; }
+                if (B == Q) { loc[2] = kk; loc[3] = 1; loc[6] = A; loc[7] = B; }
+            }
+        }
+        __syncthreads();
+        const int a = loc[0], hP = loc[1], b = loc[2], hQ = loc[3], Pa = loc[4], Qa = loc[5], Pb = loc[6], Qb = loc[7];
+        const double* Ja = Jprev + (int64_t)a * SB * SB; const double* Jbb = Jprev + (int64_t)b * SB * SB;
+        for (int e = tid; e < SB * SB; e += 1024) {
+            int i = e >> 6, j = e & 63;
+            Sb[i * SP + j] = Gp[(int64_t)gidx(Pa, Qa, i) * N + gidx(Pb, Qb, j)];                    // X = G[PQ_a, PQ_b]
+            J[i * SP + j] = (j < BW) ? Ja[i * SB + hP * BW + j] : Jbb[i * SB + hQ * BW + j - BW];   // [J_a half | J_b half]
+        }
+        __syncthreads();
+        for (int e = tid; e < BW * SB; e += 1024) {           // T1 = (J_a half)^T X   (32 x 64), parked in rows 32..63 of Sa
+            int r = e >> 6, j = e & 63;
+            double acc = 0;
+#pragma unroll 8
+            for (int i = 0; i < SB; ++i) acc += J[i * SP + r] * Sb[i * SP + j];
+            Sa[(BW + r) * SP + j] = acc;
+        }
+        __syncthreads();
+        double pq;
+        {
+            const int r = tid >> 5, c = tid & 31;                 // cross block = T1 (J_b half)   (32 x 32)
+            double acc = 0;
+#pragma unroll 8
+            for (int j = 0; j < SB; ++j) acc += Sa[(BW + r) * SP + j] * J[j * SP + BW + c];
+            pq = acc;
+        }
+        __syncthreads();
+        {
+            const int r = tid >> 5, c = tid & 31;
+            Sa[r * SP + BW + c] = pq; Sa[(BW + c) * SP + r] = pq;
+            Sa[r * SP + c] = Dprev[(int64_t)a * SB * SB + (hP * BW + r) * SB + hP * BW + c];
+            Sa[(BW + r) * SP + BW + c] = Dprev[(int64_t)b * SB * SB + (hQ * BW + r) * SB + hQ * BW + c];
+        }
     }
+    __syncthreads();
+    for (int e = tid; e < SB * SB; e += 1024) { int i = e >> 6, j = e & 63; J[i * SP + j] = (i == j) ? 1.0 : 0.0; }
     if (tid == 0) { cnt[0] = 0; cnt[1] = 0; }
     __syncthreads();
     const double floor_abs = misc[1];
@@ -232,7 +286,15 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
         }
     }
     worst = block_max(worst, red);
-    if (worst == 0.0) { if (tid == 0) active[k] = 0; return; }
+    if (worst == 0.0) {     // nothing to rotate: publish the block as it is and an identity rotation (the next round reads them)
+        if (tid == 0) active[k] = 0;
+        for (int e = tid; e < SB * SB; e += 1024) {
+            int i = e >> 6, j = e & 63;
+            Jb[(int64_t)k * SB * SB + e] = (i == j) ? 1.0 : 0.0;
+            Dg[(int64_t)k * SB * SB + e] = Sa[i * SP + j];
+        }
+        return;
+    }
     const int nrounds = mode == 0 ? SB - 1 : BW;
     const int max_sweeps = mode == 0 ? 2 : 1;
     double* S = Sa; double* T = Sb;
@@ -300,10 +362,8 @@ __global__ void __launch_bounds__(1024, 1) blk_solve2_kernel(int N, int nb, int 
         __syncthreads();
     }
     if (tid == 0) { active[k] = total > 0; if (total_sig > 0) atomicAdd(counter, total_sig); }
-    if (total > 0) {
-        for (int e = tid; e < SB * SB; e += 1024) { int i = e >> 6, j = e & 63; Jb[(int64_t)k * SB * SB + e] = J[i * SP + j]; }
-        for (int e = tid; e < SB * SB; e += 1024) { int i = e >> 6, j = e & 63; Dg[(int64_t)k * SB * SB + e] = S[i * SP + j]; }
-    }
+    for (int e = tid; e < SB * SB; e += 1024) { int i = e >> 6, j = e & 63; Jb[(int64_t)k * SB * SB + e] = J[i * SP + j]; }
+    for (int e = tid; e < SB * SB; e += 1024) { int i = e >> 6, j = e & 63; Dg[(int64_t)k * SB * SB + e] = S[i * SP + j]; }
 }
 
 // 64x64x64 tile products on FP64 tensor cores (mma.sync.m8n8k4).  256 threads = 8 warps as 4 (M) x 2 (N); a warp owns
@@ -333,10 +393,10 @@ __device__ __forceinline__ void tile_mma(const double* __restrict__ A, const dou
 // One launch applies the round's rotations to G (both sides, tile by tile, using the symmetry) and to V^T:
 //   blockIdx.y <  npair : tile (k = blockIdx.y, l = blockIdx.x), k <= l:  G[PQ_k,PQ_l] <- J_k^T G[PQ_k,PQ_l] J_l  (+ mirror)
 //   blockIdx.y >= npair : V^T[PQ_k, 64-column tile blockIdx.x] <- J_k^T V^T[...]
-__global__ void __launch_bounds__(256, 2) blk_apply2_kernel(int N, int nb, int round, double* __restrict__ Gp, double* __restrict__ Vt,
-                                                            const double* __restrict__ Jb, const double* __restrict__ Dg,
+__global__ void __launch_bounds__(256, 2) blk_apply2_kernel(int N, int nb, int round, const double* __restrict__ Gin, double* __restrict__ Gout,
+                                                            double* __restrict__ Vt, const double* __restrict__ Jb, const double* __restrict__ Dg,
                                                             const int* __restrict__ active, int64_t wstride) {
-    Gp += blockIdx.z * wstride; Vt += blockIdx.z * wstride; Jb += blockIdx.z * wstride; Dg += blockIdx.z * wstride;
+    Gin += blockIdx.z * wstride; Gout += blockIdx.z * wstride; Vt += blockIdx.z * wstride; Jb += blockIdx.z * wstride; Dg += blockIdx.z * wstride;
     active += blockIdx.z * wstride * 2;
     extern __shared__ double sh2[];
     double* Xs = sh2; double* Ja = sh2 + SB * AP; double* Jc = sh2 + 2 * SB * AP;
@@ -347,7 +407,7 @@ __global__ void __launch_bounds__(256, 2) blk_apply2_kernel(int N, int nb, int r
     for (int i = 0; i < 2; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-    if ((int)blockIdx.y >= npair) {
+    if ((int)blockIdx.y >= npair) {      // V^T rows of pair k, in place
         const int k = blockIdx.y - npair;
         if (!active[k]) return;
         int P, Q; rr_pair(nb, round, k, P, Q);
@@ -366,26 +426,31 @@ __global__ void __launch_bounds__(256, 2) blk_apply2_kernel(int N, int nb, int r
                 *reinterpret_cast<double2*>(Vt + (int64_t)gidx(P, Q, m0 + 8 * i + g) * N + c0 + n0 + 8 * j + 2 * t) = make_double2(acc[i][j][0], acc[i][j][1]);
         return;
     }
+    // G: out of place (Gin -> Gout), every tile k <= l is written (copied when neither pair rotated)
     const int k = blockIdx.y, l = blockIdx.x;
     if (l >= npair || k > l) return;
     const bool ak = active[k] != 0, al = active[l] != 0;
-    if (!ak && !al) return;
     int P, Q, R, S2; rr_pair(nb, round, k, P, Q); rr_pair(nb, round, l, R, S2);
     if (k == l) {   // the solved diagonal block: exactly what the solver left (annihilated entries are exact zeros)
         for (int e = tid; e < SB * SB; e += 256) {
             int i = e >> 6, j = e & 63;
-            Gp[(int64_t)gidx(P, Q, i) * N + gidx(P, Q, j)] = Dg[(int64_t)k * SB * SB + e];
+            Gout[(int64_t)gidx(P, Q, i) * N + gidx(P, Q, j)] = Dg[(int64_t)k * SB * SB + e];
+        }
+        return;
+    }
+    if (!ak && !al) {
+        for (int e = tid; e < SB * SB / 2; e += 256) {
+            int i = e >> 5, j = (e & 31) * 2;
+            *reinterpret_cast<double2*>(Gout + (int64_t)gidx(P, Q, i) * N + gidx(R, S2, j)) = *reinterpret_cast<const double2*>(Gin + (int64_t)gidx(P, Q, i) * N + gidx(R, S2, j));
+            *reinterpret_cast<double2*>(Gout + (int64_t)gidx(R, S2, i) * N + gidx(P, Q, j)) = *reinterpret_cast<const double2*>(Gin + (int64_t)gidx(R, S2, i) * N + gidx(P, Q, j));
         }
         return;
     }
     for (int e = tid; e < SB * SB / 2; e += 256) {
         int i = e >> 5, j = (e & 31) * 2;      // j, j+1 lie in the same 32-wide block
-        *reinterpret_cast<double2*>(Xs + i * AP + j) = *reinterpret_cast<const double2*>(Gp + (int64_t)gidx(P, Q, i) * N + gidx(R, S2, j));
-        double2 ja = make_double2(i == j ? 1.0 : 0.0, i == j + 1 ? 1.0 : 0.0), jc = ja;
-        if (ak) ja = *reinterpret_cast<const double2*>(Jb + (int64_t)k * SB * SB + i * SB + j);
-        if (al) jc = *reinterpret_cast<const double2*>(Jb + (int64_t)l * SB * SB + i * SB + j);
-        *reinterpret_cast<double2*>(Ja + i * AP + j) = ja;
-        *reinterpret_cast<double2*>(Jc + i * AP + j) = jc;
+        *reinterpret_cast<double2*>(Xs + i * AP + j) = *reinterpret_cast<const double2*>(Gin + (int64_t)gidx(P, Q, i) * N + gidx(R, S2, j));
+        *reinterpret_cast<double2*>(Ja + i * AP + j) = *reinterpret_cast<const double2*>(Jb + (int64_t)k * SB * SB + i * SB + j);
+        *reinterpret_cast<double2*>(Jc + i * AP + j) = *reinterpret_cast<const double2*>(Jb + (int64_t)l * SB * SB + i * SB + j);
     }
     __syncthreads();
     tile_mma<true>(Ja, Xs, acc, m0, n0, g, t);        // J_k^T X
@@ -404,7 +469,7 @@ __global__ void __launch_bounds__(256, 2) blk_apply2_kernel(int N, int nb, int r
     for (int i = 0; i < 2; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j)
-            *reinterpret_cast<double2*>(Gp + (int64_t)gidx(P, Q, m0 + 8 * i + g) * N + gidx(R, S2, n0 + 8 * j + 2 * t)) = make_double2(acc[i][j][0], acc[i][j][1]);
+            *reinterpret_cast<double2*>(Gout + (int64_t)gidx(P, Q, m0 + 8 * i + g) * N + gidx(R, S2, n0 + 8 * j + 2 * t)) = make_double2(acc[i][j][0], acc[i][j][1]);
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < 2; ++i)
@@ -416,7 +481,7 @@ __global__ void __launch_bounds__(256, 2) blk_apply2_kernel(int N, int nb, int r
     __syncthreads();
     for (int e = tid; e < SB * SB / 2; e += 256) {
         int i = e >> 5, j = (e & 31) * 2;
-        *reinterpret_cast<double2*>(Gp + (int64_t)gidx(R, S2, i) * N + gidx(P, Q, j)) = *reinterpret_cast<const double2*>(Ja + i * AP + j);
+        *reinterpret_cast<double2*>(Gout + (int64_t)gidx(R, S2, i) * N + gidx(P, Q, j)) = *reinterpret_cast<const double2*>(Ja + i * AP + j);
     }
 }
 __global__ void extract_diag_kernel(int N, const double* __restrict__ Gp, double* __restrict__ d) {
@@ -481,15 +546,15 @@ bool check(cudaError_t e, std::string* err, const char* what) {
 }
 constexpr int kSmallSmem = (2 * SB * SP + 96) * 8 + 3 * 32 * 4 + 64;
 constexpr int kApplySmem = 3 * SB * 68 * 8;
-constexpr int kSolve2Smem = 3 * SB * SP * 8 + 64 * 24 + 32 * 8 + 128 * 4 + 64;
+constexpr int kSolve2Smem = 3 * SB * SP * 8 + 64 * 24 + 32 * 8 + 128 * 4 + 128;
 }  // namespace
 
 static int padded_n(int n) { if (n <= SB) return n; int nb = (n + BW - 1) / BW; if (nb & 1) ++nb; return nb * BW; }
 
-// per-matrix work layout (doubles): [lam_u N][idx N][misc 64][Vt_unsorted N*N][Gp N*N][Jb npair*4096][Dg npair*4096][active npair]
+// per-matrix work layout (doubles): [lam_u N][idx N][misc 64][Vt_unsorted N*N][G0 N*N][G1 N*N][Jb 2 x npair*4096][Dg 2 x npair*4096][active 2 x npair]
 static size_t work_doubles(int N) {
     size_t nb2 = (size_t)N / BW / 2 + 1;
-    size_t d = 2 * (size_t)N + 64 + 2 * (size_t)N * N + 2 * nb2 * SB * SB + nb2;
+    size_t d = 2 * (size_t)N + 64 + 3 * (size_t)N * N + 4 * nb2 * SB * SB + 2 * nb2;
     return (d + 63) & ~(size_t)63;
 }
 size_t eigh_work_bytes(int n) { return 8 * work_doubles(padded_n(n)) + 4096; }
@@ -516,6 +581,23 @@ static int finish_one(cudaStream_t st, int n, int N, double* lam_u, int* idx, do
         fprintf(stderr, "[tatrg eigh n=%d] spectrum: >1e-4:%d >1e-8:%d >1e-12:%d >1e-14:%d >1e-16:%d\n", n, c[0], c[1], c[2], c[3], c[4]);
     }
     return TATRG_OK;
+}
+
+// auxiliary stream + events of the two-stream round pipeline (created once per process, never destroyed)
+struct Aux { cudaStream_t st = nullptr; cudaEvent_t evS[2], evA[2], ev0; bool ok = false; };
+static Aux& aux() {
+    static Aux a;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        int lo = 0, hi = 0;
+        cudaDeviceGetStreamPriorityRange(&lo, &hi);          // hi = greatest priority (numerically lowest)
+        bool ok = cudaStreamCreateWithPriority(&a.st, cudaStreamNonBlocking, hi) == cudaSuccess;
+        for (int i = 0; i < 2 && ok; ++i) ok = cudaEventCreateWithFlags(&a.evS[i], cudaEventDisableTiming) == cudaSuccess && cudaEventCreateWithFlags(&a.evA[i], cudaEventDisableTiming) == cudaSuccess;
+        if (ok) ok = cudaEventCreateWithFlags(&a.ev0, cudaEventDisableTiming) == cudaSuccess;
+        a.ok = ok;
+    }
+    return a;
 }
 
 // Eigen-decompositions of up to kMaxBatch independent symmetric matrices in the same launches: the pair solver runs
@@ -555,30 +637,53 @@ int eigh_batched(cudaStream_t st, int count, const EighItem* items, void* work, 
         const int bc = std::min(kMaxBatch, count - z0);
         BatchIn bin;
         for (int z = 0; z < bc; ++z) { bin.n[z] = items[z0 + z].n; bin.G[z] = items[z0 + z].G; }
-        double* Vu0 = Vu(z0); double* Gp0 = Vu0 + (int64_t)N * N;
-        double* Jb0 = Gp0 + (int64_t)N * N; double* Dg0 = Jb0 + (int64_t)npair * SB * SB;
-        int* active0 = (int*)(Dg0 + (int64_t)npair * SB * SB);
+        double* Vu0 = Vu(z0);
+        double* Gbuf[2] = {Vu0 + (int64_t)N * N, Vu0 + 2 * (int64_t)N * N};
+        double* Jbuf[2]; double* Dbuf[2]; int* abuf[2];
+        Jbuf[0] = Gbuf[1] + (int64_t)N * N; Jbuf[1] = Jbuf[0] + (int64_t)npair * SB * SB;
+        Dbuf[0] = Jbuf[1] + (int64_t)npair * SB * SB; Dbuf[1] = Dbuf[0] + (int64_t)npair * SB * SB;
+        abuf[0] = (int*)(Dbuf[1] + (int64_t)npair * SB * SB); abuf[1] = abuf[0] + 2 * ((npair + 1) / 2);
         double* misc0 = misc(z0);
         int* counter = (int*)misc0 + 8;
-        pad_sym_kernel<<<dim3(148 * 2, bc), 256, 0, st>>>(bin, N, Gp0, Vu0, ws);
-        diag_max_kernel<<<bc, 256, 0, st>>>(N, Gp0, misc0, kFloorRel, ws);
+        pad_sym_kernel<<<dim3(148 * 2, bc), 256, 0, st>>>(bin, N, Gbuf[0], Vu0, ws);
+        diag_max_kernel<<<bc, 256, 0, st>>>(N, Gbuf[0], misc0, kFloorRel, ws);
         count_launch(2);
-        int sweep = 0;
-        for (; sweep < kMaxSweeps; ++sweep) {
-            cudaMemsetAsync(counter, 0, sizeof(int), st);
-            for (int r = 0; r < nb - 1; ++r) {
-                blk_solve2_kernel<<<dim3(npair, bc), 1024, kSolve2Smem, st>>>(N, nb, r, r == 0 ? 0 : 1, Gp0, misc0, Jb0, Dg0, active0, counter, ws);
-                blk_apply2_kernel<<<dim3(N / SB, 2 * npair, bc), 256, kApplySmem, st>>>(N, nb, r, Gp0, Vu0, Jb0, Dg0, active0, ws);
+        // Two streams: the pair solver of round t+1 assembles its sub-problems from the previous round's solver outputs and the
+        // matrix BEFORE that round's rotations (G[t % 2]), so it does not wait for apply(t), which writes G[(t+1) % 2].  The
+        // solvers run on a high-priority auxiliary stream (their few large CTAs must get an SM as soon as one apply CTA
+        // retires), the applies on the caller's stream.  A round then costs max(solver, apply) instead of their sum.
+        Aux& ax = aux();
+        if (!ax.ok) { if (err) *err = "eigh: cannot create the auxiliary stream"; return TATRG_ECUDA; }
+        cudaStream_t ss = ax.st;                       // solver stream
+        cudaEventRecord(ax.ev0, st);
+        cudaStreamWaitEvent(ss, ax.ev0, 0);
+        int t = 0, sweep = 0;
+        for (; sweep < kMaxBlockSweeps; ++sweep) {
+            cudaMemsetAsync(counter, 0, sizeof(int), ss);
+            for (int r = 0; r < nb - 1; ++r, ++t) {
+                const int cur = t & 1, prv = cur ^ 1;
+                // solve(t): needs solve(t-1) (stream order) and apply(t-2): it wrote G[prv], the buffer read here, and was the last
+                // reader of the J/D/active buffers of parity `cur`
+                if (t >= 2) cudaStreamWaitEvent(ss, ax.evA[prv], 0);
+                const int prev_round = (t == 0) ? -1 : (r == 0 ? nb - 2 : r - 1);
+                blk_solve2_kernel<<<dim3(npair, bc), 1024, kSolve2Smem, ss>>>(N, nb, r, prev_round, r == 0 ? 0 : 1, t == 0 ? Gbuf[0] : Gbuf[prv], misc0,
+                                                                              Jbuf[prv], Dbuf[prv], Jbuf[cur], Dbuf[cur], abuf[cur], counter, ws);
+                cudaEventRecord(ax.evS[cur], ss);
+                // apply(t): G[cur] -> G[prv] with the rotations of solve(t); apply(t-1) precedes it in stream order
+                cudaStreamWaitEvent(st, ax.evS[cur], 0);
+                blk_apply2_kernel<<<dim3(N / SB, 2 * npair, bc), 256, kApplySmem, st>>>(N, nb, r, Gbuf[cur], Gbuf[prv], Vu0, Jbuf[cur], Dbuf[cur], abuf[cur], ws);
+                cudaEventRecord(ax.evA[prv], st);         // evA[p]: "the apply that wrote G[p] is done"
                 count_launch(2);
             }
             int rot = 0;
-            if (!check(cudaMemcpyAsync(&rot, counter, sizeof(int), cudaMemcpyDeviceToHost, st), err, "eigh readback")) return TATRG_ECUDA;
-            if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;
+            if (!check(cudaMemcpyAsync(&rot, counter, sizeof(int), cudaMemcpyDeviceToHost, ss), err, "eigh readback")) return TATRG_ECUDA;
+            if (!check(cudaStreamSynchronize(ss), err, "eigh sync")) return TATRG_ECUDA;
             if (verbose) fprintf(stderr, "[tatrg eigh batch=%d N=%d] sweep %d rotations %d\n", bc, N, sweep, rot);
             if (rot == 0) break;
         }
-        if (sweep == kMaxSweeps) { if (err) *err = "eigh: block Jacobi did not converge"; return TATRG_ENUMERIC; }
-        for (int z = 0; z < bc; ++z) { extract_diag_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, Gp0 + z * ws, lam_u(z0 + z)); count_launch(); }
+        if (sweep == kMaxBlockSweeps) { if (err) *err = "eigh: block Jacobi did not converge"; return TATRG_ENUMERIC; }
+        double* Gfin = Gbuf[t & 1];
+        for (int z = 0; z < bc; ++z) { extract_diag_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, Gfin + z * ws, lam_u(z0 + z)); count_launch(); }
         for (int z = 0; z < bc; ++z) {
             const EighItem& it = items[z0 + z];
             int rc = finish_one(st, it.n, N, lam_u(z0 + z), idx(z0 + z), Vu(z0 + z), it.lam, it.Vt, it.lam_host, err);
