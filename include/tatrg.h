@@ -30,6 +30,9 @@ enum {
     TATRG_OPT_TAU = 3,         /* relative gap below which values form one multiplet (R7). default 1e-6 */
     TATRG_OPT_STAGE_TIMING = 4,/* 1: CUDA-event time per stage; 2: also per DGEMM / permute launch (tatrg_gemm_profile). default 0 */
     TATRG_OPT_KEEP_TENSORS = 5,/* 1: keep copies of the step's intermediate tensors for tatrg_get_tensor (tests). default 0 */
+    TATRG_OPT_SUBSPACE = 7,    /* 1 (default): the leading eigenvectors the triad isometries (top K of D^2, Eq. 2.9 :135) and the
+                                  squeezers (top D of D^2, :171) need come from a subspace iteration (Cholesky QR on the tensor
+                                  cores + one small Rayleigh-Ritz problem); 0: full eigen-decompositions everywhere.  Same result. */
     TATRG_OPT_METHOD = 6       /* 0: Triad-ATRG (default).  1: plain ATRG, Eq. 2.7-2.8 (:104-113): no triad split, squeezers from
                                   Gamma^ATRG, O(D^9) contraction sliced so that no D^7 tensor is stored (fn 6 :205).  Before the first
                                   step only; ENOMEM unless the workspace holds tatrg_workspace_bytes_atrg(D, oversample). */

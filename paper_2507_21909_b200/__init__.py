@@ -15,7 +15,7 @@ _LIB_PATH = os.path.join(_HERE, "libtatrg.so")
 _lib = None
 
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC, ESTATE = 0, -1, -2, -3, -4, -5
-OPT_POWER_ITERS, OPT_K_TRIAD, OPT_TAU, OPT_STAGE_TIMING, OPT_KEEP_TENSORS, OPT_METHOD = 1, 2, 3, 4, 5, 6
+OPT_POWER_ITERS, OPT_K_TRIAD, OPT_TAU, OPT_STAGE_TIMING, OPT_KEEP_TENSORS, OPT_METHOD, OPT_SUBSPACE = 1, 2, 3, 4, 5, 6, 7
 METHOD_TRIAD, METHOD_ATRG = 0, 1
 SV_SIGMA, SV_S = 0, 1
 STAGES = ["decompose", "bond_swap", "_rsvd", "_lift", "triad", "_triad_tensors", "squeezer_grams", "squeezers", "contract",

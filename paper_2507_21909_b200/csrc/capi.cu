@@ -60,6 +60,7 @@ int tatrg_set_option(tatrg_handle c, int key, double value) {
         case TATRG_OPT_TAU: if (c->m > 0) return TATRG_ESTATE; if (!(value >= 0) || value > 0.1) return TATRG_EINVAL; c->tau = value; return TATRG_OK;
         case TATRG_OPT_STAGE_TIMING: c->timing = (int)value; return TATRG_OK;
         case TATRG_OPT_KEEP_TENSORS: c->keep_tensors = value != 0; return TATRG_OK;
+        case TATRG_OPT_SUBSPACE: c->use_subspace = value != 0; return TATRG_OK;
         case TATRG_OPT_METHOD:
             if (c->m > 0) return TATRG_ESTATE;
             if (value != 0 && value != 1) return TATRG_EINVAL;

@@ -85,6 +85,16 @@ size_t svd_rows_work_bytes(int nv, int len);
 int svd_rows(cudaStream_t st, int nv, int len, const double* X, double* s, double* Ut, double* Vacc, void* work,
              std::vector<double>* s_host, std::string* err);
 
+// cholesky.cu : blocked Cholesky (64-wide panels: one-CTA diagonal factor + inverse, DGEMM panel / trailing updates) and
+// the triangular solve Q = X L^-T.  All asynchronous on st.
+cudaError_t symmetrize(cudaStream_t st, int n, double* A);                      // A = (A + A^T) / 2 in place
+size_t cholesky_work_doubles(int n);
+cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, int64_t ldl, double shift, double guard_rel, double* work);
+const int* cholesky_info(const double* work, int n);                            // [dev] bit 0: a pivot was raised to the guard, bit 1: non-finite
+cudaError_t trsm_right_lt(cudaStream_t st, int64_t m, int n, double* X, int64_t ldx, double* Q, int64_t ldq, const double* L, int64_t ldl,
+                          const double* work);
+cudaError_t extract_diag(cudaStream_t st, int n, const double* A, int64_t lda, double* d);
+
 // ---- tensors and the workspace pool -------------------------------------------------------------------------
 struct Tens {
     double* p = nullptr;

@@ -127,6 +127,13 @@ struct Stepper {
         if (part) c.pool.free(part);
         return C;
     }
+    // the same into caller-provided storage (leading dimension ldc)
+    void mm_into(double* C, int64_t ldc, bool ta, bool tb, int64_t M, int64_t N, int64_t K, const double* A, int64_t lda, const double* B, int64_t ldb) {
+        int64_t need = dgemm_splitk_doubles(M, N, K);
+        double* part = need ? c.pool.alloc(need) : nullptr;
+        ck(dgemm_splitk(st, ta, tb, M, N, K, 1.0, A, lda, B, ldb, C, ldc, part), "dgemm");
+        if (part) c.pool.free(part);
+    }
     std::vector<double> to_host(const double* d, int64_t n) {
         std::vector<double> h(n);
         ck(cudaMemcpyAsync(h.data(), d, 8 * n, cudaMemcpyDeviceToHost, st), "readback");
@@ -229,6 +236,93 @@ struct Stepper {
             R[i] = make({r, n});
             ck(scale_rows(st, R[i].p, eo[i].Vt.p, eo[i].lam, r, n, 3), "scale");
             keep(Q[i]); keep(R[i]);
+        }
+    }
+
+
+    // ---- leading invariant subspaces by subspace iteration ------------------------------------------------------
+    // The triad isometries (Eq. 2.9 :135) need the top K of n = D^2 eigenvectors of a Gram matrix, the squeezers (:171,
+    // R6) the top D of the n eigenvectors of Theta_b Theta_f.  Orthogonal iteration on a block of b = 2 kmax vectors
+    // (Z <- orthonormalise(A Z), Cholesky QR on the tensor cores) converges to that subspace like (lam_{b+1}/lam_k)^q and
+    // ends with ONE b x b Rayleigh-Ritz eigen-problem instead of n x n ones.
+    //   symmetric problem  (F == nullptr): A = Bm,     Z^T Z = 1
+    //   product problem    (F != nullptr): A = Bm F,   self-adjoint in the F inner product: Z^T F Z = 1, W = F Z carried along
+    // The iteration count comes from the measured convergence ratio: the diagonal of the Cholesky factor of orthogonal
+    // iteration tends to the eigenvalues, rho = r_b / r_kmax, q = 13 digits / log10(1/rho) (+ margin).
+    struct SubProb {
+        const double* Bm; const double* F; int n, kmax, b; uint32_t sid;
+        Tens buf[2], Gm, L, H; double* cw; double* dg;
+        std::vector<double> r;
+        int done = 0, target = 0;
+        bool ok = true;
+        const double* Z() const { return buf[0].p; }
+        const double* W() const { return F ? buf[0].p + (int64_t)n * b : buf[0].p; }
+    };
+    static int sub_block(int n, int kmax) { int b = 2 * kmax; b = (b + 31) / 32 * 32; return b; }
+    static bool sub_applicable(int n, int kmax) { return n > 128 && kmax >= 8 && sub_block(n, kmax) * 2 <= n; }
+    void sub_orth(SubProb& s, double shift) {      // buf[1] = [Z'; W'] -> buf[0] = [Z; W]
+        const int64_t rows = s.F ? 2 * (int64_t)s.n : s.n;
+        const double* Wp = s.F ? s.buf[1].p + (int64_t)s.n * s.b : s.buf[1].p;
+        mm_into(s.Gm.p, s.b, true, false, s.b, s.b, s.n, s.buf[1].p, s.b, Wp, s.b);
+        ck(cholesky(st, s.b, s.Gm.p, s.b, s.L.p, s.b, shift, 1e-14, s.cw), "cholesky");
+        ck(trsm_right_lt(st, rows, s.b, s.buf[1].p, s.b, s.buf[0].p, s.b, s.L.p, s.b, s.cw), "trsm");
+    }
+    void sub_apply(SubProb& s) {                   // buf[1] = [A Z; F A Z]
+        mm_into(s.buf[1].p, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, s.W(), s.b);
+        if (s.F) mm_into(s.buf[1].p + (int64_t)s.n * s.b, s.b, false, false, s.n, s.b, s.n, s.F, s.n, s.buf[1].p, s.b);
+    }
+    // Runs the iterations of all problems (interleaved so that the host reads the convergence estimates of all of them
+    // with one synchronisation per phase) and leaves in every s.H the b x b Rayleigh-Ritz matrix.  Problems that cannot
+    // be handled (rank-deficient leading block, no convergence in sight) come back with ok = false.
+    void sub_iterate(std::vector<SubProb>& ps) {
+        constexpr int q0 = 6, qmax = 96;
+        constexpr double kShift = 1e-13;
+        static const bool verbose = getenv("TATRG_SUB_VERBOSE") != nullptr;   // debugging aid only
+        for (SubProb& s : ps) {
+            const int64_t rows = s.F ? 2 * (int64_t)s.n : s.n;
+            s.buf[0] = make({rows, s.b}); s.buf[1] = make({rows, s.b});
+            s.Gm = make({s.b, s.b}); s.L = make({s.b, s.b}); s.H = make({s.b, s.b});
+            s.cw = raw((int64_t)cholesky_work_doubles(s.b)); s.dg = raw(s.b);
+            ck(fill_zero(st, s.L.p, (int64_t)s.b * s.b), "zero");
+            ck(philox_gauss(st, c.seed, (uint32_t)call, s.sid, 0, (int64_t)s.n * s.b, s.buf[1].p), "philox");
+            if (s.F) mm_into(s.buf[1].p + (int64_t)s.n * s.b, s.b, false, false, s.n, s.b, s.n, s.F, s.n, s.buf[1].p, s.b);
+            sub_orth(s, kShift);
+            for (int i = 0; i < q0; ++i) { sub_apply(s); sub_orth(s, kShift); }
+            s.done = q0;
+            ck(extract_diag(st, s.b, s.L.p, s.b, s.dg), "diag");
+        }
+        auto estimate = [&](SubProb& s) {
+            s.r = to_host(s.dg, s.b);
+            for (double v : s.r) if (!std::isfinite(v)) { s.ok = false; return; }
+            double tail = 0; for (int j = s.b - 4; j < s.b; ++j) tail = std::max(tail, s.r[j]);
+            double head = s.r[0]; for (int j = 0; j < s.kmax; ++j) head = std::min(head, s.r[j]);
+            if (!(head > 1e-12 * s.r[0]) || !(tail > 0)) { s.ok = false; return; }     // rank-deficient leading block: full decomposition
+            const double rho = 1.1 * tail / head;
+            if (!(rho < 0.8)) { s.ok = false; return; }
+            s.target = std::max(s.target, (int)std::ceil(13.0 / std::log10(1.0 / rho)) + 2);
+            if (s.target > qmax) s.ok = false;
+            if (verbose) fprintf(stderr, "[tatrg subspace n=%d b=%d kmax=%d%s] after %d iterations: rho %.3f -> %d iterations\n", s.n, s.b, s.kmax, s.F ? " product" : "", s.done, rho, s.target);
+        };
+        for (int pass = 0; pass < 3; ++pass) {
+            bool more = false;
+            for (SubProb& s : ps) if (s.ok) { estimate(s); if (s.ok && s.target > s.done) more = true; }
+            if (!more) break;
+            for (SubProb& s : ps) {
+                if (!s.ok) continue;
+                for (; s.done < s.target; ++s.done) { sub_apply(s); sub_orth(s, kShift); }
+                ck(extract_diag(st, s.b, s.L.p, s.b, s.dg), "diag");
+            }
+        }
+        for (SubProb& s : ps) {
+            if (!s.ok) continue;
+            // second orthonormalisation pass without shift (the basis is orthonormal to ~1e-13 already), W = F Z recomputed
+            const int64_t nb = (int64_t)s.n * s.b;
+            ck(cudaMemcpyAsync(s.buf[1].p, s.buf[0].p, 8 * nb, cudaMemcpyDeviceToDevice, st), "copy"); count_launch();
+            if (s.F) mm_into(s.buf[1].p + nb, s.b, false, false, s.n, s.b, s.n, s.F, s.n, s.buf[1].p, s.b);
+            sub_orth(s, 0.0);
+            // Rayleigh-Ritz matrix H = W^T Bm W (product) or Z^T Bm Z
+            mm_into(s.buf[1].p, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, s.W(), s.b);
+            mm_into(s.H.p, s.b, true, false, s.b, s.b, s.n, s.W(), s.b, s.buf[1].p, s.b);
         }
     }
 
@@ -426,19 +520,50 @@ void Stepper::triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y,
     }
     {
         Scope s2(*this);
+        const int kmax = (int)std::min<int64_t>(c.Ktri, n);
+        const double eps_sv = std::sqrt(kEpsLambda);
+        bool have[4] = {false, false, false, false};
+        if (c.use_subspace && sub_applicable((int)n, kmax)) {
+            // top-K eigenvectors by subspace iteration + one b x b Rayleigh-Ritz problem per Gram matrix
+            std::vector<SubProb> ps(4);
+            for (int i = 0; i < 4; ++i) {
+                ck(symmetrize(st, (int)n, gram[i].p), "symmetrize");
+                ps[i].Bm = gram[i].p; ps[i].F = nullptr; ps[i].n = (int)n; ps[i].kmax = kmax; ps[i].b = sub_block((int)n, kmax); ps[i].sid = 16 + i;
+            }
+            sub_iterate(ps);
+            std::vector<Tens*> hs; std::vector<int> ns, who;
+            for (int i = 0; i < 4; ++i) if (ps[i].ok) { hs.push_back(&ps[i].H); ns.push_back(ps[i].b); who.push_back(i); }
+            std::vector<EigOut> er;
+            if (!hs.empty()) eig_batch(hs, ns, er);
+            for (size_t j = 0; j < who.size(); ++j) {
+                const int i = who[j], b = ps[i].b;
+                std::vector<double> sv(b);
+                for (int t = 0; t < b; ++t) sv[t] = std::sqrt(std::max(er[j].lh[t], 0.0));
+                if (!(sv[kmax] > eps_sv * sv[0])) continue;              // numerical rank <= kmax: the full decomposition decides
+                const int k = select_rank(sv, kmax, eps_sv, c.tau);
+                if (k <= 0) continue;
+                U[i] = mm(false, true, k, n, b, er[j].Vt.p, b, ps[i].Z(), b);     // rows: Ritz vectors Y_k^T Z^T
+                U[i] = view(U[i], {k, d2, d3});
+                keep(U[i]);
+                have[i] = true;
+            }
+        }
+        std::vector<Tens*> gs; std::vector<int> ns, who;
+        for (int i = 0; i < 4; ++i) if (!have[i]) { gs.push_back(&gram[i]); ns.push_back((int)n); who.push_back(i); }
         std::vector<EigOut> eo;
-        eig_batch({&gram[0], &gram[1], &gram[2], &gram[3]}, {(int)n, (int)n, (int)n, (int)n}, eo);
-        for (int i = 0; i < 4; ++i) {
-            drop(gram[i]);
-            const std::vector<double>& lh = eo[i].lh;
+        if (!gs.empty()) eig_batch(gs, ns, eo);
+        for (size_t j = 0; j < who.size(); ++j) {
+            const int i = who[j];
+            const std::vector<double>& lh = eo[j].lh;
             std::vector<double> sv(lh.size());
-            for (size_t j = 0; j < lh.size(); ++j) sv[j] = std::sqrt(std::max(lh[j], 0.0));    // multiplet rule on the singular-value scale
-            const int k = select_rank(sv, std::min<int64_t>(c.Ktri, n), std::sqrt(kEpsLambda), c.tau);
+            for (size_t t = 0; t < lh.size(); ++t) sv[t] = std::sqrt(std::max(lh[t], 0.0));    // multiplet rule on the singular-value scale
+            const int k = select_rank(sv, kmax, eps_sv, c.tau);
             if (k <= 0) fail(TATRG_ENUMERIC, "triad: empty isometry");
             U[i] = make({k, d2, d3});
-            ck(cudaMemcpyAsync(U[i].p, eo[i].Vt.p, 8 * (int64_t)k * n, cudaMemcpyDeviceToDevice, st), "copy"); count_launch();
+            ck(cudaMemcpyAsync(U[i].p, eo[j].Vt.p, 8 * (int64_t)k * n, cudaMemcpyDeviceToDevice, st), "copy"); count_launch();
             keep(U[i]);
         }
+        for (int i = 0; i < 4; ++i) drop(gram[i]);
     }
     e = ein("mjk,Ijkla->Imla", U[0], a);                                   // Eq. 2.10
     Tens f0 = ein("xjk,Ajklg->Axlg", U[1], x);                             // Eq. 2.11 (sigma goes into F only)
@@ -486,45 +611,100 @@ void Stepper::half_grams(const Tens& P, const Tens& Q, const Tens& Iu, const Ten
 // The six Gram matrices are eigen-decomposed in one batch, then the three (R1 R2)^T (R1 R2) in another.
 void Stepper::squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], Tens Nt[3]) {
     Scope sc(*this);
-    std::vector<EigOut> eo;
+    // per direction: s (host, leading values), wt [k x n] = (R2 V)^T, nt [k x n] = (Theta_f R2 V)^T
+    std::vector<double> sval[3]; Tens wts[3], nts[3]; int kk[3] = {0, 0, 0}; bool have[3] = {false, false, false};
+    // (1) M spans the leading eigenvectors of Theta_b Theta_f (Theta_b Theta_f M = M s^2, N = Theta_f M s^-1): subspace
+    //     iteration in the Theta_f inner product needs no factor R1, R2 at all.  With Z^T Theta_f Z = 1 and Ritz vectors Y:
+    //     R2 V = Z Y s,  Theta_f R2 V = W Y s.
     {
-        std::vector<Tens*> gs; std::vector<int> ns;
-        for (int d = 0; d < 3; ++d) { gs.push_back(&thf[d]); ns.push_back(du[d] * du[d]); gs.push_back(&thb[d]); ns.push_back(du[d] * du[d]); }
-        eig_batch(gs, ns, eo);
-        for (int d = 0; d < 3; ++d) { drop(thf[d]); drop(thb[d]); }
+        std::vector<SubProb> ps; std::vector<int> dirs;
+        for (int d = 0; d < 3; ++d) {
+            const int n = du[d] * du[d];
+            if (!c.use_subspace || !sub_applicable(n, c.D)) continue;
+            ck(symmetrize(st, n, thf[d].p), "symmetrize"); ck(symmetrize(st, n, thb[d].p), "symmetrize");
+            SubProb sp; sp.Bm = thb[d].p; sp.F = thf[d].p; sp.n = n; sp.kmax = c.D; sp.b = sub_block(n, c.D); sp.sid = 24 + (uint32_t)d;
+            ps.push_back(sp); dirs.push_back(d);
+        }
+        if (!ps.empty()) {
+            Scope s2(*this);
+            sub_iterate(ps);
+            std::vector<Tens*> hs; std::vector<int> ns, who;
+            for (size_t i = 0; i < ps.size(); ++i) if (ps[i].ok) { hs.push_back(&ps[i].H); ns.push_back(ps[i].b); who.push_back((int)i); }
+            std::vector<EigOut> er;
+            if (!hs.empty()) eig_batch(hs, ns, er);
+            for (size_t j = 0; j < who.size(); ++j) {
+                const SubProb& sp = ps[who[j]];
+                const int d = dirs[who[j]], b = sp.b, n = sp.n;
+                std::vector<double> s(b);
+                for (int t = 0; t < b; ++t) s[t] = std::sqrt(std::max(er[j].lh[t], 0.0));
+                if (!(s[c.D] > kEpsSqueezer * s[0])) continue;          // numerical rank <= D: the full decomposition decides
+                const int k = select_rank(s, c.D, kEpsSqueezer, c.tau);
+                if (k <= 0) continue;
+                std::vector<double> sk(s.begin(), s.begin() + k);
+                double* sd = to_dev(sk);
+                wts[d] = mm(false, true, k, n, b, er[j].Vt.p, b, sp.Z(), b);
+                nts[d] = mm(false, true, k, n, b, er[j].Vt.p, b, sp.W(), b);
+                ck(scale_rows(st, wts[d].p, wts[d].p, sd, k, n, 0), "scale");
+                ck(scale_rows(st, nts[d].p, nts[d].p, sd, k, n, 0), "scale");
+                keep(wts[d]); keep(nts[d]);
+                sval[d] = s; kk[d] = k; have[d] = true;
+            }
+        }
     }
-    Tens r1[3], r2t[3], cm[3], gc[3];
-    int k1[3], k2[3];
-    for (int d = 0; d < 3; ++d) {
-        const int n = du[d] * du[d];
-        const std::vector<double>&l1 = eo[2 * d].lh, &l2 = eo[2 * d + 1].lh;
-        if (!(l1[0] > 0) || !(l2[0] > 0)) fail(TATRG_ENUMERIC, "squeezer %d: zero Gram matrix", d + 2);
-        k1[d] = k2[d] = 0;
-        for (double v : l1) if (v > kEpsLambda * l1[0]) ++k1[d];
-        for (double v : l2) if (v > kEpsLambda * l2[0]) ++k2[d];
-        r1[d] = make({k1[d], n}); r2t[d] = make({k2[d], n});
-        ck(scale_rows(st, r1[d].p, eo[2 * d].Vt.p, eo[2 * d].lam, k1[d], n, 3), "scale");          // R1 = Lambda1^1/2 W1^T
-        ck(scale_rows(st, r2t[d].p, eo[2 * d + 1].Vt.p, eo[2 * d + 1].lam, k2[d], n, 3), "scale");  // R2^T
-        drop(eo[2 * d].Vt); drop(eo[2 * d + 1].Vt);
-        cm[d] = mm(false, true, k1[d], k2[d], n, r1[d].p, n, r2t[d].p, n);                            // R1 R2
-        gc[d] = mm(true, false, k2[d], k2[d], k1[d], cm[d].p, k2[d], cm[d].p, k2[d]);                 // (R1 R2)^T (R1 R2): V, s^2
+    // (2) full decompositions for the directions the iteration does not cover (small or rank-deficient problems):
+    //     the Gram matrices are eigen-decomposed in one batch, then the (R1 R2)^T (R1 R2) in another.
+    std::vector<int> todo;
+    for (int d = 0; d < 3; ++d) if (!have[d]) todo.push_back(d);
+    if (!todo.empty()) {
+        std::vector<EigOut> eo;
+        {
+            std::vector<Tens*> gs; std::vector<int> ns;
+            for (int d : todo) { gs.push_back(&thf[d]); ns.push_back(du[d] * du[d]); gs.push_back(&thb[d]); ns.push_back(du[d] * du[d]); }
+            eig_batch(gs, ns, eo);
+        }
+        Tens r1[3], r2t[3], cm[3], gc[3];
+        int k1[3], k2[3];
+        std::vector<Tens*> gcs; std::vector<int> gns;
+        for (size_t j = 0; j < todo.size(); ++j) {
+            const int d = todo[j], n = du[d] * du[d];
+            const std::vector<double>&l1 = eo[2 * j].lh, &l2 = eo[2 * j + 1].lh;
+            if (!(l1[0] > 0) || !(l2[0] > 0)) fail(TATRG_ENUMERIC, "squeezer %d: zero Gram matrix", d + 2);
+            k1[d] = k2[d] = 0;
+            for (double v : l1) if (v > kEpsLambda * l1[0]) ++k1[d];
+            for (double v : l2) if (v > kEpsLambda * l2[0]) ++k2[d];
+            r1[d] = make({k1[d], n}); r2t[d] = make({k2[d], n});
+            ck(scale_rows(st, r1[d].p, eo[2 * j].Vt.p, eo[2 * j].lam, k1[d], n, 3), "scale");          // R1 = Lambda1^1/2 W1^T
+            ck(scale_rows(st, r2t[d].p, eo[2 * j + 1].Vt.p, eo[2 * j + 1].lam, k2[d], n, 3), "scale");  // R2^T
+            drop(eo[2 * j].Vt); drop(eo[2 * j + 1].Vt);
+            cm[d] = mm(false, true, k1[d], k2[d], n, r1[d].p, n, r2t[d].p, n);                            // R1 R2
+            gc[d] = mm(true, false, k2[d], k2[d], k1[d], cm[d].p, k2[d], cm[d].p, k2[d]);                 // (R1 R2)^T (R1 R2): V, s^2
+            gcs.push_back(&gc[d]); gns.push_back(k2[d]);
+        }
+        std::vector<EigOut> ec;
+        eig_batch(gcs, gns, ec);
+        for (size_t j = 0; j < todo.size(); ++j) {
+            const int d = todo[j], n = du[d] * du[d];
+            drop(gc[d]);
+            const std::vector<double>& lc = ec[j].lh;
+            std::vector<double> s(lc.size());
+            for (size_t i = 0; i < lc.size(); ++i) s[i] = std::sqrt(std::max(lc[i], 0.0));
+            const int k = select_rank(s, c.D, kEpsSqueezer, c.tau);
+            if (k <= 0) fail(TATRG_ENUMERIC, "squeezer %d: empty", d + 2);
+            const Tens& Vc = ec[j].Vt;
+            wts[d] = mm(false, false, k, n, k2[d], Vc.p, k2[d], r2t[d].p, n);        // (R2 V)^T
+            Tens cv = mm(false, true, k, k1[d], k2[d], Vc.p, k2[d], cm[d].p, k2[d]); // (R1 R2 V)^T = (U s)^T
+            nts[d] = mm(false, false, k, n, k1[d], cv.p, k1[d], r1[d].p, n);         // (R1^T U s)^T
+            sval[d] = s; kk[d] = k;
+        }
     }
-    std::vector<EigOut> ec;
-    eig_batch({&gc[0], &gc[1], &gc[2]}, {k2[0], k2[1], k2[2]}, ec);
+    for (int d = 0; d < 3; ++d) { drop(thf[d]); drop(thb[d]); }
+    // (3) gauge (R10), s^-1/2 scalings
     for (int d = 0; d < 3; ++d) {
-        const int n = du[d] * du[d], dir = d + 2;
-        drop(gc[d]);
-        const std::vector<double>& lc = ec[d].lh;
-        std::vector<double> s(lc.size());
-        for (size_t i = 0; i < lc.size(); ++i) s[i] = std::sqrt(std::max(lc[i], 0.0));
-        const int k = select_rank(s, c.D, kEpsSqueezer, c.tau);
-        if (k <= 0) fail(TATRG_ENUMERIC, "squeezer %d: empty", dir);
+        const int n = du[d] * du[d], dir = d + 2, k = kk[d];
+        const std::vector<double>& s = sval[d];
         std::vector<double> sk(s.begin(), s.begin() + k);
         double* sd = to_dev(sk);
-        const Tens& Vc = ec[d].Vt;
-        Tens wt = mm(false, false, k, n, k2[d], Vc.p, k2[d], r2t[d].p, n);       // (R2 V)^T
-        Tens cv = mm(false, true, k, k1[d], k2[d], Vc.p, k2[d], cm[d].p, k2[d]); // (R1 R2 V)^T = (U s)^T
-        Tens nt = mm(false, false, k, n, k1[d], cv.p, k1[d], r1[d].p, n);        // (R1^T U s)^T
+        Tens& wt = wts[d]; Tens& nt = nts[d];
         Tens Gm = gauge(wt, false, s, k, (uint32_t)dir);
         ck(scale_rows(st, wt.p, wt.p, sd, k, n, 2), "scale");                    // s^-1/2
         ck(scale_rows(st, nt.p, nt.p, sd, k, n, 4), "scale");                    // s^-3/2

@@ -18,6 +18,7 @@ struct tatrg_ctx {
     uint64_t seed = 0;
     int n_pow = 2, Ktri = 0;
     int method = 0;                  // 0: Triad-ATRG, 1: plain ATRG
+    bool use_subspace = true;        // leading subspaces by subspace iteration (false: full eigen-decompositions everywhere)
     double tau = tatrg::kTauDefault;
     int timing = 0;
     bool keep_tensors = false;
