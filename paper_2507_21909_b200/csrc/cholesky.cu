@@ -148,7 +148,7 @@ cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, 
     }
     return cudaGetLastError();
 }
-const double* cholesky_linv(const double* work) { return work; }
+const double* cholesky_d0(const double* work, int n) { return work + (size_t)((n + PB - 1) / PB) * PB * PB; }
 const int* cholesky_info(const double* work, int n) { return (const int*)(work + (size_t)((n + PB - 1) / PB) * PB * PB + n); }
 
 // Q [m x n, ldq] = X [m x n, ldx] L^-T with L, Linv from cholesky().  X is overwritten (it holds the partially reduced
@@ -165,6 +165,26 @@ cudaError_t trsm_right_lt(cudaStream_t st, int64_t m, int n, double* X, int64_t 
             if (e != cudaSuccess) return e;
         }
         e = dgemm(st, false, true, m, nb, nb, 1.0, X + j0, ldx, Linv + (size_t)p * PB * PB, PB, 0.0, Q + j0, ldq);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+// X [n x n, ldx] = L^-1 (lower triangular; X must be zero-filled on entry) from the factor and the inverted diagonal blocks
+// that cholesky() left in work.  T: scratch of 64 x n doubles.  Row panel i: X[i, <i] = -Linv_ii (L[i, <i] X[<i, <i]).
+cudaError_t tri_inverse(cudaStream_t st, int n, const double* L, int64_t ldl, const double* work, double* X, int64_t ldx, double* T) {
+    const int np = (n + PB - 1) / PB;
+    const double* Linv = work;
+    for (int p = 0; p < np; ++p) {
+        const int i0 = p * PB, nb = n - i0 < PB ? n - i0 : PB;
+        cudaError_t e = cudaMemcpy2DAsync(X + (int64_t)i0 * ldx + i0, ldx * 8, Linv + (size_t)p * PB * PB, PB * 8, (size_t)nb * 8, nb,
+                                          cudaMemcpyDeviceToDevice, st);
+        count_launch();
+        if (e != cudaSuccess) return e;
+        if (i0 == 0) continue;
+        e = dgemm(st, false, false, nb, i0, i0, 1.0, L + (int64_t)i0 * ldl, ldl, X, ldx, 0.0, T, i0);
+        if (e != cudaSuccess) return e;
+        e = dgemm(st, false, false, nb, i0, nb, -1.0, Linv + (size_t)p * PB * PB, PB, T, i0, 0.0, X + (int64_t)i0 * ldx, ldx);
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;

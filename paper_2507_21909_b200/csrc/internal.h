@@ -93,6 +93,8 @@ cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, 
 const int* cholesky_info(const double* work, int n);                            // [dev] bit 0: a pivot was raised to the guard, bit 1: non-finite
 cudaError_t trsm_right_lt(cudaStream_t st, int64_t m, int n, double* X, int64_t ldx, double* Q, int64_t ldq, const double* L, int64_t ldl,
                           const double* work);
+cudaError_t tri_inverse(cudaStream_t st, int n, const double* L, int64_t ldl, const double* work, double* X, int64_t ldx, double* T);
+const double* cholesky_d0(const double* work, int n);                           // [dev] the n original diagonal entries
 cudaError_t extract_diag(cudaStream_t st, int n, const double* A, int64_t lda, double* d);
 
 // ---- tensors and the workspace pool -------------------------------------------------------------------------

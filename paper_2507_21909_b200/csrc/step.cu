@@ -216,10 +216,45 @@ struct Stepper {
         keep(Q); keep(R);
     }
 
+    // Cholesky QR of a tall matrix of full numerical rank (Eq. A.2-A.3 :345-348): G = mat^T mat = L L^T, R = L^T,
+    // Q = mat R^-1 (one GEMM with the explicit triangular inverse).  Same span and same product Q R as orth(); accepted
+    // only when the factor PROVES that orth() would drop nothing (R14): lam_min(G) = sigma_min(L)^2 >= 1 / ||L^-1||_F^2
+    // and lam_max(G) <= tr G, so 1 / (||L^-1||_F^2 tr G) > 1e-12 implies lam_min > 1e-12 lam_max.  Returns false otherwise.
+    bool orth_chol(const Tens& mat, Tens& Q, Tens& R) {
+        Scope sc(*this);
+        const int64_t m = mat.d[0], n = mat.d[1];
+        Tens G = mm(true, false, n, n, m, mat.p, n, mat.p, n);
+        Tens L = make({n, n}), X = make({n, n}), T = make({64, n});
+        double* cw = raw((int64_t)cholesky_work_doubles((int)n));
+        double* res = raw(1 + 148 * 8 + 7);
+        ck(fill_zero(st, L.p, n * n), "zero"); ck(fill_zero(st, X.p, n * n), "zero");
+        ck(cholesky(st, (int)n, G.p, n, L.p, n, 0.0, 1e-14, cw), "cholesky");
+        ck(tri_inverse(st, (int)n, L.p, n, cw, X.p, n, T.p), "tri_inverse");
+        ck(dot(st, n * n, X.p, X.p, res), "dot");
+        int info = 0;
+        ck(cudaMemcpyAsync(&info, cholesky_info(cw, (int)n), sizeof(int), cudaMemcpyDeviceToHost, st), "readback");
+        std::vector<double> d0 = to_host(cholesky_d0(cw, (int)n), n);
+        std::vector<double> xn = to_host(res, 1);
+        double tr = 0; for (double v : d0) tr += v;
+        if (getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg cholesky qr %lld x %lld] info %d, proven lam_min/lam_max >= %.3e\n", (long long)m, (long long)n, info, 1.0 / (xn[0] * tr));
+        if (info != 0 || !std::isfinite(xn[0]) || !(xn[0] > 0) || !(tr > 0)) return false;
+        if (!(1.0 / (xn[0] * tr) > kEpsOrthLambda)) return false;
+        Q = mm(false, true, m, n, n, mat.p, n, X.p, n);
+        R = perm(view(L, {n, n}), {1, 0});
+        keep(Q); keep(R);
+        return true;
+    }
+
     // orth() of two matrices of the same shape with n > 128 (single pass): the two Gram matrices are decomposed together
     void orth_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2]) {
         const int64_t m = m0.d[0], n = m0.d[1];
         if (n <= 128 || m1.d[0] != m || m1.d[1] != n) { orth(m0, Q[0], R[0]); orth(m1, Q[1], R[1]); return; }
+        if (c.use_subspace) {
+            const bool ok0 = orth_chol(m0, Q[0], R[0]), ok1 = orth_chol(m1, Q[1], R[1]);
+            if (ok0 && ok1) return;
+            if (ok0) drop(Q[0]), drop(R[0]);
+            if (ok1) drop(Q[1]), drop(R[1]);
+        }
         Scope sc(*this);
         const Tens* mats[2] = {&m0, &m1};
         Tens G[2];
