@@ -192,7 +192,7 @@ dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, co
 
 struct Args {
     cudaStream_t st; int64_t M, N, K, Klast; double alpha; const double* A; int64_t lda; const double* B; int64_t ldb; double beta;
-    double* C; int64_t ldc; int batch; int64_t sA, sB, sC;
+    double* C; int64_t ldc; int batch; int64_t sA, sB, sC; bool force_small = false;
 };
 
 template <class C_, bool A_KC, bool B_KC, bool AV, bool BV>
@@ -224,7 +224,13 @@ cudaError_t pick_order(bool a_kc, bool b_kc, bool av, bool bv, const Args& a) {
     if (!a_kc && b_kc) return pick_vec<C_, false, true>(av, bv, a);
     return pick_vec<C_, false, false>(av, bv, a);
 }
-inline bool small_cfg(int64_t M, int64_t N) { return (M < N ? M : N) <= 64; }
+// S for skinny outputs, and for launches whose L tiles would cover at most a quarter of the 148 SMs (the small products of
+// the subspace iterations): there the number of CTAs in flight matters more than the reuse inside one tile.
+inline bool small_cfg(int64_t M, int64_t N, int64_t batch = 1) {
+    if ((M < N ? M : N) <= 64) return true;
+    const int64_t tl = ((M + CfgL::BM - 1) / CfgL::BM) * ((N + CfgL::BN - 1) / CfgL::BN);
+    return tl * batch <= 37;
+}
 
 cudaError_t dgemm_raw(bool transa, bool transb, const Args& a) {
     if (a.M <= 0 || a.N <= 0 || a.batch <= 0) return cudaSuccess;
@@ -236,14 +242,14 @@ cudaError_t dgemm_raw(bool transa, bool transb, const Args& a) {
     };
     const bool kodd = (a.K % 2 != 0) || (a.Klast % 2 != 0);
     const bool av = v16(a.A, a.lda, a_kc ? (kodd ? 1 : 2) : a.M, a.sA), bv = v16(a.B, a.ldb, b_kc ? (kodd ? 1 : 2) : a.N, a.sB);
-    if (small_cfg(a.M, a.N)) return pick_order<CfgS>(a_kc, b_kc, av, bv, a);
+    if (a.force_small || small_cfg(a.M, a.N, a.batch)) return pick_order<CfgS>(a_kc, b_kc, av, bv, a);
     return pick_order<CfgL>(a_kc, b_kc, av, bv, a);
 }
 }  // namespace
 
 static cudaError_t dgemm_klast(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, int64_t Klast, double alpha,
                                const double* A, int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch,
-                               int64_t sA, int64_t sB, int64_t sC) {
+                               int64_t sA, int64_t sB, int64_t sC, bool force_small = false) {
     if (M <= 0 || N <= 0 || batch <= 0) return cudaSuccess;
     Counters* c = g_counter;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -255,7 +261,7 @@ static cudaError_t dgemm_klast(cudaStream_t st, bool transa, bool transb, int64_
     for (int b0 = 0; b0 < batch && e == cudaSuccess; b0 += 32768) {
         int nb = batch - b0 < 32768 ? batch - b0 : 32768;
         Args a{st, M, N, K, (b0 + nb == batch) ? Klast : 0, alpha, A + (int64_t)b0 * sA, lda, B + (int64_t)b0 * sB, ldb, beta,
-               C + (int64_t)b0 * sC, ldc, nb, sA, sB, sC};
+               C + (int64_t)b0 * sC, ldc, nb, sA, sB, sC, force_small};
         e = dgemm_raw(transa, transb, a);
     }
     if (e0) { cudaEventRecord(e1, st); c->gemm_ev.push_back({e0, e1}); c->gemm_shapes.push_back({M, N, (int64_t)(kk / batch), batch, transa, transb}); }
@@ -273,13 +279,16 @@ namespace {
 // Number of K-chunks for a non-batched GEMM: the smallest split whose CTA count fills whole waves of the 148 SMs
 // (>= 93 % of the last wave used), chunks of >= 256, partials capped at 64 M doubles.  1 = no split.
 int splitk_count(int64_t M, int64_t N, int64_t K) {
-    const int bm = small_cfg(M, N) ? CfgS::BM : CfgL::BM, bn = small_cfg(M, N) ? CfgS::BN : CfgL::BN;
-    const int per_sm = small_cfg(M, N) ? 2 : 1;
+    const bool sm = small_cfg(M, N);
+    const int bm = sm ? CfgS::BM : CfgL::BM, bn = sm ? CfgS::BN : CfgL::BN;
+    const int per_sm = sm ? 2 : 1;
     const int64_t tiles = ((M + bm - 1) / bm) * ((N + bn - 1) / bn);
     const int64_t slots = 148 * per_sm;
     auto eff = [&](int64_t ctas) { int64_t waves = (ctas + slots - 1) / slots; return (double)ctas / (double)(waves * slots); };
-    if (K < 512 || eff(tiles) >= 0.93) return 1;
-    int64_t maxs = K / 256;
+    if (K < 256 || eff(tiles) >= 0.93) return 1;
+    // chunks of >= 256 for outputs that already give every SM a tile; down to 64 for the small products (a few tiles only)
+    const int64_t min_chunk = tiles >= slots ? 256 : (tiles * 4 >= slots ? 128 : 64);
+    int64_t maxs = K / min_chunk;
     if (maxs > 1024) maxs = 1024;
     const int64_t cap = (64LL << 20) / (M * N > 0 ? M * N : 1);
     if (maxs > cap) maxs = cap;
@@ -287,7 +296,7 @@ int splitk_count(int64_t M, int64_t N, int64_t K) {
     for (int64_t sp = 2; sp <= maxs; ++sp) {
         const double e = eff(tiles * sp);
         if (e >= 0.93) return (int)sp;
-        if (e > best_eff + 0.02) { best_eff = e; best = (int)sp; }
+        if (e > best_eff * 1.1) { best_eff = e; best = (int)sp; }
     }
     return best;
 }
@@ -317,7 +326,7 @@ cudaError_t dgemm_splitk(cudaStream_t st, bool transa, bool transb, int64_t M, i
     int64_t tail = K - (int64_t)(nchunks - 1) * chunk;
     const int64_t stepA = transa ? chunk * lda : chunk, stepB = transb ? chunk : chunk * ldb;
     cudaError_t e = dgemm_klast(st, transa, transb, M, N, chunk, tail == chunk ? 0 : tail, 1.0, A, lda, B, ldb, 0.0, part, N, nchunks,
-                                stepA, stepB, M * N);
+                                stepA, stepB, M * N, small_cfg(M, N));
     if (e != cudaSuccess) return e;
     int64_t MN = M * N;
     int64_t blocks = (MN + 255) / 256; if (blocks > 148 * 8) blocks = 148 * 8;

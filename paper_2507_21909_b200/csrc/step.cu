@@ -288,27 +288,41 @@ struct Stepper {
         const double* Bm; const double* F; int n, kmax, b; uint32_t sid;
         Tens buf[2], Gm, L, H; double* cw; double* dg;
         std::vector<double> r;
-        int done = 0, target = 0;
+        int cur = 0;                 // the basis [Z; W] lives in buf[cur]
+        int done = 0, target = 0, deg = 1;
         bool ok = true;
-        const double* Z() const { return buf[0].p; }
-        const double* W() const { return F ? buf[0].p + (int64_t)n * b : buf[0].p; }
+        const double* Z() const { return buf[cur].p; }
+        const double* W() const { return F ? buf[cur].p + (int64_t)n * b : buf[cur].p; }
     };
     static int sub_block(int n, int kmax) { int b = 2 * kmax; b = (b + 31) / 32 * 32; return b; }
     static bool sub_applicable(int n, int kmax) { return n > 128 && kmax >= 8 && sub_block(n, kmax) * 2 <= n; }
-    void sub_orth(SubProb& s, double shift) {      // buf[1] = [Z'; W'] -> buf[0] = [Z; W]
+    void sub_orth(SubProb& s, int src, double shift) {      // buf[src] = [Z'; W'] -> buf[src^1] = [Z; W], which becomes the basis
         const int64_t rows = s.F ? 2 * (int64_t)s.n : s.n;
-        const double* Wp = s.F ? s.buf[1].p + (int64_t)s.n * s.b : s.buf[1].p;
-        mm_into(s.Gm.p, s.b, true, false, s.b, s.b, s.n, s.buf[1].p, s.b, Wp, s.b);
+        double* X = s.buf[src].p;
+        const double* Wp = s.F ? X + (int64_t)s.n * s.b : X;
+        mm_into(s.Gm.p, s.b, true, false, s.b, s.b, s.n, X, s.b, Wp, s.b);
         ck(cholesky(st, s.b, s.Gm.p, s.b, s.L.p, s.b, shift, 1e-14, s.cw), "cholesky");
-        ck(trsm_right_lt(st, rows, s.b, s.buf[1].p, s.b, s.buf[0].p, s.b, s.L.p, s.b, s.cw), "trsm");
+        ck(trsm_right_lt(st, rows, s.b, X, s.b, s.buf[src ^ 1].p, s.b, s.L.p, s.b, s.cw), "trsm");
+        s.cur = src ^ 1;
     }
-    void sub_apply(SubProb& s) {                   // buf[1] = [A Z; F A Z]
-        mm_into(s.buf[1].p, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, s.W(), s.b);
-        if (s.F) mm_into(s.buf[1].p + (int64_t)s.n * s.b, s.b, false, false, s.n, s.b, s.n, s.F, s.n, s.buf[1].p, s.b);
+    void sub_apply(SubProb& s, int from) {         // buf[from^1] = [A Z; F A Z] with [Z; W] = buf[from]
+        const double* X = s.F ? s.buf[from].p + (int64_t)s.n * s.b : s.buf[from].p;
+        double* O = s.buf[from ^ 1].p;
+        mm_into(O, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, X, s.b);
+        if (s.F) mm_into(O + (int64_t)s.n * s.b, s.b, false, false, s.n, s.b, s.n, s.F, s.n, O, s.b);
+    }
+    void sub_step(SubProb& s, int deg, double shift) {      // deg applications of A, then one orthonormalisation
+        int a = s.cur;
+        for (int i = 0; i < deg; ++i) { sub_apply(s, a); a ^= 1; }
+        sub_orth(s, a, shift);
+        s.done += deg;
     }
     // Runs the iterations of all problems (interleaved so that the host reads the convergence estimates of all of them
     // with one synchronisation per phase) and leaves in every s.H the b x b Rayleigh-Ritz matrix.  Problems that cannot
     // be handled (rank-deficient leading block, no convergence in sight) come back with ok = false.
+    // After the first q0 single steps the columns are graded like the spectrum and Cholesky (invariant under column
+    // scaling) tolerates several applications of A per orthonormalisation, as long as the dynamic range of the block,
+    // (r_1 / r_b)^deg, stays below 1e11.
     void sub_iterate(std::vector<SubProb>& ps) {
         constexpr int q0 = 6, qmax = 96;
         constexpr double kShift = 1e-13;
@@ -321,9 +335,8 @@ struct Stepper {
             ck(fill_zero(st, s.L.p, (int64_t)s.b * s.b), "zero");
             ck(philox_gauss(st, c.seed, (uint32_t)call, s.sid, 0, (int64_t)s.n * s.b, s.buf[1].p), "philox");
             if (s.F) mm_into(s.buf[1].p + (int64_t)s.n * s.b, s.b, false, false, s.n, s.b, s.n, s.F, s.n, s.buf[1].p, s.b);
-            sub_orth(s, kShift);
-            for (int i = 0; i < q0; ++i) { sub_apply(s); sub_orth(s, kShift); }
-            s.done = q0;
+            sub_orth(s, 1, kShift);
+            for (int i = 0; i < q0; ++i) sub_step(s, 1, kShift);
             ck(extract_diag(st, s.b, s.L.p, s.b, s.dg), "diag");
         }
         auto estimate = [&](SubProb& s) {
@@ -332,19 +345,24 @@ struct Stepper {
             double tail = 0; for (int j = s.b - 4; j < s.b; ++j) tail = std::max(tail, s.r[j]);
             double head = s.r[0]; for (int j = 0; j < s.kmax; ++j) head = std::min(head, s.r[j]);
             if (!(head > 1e-12 * s.r[0]) || !(tail > 0)) { s.ok = false; return; }     // rank-deficient leading block: full decomposition
-            const double rho = 1.1 * tail / head;
+            // the diagonal of R is that of the last orthonormalisation: r_j ~ lam_j^deg
+            const double rho = 1.1 * std::pow(tail / head, 1.0 / s.deg);
             if (!(rho < 0.8)) { s.ok = false; return; }
             s.target = std::max(s.target, (int)std::ceil(13.0 / std::log10(1.0 / rho)) + 2);
             if (s.target > qmax) s.ok = false;
-            if (verbose) fprintf(stderr, "[tatrg subspace n=%d b=%d kmax=%d%s] after %d iterations: rho %.3f -> %d iterations\n", s.n, s.b, s.kmax, s.F ? " product" : "", s.done, rho, s.target);
+            const double range = std::pow(s.r[0] / tail, 1.0 / s.deg);
+            int deg = 1;
+            while (deg < 3 && std::pow(range, deg + 1) <= 1e11) ++deg;
+            if (verbose) fprintf(stderr, "[tatrg subspace n=%d b=%d kmax=%d%s] after %d iterations: rho %.3f -> %d iterations, %d per orthonormalisation\n", s.n, s.b, s.kmax, s.F ? " product" : "", s.done, rho, s.target, deg);
+            s.deg = deg;
         };
         for (int pass = 0; pass < 3; ++pass) {
             bool more = false;
             for (SubProb& s : ps) if (s.ok) { estimate(s); if (s.ok && s.target > s.done) more = true; }
             if (!more) break;
             for (SubProb& s : ps) {
-                if (!s.ok) continue;
-                for (; s.done < s.target; ++s.done) { sub_apply(s); sub_orth(s, kShift); }
+                if (!s.ok || s.target <= s.done) continue;
+                while (s.done < s.target) sub_step(s, s.deg, kShift);
                 ck(extract_diag(st, s.b, s.L.p, s.b, s.dg), "diag");
             }
         }
@@ -352,12 +370,12 @@ struct Stepper {
             if (!s.ok) continue;
             // second orthonormalisation pass without shift (the basis is orthonormal to ~1e-13 already), W = F Z recomputed
             const int64_t nb = (int64_t)s.n * s.b;
-            ck(cudaMemcpyAsync(s.buf[1].p, s.buf[0].p, 8 * nb, cudaMemcpyDeviceToDevice, st), "copy"); count_launch();
-            if (s.F) mm_into(s.buf[1].p + nb, s.b, false, false, s.n, s.b, s.n, s.F, s.n, s.buf[1].p, s.b);
-            sub_orth(s, 0.0);
+            if (s.F) mm_into(s.buf[s.cur].p + nb, s.b, false, false, s.n, s.b, s.n, s.F, s.n, s.buf[s.cur].p, s.b);
+            sub_orth(s, s.cur, 0.0);
             // Rayleigh-Ritz matrix H = W^T Bm W (product) or Z^T Bm Z
-            mm_into(s.buf[1].p, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, s.W(), s.b);
-            mm_into(s.H.p, s.b, true, false, s.b, s.b, s.n, s.W(), s.b, s.buf[1].p, s.b);
+            double* T = s.buf[s.cur ^ 1].p;
+            mm_into(T, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, s.W(), s.b);
+            mm_into(s.H.p, s.b, true, false, s.b, s.b, s.n, s.W(), s.b, T, s.b);
         }
     }
 
