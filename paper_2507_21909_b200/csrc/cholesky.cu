@@ -20,7 +20,6 @@ namespace tatrg {
 namespace {
 constexpr int PB = 64;        // panel width
 constexpr int PP = PB + 1;    // shared-memory pitch
-constexpr int kPotrfSmem = (2 * PB * PP + 2 * PB) * 8;
 
 __global__ void symmetrize_kernel(int n, double* __restrict__ A) {
     const int64_t total = (int64_t)n * n;
@@ -43,65 +42,87 @@ __global__ void diag_shift_kernel(int n, double* __restrict__ A, int64_t lda, do
 
 // Diagonal block [j0, j0+nb) of A -> L block (upper part of the block zeroed) and its inverse Linv (PB x PB, zero padded).
 // info[0] |= 1 when a pivot had to be raised to the guard, |= 2 when a pivot was not finite.
+// 256 threads: thread (i = tid & 63, g = tid >> 6) keeps the 16 entries [i][16 g .. 16 g + 15] of its row in registers.
+// Factorisation, right-looking: step j publishes column j through shared memory (double-buffered: one barrier per step),
+// every thread scales it by 1/sqrt(pivot) and updates its 16 entries.  Inverse, also right-looking: once row k of
+// X = L^-1 is final, every row i > k accumulates l_ik x_k; row k+1 is finished by its own four threads.
 __global__ void __launch_bounds__(256, 1) potrf_block_kernel(int nb, int j0, const double* __restrict__ A, int64_t lda, double* __restrict__ L,
                                                              int64_t ldl, double* __restrict__ Linv, const double* __restrict__ d0,
                                                              double guard_rel, int* __restrict__ info) {
-    extern __shared__ double sh_potrf[];
-    double* S = sh_potrf; double* X = S + PB * PP; double* dg = X + PB * PP; double* rdg = dg + PB;
-    const int tid = threadIdx.x;
-    for (int e = tid; e < PB * PB; e += 256) {
-        const int i = e >> 6, j = e & 63;
-        S[i * PP + j] = (i < nb && j <= i) ? A[(int64_t)(j0 + i) * lda + j0 + j] : 0.0;
-        X[i * PP + j] = 0.0;
+    __shared__ double col[2][PB];        // published column (factorisation) / row of X (inverse)
+    __shared__ double Ls[PB * PP];       // the factor, for the inverse
+    const int tid = threadIdx.x, i = tid & 63, g = tid >> 6, c0 = g * 16;
+    double a[16];
+#pragma unroll
+    for (int cc = 0; cc < 16; ++cc) {
+        const int c = c0 + cc;
+        a[cc] = (i < nb && c <= i) ? A[(int64_t)(j0 + i) * lda + j0 + c] : ((i == c) ? 1.0 : 0.0);   // identity padding beyond nb
     }
-    __syncthreads();
     int flag = 0;
-    for (int j = 0; j < nb; ++j) {
-        // left-looking: s_i = a_ij - sum_{k<j} l_ik l_jk   (thread i, i >= j)
-        if (tid >= j && tid < nb) {
-            double s0 = S[tid * PP + j], s1 = 0, s2 = 0, s3 = 0;
-            int k = 0;
-            for (; k + 3 < j; k += 4) {
-                s0 -= S[tid * PP + k] * S[j * PP + k];
-                s1 -= S[tid * PP + k + 1] * S[j * PP + k + 1];
-                s2 -= S[tid * PP + k + 2] * S[j * PP + k + 2];
-                s3 -= S[tid * PP + k + 3] * S[j * PP + k + 3];
+    for (int j = 0; j < PB; ++j) {
+        const int gj = j >> 4, jj = j & 15, buf = j & 1;
+        if (g == gj) {
+            double v = 0;
+#pragma unroll
+            for (int cc = 0; cc < 16; ++cc) if (cc == jj) v = a[cc];
+            col[buf][i] = v;
+        }
+        __syncthreads();
+        double p = col[buf][j];
+        const double dref = j < nb ? fabs(d0[j0 + j]) : 1.0;
+        const double floor_p = fmax(guard_rel * dref, 1e-290);
+        if (!(p == p) || fabs(p) > 1e300) { flag |= 2; p = floor_p; }
+        if (p < floor_p) { flag |= 1; p = floor_p; }
+        const double r = rsqrt(p);
+        const double li = (i == j) ? p * r : (i > j ? col[buf][i] * r : 0.0);
+#pragma unroll
+        for (int cc = 0; cc < 16; ++cc) {
+            const int c = c0 + cc;
+            if (c > j) a[cc] -= li * (col[buf][c] * r);
+            else if (c == j) a[cc] = li;
+        }
+    }
+    if (flag && tid == 0) atomicOr(info, flag);
+    // factor to shared memory and to L
+#pragma unroll
+    for (int cc = 0; cc < 16; ++cc) {
+        const int c = c0 + cc;
+        const double v = (c <= i) ? a[cc] : 0.0;
+        Ls[i * PP + c] = v;
+        if (i < nb && c < nb) L[(int64_t)(j0 + i) * ldl + j0 + c] = v;
+    }
+    __syncthreads();
+    // X = L^-1: x[cc] accumulates sum_{k<i} l_ik x_kc for the thread's 16 columns
+    double x[16];
+#pragma unroll
+    for (int cc = 0; cc < 16; ++cc) x[cc] = 0.0;
+    const double rii = 1.0 / Ls[i * PP + i];
+    if (i == 0) {
+#pragma unroll
+        for (int cc = 0; cc < 16; ++cc) { x[cc] = (c0 + cc == 0) ? rii : 0.0; }
+    }
+    __shared__ double xr[2][PB];
+    for (int k = 0; k < PB; ++k) {
+        const int buf = k & 1;
+        if (i == k) {
+#pragma unroll
+            for (int cc = 0; cc < 16; ++cc) xr[buf][c0 + cc] = x[cc];      // row k of X is final
+        }
+        __syncthreads();
+        if (i > k) {
+            const double lik = Ls[i * PP + k];
+#pragma unroll
+            for (int cc = 0; cc < 16; ++cc) x[cc] += lik * xr[buf][c0 + cc];
+            if (i == k + 1) {       // finish row k+1: x_ic = (delta_ic - sum) / l_ii
+#pragma unroll
+                for (int cc = 0; cc < 16; ++cc) { const int c = c0 + cc; x[cc] = (c > i) ? 0.0 : (((c == i) ? 1.0 : 0.0) - x[cc]) * rii; }
             }
-            for (; k < j; ++k) s0 -= S[tid * PP + k] * S[j * PP + k];
-            S[tid * PP + j] = (s0 + s1) + (s2 + s3);
-        }
-        __syncthreads();
-        if (tid >= j && tid < nb) {
-            double p = S[j * PP + j];
-            const double floor_p = fmax(guard_rel * fabs(d0[j0 + j]), 1e-290);
-            if (!(p == p) || fabs(p) > 1e300) { flag |= 2; p = floor_p; }
-            if (p < floor_p) { flag |= 1; p = floor_p; }
-            const double r = 1.0 / sqrt(p);
-            if (tid == j) { dg[j] = p * r; rdg[j] = r; }
-            else S[tid * PP + j] *= r;
-        }
-        __syncthreads();
-    }
-    if (tid < nb) S[tid * PP + tid] = dg[tid];
-    if (flag) atomicOr(info, flag);
-    __syncthreads();
-    // inverse of the lower-triangular block, one column per thread: x_c = 1/l_cc, x_i = -(sum_{k<i} l_ik x_k) / l_ii
-    if (tid < nb) {
-        const int c = tid;
-        for (int i = 0; i < nb; ++i) {
-            double a0 = 0, a1 = 0;
-            int k = 0;
-            for (; k + 1 < i; k += 2) { a0 += S[i * PP + k] * X[k * PP + c]; a1 += S[i * PP + k + 1] * X[(k + 1) * PP + c]; }
-            for (; k < i; ++k) a0 += S[i * PP + k] * X[k * PP + c];
-            const double rhs = (i == c) ? 1.0 : 0.0;
-            X[i * PP + c] = (i < c) ? 0.0 : (rhs - (a0 + a1)) * rdg[i];
         }
     }
-    __syncthreads();
-    for (int e = tid; e < PB * PB; e += 256) {
-        const int i = e >> 6, j = e & 63;
-        Linv[e] = (i < nb && j < nb) ? X[i * PP + j] : 0.0;
-        if (i < nb && j < nb) L[(int64_t)(j0 + i) * ldl + j0 + j] = (j <= i) ? S[i * PP + j] : 0.0;
+#pragma unroll
+    for (int cc = 0; cc < 16; ++cc) {
+        const int c = c0 + cc;
+        Linv[i * PB + c] = (i < nb && c < nb) ? x[cc] : 0.0;
     }
 }
 
@@ -124,18 +145,12 @@ size_t cholesky_work_doubles(int n) { return (size_t)((n + PB - 1) / PB) * PB * 
 cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, int64_t ldl, double shift, double guard_rel, double* work) {
     const int np = (n + PB - 1) / PB;
     double* Linv = work; double* d0 = work + (size_t)np * PB * PB; int* info = (int*)(d0 + n);
-    static bool cfg = false;
-    if (!cfg) {
-        cudaError_t ea = cudaFuncSetAttribute(potrf_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPotrfSmem);
-        if (ea != cudaSuccess) return ea;
-        cfg = true;
-    }
     cudaError_t e = cudaMemsetAsync(info, 0, sizeof(int), st);
     if (e != cudaSuccess) return e;
     diag_shift_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, A, lda, shift, d0); count_launch();
     for (int p = 0; p < np; ++p) {
         const int j0 = p * PB, nb = n - j0 < PB ? n - j0 : PB, m = n - j0 - nb;
-        potrf_block_kernel<<<1, 256, kPotrfSmem, st>>>(nb, j0, A, lda, L, ldl, Linv + (size_t)p * PB * PB, d0, guard_rel, info); count_launch();
+        potrf_block_kernel<<<1, 256, 0, st>>>(nb, j0, A, lda, L, ldl, Linv + (size_t)p * PB * PB, d0, guard_rel, info); count_launch();
         if (m <= 0) break;
         // panel below: L[i, j0:j0+nb] = A[i, j0:j0+nb] Linv^T
         e = dgemm(st, false, true, m, nb, nb, 1.0, A + (int64_t)(j0 + nb) * lda + j0, lda, Linv + (size_t)p * PB * PB, PB, 0.0,

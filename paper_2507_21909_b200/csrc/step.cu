@@ -191,6 +191,7 @@ struct Stepper {
     // Gram matrix -> eigen-decomposition -> Q = mat V lam^-1/2 (directions with lam <= 1e-12 lam_max dropped), and a
     // second identical pass on Q for narrow matrices (n <= 128), where it is cheap, to restore orthogonality to eps.
     void orth(const Tens& mat, Tens& Q, Tens& R) {
+        if (c.use_subspace && mat.d[1] >= 8 && mat.d[1] <= 128 && mat.d[0] >= 4 * mat.d[1] && orth_chol(mat, Q, R, 2)) return;
         Scope sc(*this);
         const int64_t m = mat.d[0], n = mat.d[1];
         Tens G = mm(true, false, n, n, m, mat.p, n, mat.p, n);
@@ -220,7 +221,7 @@ struct Stepper {
     // Q = mat R^-1 (one GEMM with the explicit triangular inverse).  Same span and same product Q R as orth(); accepted
     // only when the factor PROVES that orth() would drop nothing (R14): lam_min(G) = sigma_min(L)^2 >= 1 / ||L^-1||_F^2
     // and lam_max(G) <= tr G, so 1 / (||L^-1||_F^2 tr G) > 1e-12 implies lam_min > 1e-12 lam_max.  Returns false otherwise.
-    bool orth_chol(const Tens& mat, Tens& Q, Tens& R) {
+    bool orth_chol(const Tens& mat, Tens& Q, Tens& R, int passes = 1) {
         Scope sc(*this);
         const int64_t m = mat.d[0], n = mat.d[1];
         Tens G = mm(true, false, n, n, m, mat.p, n, mat.p, n);
@@ -240,7 +241,20 @@ struct Stepper {
         if (info != 0 || !std::isfinite(xn[0]) || !(xn[0] > 0) || !(tr > 0)) return false;
         if (!(1.0 / (xn[0] * tr) > kEpsOrthLambda)) return false;
         Q = mm(false, true, m, n, n, mat.p, n, X.p, n);
-        R = perm(view(L, {n, n}), {1, 0});
+        if (passes < 2) {
+            R = perm(view(L, {n, n}), {1, 0});
+        } else {
+            // second pass on the almost orthonormal Q (CholeskyQR2): Q^T Q = L2 L2^T, Q <- Q L2^-T, R = (L L2)^T
+            Tens G2 = mm(true, false, n, n, m, Q.p, n, Q.p, n);
+            Tens L2 = make({n, n}), X2 = make({n, n});
+            ck(fill_zero(st, L2.p, n * n), "zero"); ck(fill_zero(st, X2.p, n * n), "zero");
+            ck(cholesky(st, (int)n, G2.p, n, L2.p, n, 0.0, 1e-14, cw), "cholesky");
+            ck(tri_inverse(st, (int)n, L2.p, n, cw, X2.p, n, T.p), "tri_inverse");
+            Tens Q2 = mm(false, true, m, n, n, Q.p, n, X2.p, n);
+            Tens LL = mm(false, false, n, n, n, L.p, n, L2.p, n);
+            R = perm(LL, {1, 0});
+            drop(Q); Q = Q2;
+        }
         keep(Q); keep(R);
         return true;
     }
