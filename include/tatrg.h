@@ -146,6 +146,16 @@ int tatrg_eigh(void* cuda_stream, int n, double* G, double* lam, double* Vt, voi
 size_t tatrg_svd_work_bytes(int nv, int len);
 int tatrg_svd(void* cuda_stream, int nv, int len, const double* X, double* s, double* Ut, double* Vacc, void* work);
 
+/* Cholesky QR of a tall matrix (the orthonormalisation of the QR pre-reduction, Eq. A.2-A.3 :345-348, of the RSVD
+ * sketches, Eq. A.4-A.6 :352-369, and of the subspace iterations behind Eq. 2.9 :135 and the squeezers :171):
+ * X [dev] m x n row-major (m >= n; DESTROYED), Q [dev] m x n with orthonormal columns up to cond(X)^2 eps (one pass),
+ * R [dev] n x n upper triangular with positive diagonal, X = Q R.  Blocked Cholesky of X^T X over 64-wide panels
+ * (one-CTA diagonal factor, DGEMM panel/trailing updates), Q by forward substitution over the panels.
+ * work [dev] >= tatrg_cholqr_work_bytes(n), 256-byte aligned.  Synchronises.  ENUMERIC when a pivot of the factorisation
+ * fell below 1e-14 of its diagonal entry (X numerically rank-deficient): Q, R are then not usable. */
+size_t tatrg_cholqr_work_bytes(int n);
+int tatrg_cholqr(void* cuda_stream, long long m, int n, double* X, double* Q, double* R, void* work);
+
 /* result[0] [dev] = sum_i x[i]*y[i]  (the tensor trace tTr of Eq. 2.1 :48 on the factored tensor).
  * result must have room for 1200 doubles (partial sums of the first pass follow result[0]). */
 int tatrg_dot(void* cuda_stream, long long n, const double* x, const double* y, double* result);

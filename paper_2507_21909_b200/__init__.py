@@ -61,6 +61,8 @@ _SIGNATURES = {
     "tatrg_svd_work_bytes": (_c.c_size_t, [_c.c_int, _c.c_int]),
     "tatrg_svd": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_void_p,
                              _c.c_void_p]),
+    "tatrg_cholqr_work_bytes": (_c.c_size_t, [_c.c_int]),
+    "tatrg_cholqr": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
     "tatrg_dot": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
     "tatrg_dmma_issue_rate": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_int, _dp, _c.c_void_p]),
 }
@@ -323,6 +325,18 @@ def svd_rows(X):
     work = torch.empty(lib().tatrg_svd_work_bytes(nv, ln), dtype=torch.uint8, device=X.device)
     _check(lib().tatrg_svd(_stream_ptr(), nv, ln, _p(x), _p(s), _p(ut), _p(va), _p(work)), "tatrg_svd")
     return s, ut, va
+
+
+def cholqr(X):
+    """X = Q R by Cholesky QR (torch CUDA float64, m x n with m >= n): (Q, R), R upper triangular with positive diagonal."""
+    torch = _torch_cuda()
+    m, n = X.shape
+    x = X.clone().contiguous()
+    q = torch.empty((m, n), dtype=torch.float64, device=X.device)
+    r = torch.empty((n, n), dtype=torch.float64, device=X.device)
+    work = torch.empty(lib().tatrg_cholqr_work_bytes(n), dtype=torch.uint8, device=X.device)
+    _check(lib().tatrg_cholqr(_stream_ptr(), m, n, _p(x), _p(q), _p(r), _p(work)), "tatrg_cholqr")
+    return q, r
 
 
 def dot(x, y):

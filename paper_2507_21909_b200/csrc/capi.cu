@@ -239,6 +239,23 @@ int tatrg_svd(void* st, int nv, int len, const double* X, double* s, double* Ut,
     std::string err;
     try { return svd_rows((cudaStream_t)st, nv, len, X, s, Ut, Vacc, work, nullptr, &err); } catch (...) { return TATRG_ECUDA; }
 }
+size_t tatrg_cholqr_work_bytes(int n) { return n > 0 ? 8 * (2 * (size_t)n * n + cholesky_work_doubles(n)) + 4096 : 0; }
+int tatrg_cholqr(void* stp, long long m, int n, double* X, double* Q, double* R, void* work) {
+    if (m < n || n < 1 || !X || !Q || !R || !work) return TATRG_EINVAL;
+    cudaStream_t st = (cudaStream_t)stp;
+    double* G = (double*)work; double* L = G + (size_t)n * n; double* cw = L + (size_t)n * n;
+    cudaError_t e = dgemm(st, true, false, n, n, m, 1.0, X, n, X, n, 0.0, G, n);
+    if (e == cudaSuccess) e = fill_zero(st, L, (int64_t)n * n);
+    if (e == cudaSuccess) e = cholesky(st, n, G, n, L, n, 0.0, 1e-14, cw);
+    if (e == cudaSuccess) e = trsm_right_lt(st, m, n, X, n, Q, n, L, n, cw);
+    const int64_t dims[2] = {n, n}; const int perm[2] = {1, 0};
+    if (e == cudaSuccess) e = permute(st, 2, dims, perm, L, R);
+    int info = 0;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&info, cholesky_info(cw, n), sizeof(int), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return TATRG_ECUDA;
+    return info == 0 ? TATRG_OK : TATRG_ENUMERIC;
+}
 int tatrg_dot(void* st, long long n, const double* x, const double* y, double* result) {
     if (n < 0 || !x || !y || !result) return TATRG_EINVAL;
     return dot((cudaStream_t)st, n, x, y, result) == cudaSuccess ? TATRG_OK : TATRG_ECUDA;

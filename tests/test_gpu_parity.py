@@ -28,8 +28,9 @@ def golden(name):
     return json.load(open(path))["runs"]
 
 
-def run_against(rec, max_steps=None):
+def run_against(rec, max_steps=None, subspace=1):
     t = T.Tatrg(rec["beta"], rec["h"], rec["D"], rec["oversample"], rec["seed"], power_iters=rec["n_pow"])
+    t.set_option(T.OPT_SUBSPACE, subspace)
     n = len(rec["lnZ"]) if max_steps is None else min(max_steps, len(rec["lnZ"]))
     worst = [0.0, 0.0, 0.0]
     for m in range(n):
@@ -64,19 +65,41 @@ def test_config2_beta_sweep(idx):
 
 
 @pytest.mark.parametrize("idx", range(2))
-def test_config3_field(idx):
-    """configs[2]: 2^12 per axis (48 steps), D=16, p=16, h = +-1e-3, seed 7."""
+@pytest.mark.parametrize("subspace", [1, 0])
+def test_config3_field(idx, subspace):
+    """configs[2]: 2^12 per axis (48 steps), D=16, p=16, h = +-1e-3, seed 7.  subspace = 1: leading eigenvectors by subspace
+    iteration + Cholesky QR (the default path); 0: full eigen-decompositions everywhere (TATRG_OPT_SUBSPACE)."""
     rec = golden("c3")[idx]
-    w = run_against(rec)
+    w = run_against(rec, subspace=subspace)
     assert w[0] <= TOL_LNZ and w[1] <= TOL_SV and w[2] <= TOL_SV, w
 
 
-def test_config4_first_steps_at_full_size():
+@pytest.mark.parametrize("subspace", [1, 0])
+def test_config4_first_steps_at_full_size(subspace):
     """configs[3] (headline, D=32, p=32): as many steps as the oracle could afford (the weight of step m in ln Z/V is
     2^-m); the remaining steps are covered by test_d32_stage_properties."""
     (rec,) = golden("c4")
-    w = run_against(rec)
+    w = run_against(rec, subspace=subspace)
     assert w[0] <= TOL_LNZ and w[1] <= TOL_SV and w[2] <= TOL_SV, w
+
+
+def test_subspace_and_full_decompositions_agree_at_d32():
+    """The two ways of getting the triad isometries / squeezers / QR factors (TATRG_OPT_SUBSPACE 1 / 0) give the same
+    physics over 10 steps at D = 32, well inside the parity tolerance, and the iteration is the faster one."""
+    runs = []
+    for sub in (1, 0):
+        t = T.Tatrg(0.1497, 0.0, 32, 32, 42)
+        t.set_option(T.OPT_SUBSPACE, sub)
+        out = []
+        for _ in range(10):
+            t.step()
+            out.append((t.lnZ_per_site(), t.singular_values(T.SV_SIGMA, 32), t.singular_values(T.SV_S, 32), t.launches()))
+        runs.append(out)
+        t.close()
+    for a, b in zip(*runs):
+        assert abs(a[0] - b[0]) <= 1e-12 * abs(b[0])
+        assert np.abs(a[1] - b[1]).max() <= 1e-10 and np.abs(a[2] - b[2]).max() <= 1e-10
+    assert runs[0][-1][3] < runs[1][-1][3]
 
 
 # ---- pins that need no oracle run: exact values the mathematics fixes ------------------------------------------------------

@@ -174,3 +174,33 @@ def test_svd_rows_rank_deficient_gives_exact_zero_structure(torch):
     s, ut, va = T.svd_rows(dev(torch, x))
     s = s.cpu().numpy()
     assert (s[2:] <= 1e-13 * s[0]).all() and s[1] > 1e-3 * s[0]
+
+
+# ---- Cholesky QR (blocked Cholesky + triangular solve) ----------------------------------------------------------------------
+@pytest.mark.parametrize("m,n,cond", [(7, 7, 1.0), (100, 7, 10.0), (1000, 64, 1e3), (3000, 130, 1e2), (2500, 200, 1e4), (4096, 257, 30.0)])
+def test_cholqr_is_the_qr_factorisation(torch, m, n, cond):
+    """X = Q R with Q^T Q = 1 and R upper triangular with positive diagonal is unique: the three properties pin the result.
+    One pass of Cholesky QR loses orthogonality like cond(X)^2 eps, X = Q R holds to eps."""
+    rng = np.random.default_rng(m + n)
+    x = inputs.random_tensor((m, n), 11) * (cond ** (-np.arange(n) / max(n - 1, 1)))      # graded columns
+    if n > 1:
+        x = x @ np.linalg.qr(rng.standard_normal((n, n)))[0]                              # and mixed: cond(X) ~ cond
+    q, r = T.cholqr(dev(torch, x))
+    q, r = q.cpu().numpy(), r.cpu().numpy()
+    assert np.all(np.diag(r) > 0) and np.abs(np.tril(r, -1)).max() == 0.0
+    scale = np.abs(x).max()
+    assert np.abs(q @ r - x).max() <= 64 * EPS * n * scale
+    assert np.abs(q.T @ q - np.eye(n)).max() <= 64 * EPS * n * max(1.0, np.linalg.cond(x) ** 2)
+    # against the definition through the oracle's LAPACK-free Jacobi: R^T R = X^T X has the eigenvalues of the Gram matrix
+    from oracle import tatrg_oracle as O
+    if n <= 130:
+        lam = np.sort(O.jacobi_eigh(x.T @ x)[0])
+        lam_r = np.sort(O.jacobi_eigh(r.T @ r)[0])
+        assert np.abs(lam - lam_r).max() <= 64 * EPS * n * lam.max()
+
+
+def test_cholqr_reports_rank_deficiency(torch):
+    x = inputs.random_tensor((500, 40), 3)
+    x[:, 17] = x[:, 3] - 2.0 * x[:, 5]
+    with pytest.raises(T.TatrgError):
+        T.cholqr(dev(torch, x))
