@@ -18,7 +18,7 @@ OK, EINVAL, ENOMEM, ECUDA, ENUMERIC, ESTATE = 0, -1, -2, -3, -4, -5
 OPT_POWER_ITERS, OPT_K_TRIAD, OPT_TAU, OPT_STAGE_TIMING, OPT_KEEP_TENSORS, OPT_METHOD, OPT_SUBSPACE = 1, 2, 3, 4, 5, 6, 7
 METHOD_TRIAD, METHOD_ATRG = 0, 1
 SV_SIGMA, SV_S = 0, 1
-STAGES = ["decompose", "bond_swap", "_rsvd", "_lift", "triad", "_triad_tensors", "squeezer_grams", "squeezers", "contract",
+STAGES = ["decompose", "qr", "rsvd", "lift", "triad", "triad_tensors", "squeezer_grams", "squeezers", "contract",
           "rotate_trace"]
 
 _c = ctypes

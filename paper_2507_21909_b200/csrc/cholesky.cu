@@ -32,6 +32,21 @@ __global__ void symmetrize_kernel(int n, double* __restrict__ A) {
     }
 }
 
+__global__ void mirror_lower_kernel(int n, double* __restrict__ A) {      // 32 x 32 tiles through shared memory
+    __shared__ double t[32][33];
+    const int bi = blockIdx.y, bj = blockIdx.x;
+    if (bj < bi) return;                                                   // (bi, bj) upper tile <- transpose of lower tile (bj, bi)
+    for (int r = threadIdx.y; r < 32; r += 8) {
+        const int i = bj * 32 + r, j = bi * 32 + threadIdx.x;
+        t[r][threadIdx.x] = (i < n && j < n) ? A[(int64_t)i * n + j] : 0.0;
+    }
+    __syncthreads();
+    for (int r = threadIdx.y; r < 32; r += 8) {
+        const int i = bi * 32 + r, j = bj * 32 + threadIdx.x;
+        if (i < n && j < n && i < j) A[(int64_t)i * n + j] = t[threadIdx.x][r];
+    }
+}
+
 __global__ void diag_shift_kernel(int n, double* __restrict__ A, int64_t lda, double shift, double* __restrict__ d0) {
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const double v = A[(int64_t)i * lda + i];
@@ -137,6 +152,12 @@ cudaError_t symmetrize(cudaStream_t st, int n, double* A) {
     return cudaGetLastError();
 }
 
+cudaError_t mirror_lower(cudaStream_t st, int n, double* A) {
+    const int nt = (n + 31) / 32;
+    mirror_lower_kernel<<<dim3(nt, nt), dim3(32, 8), 0, st>>>(n, A); count_launch();
+    return cudaGetLastError();
+}
+
 size_t cholesky_work_doubles(int n) { return (size_t)((n + PB - 1) / PB) * PB * PB + (size_t)n + 64; }
 
 // A [n x n, lda] (lower triangle read, destroyed) -> L [n x n, ldl] lower triangular (strict upper part of the diagonal
@@ -186,22 +207,34 @@ cudaError_t trsm_right_lt(cudaStream_t st, int64_t m, int n, double* X, int64_t 
 }
 
 // X [n x n, ldx] = L^-1 (lower triangular; X must be zero-filled on entry) from the factor and the inverted diagonal blocks
-// that cholesky() left in work.  T: scratch of 64 x n doubles.  Row panel i: X[i, <i] = -Linv_ii (L[i, <i] X[<i, <i]).
+// that cholesky() left in work.  T: scratch of tri_inverse_scratch_doubles(n).
+//   n = 64 * 2^k: recursive doubling, [[X11, 0], [-X22 L21 X11, X22]] for all pairs of a level in two batched DGEMMs
+//   (2 log2(n/64) launches, square products);  otherwise row panels: X[i, <i] = -Linv_ii (L[i, <i] X[<i, <i]).
+size_t tri_inverse_scratch_doubles(int n) { const size_t a = (size_t)n * n / 4, b = (size_t)PB * n; return a > b ? a : b; }
 cudaError_t tri_inverse(cudaStream_t st, int n, const double* L, int64_t ldl, const double* work, double* X, int64_t ldx, double* T) {
     const int np = (n + PB - 1) / PB;
     const double* Linv = work;
+    const bool pow2 = (n % PB == 0) && ((np & (np - 1)) == 0);
     for (int p = 0; p < np; ++p) {
         const int i0 = p * PB, nb = n - i0 < PB ? n - i0 : PB;
         cudaError_t e = cudaMemcpy2DAsync(X + (int64_t)i0 * ldx + i0, ldx * 8, Linv + (size_t)p * PB * PB, PB * 8, (size_t)nb * 8, nb,
                                           cudaMemcpyDeviceToDevice, st);
         count_launch();
         if (e != cudaSuccess) return e;
-        if (i0 == 0) continue;
+        if (pow2 || i0 == 0) continue;
         e = dgemm(st, false, false, nb, i0, i0, 1.0, L + (int64_t)i0 * ldl, ldl, X, ldx, 0.0, T, i0);
         if (e != cudaSuccess) return e;
         e = dgemm(st, false, false, nb, i0, nb, -1.0, Linv + (size_t)p * PB * PB, PB, T, i0, 0.0, X + (int64_t)i0 * ldx, ldx);
         if (e != cudaSuccess) return e;
     }
+    if (pow2)
+        for (int64_t s = PB; s < n; s *= 2) {
+            const int pairs = (int)(n / (2 * s));
+            cudaError_t e = dgemm(st, false, false, s, s, s, 1.0, L + s * ldl, ldl, X, ldx, 0.0, T, s, pairs, 2 * s * (ldl + 1), 2 * s * (ldx + 1), s * s);
+            if (e != cudaSuccess) return e;
+            e = dgemm(st, false, false, s, s, s, -1.0, X + s * ldx + s, ldx, T, s, 0.0, X + s * ldx, ldx, pairs, 2 * s * (ldx + 1), s * s, 2 * s * (ldx + 1));
+            if (e != cudaSuccess) return e;
+        }
     return cudaSuccess;
 }
 

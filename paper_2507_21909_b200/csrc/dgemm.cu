@@ -13,6 +13,7 @@
 // 16 distinct bank pairs for both storage orders.
 // Batched launches take a K of their own for the last batch entry (klast): split-K passes its ragged tail that way.
 #include "internal.h"
+#include <algorithm>
 
 namespace tatrg {
 thread_local Counters* g_counter = nullptr;
@@ -104,7 +105,7 @@ template <class C_, bool A_KC, bool B_KC, bool AV16, bool BV16>
 __global__ void __launch_bounds__(C_::NT, C_::NT == 256 ? 1 : 2)
 dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, const double* __restrict__ A, int64_t lda,
              const double* __restrict__ B, int64_t ldb, double beta, double* __restrict__ C, int64_t ldc, int64_t sA,
-             int64_t sB, int64_t sC, int tiles_m) {
+             int64_t sB, int64_t sC, int tiles_m, int lower_only) {
     constexpr int BM = C_::BM, BN = C_::BN, NT = C_::NT, MI = C_::MI, NI = C_::NI, TILE_D = C_::TILE_D;
     constexpr int PA = BM + 4, PB = BN + 4;
     extern __shared__ __align__(16) double smem[];
@@ -114,6 +115,7 @@ dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, co
     // tile order: consecutive CTAs walk down M for a fixed N-panel so that the B panel stays in L2
     const int64_t tile = blockIdx.x;
     const int64_t m0 = (tile % tiles_m) * BM, n0 = (tile / tiles_m) * BN;
+    if (lower_only && n0 >= m0 + BM) return;          // symmetric result: tiles strictly above the diagonal are mirrored later
     const int64_t K = (Klast > 0 && blockIdx.z == gridDim.z - 1) ? Klast : Kall;
     A += (int64_t)blockIdx.z * sA; B += (int64_t)blockIdx.z * sB; C += (int64_t)blockIdx.z * sC;
 
@@ -192,7 +194,7 @@ dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, co
 
 struct Args {
     cudaStream_t st; int64_t M, N, K, Klast; double alpha; const double* A; int64_t lda; const double* B; int64_t ldb; double beta;
-    double* C; int64_t ldc; int batch; int64_t sA, sB, sC; bool force_small = false;
+    double* C; int64_t ldc; int batch; int64_t sA, sB, sC; bool force_small = false; bool lower_only = false;
 };
 
 template <class C_, bool A_KC, bool B_KC, bool AV, bool BV>
@@ -206,7 +208,7 @@ cudaError_t launch(const Args& a) {
     }
     int64_t tm = (a.M + C_::BM - 1) / C_::BM, tn = (a.N + C_::BN - 1) / C_::BN;
     dim3 grid((unsigned)(tm * tn), 1, (unsigned)a.batch);
-    kern<<<grid, C_::NT, C_::SMEM, a.st>>>(a.M, a.N, a.K, a.Klast, a.alpha, a.A, a.lda, a.B, a.ldb, a.beta, a.C, a.ldc, a.sA, a.sB, a.sC, (int)tm);
+    kern<<<grid, C_::NT, C_::SMEM, a.st>>>(a.M, a.N, a.K, a.Klast, a.alpha, a.A, a.lda, a.B, a.ldb, a.beta, a.C, a.ldc, a.sA, a.sB, a.sC, (int)tm, a.lower_only ? 1 : 0);
     count_launch();
     return cudaGetLastError();
 }
@@ -249,22 +251,31 @@ cudaError_t dgemm_raw(bool transa, bool transb, const Args& a) {
 
 static cudaError_t dgemm_klast(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, int64_t Klast, double alpha,
                                const double* A, int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch,
-                               int64_t sA, int64_t sB, int64_t sC, bool force_small = false) {
+                               int64_t sA, int64_t sB, int64_t sC, bool force_small = false, bool lower_only = false) {
     if (M <= 0 || N <= 0 || batch <= 0) return cudaSuccess;
     Counters* c = g_counter;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     const double kk = Klast > 0 ? (double)K * (batch - 1) + (double)Klast : (double)K * batch;
-    if (c) { c->gemm_flops += 2.0 * (double)M * (double)N * kk; c->gemm_calls += 1; }
+    // lower_only: only the tiles on and below the diagonal are computed (counted as such)
+    double mn = (double)M * (double)N;
+    if (lower_only) {
+        const bool sm = force_small || small_cfg(M, N, batch);
+        const int64_t bm = sm ? CfgS::BM : CfgL::BM, bn = sm ? CfgS::BN : CfgL::BN;
+        mn = 0;
+        for (int64_t m0 = 0; m0 < M; m0 += bm)
+            for (int64_t n0 = 0; n0 < N && n0 < m0 + bm; n0 += bn) mn += (double)std::min(bm, M - m0) * (double)std::min(bn, N - n0);
+    }
+    if (c) { c->gemm_flops += 2.0 * mn * kk; c->gemm_calls += 1; }
     if (c && c->time_kernels) { e0 = c->next_event(); e1 = c->next_event(); cudaEventRecord(e0, st); }
     cudaError_t e = cudaSuccess;
     // grid.z carries the batch: split very large batches
     for (int b0 = 0; b0 < batch && e == cudaSuccess; b0 += 32768) {
         int nb = batch - b0 < 32768 ? batch - b0 : 32768;
         Args a{st, M, N, K, (b0 + nb == batch) ? Klast : 0, alpha, A + (int64_t)b0 * sA, lda, B + (int64_t)b0 * sB, ldb, beta,
-               C + (int64_t)b0 * sC, ldc, nb, sA, sB, sC, force_small};
+               C + (int64_t)b0 * sC, ldc, nb, sA, sB, sC, force_small, lower_only};
         e = dgemm_raw(transa, transb, a);
     }
-    if (e0) { cudaEventRecord(e1, st); c->gemm_ev.push_back({e0, e1}); c->gemm_shapes.push_back({M, N, (int64_t)(kk / batch), batch, transa, transb}); }
+    if (e0) { cudaEventRecord(e1, st); c->gemm_ev.push_back({e0, e1}); c->gemm_shapes.push_back({M, N, (int64_t)(kk / batch), batch, transa, transb, mn / ((double)M * (double)N)}); }
     return e;
 }
 
@@ -278,11 +289,15 @@ cudaError_t dgemm(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t 
 namespace {
 // Number of K-chunks for a non-batched GEMM: the smallest split whose CTA count fills whole waves of the 148 SMs
 // (>= 93 % of the last wave used), chunks of >= 256, partials capped at 64 M doubles.  1 = no split.
-int splitk_count(int64_t M, int64_t N, int64_t K) {
+int splitk_count(int64_t M, int64_t N, int64_t K, bool lower_only = false) {
     const bool sm = small_cfg(M, N);
     const int bm = sm ? CfgS::BM : CfgL::BM, bn = sm ? CfgS::BN : CfgL::BN;
     const int per_sm = sm ? 2 : 1;
-    const int64_t tiles = ((M + bm - 1) / bm) * ((N + bn - 1) / bn);
+    int64_t tiles = ((M + bm - 1) / bm) * ((N + bn - 1) / bn);
+    if (lower_only) {      // only the tiles on and below the diagonal do work
+        tiles = 0;
+        for (int64_t m0 = 0; m0 < M; m0 += bm) for (int64_t n0 = 0; n0 < N && n0 < m0 + bm; n0 += bn) ++tiles;
+    }
     const int64_t slots = 148 * per_sm;
     auto eff = [&](int64_t ctas) { int64_t waves = (ctas + slots - 1) / slots; return (double)ctas / (double)(waves * slots); };
     if (K < 256 || eff(tiles) >= 0.93) return 1;
@@ -311,22 +326,22 @@ __global__ void splitk_reduce_kernel(const double* __restrict__ part, int nsplit
 }
 }  // namespace
 
-int64_t dgemm_splitk_doubles(int64_t M, int64_t N, int64_t K) {
-    int s = splitk_count(M, N, K);
+int64_t dgemm_splitk_doubles(int64_t M, int64_t N, int64_t K, bool lower_only) {
+    int s = splitk_count(M, N, K, lower_only);
     return s > 1 ? (int64_t)s * M * N : 0;
 }
 
 cudaError_t dgemm_splitk(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
-                         int64_t lda, const double* B, int64_t ldb, double* C, int64_t ldc, double* part) {
-    int ns = splitk_count(M, N, K);
-    if (ns <= 1 || part == nullptr) return dgemm(st, transa, transb, M, N, K, alpha, A, lda, B, ldb, 0.0, C, ldc);
+                         int64_t lda, const double* B, int64_t ldb, double* C, int64_t ldc, double* part, bool lower_only) {
+    int ns = splitk_count(M, N, K, lower_only);
+    if (ns <= 1 || part == nullptr) return dgemm_klast(st, transa, transb, M, N, K, 0, alpha, A, lda, B, ldb, 0.0, C, ldc, 1, 0, 0, 0, false, lower_only);
     // chunk: multiple of BK; the last batch entry takes the ragged tail (klast)
     int64_t chunk = ((K + ns - 1) / ns + BK - 1) / BK * BK;
     int nchunks = (int)((K + chunk - 1) / chunk);
     int64_t tail = K - (int64_t)(nchunks - 1) * chunk;
     const int64_t stepA = transa ? chunk * lda : chunk, stepB = transb ? chunk : chunk * ldb;
     cudaError_t e = dgemm_klast(st, transa, transb, M, N, chunk, tail == chunk ? 0 : tail, 1.0, A, lda, B, ldb, 0.0, part, N, nchunks,
-                                stepA, stepB, M * N, small_cfg(M, N));
+                                stepA, stepB, M * N, small_cfg(M, N), lower_only);
     if (e != cudaSuccess) return e;
     int64_t MN = M * N;
     int64_t blocks = (MN + 255) / 256; if (blocks > 148 * 8) blocks = 148 * 8;

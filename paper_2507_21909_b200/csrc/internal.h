@@ -28,7 +28,7 @@ struct Counters {
     // optional device timing of the two kernel families (TATRG_OPT_STAGE_TIMING = 2): events bracket each launch
     bool time_kernels = false;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> gemm_ev, perm_ev;
-    struct GemmShape { int64_t M, N, K; int batch; bool ta, tb; };
+    struct GemmShape { int64_t M, N, K; int batch; bool ta, tb; double frac = 1.0; };   // frac < 1: lower-triangular tiles only
     std::vector<GemmShape> gemm_shapes;   // parallel to gemm_ev (time_kernels only)
     std::vector<cudaEvent_t> ev_pool;
     size_t ev_used = 0;
@@ -45,9 +45,9 @@ cudaError_t dgemm(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t 
 // split-K variant for skinny outputs (Gram matrices of tall operands): partial products of K-chunks go to `part`
 // (>= dgemm_splitk_doubles(M,N,K) doubles, [dev]) and are summed by a second kernel.  Falls back to dgemm when
 // the output already fills the machine.  part may be null when dgemm_splitk_doubles() == 0.
-int64_t dgemm_splitk_doubles(int64_t M, int64_t N, int64_t K);
+int64_t dgemm_splitk_doubles(int64_t M, int64_t N, int64_t K, bool lower_only = false);
 cudaError_t dgemm_splitk(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
-                         int64_t lda, const double* B, int64_t ldb, double* C, int64_t ldc, double* part);
+                         int64_t lda, const double* B, int64_t ldb, double* C, int64_t ldc, double* part, bool lower_only = false);
 
 // permute.cu
 cudaError_t permute(cudaStream_t st, int nd, const int64_t* dims, const int* perm, const double* in, double* out);
@@ -88,11 +88,13 @@ int svd_rows(cudaStream_t st, int nv, int len, const double* X, double* s, doubl
 // cholesky.cu : blocked Cholesky (64-wide panels: one-CTA diagonal factor + inverse, DGEMM panel / trailing updates) and
 // the triangular solve Q = X L^-T.  All asynchronous on st.
 cudaError_t symmetrize(cudaStream_t st, int n, double* A);                      // A = (A + A^T) / 2 in place
+cudaError_t mirror_lower(cudaStream_t st, int n, double* A);                    // A[i][j] = A[j][i] for i < j
 size_t cholesky_work_doubles(int n);
 cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, int64_t ldl, double shift, double guard_rel, double* work);
 const int* cholesky_info(const double* work, int n);                            // [dev] bit 0: a pivot was raised to the guard, bit 1: non-finite
 cudaError_t trsm_right_lt(cudaStream_t st, int64_t m, int n, double* X, int64_t ldx, double* Q, int64_t ldq, const double* L, int64_t ldl,
                           const double* work);
+size_t tri_inverse_scratch_doubles(int n);
 cudaError_t tri_inverse(cudaStream_t st, int n, const double* L, int64_t ldl, const double* work, double* X, int64_t ldx, double* T);
 const double* cholesky_d0(const double* work, int n);                           // [dev] the n original diagonal entries
 cudaError_t extract_diag(cudaStream_t st, int n, const double* A, int64_t lda, double* d);

@@ -129,8 +129,14 @@ __device__ __forceinline__ double block_max(double v, double* red) {
 }
 
 // ---- n <= 64 ---------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(512, 1) eigh_small_kernel(int n, const double* __restrict__ G, double* __restrict__ lam, double* __restrict__ Vt) {
+struct SmallBatch { int n[8]; const double* G[8]; double* lam[8]; double* Vt[8]; };
+// one CTA per matrix of the batch (independent problems of a stage share one launch)
+__global__ void __launch_bounds__(512, 1) eigh_small_kernel(SmallBatch sb) {
     extern __shared__ double sh[];
+    const int n = sb.n[blockIdx.x];
+    const double* __restrict__ G = sb.G[blockIdx.x];
+    double* __restrict__ lam = sb.lam[blockIdx.x];
+    double* __restrict__ Vt = sb.Vt[blockIdx.x];
     double* S = sh; double* J = S + SB * SP;
     double* cs = J + SB * SP; double* sn = cs + 32; double* red = sn + 32;
     int* pp = (int*)(red + 32); int* qq = pp + 32; int* cnt = qq + 32;
@@ -622,8 +628,11 @@ int eigh_batched(cudaStream_t st, int count, const EighItem* items, void* work, 
     auto misc = [&](int z) { return base + z * ws + 2 * (int64_t)N; };
     auto Vu = [&](int z) { return base + z * ws + 2 * (int64_t)N + 64; };
     if (nmax <= SB) {
-        for (int z = 0; z < count; ++z) {
-            eigh_small_kernel<<<1, 512, kSmallSmem, st>>>(items[z].n, items[z].G, lam_u(z), Vu(z)); count_launch();
+        for (int z0 = 0; z0 < count; z0 += 8) {
+            const int bc = std::min(8, count - z0);
+            SmallBatch sb;
+            for (int z = 0; z < bc; ++z) { sb.n[z] = items[z0 + z].n; sb.G[z] = items[z0 + z].G; sb.lam[z] = lam_u(z0 + z); sb.Vt[z] = Vu(z0 + z); }
+            eigh_small_kernel<<<bc, 512, kSmallSmem, st>>>(sb); count_launch();
         }
         for (int z = 0; z < count; ++z) {
             int rc = finish_one(st, items[z].n, items[z].n, lam_u(z), idx(z), Vu(z), items[z].lam, items[z].Vt, items[z].lam_host, err);

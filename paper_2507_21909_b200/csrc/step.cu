@@ -15,6 +15,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
+#include <functional>
 
 namespace tatrg {
 namespace {
@@ -49,6 +50,8 @@ struct Stepper {
     cudaStream_t st;
     std::vector<std::vector<double*>> scopes;
     int call;
+
+    std::function<void()> submark;   // closes a timing sub-stage from inside a stage function (set by run())
 
     Stepper(tatrg_ctx& ctx, cudaStream_t s) : c(ctx), st(s), call(ctx.m + 1) { scopes.emplace_back(); }
     ~Stepper() { while (!scopes.empty()) pop(); }
@@ -119,17 +122,27 @@ struct Stepper {
         return o;
     }
     // C[M,N] = op(A) op(B), plain 2-D, with split-K when the output is small
-    Tens mm(bool ta, bool tb, int64_t M, int64_t N, int64_t K, const double* A, int64_t lda, const double* B, int64_t ldb) {
+    // sym: the result is symmetric (a Gram matrix): only the tiles on and below the diagonal are computed, then mirrored
+    Tens mm(bool ta, bool tb, int64_t M, int64_t N, int64_t K, const double* A, int64_t lda, const double* B, int64_t ldb, bool sym = false) {
         Tens C = make({M, N});
-        int64_t need = dgemm_splitk_doubles(M, N, K);
+        const bool lower = sym && M == N && M >= 256;
+        int64_t need = dgemm_splitk_doubles(M, N, K, lower);
         double* part = need ? c.pool.alloc(need) : nullptr;
-        ck(dgemm_splitk(st, ta, tb, M, N, K, 1.0, A, lda, B, ldb, C.p, N, part), "dgemm");
+        ck(dgemm_splitk(st, ta, tb, M, N, K, 1.0, A, lda, B, ldb, C.p, N, part, lower), "dgemm");
         if (part) c.pool.free(part);
+        if (lower) ck(mirror_lower(st, (int)M, C.p), "mirror");
         return C;
     }
     // the same into caller-provided storage (leading dimension ldc)
+    // While several problems are in flight on their own streams (sub_iterate) the split-K partials must not come from the
+    // pool's enqueue-order reuse: part_fixed then points to the problem's own scratch of part_cap doubles.
+    double* part_fixed = nullptr; int64_t part_cap = 0;
     void mm_into(double* C, int64_t ldc, bool ta, bool tb, int64_t M, int64_t N, int64_t K, const double* A, int64_t lda, const double* B, int64_t ldb) {
         int64_t need = dgemm_splitk_doubles(M, N, K);
+        if (part_fixed) {
+            ck(dgemm_splitk(st, ta, tb, M, N, K, 1.0, A, lda, B, ldb, C, ldc, need <= part_cap ? part_fixed : nullptr), "dgemm");
+            return;
+        }
         double* part = need ? c.pool.alloc(need) : nullptr;
         ck(dgemm_splitk(st, ta, tb, M, N, K, 1.0, A, lda, B, ldb, C, ldc, part), "dgemm");
         if (part) c.pool.free(part);
@@ -224,8 +237,8 @@ struct Stepper {
     bool orth_chol(const Tens& mat, Tens& Q, Tens& R, int passes = 1) {
         Scope sc(*this);
         const int64_t m = mat.d[0], n = mat.d[1];
-        Tens G = mm(true, false, n, n, m, mat.p, n, mat.p, n);
-        Tens L = make({n, n}), X = make({n, n}), T = make({64, n});
+        Tens G = mm(true, false, n, n, m, mat.p, n, mat.p, n, true);
+        Tens L = make({n, n}), X = make({n, n}), T = make({(int64_t)tri_inverse_scratch_doubles((int)n)});
         double* cw = raw((int64_t)cholesky_work_doubles((int)n));
         double* res = raw(1 + 148 * 8 + 7);
         ck(fill_zero(st, L.p, n * n), "zero"); ck(fill_zero(st, X.p, n * n), "zero");
@@ -272,7 +285,7 @@ struct Stepper {
         Scope sc(*this);
         const Tens* mats[2] = {&m0, &m1};
         Tens G[2];
-        for (int i = 0; i < 2; ++i) G[i] = mm(true, false, n, n, m, mats[i]->p, n, mats[i]->p, n);
+        for (int i = 0; i < 2; ++i) G[i] = mm(true, false, n, n, m, mats[i]->p, n, mats[i]->p, n, true);
         std::vector<EigOut> eo;
         eig_batch({&G[0], &G[1]}, {(int)n, (int)n}, eo);
         for (int i = 0; i < 2; ++i) {
@@ -302,6 +315,7 @@ struct Stepper {
         const double* Bm; const double* F; int n, kmax, b; uint32_t sid;
         Tens buf[2], Gm, L, H; double* cw; double* dg;
         std::vector<double> r;
+        cudaStream_t stream = nullptr; double* part = nullptr; int64_t part_cap = 0;
         int cur = 0;                 // the basis [Z; W] lives in buf[cur]
         int done = 0, target = 0, deg = 1;
         bool ok = true;
@@ -331,6 +345,27 @@ struct Stepper {
         sub_orth(s, a, shift);
         s.done += deg;
     }
+    // The problems of a stage are independent chains of small launches: each runs on a stream of its own (created once
+    // per process), forked from and joined to the caller's stream by events, so that their kernels overlap on the device.
+    struct SubStreams { cudaStream_t s[4]; cudaEvent_t fork, join[4]; bool ok = false; };
+    static SubStreams& sub_streams() {
+        static SubStreams ss; static bool tried = false;
+        if (!tried) {
+            tried = true;
+            bool ok = cudaEventCreateWithFlags(&ss.fork, cudaEventDisableTiming) == cudaSuccess;
+            for (int i = 0; i < 4 && ok; ++i)
+                ok = cudaStreamCreateWithFlags(&ss.s[i], cudaStreamNonBlocking) == cudaSuccess && cudaEventCreateWithFlags(&ss.join[i], cudaEventDisableTiming) == cudaSuccess;
+            ss.ok = ok;
+        }
+        return ss;
+    }
+    struct OnStream {      // issue the enclosed work of problem p on its stream, with its own split-K scratch
+        Stepper& s; cudaStream_t saved; double* pf; int64_t pc;
+        OnStream(Stepper& s_, const SubProb& p) : s(s_), saved(s_.st), pf(s_.part_fixed), pc(s_.part_cap) {
+            if (p.stream) { s.st = p.stream; s.part_fixed = p.part; s.part_cap = p.part_cap; }
+        }
+        ~OnStream() { s.st = saved; s.part_fixed = pf; s.part_cap = pc; }
+    };
     // Runs the iterations of all problems (interleaved so that the host reads the convergence estimates of all of them
     // with one synchronisation per phase) and leaves in every s.H the b x b Rayleigh-Ritz matrix.  Problems that cannot
     // be handled (rank-deficient leading block, no convergence in sight) come back with ok = false.
@@ -341,7 +376,21 @@ struct Stepper {
         constexpr int q0 = 6, qmax = 96;
         constexpr double kShift = 1e-13;
         static const bool verbose = getenv("TATRG_SUB_VERBOSE") != nullptr;   // debugging aid only
+        SubStreams& ss = sub_streams();
+        const bool multi = ss.ok && ps.size() > 1 && ps.size() <= 4;
+        if (multi) {
+            ck(cudaEventRecord(ss.fork, st), "event");
+            for (size_t i = 0; i < ps.size(); ++i) {
+                SubProb& s = ps[i];
+                s.stream = ss.s[i];
+                ck(cudaStreamWaitEvent(s.stream, ss.fork, 0), "wait");
+                s.part_cap = std::max(dgemm_splitk_doubles(s.b, s.b, s.n), dgemm_splitk_doubles(s.n, s.b, s.n));
+                s.part = s.part_cap ? raw(s.part_cap) : nullptr;
+                if (!s.part) s.part_cap = 0;
+            }
+        }
         for (SubProb& s : ps) {
+            OnStream on(*this, s);
             const int64_t rows = s.F ? 2 * (int64_t)s.n : s.n;
             s.buf[0] = make({rows, s.b}); s.buf[1] = make({rows, s.b});
             s.Gm = make({s.b, s.b}); s.L = make({s.b, s.b}); s.H = make({s.b, s.b});
@@ -354,6 +403,7 @@ struct Stepper {
             ck(extract_diag(st, s.b, s.L.p, s.b, s.dg), "diag");
         }
         auto estimate = [&](SubProb& s) {
+            OnStream on(*this, s);
             s.r = to_host(s.dg, s.b);
             for (double v : s.r) if (!std::isfinite(v)) { s.ok = false; return; }
             double tail = 0; for (int j = s.b - 4; j < s.b; ++j) tail = std::max(tail, s.r[j]);
@@ -376,12 +426,14 @@ struct Stepper {
             if (!more) break;
             for (SubProb& s : ps) {
                 if (!s.ok || s.target <= s.done) continue;
+                OnStream on(*this, s);
                 while (s.done < s.target) sub_step(s, s.deg, kShift);
                 ck(extract_diag(st, s.b, s.L.p, s.b, s.dg), "diag");
             }
         }
         for (SubProb& s : ps) {
             if (!s.ok) continue;
+            OnStream on(*this, s);
             // second orthonormalisation pass without shift (the basis is orthonormal to ~1e-13 already), W = F Z recomputed
             const int64_t nb = (int64_t)s.n * s.b;
             if (s.F) mm_into(s.buf[s.cur].p + nb, s.b, false, false, s.n, s.b, s.n, s.F, s.n, s.buf[s.cur].p, s.b);
@@ -391,6 +443,11 @@ struct Stepper {
             mm_into(T, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, s.W(), s.b);
             mm_into(s.H.p, s.b, true, false, s.b, s.b, s.n, s.W(), s.b, T, s.b);
         }
+        if (multi)
+            for (size_t i = 0; i < ps.size(); ++i) {
+                ck(cudaEventRecord(ss.join[i], ps[i].stream), "event");
+                ck(cudaStreamWaitEvent(st, ss.join[i], 0), "wait");
+            }
     }
 
     // R10: block-diagonal gauge rotation Gm (k x k) from wt [k x n] (rows = the vectors to fix) and the multiplet
@@ -485,6 +542,7 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
         QB = Qs[0]; RB = Rs[0]; QC = Qs[1]; RC = Rs[1];
         keep(QB); keep(RB); keep(QC); keep(RC);
     }
+    if (submark) submark();                                              // end of TATRG_ST_QR
     const int64_t npb = QB.d[1], npc = QC.d[1];
     Tens RB3 = view(RB, {npb, d1, chi}), RC3 = view(RC, {npc, d1, chi});
     const int64_t l = std::min<int64_t>(c.D + c.p, std::min(chi * npc, chi * npb));     // R3: sketch width
@@ -523,6 +581,7 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
             keep(omega);
         }
     }
+    if (submark) submark();                                              // end of TATRG_ST_RSVD
     // Eq. A.7-A.8 :373-376: SVD of the projected tensor, via an orthonormal basis of its columns and a small Jacobi SVD
     const int64_t rk = yt.d[2];
     Tens Qy, Ry;
@@ -572,7 +631,7 @@ void Stepper::triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y,
         ck(scale_last(st, xs.p, xx.p, sig, chi * J, gr, 0), "scale");
         // G^X[(i2 i3),(i2' i3')] = sum_{al,i4,g} Xs Xs
         Tens xp = perm(xs, {0, 3, 4, 1, 2});
-        Tens gx = mm(true, false, n, n, chi * d4 * gr, xp.p, n, xp.p, n);
+        Tens gx = mm(true, false, n, n, chi * d4 * gr, xp.p, n, xp.p, n, true);
         drop(xp);
         // kappa[al,al'] = sum_{i',g} Xs Xs ;  G^A = sum_{i1,i4,al,al'} A kappa A
         Tens ka = mm(false, true, chi, chi, J * gr, xs.p, J * gr, xs.p, J * gr);
@@ -581,7 +640,7 @@ void Stepper::triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y,
         Tens ap = perm(aa, {0, 3, 4, 1, 2});
         Tens tp = perm(view(ta, {d1, d2, d3, d4, chi}), {0, 3, 4, 1, 2});
         drop(ta);
-        Tens ga = mm(true, false, n, n, d1 * d4 * chi, ap.p, n, tp.p, n);
+        Tens ga = mm(true, false, n, n, d1 * d4 * chi, ap.p, n, tp.p, n, true);      // A kappa A: symmetric because kappa is
         gram[side == 0 ? 0 : 3] = ga; gram[side == 0 ? 1 : 2] = gx;
         keep(ga); keep(gx);
     }
@@ -632,6 +691,7 @@ void Stepper::triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y,
         }
         for (int i = 0; i < 4; ++i) drop(gram[i]);
     }
+    if (submark) submark();                                                // end of TATRG_ST_TRIAD_ISO
     e = ein("mjk,Ijkla->Imla", U[0], a);                                   // Eq. 2.10
     Tens f0 = ein("xjk,Ajklg->Axlg", U[1], x);                             // Eq. 2.11 (sigma goes into F only)
     ck(scale_last(st, f0.p, f0.p, sig, f0.size() / gr, gr, 0), "scale");
@@ -845,9 +905,11 @@ void Stepper::run() {
     mark();
     // (b) the QR / RSVD / lift stages are timed together under TATRG_ST_QR..LIFT: QR and RSVD flops are attributed by bond_swap
     Tens x, y; double* sig; int gr;
+    submark = mark;
     bond_swap(a, dt, core, x, y, sig, gr);
+    submark = nullptr;
     save("X", x); save("Y", y); { Tens s; s.p = sig; s.nd = 1; s.d[0] = gr; save("sigma", s); }
-    mark(); mark(); mark();
+    mark();
     Tens phin, psin;
     if (c.method == 1) {
         // ---- plain ATRG: squeezers from Gamma^ATRG = A (X sigma) | (sigma Y) Dt, contraction by Eq. 2.7-2.8 ----
@@ -889,11 +951,13 @@ void Stepper::run() {
         mark();
     } else {
         Tens U[4], e, f, g, h;
+        submark = mark;
         triad(a, dt, x, y, sig, U, e, f, g, h);                         // (c)
+        submark = nullptr;
         save("E", e); save("F", f); save("G", g); save("H", h);
         save("UA", U[0]); save("UX", U[1]); save("UY", U[2]); save("UD", U[3]);
         drop(a); drop(dt); drop(core); drop(x); drop(y);
-        mark(); mark();
+        mark();
         // (d) squeezer Gram matrices of the upper half (E F I J) and of the sigma-weighted lower half (G sigma, H, K, L)
         Tens thf[3], thb[3];
         half_grams(e, f, U[0], U[1], thf);
@@ -985,7 +1049,7 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
             if (verbose && i < cn.gemm_shapes.size()) {
                 const auto& g = cn.gemm_shapes[i];
                 fprintf(stderr, "[tatrg gemm] M=%lld N=%lld K=%lld batch=%d ta=%d tb=%d  %.3f ms  %.2f TF/s\n", (long long)g.M, (long long)g.N,
-                        (long long)g.K, g.batch, (int)g.ta, (int)g.tb, ms, 2.0 * g.M * g.N * g.K * g.batch / (ms * 1e-3) / 1e12);
+                        (long long)g.K, g.batch, (int)g.ta, (int)g.tb, ms, 2.0 * g.frac * g.M * g.N * g.K * g.batch / (ms * 1e-3) / 1e12);
             }
         }
         for (auto& ev : cn.perm_ev) { float ms = 0; cudaEventElapsedTime(&ms, ev.first, ev.second); c->perm_ms += ms; }
