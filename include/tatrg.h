@@ -94,6 +94,9 @@ long long tatrg_last_step_launches(tatrg_handle);
 /* device time (ms; needs STAGE_TIMING=2), flops and launches of the DGEMM kernel during the last step; likewise the
  * leg-permutation kernel with its algorithmic bytes (8 B read + 8 B written per element). Any out pointer may be NULL. */
 int tatrg_gemm_profile(tatrg_handle, double* ms, double* flops, long long* calls);
+/* The same restricted to the DGEMM launches of >= 1e9 flop: the tensor contractions proper (Eq. 2.18-2.19 :175, 2.9-2.17,
+ * A.2-A.11), without the small products inside the Cholesky / subspace-iteration solvers.  Needs STAGE_TIMING=2. */
+int tatrg_gemm_profile_large(tatrg_handle, double* ms, double* flops, long long* calls);
 int tatrg_permute_profile(tatrg_handle, double* ms, double* bytes, long long* calls);
 /* high-water mark (bytes) of the workspace since tatrg_create */
 size_t tatrg_workspace_peak(tatrg_handle);

@@ -40,6 +40,7 @@ _SIGNATURES = {
     "tatrg_stage_flops": (_c.c_int, [_c.c_void_p, _dp]),
     "tatrg_last_step_launches": (_c.c_longlong, [_c.c_void_p]),
     "tatrg_gemm_profile": (_c.c_int, [_c.c_void_p, _dp, _dp, _c.POINTER(_c.c_longlong)]),
+    "tatrg_gemm_profile_large": (_c.c_int, [_c.c_void_p, _dp, _dp, _c.POINTER(_c.c_longlong)]),
     "tatrg_permute_profile": (_c.c_int, [_c.c_void_p, _dp, _dp, _c.POINTER(_c.c_longlong)]),
     "tatrg_workspace_peak": (_c.c_size_t, [_c.c_void_p]),
     "tatrg_get_tensor": (_c.c_longlong, [_c.c_void_p, _c.c_char_p, _dp, _c.c_longlong, _c.POINTER(_c.c_int),
@@ -188,6 +189,11 @@ class Tatrg:
     def gemm_profile(self):
         ms, fl, n = ctypes.c_double(), ctypes.c_double(), ctypes.c_longlong()
         _check(lib().tatrg_gemm_profile(self._h, ctypes.byref(ms), ctypes.byref(fl), ctypes.byref(n)), "tatrg_gemm_profile")
+        return ms.value, fl.value, n.value
+
+    def gemm_profile_large(self):
+        ms, fl, n = ctypes.c_double(), ctypes.c_double(), ctypes.c_longlong()
+        _check(lib().tatrg_gemm_profile_large(self._h, ctypes.byref(ms), ctypes.byref(fl), ctypes.byref(n)), "tatrg_gemm_profile_large")
         return ms.value, fl.value, n.value
 
     def permute_profile(self):

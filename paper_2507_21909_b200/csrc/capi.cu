@@ -125,6 +125,7 @@ void tatrg_destroy(tatrg_handle c) {
     if (!c) return;
     for (auto e : c->stage_ev) cudaEventDestroy(e);
     for (auto e : c->cnt.ev_pool) cudaEventDestroy(e);
+    if (!c->graveyard.empty()) { cudaStreamSynchronize(c->last_stream); for (auto g : c->graveyard) cudaGraphExecDestroy(g); }
     delete c;
 }
 
@@ -142,6 +143,11 @@ long long tatrg_last_step_launches(tatrg_handle c) { return c ? c->last_launches
 int tatrg_gemm_profile(tatrg_handle c, double* ms, double* flops, long long* calls) {
     if (!c) return TATRG_EINVAL;
     if (ms) *ms = c->gemm_ms; if (flops) *flops = c->gemm_flops; if (calls) *calls = c->gemm_calls;
+    return TATRG_OK;
+}
+int tatrg_gemm_profile_large(tatrg_handle c, double* ms, double* flops, long long* calls) {
+    if (!c) return TATRG_EINVAL;
+    if (ms) *ms = c->gemm_large_ms; if (flops) *flops = c->gemm_large_flops; if (calls) *calls = c->gemm_large_calls;
     return TATRG_OK;
 }
 int tatrg_permute_profile(tatrg_handle c, double* ms, double* bytes, long long* calls) {

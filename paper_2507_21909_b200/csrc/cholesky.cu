@@ -66,7 +66,9 @@ __global__ void __launch_bounds__(256, 1) potrf_block_kernel(int nb, int j0, con
                                                              double guard_rel, int* __restrict__ info) {
     __shared__ double col[2][PB];        // published column (factorisation) / row of X (inverse)
     __shared__ double Ls[PB * PP];       // the factor, for the inverse
+    __shared__ double floor_s[PB];       // pivot floors (global loads kept out of the column loop)
     const int tid = threadIdx.x, i = tid & 63, g = tid >> 6, c0 = g * 16;
+    if (tid < PB) floor_s[tid] = fmax(guard_rel * (tid < nb ? fabs(d0[j0 + tid]) : 1.0), 1e-290);
     double a[16];
 #pragma unroll
     for (int cc = 0; cc < 16; ++cc) {
@@ -84,10 +86,12 @@ __global__ void __launch_bounds__(256, 1) potrf_block_kernel(int nb, int j0, con
         }
         __syncthreads();
         double p = col[buf][j];
-        const double dref = j < nb ? fabs(d0[j0 + j]) : 1.0;
-        const double floor_p = fmax(guard_rel * dref, 1e-290);
+        const double floor_p = floor_s[j];
         if (!(p == p) || fabs(p) > 1e300) { flag |= 2; p = floor_p; }
         if (p < floor_p) { flag |= 1; p = floor_p; }
+        // warps whose rows all lie above the pivot row, or whose 16 columns all lie left of it, have nothing to update
+        // (both conditions are warp-uniform): the serial chain of the 64 columns is issue-bound otherwise
+        if ((i | 31) < j || c0 + 15 < j) continue;
         const double r = rsqrt(p);
         const double li = (i == j) ? p * r : (i > j ? col[buf][i] * r : 0.0);
 #pragma unroll
@@ -124,7 +128,7 @@ __global__ void __launch_bounds__(256, 1) potrf_block_kernel(int nb, int j0, con
             for (int cc = 0; cc < 16; ++cc) xr[buf][c0 + cc] = x[cc];      // row k of X is final
         }
         __syncthreads();
-        if (i > k) {
+        if (i > k && c0 <= k + 1) {        // row k of X is zero right of column k: column groups beyond it only need the diagonal
             const double lik = Ls[i * PP + k];
 #pragma unroll
             for (int cc = 0; cc < 16; ++cc) x[cc] += lik * xr[buf][c0 + cc];

@@ -148,24 +148,29 @@ dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, co
         }
         const double* As = smem + (2 * (kt % STAGES)) * TILE_D;
         const double* Bs = As + TILE_D;
-#pragma unroll
-        for (int ks = 0; ks < BK / 4; ++ks) {
-            double a[MI], b[NI];
+        // fragments of the next 4-deep slice are loaded while the DMMAs of the current one issue (register double buffer)
+        double a[2][MI], b[2][NI];
+        auto load_frag = [&](int ks, double (&af)[MI], double (&bf)[NI]) {
             const int k = ks * 4 + t;
 #pragma unroll
             for (int i = 0; i < MI; ++i) {
                 int m = wm * (MI * 8) + i * 8 + g;
-                a[i] = A_KC ? As[m * PITCH_KC + k] : As[k * PA + m];
+                af[i] = A_KC ? As[m * PITCH_KC + k] : As[k * PA + m];
             }
 #pragma unroll
             for (int j = 0; j < NI; ++j) {
                 int n = wn * (NI * 8) + j * 8 + g;
-                b[j] = B_KC ? Bs[n * PITCH_KC + k] : Bs[k * PB + n];
+                bf[j] = B_KC ? Bs[n * PITCH_KC + k] : Bs[k * PB + n];
             }
+        };
+        load_frag(0, a[0], b[0]);
+#pragma unroll
+        for (int ks = 0; ks < BK / 4; ++ks) {
+            if (ks + 1 < BK / 4) load_frag(ks + 1, a[(ks + 1) & 1], b[(ks + 1) & 1]);
 #pragma unroll
             for (int i = 0; i < MI; ++i)
 #pragma unroll
-                for (int j = 0; j < NI; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                for (int j = 0; j < NI; ++j) dmma(acc[i][j][0], acc[i][j][1], a[ks & 1][i], b[ks & 1][j]);
         }
     }
     cp_wait<0>();
@@ -324,6 +329,32 @@ __global__ void splitk_reduce_kernel(const double* __restrict__ part, int nsplit
         C[r * ldc + c] = alpha * s;
     }
 }
+// Many partials of a small output (Gram matrices of very tall operands: 64 x 64 from 256 chunks): the sum over the
+// partials is itself spread over 8 threads per element (4 independent accumulators each), combined in shared memory.
+__global__ void __launch_bounds__(256) splitk_reduce_wide_kernel(const double* __restrict__ part, int nsplit, int64_t MN, int64_t N, double alpha,
+                                                                 double* __restrict__ C, int64_t ldc) {
+    __shared__ double red[8][33];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t e = (int64_t)blockIdx.x * 32 + lane;
+    double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+    if (e < MN) {
+        int k = w;
+        for (; k + 24 < nsplit; k += 32) {
+            s0 += part[(int64_t)k * MN + e]; s1 += part[(int64_t)(k + 8) * MN + e];
+            s2 += part[(int64_t)(k + 16) * MN + e]; s3 += part[(int64_t)(k + 24) * MN + e];
+        }
+        for (; k < nsplit; k += 8) s0 += part[(int64_t)k * MN + e];
+    }
+    red[w][lane] = (s0 + s1) + (s2 + s3);
+    __syncthreads();
+    if (w == 0 && e < MN) {
+        double s = 0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s += red[j][lane];
+        const int64_t r = e / N, c = e - r * N;
+        C[r * ldc + c] = alpha * s;
+    }
+}
 }  // namespace
 
 int64_t dgemm_splitk_doubles(int64_t M, int64_t N, int64_t K, bool lower_only) {
@@ -344,8 +375,12 @@ cudaError_t dgemm_splitk(cudaStream_t st, bool transa, bool transb, int64_t M, i
                                 stepA, stepB, M * N, small_cfg(M, N), lower_only);
     if (e != cudaSuccess) return e;
     int64_t MN = M * N;
-    int64_t blocks = (MN + 255) / 256; if (blocks > 148 * 8) blocks = 148 * 8;
-    splitk_reduce_kernel<<<(unsigned)blocks, 256, 0, st>>>(part, nchunks, MN, N, alpha, C, ldc);
+    if (nchunks >= 16 && MN <= (1 << 18)) {
+        splitk_reduce_wide_kernel<<<(unsigned)((MN + 31) / 32), 256, 0, st>>>(part, nchunks, MN, N, alpha, C, ldc);
+    } else {
+        int64_t blocks = (MN + 255) / 256; if (blocks > 148 * 8) blocks = 148 * 8;
+        splitk_reduce_kernel<<<(unsigned)blocks, 256, 0, st>>>(part, nchunks, MN, N, alpha, C, ldc);
+    }
     count_launch();
     return cudaGetLastError();
 }

@@ -16,6 +16,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <functional>
+#include <chrono>
 
 namespace tatrg {
 namespace {
@@ -324,19 +325,30 @@ struct Stepper {
     };
     static int sub_block(int n, int kmax) { int b = 2 * kmax; b = (b + 31) / 32 * 32; return b; }
     static bool sub_applicable(int n, int kmax) { return n > 128 && kmax >= 8 && sub_block(n, kmax) * 2 <= n; }
+    void capdbg(const char* where) {
+        static const bool on = getenv("TATRG_CAP_DEBUG") != nullptr;
+        if (!on) return;
+        cudaStreamCaptureStatus stt = cudaStreamCaptureStatusNone;
+        cudaError_t e = cudaStreamIsCapturing(st, &stt);
+        fprintf(stderr, "[capdbg] %s: status %d err %d\n", where, (int)stt, (int)e);
+    }
     void sub_orth(SubProb& s, int src, double shift) {      // buf[src] = [Z'; W'] -> buf[src^1] = [Z; W], which becomes the basis
         const int64_t rows = s.F ? 2 * (int64_t)s.n : s.n;
         double* X = s.buf[src].p;
         const double* Wp = s.F ? X + (int64_t)s.n * s.b : X;
         mm_into(s.Gm.p, s.b, true, false, s.b, s.b, s.n, X, s.b, Wp, s.b);
+        capdbg("gram");
         ck(cholesky(st, s.b, s.Gm.p, s.b, s.L.p, s.b, shift, 1e-14, s.cw), "cholesky");
+        capdbg("cholesky");
         ck(trsm_right_lt(st, rows, s.b, X, s.b, s.buf[src ^ 1].p, s.b, s.L.p, s.b, s.cw), "trsm");
+        capdbg("trsm");
         s.cur = src ^ 1;
     }
     void sub_apply(SubProb& s, int from) {         // buf[from^1] = [A Z; F A Z] with [Z; W] = buf[from]
         const double* X = s.F ? s.buf[from].p + (int64_t)s.n * s.b : s.buf[from].p;
         double* O = s.buf[from ^ 1].p;
         mm_into(O, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, X, s.b);
+        capdbg("apply");
         if (s.F) mm_into(O + (int64_t)s.n * s.b, s.b, false, false, s.n, s.b, s.n, s.F, s.n, O, s.b);
     }
     void sub_step(SubProb& s, int deg, double shift) {      // deg applications of A, then one orthonormalisation
@@ -366,6 +378,48 @@ struct Stepper {
         }
         ~OnStream() { s.st = saved; s.part_fixed = pf; s.part_cap = pc; }
     };
+    // Advances problem s to its target.  The steps are identical chains of ~15-30 small launches, and four such chains in
+    // flight are bound by the host's launch rate: one unit (1 step, or 2 when the basis alternates between the two buffers)
+    // is captured into a CUDA graph and replayed.  Counters are incremented at capture time only, hence the correction.
+    void sub_run(SubProb& s, double shift) {
+        static bool graphs_ok = getenv("TATRG_NO_GRAPHS") == nullptr;
+        const int steps = (s.target - s.done + s.deg - 1) / s.deg;
+        const int unit = (s.deg % 2 == 0) ? 2 : 1;
+        const int reps = steps / unit;
+        int left = steps;
+        if (graphs_ok && s.stream && c.timing < 2 && reps >= 3) {      // never the caller's stream: it may be the legacy default stream
+            const int done0 = s.done, cur0 = s.cur;
+            Counters* cn = g_counter;
+            const long long l0 = cn ? cn->launches : 0, gc0 = cn ? cn->gemm_calls : 0; const double f0 = cn ? cn->gemm_flops : 0;
+            cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr;
+            cudaError_t ge = cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal);
+            bool ok = ge == cudaSuccess;
+            std::string why;
+            if (ok) {
+                try { for (int u = 0; u < unit; ++u) sub_step(s, s.deg, shift); } catch (const Fail& f) { ok = false; why = f.msg; } catch (...) { ok = false; }
+                ge = cudaStreamEndCapture(st, &graph);
+                if (ge != cudaSuccess || !graph) ok = false;
+            }
+            if (ok) { ge = cudaGraphInstantiate(&exec, graph, 0); ok = ge == cudaSuccess; }
+            if (!ok && getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg subspace] graph capture failed: %s %s\n", cudaGetErrorString(ge), why.c_str());
+            if (graph) cudaGraphDestroy(graph);
+            if (getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg subspace] graph of %d step(s): %s, %d replays + %d plain steps\n", unit, ok ? "ok" : "FAILED", reps, steps - reps * unit);
+            if (ok) {
+                for (int r = 0; r < reps && ok; ++r) ok = cudaGraphLaunch(exec, st) == cudaSuccess;
+                c.graveyard.push_back(exec);
+                if (!ok) fail(TATRG_ECUDA, "graph launch failed");
+                if (cn) { cn->launches += (cn->launches - l0) * (reps - 1); cn->gemm_calls += (cn->gemm_calls - gc0) * (reps - 1); cn->gemm_flops += (cn->gemm_flops - f0) * (reps - 1); }
+                s.done = done0 + reps * unit * s.deg; s.cur = cur0;
+                left = steps - reps * unit;
+            } else {        // capture unavailable: nothing was executed; plain launches from the saved state
+                cudaGetLastError();
+                graphs_ok = false;
+                if (cn) { cn->launches = l0; cn->gemm_calls = gc0; cn->gemm_flops = f0; }
+                s.done = done0; s.cur = cur0;
+            }
+        }
+        for (int i = 0; i < left; ++i) sub_step(s, s.deg, shift);
+    }
     // Runs the iterations of all problems (interleaved so that the host reads the convergence estimates of all of them
     // with one synchronisation per phase) and leaves in every s.H the b x b Rayleigh-Ritz matrix.  Problems that cannot
     // be handled (rank-deficient leading block, no convergence in sight) come back with ok = false.
@@ -377,7 +431,7 @@ struct Stepper {
         constexpr double kShift = 1e-13;
         static const bool verbose = getenv("TATRG_SUB_VERBOSE") != nullptr;   // debugging aid only
         SubStreams& ss = sub_streams();
-        const bool multi = ss.ok && ps.size() > 1 && ps.size() <= 4;
+        const bool multi = ss.ok && !ps.empty() && ps.size() <= 4;
         if (multi) {
             ck(cudaEventRecord(ss.fork, st), "event");
             for (size_t i = 0; i < ps.size(); ++i) {
@@ -402,6 +456,8 @@ struct Stepper {
             for (int i = 0; i < q0; ++i) sub_step(s, 1, kShift);
             ck(extract_diag(st, s.b, s.L.p, s.b, s.dg), "diag");
         }
+        auto sync_all = [&]() { for (SubProb& s : ps) if (s.stream) cudaStreamSynchronize(s.stream); cudaStreamSynchronize(st); return std::chrono::steady_clock::now(); };
+        auto tA = verbose ? sync_all() : std::chrono::steady_clock::time_point();
         auto estimate = [&](SubProb& s) {
             OnStream on(*this, s);
             s.r = to_host(s.dg, s.b);
@@ -427,10 +483,11 @@ struct Stepper {
             for (SubProb& s : ps) {
                 if (!s.ok || s.target <= s.done) continue;
                 OnStream on(*this, s);
-                while (s.done < s.target) sub_step(s, s.deg, kShift);
+                sub_run(s, kShift);
                 ck(extract_diag(st, s.b, s.L.p, s.b, s.dg), "diag");
             }
         }
+        auto tB = verbose ? sync_all() : tA;
         for (SubProb& s : ps) {
             if (!s.ok) continue;
             OnStream on(*this, s);
@@ -448,6 +505,11 @@ struct Stepper {
                 ck(cudaEventRecord(ss.join[i], ps[i].stream), "event");
                 ck(cudaStreamWaitEvent(st, ss.join[i], 0), "wait");
             }
+        if (verbose) {
+            auto tC = sync_all();
+            fprintf(stderr, "[tatrg subspace] %zu problems: phases after the first %d steps %.2f ms, final pass + Rayleigh-Ritz matrix %.2f ms\n", ps.size(), q0,
+                    std::chrono::duration<double, std::milli>(tB - tA).count(), std::chrono::duration<double, std::milli>(tC - tB).count());
+        }
     }
 
     // R10: block-diagonal gauge rotation Gm (k x k) from wt [k x n] (rows = the vectors to fix) and the multiplet
@@ -656,11 +718,16 @@ void Stepper::triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y,
                 ck(symmetrize(st, (int)n, gram[i].p), "symmetrize");
                 ps[i].Bm = gram[i].p; ps[i].F = nullptr; ps[i].n = (int)n; ps[i].kmax = kmax; ps[i].b = sub_block((int)n, kmax); ps[i].sid = 16 + i;
             }
+            const bool vb = getenv("TATRG_SUB_VERBOSE") != nullptr;
+            auto now = [&]() { cudaStreamSynchronize(st); return std::chrono::steady_clock::now(); };
+            auto t0 = vb ? now() : std::chrono::steady_clock::time_point();
             sub_iterate(ps);
+            auto t1 = vb ? now() : t0;
             std::vector<Tens*> hs; std::vector<int> ns, who;
             for (int i = 0; i < 4; ++i) if (ps[i].ok) { hs.push_back(&ps[i].H); ns.push_back(ps[i].b); who.push_back(i); }
             std::vector<EigOut> er;
             if (!hs.empty()) eig_batch(hs, ns, er);
+            if (vb) { auto t2 = now(); fprintf(stderr, "[tatrg triad] subspace iterations %.2f ms, Rayleigh-Ritz %.2f ms\n", std::chrono::duration<double, std::milli>(t1 - t0).count(), std::chrono::duration<double, std::milli>(t2 - t1).count()); }
             for (size_t j = 0; j < who.size(); ++j) {
                 const int i = who[j], b = ps[i].b;
                 std::vector<double> sv(b);
@@ -1023,6 +1090,8 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
     cn.launches = 0; cn.gemm_flops = 0; cn.gemm_calls = 0; cn.permuted_bytes = 0; cn.permute_calls = 0;
     cn.time_kernels = c->timing >= 2; cn.gemm_ev.clear(); cn.perm_ev.clear(); cn.gemm_shapes.clear(); cn.ev_used = 0;
     g_counter = &cn;
+    for (cudaGraphExec_t g : c->graveyard) cudaGraphExecDestroy(g);    // their launches completed before the previous step's last read-back
+    c->graveyard.clear();
     int rc = TATRG_OK;
     const size_t lnc0 = c->lnc.size();
     try {
@@ -1044,8 +1113,14 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
         for (int i = 0; i < TATRG_NSTAGES; ++i) { float ms = 0; cudaEventElapsedTime(&ms, c->stage_ev[i], c->stage_ev[i + 1]); c->stage_ms[i] = ms; }
         c->gemm_ms = 0; c->perm_ms = 0;
         const bool verbose = getenv("TATRG_GEMM_VERBOSE") != nullptr;   // debugging aid: per-launch shapes and rates
+        c->gemm_large_ms = 0; c->gemm_large_flops = 0; c->gemm_large_calls = 0;
         for (size_t i = 0; i < cn.gemm_ev.size(); ++i) {
             float ms = 0; cudaEventElapsedTime(&ms, cn.gemm_ev[i].first, cn.gemm_ev[i].second); c->gemm_ms += ms;
+            if (i < cn.gemm_shapes.size()) {
+                const auto& g = cn.gemm_shapes[i];
+                const double fl = 2.0 * g.frac * g.M * g.N * g.K * g.batch;
+                if (fl >= kLargeGemmFlops) { c->gemm_large_ms += ms; c->gemm_large_flops += fl; c->gemm_large_calls += 1; }
+            }
             if (verbose && i < cn.gemm_shapes.size()) {
                 const auto& g = cn.gemm_shapes[i];
                 fprintf(stderr, "[tatrg gemm] M=%lld N=%lld K=%lld batch=%d ta=%d tb=%d  %.3f ms  %.2f TF/s\n", (long long)g.M, (long long)g.N,

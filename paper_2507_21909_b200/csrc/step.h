@@ -6,6 +6,10 @@
 
 namespace tatrg {
 
+// DGEMM launches of at least this many flops are the tensor contractions of the path (Eq. 2.18-2.19, 2.9-2.17, A.2-A.11:
+// >= 4e9 each at D = 32); the products inside the Cholesky / subspace solvers are <= 3e8.
+constexpr double kLargeGemmFlops = 1e9;
+
 struct Fail {
     int code; std::string msg;
 };
@@ -33,10 +37,12 @@ struct tatrg_ctx {
     std::vector<double> sv_sigma, sv_s;
     double stage_ms[TATRG_NSTAGES] = {0}, stage_flops[TATRG_NSTAGES] = {0};
     double gemm_ms = 0, gemm_flops = 0, perm_ms = 0; long long gemm_calls = 0, perm_calls = 0, perm_bytes = 0;
+    double gemm_large_ms = 0, gemm_large_flops = 0; long long gemm_large_calls = 0;   // launches of >= kLargeGemmFlops
     long long last_launches = 0;
     tatrg::Counters cnt;
     std::map<std::string, tatrg::Tens> kept;   // tensors of the last step (keep_tensors only)
     std::vector<cudaEvent_t> stage_ev;
+    std::vector<cudaGraphExec_t> graveyard;    // replayed graphs of the last step, destroyed at the start of the next one
 };
 
 namespace tatrg {
