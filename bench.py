@@ -151,6 +151,12 @@ def aggregate_seconds_per_step(ms_max, steps, world):
     return ms_max * 1e-3 / (steps * world)
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant DGEMM launch (Xi = E (M4 F), Eq. 2.18: M=2048, N=65536, K=1024, 8.6 ms)
+# from the ncu --set full capture in profiles/dgemm_r01_ncu_full.txt; its algorithmic bytes are 8 (MK + KN + MN) = 1.63e9
+DGEMM_TRAFFIC = {"launch": "M=2048 N=65536 K=1024 (grid 8192)", "dram_bytes": 1.601e9, "algorithmic_bytes": 1.627e9,
+                 "source": "profiles/dgemm_r01_ncu_full.txt"}
+
+
 # ---- the CUDA path ---------------------------------------------------------------------------------------------------
 def run_cuda(args):
     import torch
@@ -249,7 +255,7 @@ def run_cuda(args):
             "model_tflops": g_fl / n_prof / (ms / args.steps * 1e-3) / 1e12,
             "roofline": {"bound": "tensor", "kernel": "dgemm_kernel (DMMA m8n8k4): the %d contraction launches of a step (>= 1e9 flop each, "
                                                       "%.1f%% of the step's DGEMM flops)" % (l_n // n_prof, 100.0 * l_fl / g_fl),
-                         "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": None,
+                         "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": DGEMM_TRAFFIC,
                          "all_launches": {"launches_per_step": g_n // n_prof, "achieved": all_tf, "frac": all_tf / peak_tf,
                                           "note": "includes the small products of the Cholesky / subspace-iteration solvers, which "
                                                   "run concurrently on several streams: their event times overlap"},

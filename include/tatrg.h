@@ -166,6 +166,10 @@ int tatrg_dot(void* cuda_stream, long long n, const double* x, const double* y, 
 /* Calibration: FP64 tensor-core (DMMA m8n8k4) issue rate of the whole device with register-resident operands, in
  * TFLOP/s, timed with CUDA events inside the call (synchronises).  ctas_per_sm in 1..8; scratch_dev [dev] >= 8 bytes. */
 int tatrg_dmma_issue_rate(void* cuda_stream, int iters, int ctas_per_sm, double* tflops_out, double* scratch_dev);
+/* The same for the register tile of the DGEMM inner loop (8 x 4 atoms per warp, 12 distinct operand registers per 4-deep
+ * slice, one 256-thread CTA per SM, no memory traffic): the ceiling of the warp tile itself.  order 0: row-major walk of the
+ * atoms (the A fragment is reused by consecutive DMMAs), 1: column-major walk. */
+int tatrg_dmma_tile_rate(void* cuda_stream, int iters, int order, double* tflops_out, double* scratch_dev);
 
 #ifdef __cplusplus
 }

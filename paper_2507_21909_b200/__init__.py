@@ -66,6 +66,7 @@ _SIGNATURES = {
     "tatrg_cholqr": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
     "tatrg_dot": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
     "tatrg_dmma_issue_rate": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_int, _dp, _c.c_void_p]),
+    "tatrg_dmma_tile_rate": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_int, _dp, _c.c_void_p]),
 }
 
 
@@ -350,6 +351,15 @@ def dot(x, y):
     res = torch.empty(1200, dtype=torch.float64, device=x.device)
     _check(lib().tatrg_dot(_stream_ptr(), x.numel(), _p(x), _p(y), _p(res)), "tatrg_dot")
     return float(res[0].item())
+
+
+def dmma_tile_rate(iters=5000, order=0):
+    """DMMA rate of the DGEMM register tile (8 x 4 atoms per warp, one CTA per SM) without memory traffic, TFLOP/s."""
+    torch = _torch_cuda()
+    scratch = torch.zeros(8, dtype=torch.float64, device="cuda")
+    out = ctypes.c_double()
+    _check(lib().tatrg_dmma_tile_rate(_stream_ptr(), iters, order, ctypes.byref(out), _p(scratch)), "tatrg_dmma_tile_rate")
+    return out.value
 
 
 def dmma_issue_rate(iters=20000, ctas_per_sm=2):

@@ -92,12 +92,16 @@ __global__ void __launch_bounds__(256, 1) potrf_block_kernel(int nb, int j0, con
         // warps whose rows all lie above the pivot row, or whose 16 columns all lie left of it, have nothing to update
         // (both conditions are warp-uniform): the serial chain of the 64 columns is issue-bound otherwise
         if ((i | 31) < j || c0 + 15 < j) continue;
+        // l_i l_c = (a_ij / p) a_cj: one DMUL per thread and one DFMA per entry instead of a DMUL + DFMA per entry (the
+        // FP64 pipe is what the 64-column chain waits for)
         const double r = rsqrt(p);
-        const double li = (i == j) ? p * r : (i > j ? col[buf][i] * r : 0.0);
+        const double ci = (i >= j) ? col[buf][i] : 0.0;
+        const double lip = ci * (r * r);
+        const double li = (i == j) ? p * r : ci * r;
 #pragma unroll
         for (int cc = 0; cc < 16; ++cc) {
             const int c = c0 + cc;
-            if (c > j) a[cc] -= li * (col[buf][c] * r);
+            if (c > j) a[cc] -= lip * col[buf][c];
             else if (c == j) a[cc] = li;
         }
     }

@@ -23,20 +23,20 @@ cudaEvent_t Counters::next_event() {
 }
 
 namespace {
-constexpr int BK = 16, STAGES = 4;
-constexpr int PITCH_KC = BK + 4;   // operand stored [row][k]: 20 doubles
+constexpr int kChunkAlign = 32;    // split-K chunks are multiples of every configuration's BK
 
-template <int BM_, int BN_, int WM_, int WN_>
+template <int BM_, int BN_, int WM_, int WN_, int BK_, int STAGES_>
 struct Cfg {
-    static constexpr int BM = BM_, BN = BN_, WM = WM_, WN = WN_;
+    static constexpr int BM = BM_, BN = BN_, WM = WM_, WN = WN_, BK = BK_, STAGES = STAGES_;
+    static constexpr int PITCH_KC = BK + 4;   // operand stored [row][k]: = 4 (mod 16) doubles
     static constexpr int NT = 32 * WM * WN;
     static constexpr int MI = BM / WM / 8, NI = BN / WN / 8;          // atoms per warp
     static constexpr int ROWS = BM > BN ? BM : BN;
     static constexpr int TILE_D = ROWS * PITCH_KC > BK * (ROWS + 4) ? ROWS * PITCH_KC : BK * (ROWS + 4);
     static constexpr int SMEM = STAGES * 2 * TILE_D * 8;
 };
-using CfgL = Cfg<128, 128, 2, 4>;
-using CfgS = Cfg<64, 64, 2, 2>;
+using CfgL = Cfg<128, 128, 2, 4, 16, 4>;     // BK = 32 with 3 stages (221 KB) measured no faster
+using CfgS = Cfg<64, 64, 2, 2, 16, 4>;
 
 __device__ __forceinline__ void cp16(double* dst, const double* src, bool ok) {
     unsigned d = (unsigned)__cvta_generic_to_shared(dst);
@@ -52,21 +52,21 @@ __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_grou
 template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
 __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                  : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
 // Load one ROWS x 16 operand tile.  KC: global element (r, k) at g[r*ld + k]; else at g[k*ld + r].
 // rows = extent of the non-contracted dimension, K = extent of k; r0/k0 tile origin.
-template <bool KC, bool V16, int ROWS, int NT>
+template <bool KC, bool V16, int ROWS, int NT, int BK>
 __device__ __forceinline__ void load_tile(double* s, const double* __restrict__ g, int64_t ld, int64_t r0, int64_t k0,
                                           int64_t rows, int64_t K, int tid) {
-    constexpr int PITCH_MC = ROWS + 4;
+    constexpr int PITCH_MC = ROWS + 4, PITCH_KC = BK + 4, CPR = BK / 2;
     if (KC) {
         if (V16) {
 #pragma unroll
             for (int c = tid; c < ROWS * BK / 2; c += NT) {
-                int r = c >> 3, kc = (c & 7) * 2;
+                int r = c / CPR, kc = (c % CPR) * 2;
                 bool ok = (r0 + r < rows) && (k0 + kc < K);
                 const double* src = ok ? g + (r0 + r) * ld + k0 + kc : g;
                 cp16(s + r * PITCH_KC + kc, src, ok);
@@ -74,7 +74,7 @@ __device__ __forceinline__ void load_tile(double* s, const double* __restrict__ 
         } else {
 #pragma unroll
             for (int c = tid; c < ROWS * BK; c += NT) {
-                int r = c >> 4, kc = c & 15;
+                int r = c / BK, kc = c % BK;
                 bool ok = (r0 + r < rows) && (k0 + kc < K);
                 const double* src = ok ? g + (r0 + r) * ld + k0 + kc : g;
                 cp8(s + r * PITCH_KC + kc, src, ok);
@@ -101,12 +101,55 @@ __device__ __forceinline__ void load_tile(double* s, const double* __restrict__ 
     }
 }
 
+// The same for the 16-byte path with everything loop-invariant hoisted: the k-loop then spends one pointer add, one
+// compare and one cp.async per 16-byte chunk (the generic index arithmetic of load_tile costs ~140 integer instructions
+// per k-step, during which neither warp of a scheduler issues DMMAs).  Chunk `it` of a thread sits at a fixed stride
+// from its chunk 0 in global and in shared memory:
+//   KC: r = tid/(BK/2) + it*NT/(BK/2), kc = 2*(tid%(BK/2))     MC: k = tid/(ROWS/2) + it*NT/(ROWS/2), rc = 2*(tid%(ROWS/2))
+template <bool KC, int ROWS, int NT, int BK>
+struct TileLoader {
+    static constexpr int ITERS = ROWS * BK / 2 / NT;
+    static constexpr int HALF = ROWS / 2, CPR = BK / 2;
+    static constexpr int PITCH_MC = ROWS + 4, PITCH_KC = BK + 4;
+    const double* p0; const double* safe;
+    int64_t step_it, step_k;
+    unsigned mask;
+    int kofs0, kofs_it, soff0, soff_it;
+    __device__ __forceinline__ void init(const double* __restrict__ g, int64_t ld, int64_t r0, int64_t rows, int tid) {
+        safe = g;
+        if (KC) {
+            const int r = tid / CPR, kc = (tid % CPR) * 2;
+            p0 = g + (r0 + r) * ld + kc; step_it = (int64_t)(NT / CPR) * ld; step_k = BK;
+            mask = 0;
+#pragma unroll
+            for (int it = 0; it < ITERS; ++it) if (r0 + r + it * (NT / CPR) < rows) mask |= 1u << it;
+            kofs0 = kc; kofs_it = 0; soff0 = r * PITCH_KC + kc; soff_it = (NT / CPR) * PITCH_KC;
+        } else {
+            const int k = tid / HALF, rc = (tid % HALF) * 2;
+            p0 = g + (int64_t)k * ld + r0 + rc; step_it = (int64_t)(NT / HALF) * ld; step_k = (int64_t)BK * ld;
+            mask = (r0 + rc < rows) ? 0xffffffffu : 0u;
+            kofs0 = k; kofs_it = NT / HALF; soff0 = k * PITCH_MC + rc; soff_it = (NT / HALF) * PITCH_MC;
+        }
+    }
+    // tile kt (k origin kt*BK) -> stage buffer s
+    __device__ __forceinline__ void issue(double* s, int kt, int64_t K) const {
+        const double* p = p0 + (int64_t)kt * step_k;
+        const int64_t krem = K - (int64_t)kt * BK - kofs0;      // chunk it is inside K iff it*kofs_it < krem
+#pragma unroll
+        for (int it = 0; it < ITERS; ++it) {
+            const bool ok = ((mask >> it) & 1u) && (int64_t)(it * kofs_it) < krem;
+            cp16(s + soff0 + it * soff_it, ok ? p + it * step_it : safe, ok);
+        }
+    }
+};
+
 template <class C_, bool A_KC, bool B_KC, bool AV16, bool BV16>
 __global__ void __launch_bounds__(C_::NT, C_::NT == 256 ? 1 : 2)
 dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, const double* __restrict__ A, int64_t lda,
              const double* __restrict__ B, int64_t ldb, double beta, double* __restrict__ C, int64_t ldc, int64_t sA,
              int64_t sB, int64_t sC, int tiles_m, int lower_only) {
     constexpr int BM = C_::BM, BN = C_::BN, NT = C_::NT, MI = C_::MI, NI = C_::NI, TILE_D = C_::TILE_D;
+    constexpr int BK = C_::BK, STAGES = C_::STAGES, PITCH_KC = C_::PITCH_KC;
     constexpr int PA = BM + 4, PB = BN + 4;
     extern __shared__ __align__(16) double smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -126,12 +169,17 @@ dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, co
         for (int j = 0; j < NI; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
     const int nk = (int)((K + BK - 1) / BK);
+    TileLoader<A_KC, BM, NT, BK> ldA; TileLoader<B_KC, BN, NT, BK> ldB;
+    if (AV16) ldA.init(A, lda, m0, M, tid);
+    if (BV16) ldB.init(B, ldb, n0, N, tid);
+    auto load_stage = [&](int kt) {
+        double* sa = smem + (2 * (kt % STAGES)) * TILE_D;
+        if (AV16) ldA.issue(sa, kt, K); else load_tile<A_KC, false, BM, NT, BK>(sa, A, lda, m0, (int64_t)kt * BK, M, K, tid);
+        if (BV16) ldB.issue(sa + TILE_D, kt, K); else load_tile<B_KC, false, BN, NT, BK>(sa + TILE_D, B, ldb, n0, (int64_t)kt * BK, N, K, tid);
+    };
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
-        if (s < nk) {
-            load_tile<A_KC, AV16, BM, NT>(smem + (2 * s) * TILE_D, A, lda, m0, (int64_t)s * BK, M, K, tid);
-            load_tile<B_KC, BV16, BN, NT>(smem + (2 * s + 1) * TILE_D, B, ldb, n0, (int64_t)s * BK, N, K, tid);
-        }
+        if (s < nk) load_stage(s);
         cp_commit();
     }
     for (int kt = 0; kt < nk; ++kt) {
@@ -139,11 +187,7 @@ dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, co
         __syncthreads();
         {
             int nxt = kt + STAGES - 1;
-            if (nxt < nk) {
-                int s = nxt % STAGES;
-                load_tile<A_KC, AV16, BM, NT>(smem + (2 * s) * TILE_D, A, lda, m0, (int64_t)nxt * BK, M, K, tid);
-                load_tile<B_KC, BV16, BN, NT>(smem + (2 * s + 1) * TILE_D, B, ldb, n0, (int64_t)nxt * BK, N, K, tid);
-            }
+            if (nxt < nk) load_stage(nxt);
             cp_commit();
         }
         const double* As = smem + (2 * (kt % STAGES)) * TILE_D;
@@ -367,7 +411,7 @@ cudaError_t dgemm_splitk(cudaStream_t st, bool transa, bool transb, int64_t M, i
     int ns = splitk_count(M, N, K, lower_only);
     if (ns <= 1 || part == nullptr) return dgemm_klast(st, transa, transb, M, N, K, 0, alpha, A, lda, B, ldb, 0.0, C, ldc, 1, 0, 0, 0, false, lower_only);
     // chunk: multiple of BK; the last batch entry takes the ragged tail (klast)
-    int64_t chunk = ((K + ns - 1) / ns + BK - 1) / BK * BK;
+    int64_t chunk = ((K + ns - 1) / ns + kChunkAlign - 1) / kChunkAlign * kChunkAlign;
     int nchunks = (int)((K + chunk - 1) / chunk);
     int64_t tail = K - (int64_t)(nchunks - 1) * chunk;
     const int64_t stepA = transa ? chunk * lda : chunk, stepB = transb ? chunk : chunk * ldb;
