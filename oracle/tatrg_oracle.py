@@ -376,9 +376,15 @@ def contract_psi(g, h, k_, l_, n2, n3, n4):
 class TatrgOracle:
     """State = (Phi, Psi, [ln c_m], step counter).  step() = Fig. 5 (a)-(f) :193."""
 
-    def __init__(self, beta, h, D, oversample, seed, n_pow=2, K=None, tau=TAU_MULTIPLET, exact_swap=False, method="triad"):
+    def __init__(self, beta, h, D, oversample, seed, n_pow=2, K=None, tau=TAU_MULTIPLET, exact_swap=False, method="triad",
+                 bond_rank=None):
         self.beta, self.h, self.D, self.p, self.seed = beta, h, D, oversample, seed
         self.method = method                                   # "triad" (Eq. 2.9-2.19) or "atrg" (Eq. 2.7-2.8)
+        # ILO Triad-ATRG (PAPER.md section 2.3 :183-209, App. A :331-394): the bond swap keeps r_bond D values (the sum over gamma in
+        # Eq. A.1 :337 runs to r_bond D) and, one step later, so does the decomposition of T (fn 5 :203: "the subscripts alpha and
+        # beta in Eq. (2.4) are also overspanned"); the RSVD sketch is r_bond D + p wide (fn 9 :381).  bond_rank = r_bond D; the
+        # squeezed legs stay at D.  bond_rank = D is the Triad-ATRG of section 2.2.
+        self.bond_rank = bond_rank if bond_rank is not None else D
         self.n_pow, self.tau, self.exact_swap = n_pow, tau, exact_swap
         self.K = K if K is not None else D + oversample        # R3: triad internal-line dimension rD = D + p
         self.phi, self.psi = init_tensor(beta, h)
@@ -388,8 +394,8 @@ class TatrgOracle:
 
     def step(self):
         D, tau, call = self.D, self.tau, self.m + 1
-        a, dt, core, s_all, lnc = decompose(self.phi, self.psi, D, self.seed, call, tau)          # (a)
-        x, y, sig, sig_all = bond_swap(a, dt, core, D, self.p, self.n_pow, self.seed, call, tau,
+        a, dt, core, s_all, lnc = decompose(self.phi, self.psi, self.bond_rank, self.seed, call, tau)          # (a)
+        x, y, sig, sig_all = bond_swap(a, dt, core, self.bond_rank, self.p, self.n_pow, self.seed, call, tau,
                                        exact=self.exact_swap)                                        # (b)
         if self.method == "atrg":
             return self._finish_atrg(a, dt, core, s_all, lnc, x, y, sig, sig_all, call)

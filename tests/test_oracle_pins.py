@@ -516,3 +516,74 @@ def test_atrg_staged_gram_equals_definition_on_random_tensors():
     half = np.einsum("iucda,alefg->iuclefdg", p, q)               # [o1,u2,u3,l2,l3,l4,u4,o2]
     th2 = np.einsum("iuclefdg,ivcwefdg->ulvw", half, half)
     assert np.abs(O.atrg_grams(p, q, 2) - th2).max() <= 1e-12
+
+
+# ------------------------------------------------------------------------------------------------ ILO Triad-ATRG (section 2.3)
+def test_ilo_bond_rank_equal_D_is_plain_triad_atrg():
+    """':331 When r_bond = 1 is set, it returns to the conventional ATRG bond-swapping process.'"""
+    o0 = O.TatrgOracle(0.1497, 0.0, 4, 4, 3, n_pow=1)
+    o1 = O.TatrgOracle(0.1497, 0.0, 4, 4, 3, n_pow=1, bond_rank=4)
+    for _ in range(5):
+        o0.step(); o1.step()
+        assert o0.lnZ_per_site() == o1.lnZ_per_site()
+
+
+def test_ilo_shapes_follow_footnote_5():
+    """fn 5 :203: with overspanning, X and Y become (r_bond D) x D x D x D x (r_bond D) once the overspanned gamma of one step
+    has become the alpha, beta of the next; the squeezed legs stay at D; sigma has r_bond D entries (Eq. A.1 :337)."""
+    D, Db = 3, 6
+    o = O.TatrgOracle(0.1497, 0.0, D, D, 5, n_pow=2, bond_rank=Db)
+    for _ in range(6):
+        o.step()
+    assert o.phi.shape == (D, D, D, D, Db) and o.psi.shape == (D, D, D, D, Db)
+    assert o.last["x"].shape == (Db, D, D, D, Db) and o.last["y"].shape == (Db, D, D, D, Db)
+    assert len(o.last["sig"]) == Db and o.last["a"].shape == (D, D, D, D, Db)
+    for t in (o.last["x"], o.last["y"], o.last["a"], o.last["dt"]):      # still isometries (:137, :339)
+        m = t.reshape(-1, t.shape[-1])
+        assert np.abs(m.T @ m - np.eye(m.shape[1])).max() < 1e-12
+
+
+def test_ilo_decomposition_keeps_the_whole_overspanned_bond():
+    """fn 5: 'the subscripts alpha and beta in Eq. (2.4) are also overspanned': T = Phi Psi^T of an ILO state (factor bond
+    r_bond D) is reproduced exactly by A c Dt^T -- the decomposition at rank r_bond D truncates nothing."""
+    D, Db = 3, 6
+    o = O.TatrgOracle(0.1497, 0.0, D, D, 5, n_pow=2, bond_rank=Db)
+    for _ in range(5):
+        o.step()
+    a, dt, core, s, lnc = O.decompose(o.phi, o.psi, Db, 5, 6)
+    chi = a.shape[-1]
+    t = o.phi.reshape(-1, Db) @ o.psi.reshape(-1, Db).T
+    assert chi == Db and np.abs(a.reshape(-1, chi) @ core @ dt.reshape(-1, chi).T * math.exp(lnc) - t).max() < 1e-12 * np.abs(t).max()
+    a3, dt3, core3, _, lnc3 = O.decompose(o.phi, o.psi, D, 5, 6)             # rank D would truncate it
+    assert np.abs(a3.reshape(-1, D) @ core3 @ dt3.reshape(-1, D).T * math.exp(lnc3) - t).max() > 1e-6 * np.abs(t).max()
+
+
+def test_ilo_bond_swap_is_the_best_rank_rbondD_approximation():
+    """App. A :339 'this decomposition ... yields an optimal low-rank approximation of the unit-cell tensor in terms of the
+    Frobenius norm' (Eckart-Young): at rank r_bond D the squared error of X sigma Y against sum_i1 B C is the sum of the
+    discarded squared singular values, and it is smaller than at rank D."""
+    o = _state_after(2, D=4, p=4)
+    a, dt, core, s, _ = O.decompose(o.phi, o.psi, 4, 11, 3)
+    b = np.einsum("ijklc,ac->ijkla", dt, core)
+    c = np.einsum("ijklc,cb->ijklb", a, core)
+    lhs = np.einsum("ijkla,imnob->amnobjkl", b, c)
+    errs = []
+    for rank in (4, 8, 12):
+        x, y, sig, sig_all = O.bond_swap(a, dt, core, rank, 0, 0, 11, 3, exact=True)
+        assert len(sig) == rank
+        rhs = np.einsum("amnog,g,bjklg->amnobjkl", x, sig, y)
+        err2 = float(((lhs - rhs) ** 2).sum())
+        tail2 = float(((sig_all[rank:] * sig[0]) ** 2).sum())
+        assert abs(err2 - tail2) < 1e-12 * float((lhs ** 2).sum())
+        errs.append(err2)
+    assert errs[0] > errs[1] > errs[2]
+
+
+@pytest.mark.parametrize("beta,h", [(0.14, 0.0), (0.1497, 1e-3)])
+def test_ilo_first_steps_stay_exact(beta, h):
+    """Overspanning never truncates more: one and two steps remain exact against brute-force enumeration."""
+    o = O.TatrgOracle(beta, h, 16, 16, 2, n_pow=2, bond_rank=32)
+    o.step()
+    assert abs(o.lnZ_per_site() - enumerate_lnz_per_site((2, 1, 1, 1), beta, h)) < 2e-14
+    o.step()
+    assert abs(o.lnZ_per_site() - enumerate_lnz_per_site((2, 2, 1, 1), beta, h)) < 1e-13
