@@ -33,6 +33,11 @@ enum {
     TATRG_OPT_SUBSPACE = 7,    /* 1 (default): the leading eigenvectors the triad isometries (top K of D^2, Eq. 2.9 :135) and the
                                   squeezers (top D of D^2, :171) need come from a subspace iteration (Cholesky QR on the tensor
                                   cores + one small Rayleigh-Ritz problem); 0: full eigen-decompositions everywhere.  Same result. */
+    TATRG_OPT_BOND_RANK = 8,   /* ILO Triad-ATRG (section 2.3 :183-209, App. A): r_bond D, the number of singular values the bond swap keeps
+                                  (Eq. A.1 :337) and hence the rank of the next decomposition (fn 5 :203); the RSVD sketch is
+                                  r_bond D + oversample wide (fn 9 :381); the squeezed legs stay at D.  default D (r_bond = 1, :331).
+                                  Before the first step only; integer in [D, 4D]; ENOMEM unless the workspace holds
+                                  tatrg_workspace_bytes_ilo(D, oversample, value). */
     TATRG_OPT_METHOD = 6       /* 0: Triad-ATRG (default).  1: plain ATRG, Eq. 2.7-2.8 (:104-113): no triad split, squeezers from
                                   Gamma^ATRG, O(D^9) contraction sliced so that no D^7 tensor is stored (fn 6 :205).  Before the first
                                   step only; ENOMEM unless the workspace holds tatrg_workspace_bytes_atrg(D, oversample). */
@@ -49,6 +54,8 @@ enum { TATRG_ST_DECOMPOSE = 0, TATRG_ST_QR, TATRG_ST_RSVD, TATRG_ST_LIFT, TATRG_
 
 /* Device bytes a handle with truncation D (Eq. 2.4 :76) and RSVD oversampling p (l = D+p, :371) needs. */
 size_t tatrg_workspace_bytes(int D, int oversample);
+/* The same for TATRG_OPT_BOND_RANK = bond_rank (ILO Triad-ATRG: X, Y, F, G carry two legs of dimension r_bond D, fn 5 :203). */
+size_t tatrg_workspace_bytes_ilo(int D, int oversample, int bond_rank);
 /* The same for TATRG_OPT_METHOD = 1 (plain ATRG keeps three D^6 slabs). */
 size_t tatrg_workspace_bytes_atrg(int D, int oversample);
 

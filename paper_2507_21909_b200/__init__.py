@@ -15,7 +15,7 @@ _LIB_PATH = os.path.join(_HERE, "libtatrg.so")
 _lib = None
 
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC, ESTATE = 0, -1, -2, -3, -4, -5
-OPT_POWER_ITERS, OPT_K_TRIAD, OPT_TAU, OPT_STAGE_TIMING, OPT_KEEP_TENSORS, OPT_METHOD, OPT_SUBSPACE = 1, 2, 3, 4, 5, 6, 7
+OPT_POWER_ITERS, OPT_K_TRIAD, OPT_TAU, OPT_STAGE_TIMING, OPT_KEEP_TENSORS, OPT_METHOD, OPT_SUBSPACE, OPT_BOND_RANK = 1, 2, 3, 4, 5, 6, 7, 8
 METHOD_TRIAD, METHOD_ATRG = 0, 1
 SV_SIGMA, SV_S = 0, 1
 STAGES = ["decompose", "qr", "rsvd", "lift", "triad", "triad_tensors", "squeezer_grams", "squeezers", "contract",
@@ -26,6 +26,7 @@ _dp = _c.POINTER(_c.c_double)
 _SIGNATURES = {
     "tatrg_workspace_bytes": (_c.c_size_t, [_c.c_int, _c.c_int]),
     "tatrg_workspace_bytes_atrg": (_c.c_size_t, [_c.c_int, _c.c_int]),
+    "tatrg_workspace_bytes_ilo": (_c.c_size_t, [_c.c_int, _c.c_int, _c.c_int]),
     "tatrg_create": (_c.c_int, [_c.c_double, _c.c_double, _c.c_int, _c.c_int, _c.c_uint64, _c.c_void_p, _c.c_size_t,
                                 _c.POINTER(_c.c_void_p)]),
     "tatrg_set_option": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_double]),
@@ -119,12 +120,14 @@ class Tatrg:
     """One 4D Ising tensor network being coarse-grained on one GPU (tatrg_create .. tatrg_destroy)."""
 
     def __init__(self, beta, h, D, oversample, seed, power_iters=2, K=None, tau=None, device="cuda:0", workspace=None,
-                 method=METHOD_TRIAD):
+                 method=METHOD_TRIAD, bond_rank=None):
         torch = _torch_cuda()
         L = lib()
         need = L.tatrg_workspace_bytes_atrg(D, oversample) if method == METHOD_ATRG else L.tatrg_workspace_bytes(D, oversample)
+        if bond_rank is not None and bond_rank != D:      # ILO Triad-ATRG (PAPER.md section 2.3): bond_rank = r_bond * D
+            need = max(need, L.tatrg_workspace_bytes_ilo(D, oversample, bond_rank)) if L.tatrg_workspace_bytes_ilo(D, oversample, bond_rank) else 0
         if need == 0:
-            raise TatrgError("unsupported (D, oversample) = (%d, %d)" % (D, oversample))
+            raise TatrgError("unsupported (D, oversample, bond_rank) = (%d, %d, %s)" % (D, oversample, bond_rank))
         self.device = torch.device(device)
         with torch.cuda.device(self.device):
             self.workspace = workspace if workspace is not None else torch.empty(need, dtype=torch.uint8, device=self.device)
@@ -142,6 +145,8 @@ class Tatrg:
             self.set_option(OPT_TAU, tau)
         if method != METHOD_TRIAD:
             self.set_option(OPT_METHOD, method)
+        if bond_rank is not None and bond_rank != D:
+            self.set_option(OPT_BOND_RANK, bond_rank)
 
     def set_option(self, key, value):
         _check(lib().tatrg_set_option(self._h, key, float(value)), "tatrg_set_option", self._h)

@@ -22,6 +22,14 @@ size_t tatrg_workspace_bytes(int D, int oversample) {
     return (size_t)workspace_doubles(D, oversample) * 8;
 }
 
+size_t tatrg_workspace_bytes_ilo(int D, int oversample, int bond_rank) {
+    const size_t base = tatrg_workspace_bytes(D, oversample);
+    if (base == 0 || bond_rank < D || bond_rank > 4 * D || bond_rank + oversample > 112) return 0;
+    // every tensor carries at most two overspanned legs (X, Y, F, G of fn 5 :203): the plain bound times (r_bond)^2
+    const double r = (double)bond_rank / D;
+    return (size_t)((double)base * r * r);
+}
+
 size_t tatrg_workspace_bytes_atrg(int D, int oversample) {
     const size_t base = tatrg_workspace_bytes(D, oversample);
     if (base == 0) return 0;
@@ -37,7 +45,7 @@ int tatrg_create(double beta, double h, int D, int oversample, uint64_t seed, vo
     if (workspace_bytes < tatrg_workspace_bytes(D, oversample)) return TATRG_ENOMEM;
     tatrg_ctx* c = new (std::nothrow) tatrg_ctx();
     if (!c) return TATRG_ENOMEM;
-    c->beta = beta; c->h = h; c->D = D; c->p = oversample; c->seed = seed; c->Ktri = D + oversample;
+    c->beta = beta; c->h = h; c->D = D; c->p = oversample; c->seed = seed; c->Ktri = D + oversample; c->Dbond = D;
     c->pool.reset(workspace, workspace_bytes);
     c->trace_dev = c->pool.alloc(kTraceDoubles);
     c->phi.nd = c->psi.nd = 5;
@@ -61,6 +69,14 @@ int tatrg_set_option(tatrg_handle c, int key, double value) {
         case TATRG_OPT_STAGE_TIMING: c->timing = (int)value; return TATRG_OK;
         case TATRG_OPT_KEEP_TENSORS: c->keep_tensors = value != 0; return TATRG_OK;
         case TATRG_OPT_SUBSPACE: c->use_subspace = value != 0; return TATRG_OK;
+        case TATRG_OPT_BOND_RANK: {
+            if (c->m > 0) return TATRG_ESTATE;
+            if (value != std::floor(value) || value < c->D) return TATRG_EINVAL;
+            const size_t need = tatrg_workspace_bytes_ilo(c->D, c->p, (int)value);
+            if (need == 0) return TATRG_EINVAL;
+            if (c->pool.capacity() < (need & ~(size_t)255)) return TATRG_ENOMEM;
+            c->Dbond = (int)value; return TATRG_OK;
+        }
         case TATRG_OPT_METHOD:
             if (c->m > 0) return TATRG_ESTATE;
             if (value != 0 && value != 1) return TATRG_EINVAL;

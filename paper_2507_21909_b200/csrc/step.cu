@@ -565,7 +565,7 @@ void Stepper::decompose(Tens& a, Tens& dt, Tens& core) {
     c.lnc.push_back(std::log(cm));
     for (double& v : sh) v /= cm;
     c.sv_s = sh;
-    const int chi = select_rank(sh, c.D, kEpsSV, c.tau);
+    const int chi = select_rank(sh, c.Dbond, kEpsSV, c.tau);          // fn 5 :203: alpha, beta carry the overspanned bond
     // rows of Va are the singular vectors on the side of X's rows, rows of Ut those on the side of its columns
     const Tens& urows = flip ? Ut : Va;    // [nv x r1]
     const Tens& vrows = flip ? Va : Ut;    // [nv x r2]
@@ -607,7 +607,7 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
     if (submark) submark();                                              // end of TATRG_ST_QR
     const int64_t npb = QB.d[1], npc = QC.d[1];
     Tens RB3 = view(RB, {npb, d1, chi}), RC3 = view(RC, {npc, d1, chi});
-    const int64_t l = std::min<int64_t>(c.D + c.p, std::min(chi * npc, chi * npb));     // R3: sketch width
+    const int64_t l = std::min<int64_t>(c.Dbond + c.p, std::min(chi * npc, chi * npb));     // R3: sketch width (fn 9 :381)
     // Omega drawn in the physical basis (be, j', m) and projected on Q^B  (R11, R12)
     Tens omega;
     {
@@ -658,7 +658,7 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
         if (rc != TATRG_OK) fail(rc, "%s", e.c_str());
     }
     if (!(sh[0] > 0)) fail(TATRG_ENUMERIC, "bond swap: zero spectrum");
-    gr = select_rank(sh, c.D, kEpsSV, c.tau);
+    gr = select_rank(sh, c.Dbond, kEpsSV, c.tau);                     // Eq. A.1 :337: gamma runs to r_bond D
     c.sv_sigma.assign((size_t)rk, 0.0);
     for (int i = 0; i < ry; ++i) c.sv_sigma[i] = sh[i] / sh[0];
     // Eq. A.9 :379 and A.10-A.11 :389-392

@@ -21,6 +21,7 @@ struct tatrg_ctx {
     int D = 0, p = 0;
     uint64_t seed = 0;
     int n_pow = 2, Ktri = 0;
+    int Dbond = 0;                   // ILO Triad-ATRG (section 2.3): rank r_bond D of the bond swap and of the decomposition; = D otherwise
     int method = 0;                  // 0: Triad-ATRG, 1: plain ATRG
     bool use_subspace = true;        // leading subspaces by subspace iteration (false: full eigen-decompositions everywhere)
     double tau = tatrg::kTauDefault;

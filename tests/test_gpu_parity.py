@@ -320,3 +320,47 @@ def test_plain_atrg_method_matches_untriaded_oracle(D, p, n_pow, steps):
             tt.step()
             ta.step()
         assert abs(tt.lnZ_per_site() - ta.lnZ_per_site()) > 1e-8
+
+
+@pytest.mark.parametrize("D,bond_rank,p,n_pow,steps", [(3, 6, 3, 2, 8), (4, 8, 4, 1, 8), (4, 12, 4, 2, 6), (6, 9, 6, 2, 6)])
+def test_ilo_triad_atrg_matches_oracle(D, bond_rank, p, n_pow, steps):
+    """SURVEY A10 / PAPER.md section 2.3 :183-209, App. A: ILO Triad-ATRG -- the bond swap keeps r_bond D values (Eq. A.1 :337), the
+    next decomposition keeps the whole overspanned bond (fn 5 :203), the squeezed legs stay at D -- against the oracle run with
+    the same bond_rank; and the state has the shape fn 5 states."""
+    from oracle import tatrg_oracle as O
+    beta, seed = 0.1497, 17
+    t = T.Tatrg(beta, 0.0, D, p, seed, power_iters=n_pow, bond_rank=bond_rank)
+    t.set_option(T.OPT_KEEP_TENSORS, 1)
+    o = O.TatrgOracle(beta, 0.0, D, p, seed, n_pow=n_pow, bond_rank=bond_rank)
+    for m in range(steps):
+        t.step()
+        o.step()
+        lo = o.lnZ_per_site()
+        assert abs(t.lnZ_per_site() - lo) <= TOL_LNZ * abs(lo), m
+        for which, key in ((T.SV_SIGMA, "sigma"), (T.SV_S, "s")):
+            got, ref = t.singular_values(which, bond_rank), o.last[key][:bond_rank]
+            k = min(len(got), len(ref))
+            assert np.abs(got[:k] - ref[:k]).max() <= TOL_SV, (m, key)
+    assert t.get_tensor("phi").shape == o.phi.shape == (D, D, D, D, bond_rank)
+    assert t.get_tensor("X").shape == (bond_rank, D, D, D, bond_rank)
+
+
+def test_ilo_at_d16_runs_and_differs_from_plain():
+    """r_bond = 2 at D = 16 (bond rank 32, sketch 48 wide): properties at a size the oracle cannot reach in seconds -- workspace
+    bound, isometries, ordered spectrum of 32 values -- and a free energy that differs from (and, near T_c, lies above) r_bond = 1."""
+    D, p = 16, 16
+    ti = T.Tatrg(0.1497, 0.0, D, p, 7, bond_rank=32)
+    ti.set_option(T.OPT_KEEP_TENSORS, 1)
+    tp = T.Tatrg(0.1497, 0.0, D, p, 7)
+    for _ in range(12):
+        ti.step()
+        tp.step()
+    assert ti.workspace_peak() <= T.lib().tatrg_workspace_bytes_ilo(D, p, 32)
+    x = ti.get_tensor("X")
+    assert x.shape == (32, D, D, D, 32)
+    xm = x.reshape(-1, 32)
+    assert np.abs(xm.T @ xm - np.eye(32)).max() <= 1e-10
+    sig = ti.singular_values(T.SV_SIGMA, 32)
+    assert len(sig) == 32 and np.all(np.diff(sig) <= 0) and sig[-1] > 0
+    zi, zp = ti.lnZ_per_site(), tp.lnZ_per_site()
+    assert np.isfinite(zi) and 1e-7 < zi - zp < 5e-3
