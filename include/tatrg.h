@@ -156,6 +156,13 @@ int tatrg_eigh(void* cuda_stream, int n, double* G, double* lam, double* Vt, voi
 size_t tatrg_svd_work_bytes(int nv, int len);
 int tatrg_svd(void* cuda_stream, int nv, int len, const double* X, double* s, double* Ut, double* Vacc, void* work);
 
+/* Gram matrix G [dev] n x n (row-major, ld n) = X^T X of X [dev] m x n (row-major, ld n): the DGEMM in its symmetric mode -- only
+ * the tiles on and below the diagonal are computed (split along K into partial products when the grid would not fill the SMs),
+ * the upper triangle is mirrored.  This is how the Gram matrices of Eq. A.2-A.3 and Eq. 2.9 are formed.
+ * scratch [dev] >= tatrg_gram_scratch_bytes(m, n) (may be NULL when that is 0). */
+size_t tatrg_gram_scratch_bytes(long long m, int n);
+int tatrg_gram(void* cuda_stream, long long m, int n, const double* X, double* G, void* scratch);
+
 /* Cholesky QR of a tall matrix (the orthonormalisation of the QR pre-reduction, Eq. A.2-A.3 :345-348, of the RSVD
  * sketches, Eq. A.4-A.6 :352-369, and of the subspace iterations behind Eq. 2.9 :135 and the squeezers :171):
  * X [dev] m x n row-major (m >= n; DESTROYED), Q [dev] m x n with orthonormal columns up to cond(X)^2 eps (one pass),

@@ -63,6 +63,8 @@ _SIGNATURES = {
     "tatrg_svd_work_bytes": (_c.c_size_t, [_c.c_int, _c.c_int]),
     "tatrg_svd": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_void_p,
                              _c.c_void_p]),
+    "tatrg_gram_scratch_bytes": (_c.c_size_t, [_c.c_longlong, _c.c_int]),
+    "tatrg_gram": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
     "tatrg_cholqr_work_bytes": (_c.c_size_t, [_c.c_int]),
     "tatrg_cholqr": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
     "tatrg_dot": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
@@ -337,6 +339,18 @@ def svd_rows(X):
     work = torch.empty(lib().tatrg_svd_work_bytes(nv, ln), dtype=torch.uint8, device=X.device)
     _check(lib().tatrg_svd(_stream_ptr(), nv, ln, _p(x), _p(s), _p(ut), _p(va), _p(work)), "tatrg_svd")
     return s, ut, va
+
+
+def gram(X):
+    """X^T X (torch CUDA float64, m x n) through the symmetric mode of the DGEMM (lower tiles + mirror)."""
+    torch = _torch_cuda()
+    m, n = X.shape
+    x = X.contiguous()
+    g = torch.empty((n, n), dtype=torch.float64, device=X.device)
+    nb = lib().tatrg_gram_scratch_bytes(m, n)
+    scratch = torch.empty(max(nb, 8), dtype=torch.uint8, device=X.device)
+    _check(lib().tatrg_gram(_stream_ptr(), m, n, _p(x), _p(g), _p(scratch)), "tatrg_gram")
+    return g
 
 
 def cholqr(X):

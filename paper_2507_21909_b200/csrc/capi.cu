@@ -261,6 +261,15 @@ int tatrg_svd(void* st, int nv, int len, const double* X, double* s, double* Ut,
     std::string err;
     try { return svd_rows((cudaStream_t)st, nv, len, X, s, Ut, Vacc, work, nullptr, &err); } catch (...) { return TATRG_ECUDA; }
 }
+size_t tatrg_gram_scratch_bytes(long long m, int n) { return (m > 0 && n > 0) ? 8 * (size_t)dgemm_splitk_doubles(n, n, m, n >= 256) : 0; }
+int tatrg_gram(void* stp, long long m, int n, const double* X, double* G, void* scratch) {
+    if (m < 1 || n < 1 || !X || !G) return TATRG_EINVAL;
+    cudaStream_t st = (cudaStream_t)stp;
+    const bool lower = n >= 256;
+    cudaError_t e = dgemm_splitk(st, true, false, n, n, m, 1.0, X, n, X, n, G, n, (double*)scratch, lower);
+    if (e == cudaSuccess && lower) e = mirror_lower(st, n, G);
+    return e == cudaSuccess ? TATRG_OK : TATRG_ECUDA;
+}
 size_t tatrg_cholqr_work_bytes(int n) { return n > 0 ? 8 * (2 * (size_t)n * n + cholesky_work_doubles(n)) + 4096 : 0; }
 int tatrg_cholqr(void* stp, long long m, int n, double* X, double* Q, double* R, void* work) {
     if (m < n || n < 1 || !X || !Q || !R || !work) return TATRG_EINVAL;

@@ -204,3 +204,14 @@ def test_cholqr_reports_rank_deficiency(torch):
     x[:, 17] = x[:, 3] - 2.0 * x[:, 5]
     with pytest.raises(T.TatrgError):
         T.cholqr(dev(torch, x))
+
+
+@pytest.mark.parametrize("m,n", [(5, 3), (1000, 64), (4096, 256), (33000, 300), (2048, 1024), (777, 513)])
+def test_gram_symmetric_mode_matches_definition(torch, m, n):
+    """X^T X with only the lower tiles computed (n >= 256), split along K, mirrored: against the definition, and exactly symmetric."""
+    x = inputs.random_tensor((m, n), 5)
+    g = T.gram(dev(torch, x)).cpu().numpy()
+    ref = x.T @ x
+    assert np.abs(g - ref).max() <= 8 * EPS * m * np.abs(x).max() ** 2
+    if n >= 256:
+        assert np.array_equal(g, g.T)
