@@ -427,7 +427,7 @@ struct Stepper {
     // scaling) tolerates several applications of A per orthonormalisation, as long as the dynamic range of the block,
     // (r_1 / r_b)^deg, stays below 1e11.
     void sub_iterate(std::vector<SubProb>& ps) {
-        constexpr int q0 = 6, qmax = 96;
+        constexpr int q0 = 4, qmax = 96;
         constexpr double kShift = 1e-13;
         static const bool verbose = getenv("TATRG_SUB_VERBOSE") != nullptr;   // debugging aid only
         SubStreams& ss = sub_streams();
@@ -478,7 +478,8 @@ struct Stepper {
         };
         for (int pass = 0; pass < 3; ++pass) {
             bool more = false;
-            for (SubProb& s : ps) if (s.ok) { estimate(s); if (s.ok && s.target > s.done) more = true; }
+            // a re-estimate within 1 of the count already done is the noise of the estimator (+-10 % in rho), not missing work
+            for (SubProb& s : ps) if (s.ok) { estimate(s); if (s.ok && s.target > s.done + (pass > 0 ? 1 : 0)) more = true; else if (s.ok) s.target = std::min(s.target, s.done); }
             if (!more) break;
             for (SubProb& s : ps) {
                 if (!s.ok || s.target <= s.done) continue;
