@@ -73,6 +73,10 @@ int tatrg_set_option(tatrg_handle, int key, double value);
  * by RSVD (Eq. 2.5, App. A), triad isometries and tensors (Eq. 2.9-2.17), squeezers (:171), contraction
  * (Eq. 2.18-2.19), axis rotation and normalisation.  Work is enqueued on cuda_stream (a cudaStream_t; NULL =
  * default stream); small spectra are read back inside the call to take the rank decisions.
+ * The independent solver chains of a stage (subspace iterations, block-Jacobi rounds) run on up to five auxiliary
+ * non-blocking streams that the library creates once per device; they are forked from and joined to cuda_stream by
+ * events, so that all work of the step is ordered after what was enqueued on cuda_stream before the call and before
+ * what is enqueued on it afterwards.  Handles on the same device must not be stepped from several host threads at once.
  * Errors: ECUDA, ENUMERIC (non-finite or non-positive normalisation), ENOMEM, ESTATE (after an earlier failure). */
 int tatrg_step(tatrg_handle, void* cuda_stream);
 

@@ -15,6 +15,8 @@
 #include <algorithm>
 #include <cmath>
 #include <numeric>
+#include <map>
+#include <mutex>
 #include <cstdio>
 #include <cstdlib>
 
@@ -590,12 +592,18 @@ static int finish_one(cudaStream_t st, int n, int N, double* lam_u, int* idx, do
 }
 
 // auxiliary stream + events of the two-stream round pipeline (created once per process, never destroyed)
-struct Aux { cudaStream_t st = nullptr; cudaEvent_t evS[2], evA[2], ev0; bool ok = false; };
+struct Aux { cudaStream_t st = nullptr; cudaEvent_t evS[2], evA[2], ev0; bool ok = false; bool tried = false; };
+// one set per device (streams belong to the device that was current when they were created); calls on the same device
+// from several host threads at once are not supported
 static Aux& aux() {
-    static Aux a;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
+    static std::map<int, Aux> per_device;
+    static std::mutex mu;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    std::lock_guard<std::mutex> lock(mu);
+    Aux& a = per_device[dev];
+    if (!a.tried) {
+        a.tried = true;
         int lo = 0, hi = 0;
         cudaDeviceGetStreamPriorityRange(&lo, &hi);          // hi = greatest priority (numerically lowest)
         bool ok = cudaStreamCreateWithPriority(&a.st, cudaStreamNonBlocking, hi) == cudaSuccess;

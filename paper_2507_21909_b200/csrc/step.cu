@@ -16,6 +16,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <functional>
+#include <mutex>
 #include <chrono>
 
 namespace tatrg {
@@ -359,11 +360,16 @@ struct Stepper {
     }
     // The problems of a stage are independent chains of small launches: each runs on a stream of its own (created once
     // per process), forked from and joined to the caller's stream by events, so that their kernels overlap on the device.
-    struct SubStreams { cudaStream_t s[4]; cudaEvent_t fork, join[4]; bool ok = false; };
-    static SubStreams& sub_streams() {
-        static SubStreams ss; static bool tried = false;
-        if (!tried) {
-            tried = true;
+    struct SubStreams { cudaStream_t s[4]; cudaEvent_t fork, join[4]; bool ok = false; bool tried = false; };
+    static SubStreams& sub_streams() {      // one set per device; not for concurrent use from several host threads
+        static std::map<int, SubStreams> per_device;
+        static std::mutex mu;
+        int dev = 0;
+        cudaGetDevice(&dev);
+        std::lock_guard<std::mutex> lock(mu);
+        SubStreams& ss = per_device[dev];
+        if (!ss.tried) {
+            ss.tried = true;
             bool ok = cudaEventCreateWithFlags(&ss.fork, cudaEventDisableTiming) == cudaSuccess;
             for (int i = 0; i < 4 && ok; ++i)
                 ok = cudaStreamCreateWithFlags(&ss.s[i], cudaStreamNonBlocking) == cudaSuccess && cudaEventCreateWithFlags(&ss.join[i], cudaEventDisableTiming) == cudaSuccess;
