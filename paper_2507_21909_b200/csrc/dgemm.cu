@@ -31,17 +31,25 @@ struct Cfg {
     static constexpr int PITCH_KC = BK + 4;   // operand stored [row][k]: = 4 (mod 16) doubles
     static constexpr int NT = 32 * WM * WN;
     static constexpr int MI = BM / WM / 8, NI = BN / WN / 8;          // atoms per warp
-    static constexpr int ROWS = BM > BN ? BM : BN;
-    static constexpr int TILE_D = ROWS * PITCH_KC > BK * (ROWS + 4) ? ROWS * PITCH_KC : BK * (ROWS + 4);
-    static constexpr int SMEM = STAGES * 2 * TILE_D * 8;
+    // an operand tile holds ROWS x BK doubles in either storage order
+    static constexpr int tile_doubles(int rows) { return rows * PITCH_KC > BK * (rows + 4) ? rows * PITCH_KC : BK * (rows + 4); }
+    static constexpr int TILE_A = tile_doubles(BM), TILE_B = tile_doubles(BN);
+    static constexpr int SMEM = STAGES * (TILE_A + TILE_B) * 8;
 };
 using CfgL = Cfg<128, 128, 2, 4, 16, 4>;     // BK = 32 with 3 stages (221 KB) measured no faster
 using CfgS = Cfg<64, 64, 2, 2, 16, 4>;
+using CfgT = Cfg<128, 32, 4, 1, 16, 4>;      // tall and skinny: C = A G with G = D x D (M = D^4): HBM-bound, no padded DMMAs along N
+using CfgU = Cfg<32, 32, 2, 2, 16, 4>;       // 32 x 32 outputs (Gram matrices of D^4 x D operands, batched over K-chunks)
+enum { CFG_AUTO = -1, CFG_L = 0, CFG_S = 1, CFG_T = 2, CFG_U = 3 };
 
 __device__ __forceinline__ void cp16(double* dst, const double* src, bool ok) {
     unsigned d = (unsigned)__cvta_generic_to_shared(dst);
     int n = ok ? 16 : 0;
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(d), "l"(src), "r"(n));
+}
+__device__ __forceinline__ void cp16u(double* dst, const double* src) {      // unpredicated
+    unsigned d = (unsigned)__cvta_generic_to_shared(dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(src));
 }
 __device__ __forceinline__ void cp8(double* dst, const double* src, bool ok) {
     unsigned d = (unsigned)__cvta_generic_to_shared(dst);
@@ -111,29 +119,37 @@ struct TileLoader {
     static constexpr int ITERS = ROWS * BK / 2 / NT;
     static constexpr int HALF = ROWS / 2, CPR = BK / 2;
     static constexpr int PITCH_MC = ROWS + 4, PITCH_KC = BK + 4;
-    const double* p0; const double* safe;
+    const double* pk; const double* safe;
     int64_t step_it, step_k;
-    unsigned mask;
+    unsigned mask; bool full;
     int kofs0, kofs_it, soff0, soff_it;
     __device__ __forceinline__ void init(const double* __restrict__ g, int64_t ld, int64_t r0, int64_t rows, int tid) {
         safe = g;
         if (KC) {
             const int r = tid / CPR, kc = (tid % CPR) * 2;
-            p0 = g + (r0 + r) * ld + kc; step_it = (int64_t)(NT / CPR) * ld; step_k = BK;
+            pk = g + (r0 + r) * ld + kc; step_it = (int64_t)(NT / CPR) * ld; step_k = BK;
             mask = 0;
 #pragma unroll
             for (int it = 0; it < ITERS; ++it) if (r0 + r + it * (NT / CPR) < rows) mask |= 1u << it;
             kofs0 = kc; kofs_it = 0; soff0 = r * PITCH_KC + kc; soff_it = (NT / CPR) * PITCH_KC;
         } else {
             const int k = tid / HALF, rc = (tid % HALF) * 2;
-            p0 = g + (int64_t)k * ld + r0 + rc; step_it = (int64_t)(NT / HALF) * ld; step_k = (int64_t)BK * ld;
+            pk = g + (int64_t)k * ld + r0 + rc; step_it = (int64_t)(NT / HALF) * ld; step_k = (int64_t)BK * ld;
             mask = (r0 + rc < rows) ? 0xffffffffu : 0u;
             kofs0 = k; kofs_it = NT / HALF; soff0 = k * PITCH_MC + rc; soff_it = (NT / HALF) * PITCH_MC;
         }
+        full = r0 + ROWS <= rows;       // CTA-uniform
     }
-    // tile kt (k origin kt*BK) -> stage buffer s
-    __device__ __forceinline__ void issue(double* s, int kt, int64_t K) const {
-        const double* p = p0 + (int64_t)kt * step_k;
+    // tile kt (k origin kt*BK) -> stage buffer s.  Tiles are issued in order kt = 0, 1, 2, ...: `pk` runs along.
+    // A tile that lies inside the matrix in both directions takes the unpredicated path: per chunk one 64-bit add and one cp.async.
+    __device__ __forceinline__ void issue(double* s, int kt, int64_t K) {
+        const double* p = pk;
+        pk += step_k;
+        if (full && (int64_t)(kt + 1) * BK <= K) {
+#pragma unroll
+            for (int it = 0; it < ITERS; ++it) { cp16u(s + soff0 + it * soff_it, p); p += step_it; }
+            return;
+        }
         const int64_t krem = K - (int64_t)kt * BK - kofs0;      // chunk it is inside K iff it*kofs_it < krem
 #pragma unroll
         for (int it = 0; it < ITERS; ++it) {
@@ -148,7 +164,7 @@ __global__ void __launch_bounds__(C_::NT, C_::NT == 256 ? 1 : 2)
 dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, const double* __restrict__ A, int64_t lda,
              const double* __restrict__ B, int64_t ldb, double beta, double* __restrict__ C, int64_t ldc, int64_t sA,
              int64_t sB, int64_t sC, int tiles_m, int lower_only) {
-    constexpr int BM = C_::BM, BN = C_::BN, NT = C_::NT, MI = C_::MI, NI = C_::NI, TILE_D = C_::TILE_D;
+    constexpr int BM = C_::BM, BN = C_::BN, NT = C_::NT, MI = C_::MI, NI = C_::NI, TILE_A = C_::TILE_A, TILE_S = C_::TILE_A + C_::TILE_B;
     constexpr int BK = C_::BK, STAGES = C_::STAGES, PITCH_KC = C_::PITCH_KC;
     constexpr int PA = BM + 4, PB = BN + 4;
     extern __shared__ __align__(16) double smem[];
@@ -173,9 +189,9 @@ dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, co
     if (AV16) ldA.init(A, lda, m0, M, tid);
     if (BV16) ldB.init(B, ldb, n0, N, tid);
     auto load_stage = [&](int kt) {
-        double* sa = smem + (2 * (kt % STAGES)) * TILE_D;
+        double* sa = smem + (kt % STAGES) * TILE_S;
         if (AV16) ldA.issue(sa, kt, K); else load_tile<A_KC, false, BM, NT, BK>(sa, A, lda, m0, (int64_t)kt * BK, M, K, tid);
-        if (BV16) ldB.issue(sa + TILE_D, kt, K); else load_tile<B_KC, false, BN, NT, BK>(sa + TILE_D, B, ldb, n0, (int64_t)kt * BK, N, K, tid);
+        if (BV16) ldB.issue(sa + TILE_A, kt, K); else load_tile<B_KC, false, BN, NT, BK>(sa + TILE_A, B, ldb, n0, (int64_t)kt * BK, N, K, tid);
     };
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
@@ -190,8 +206,8 @@ dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, co
             if (nxt < nk) load_stage(nxt);
             cp_commit();
         }
-        const double* As = smem + (2 * (kt % STAGES)) * TILE_D;
-        const double* Bs = As + TILE_D;
+        const double* As = smem + (kt % STAGES) * TILE_S;
+        const double* Bs = As + TILE_A;
         // fragments of the next 4-deep slice are loaded while the DMMAs of the current one issue (register double buffer)
         double a[2][MI], b[2][NI];
         auto load_frag = [&](int ks, double (&af)[MI], double (&bf)[NI]) {
@@ -243,7 +259,7 @@ dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, co
 
 struct Args {
     cudaStream_t st; int64_t M, N, K, Klast; double alpha; const double* A; int64_t lda; const double* B; int64_t ldb; double beta;
-    double* C; int64_t ldc; int batch; int64_t sA, sB, sC; bool force_small = false; bool lower_only = false;
+    double* C; int64_t ldc; int batch; int64_t sA, sB, sC; int force_cfg = CFG_AUTO; bool lower_only = false;
 };
 
 template <class C_, bool A_KC, bool B_KC, bool AV, bool BV>
@@ -275,12 +291,23 @@ cudaError_t pick_order(bool a_kc, bool b_kc, bool av, bool bv, const Args& a) {
     if (!a_kc && b_kc) return pick_vec<C_, false, true>(av, bv, a);
     return pick_vec<C_, false, false>(av, bv, a);
 }
-// S for skinny outputs, and for launches whose L tiles would cover at most a quarter of the 148 SMs (the small products of
-// the subspace iterations): there the number of CTAs in flight matters more than the reuse inside one tile.
-inline bool small_cfg(int64_t M, int64_t N, int64_t batch = 1) {
-    if ((M < N ? M : N) <= 64) return true;
+// U for outputs of at most 32 x 32, T for N <= 32 below a tall M, S for the other skinny outputs and for launches whose L tiles
+// would cover at most a quarter of the 148 SMs (the small products of the subspace iterations: there the number of CTAs in
+// flight matters more than the reuse inside one tile), L otherwise.
+inline int pick_cfg(int64_t M, int64_t N, int64_t batch = 1) {
+    if (M <= 32 && N <= 32) return CFG_U;
+    if (N <= 32 && M >= 128) return CFG_T;
+    if ((M < N ? M : N) <= 64) return CFG_S;
     const int64_t tl = ((M + CfgL::BM - 1) / CfgL::BM) * ((N + CfgL::BN - 1) / CfgL::BN);
-    return tl * batch <= 37;
+    return tl * batch <= 37 ? CFG_S : CFG_L;
+}
+inline void cfg_dims(int cfg, int& bm, int& bn, int& per_sm) {
+    switch (cfg) {
+        case CFG_L: bm = CfgL::BM; bn = CfgL::BN; per_sm = 1; break;
+        case CFG_S: bm = CfgS::BM; bn = CfgS::BN; per_sm = 2; break;
+        case CFG_T: bm = CfgT::BM; bn = CfgT::BN; per_sm = 2; break;
+        default: bm = CfgU::BM; bn = CfgU::BN; per_sm = 4; break;
+    }
 }
 
 cudaError_t dgemm_raw(bool transa, bool transb, const Args& a) {
@@ -293,14 +320,18 @@ cudaError_t dgemm_raw(bool transa, bool transb, const Args& a) {
     };
     const bool kodd = (a.K % 2 != 0) || (a.Klast % 2 != 0);
     const bool av = v16(a.A, a.lda, a_kc ? (kodd ? 1 : 2) : a.M, a.sA), bv = v16(a.B, a.ldb, b_kc ? (kodd ? 1 : 2) : a.N, a.sB);
-    if (a.force_small || small_cfg(a.M, a.N, a.batch)) return pick_order<CfgS>(a_kc, b_kc, av, bv, a);
-    return pick_order<CfgL>(a_kc, b_kc, av, bv, a);
+    switch (a.force_cfg != CFG_AUTO ? a.force_cfg : pick_cfg(a.M, a.N, a.batch)) {
+        case CFG_L: return pick_order<CfgL>(a_kc, b_kc, av, bv, a);
+        case CFG_S: return pick_order<CfgS>(a_kc, b_kc, av, bv, a);
+        case CFG_T: return pick_order<CfgT>(a_kc, b_kc, av, bv, a);
+        default: return pick_order<CfgU>(a_kc, b_kc, av, bv, a);
+    }
 }
 }  // namespace
 
 static cudaError_t dgemm_klast(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, int64_t Klast, double alpha,
                                const double* A, int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc, int batch,
-                               int64_t sA, int64_t sB, int64_t sC, bool force_small = false, bool lower_only = false) {
+                               int64_t sA, int64_t sB, int64_t sC, int force_cfg = CFG_AUTO, bool lower_only = false) {
     if (M <= 0 || N <= 0 || batch <= 0) return cudaSuccess;
     Counters* c = g_counter;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -308,8 +339,9 @@ static cudaError_t dgemm_klast(cudaStream_t st, bool transa, bool transb, int64_
     // lower_only: only the tiles on and below the diagonal are computed (counted as such)
     double mn = (double)M * (double)N;
     if (lower_only) {
-        const bool sm = force_small || small_cfg(M, N, batch);
-        const int64_t bm = sm ? CfgS::BM : CfgL::BM, bn = sm ? CfgS::BN : CfgL::BN;
+        int bm_, bn_, psm_;
+        cfg_dims(force_cfg != CFG_AUTO ? force_cfg : pick_cfg(M, N, batch), bm_, bn_, psm_);
+        const int64_t bm = bm_, bn = bn_;
         mn = 0;
         for (int64_t m0 = 0; m0 < M; m0 += bm)
             for (int64_t n0 = 0; n0 < N && n0 < m0 + bm; n0 += bn) mn += (double)std::min(bm, M - m0) * (double)std::min(bn, N - n0);
@@ -321,7 +353,7 @@ static cudaError_t dgemm_klast(cudaStream_t st, bool transa, bool transb, int64_
     for (int b0 = 0; b0 < batch && e == cudaSuccess; b0 += 32768) {
         int nb = batch - b0 < 32768 ? batch - b0 : 32768;
         Args a{st, M, N, K, (b0 + nb == batch) ? Klast : 0, alpha, A + (int64_t)b0 * sA, lda, B + (int64_t)b0 * sB, ldb, beta,
-               C + (int64_t)b0 * sC, ldc, nb, sA, sB, sC, force_small, lower_only};
+               C + (int64_t)b0 * sC, ldc, nb, sA, sB, sC, force_cfg, lower_only};
         e = dgemm_raw(transa, transb, a);
     }
     if (e0) { cudaEventRecord(e1, st); c->gemm_ev.push_back({e0, e1}); c->gemm_shapes.push_back({M, N, (int64_t)(kk / batch), batch, transa, transb, mn / ((double)M * (double)N)}); }
@@ -339,9 +371,8 @@ namespace {
 // Number of K-chunks for a non-batched GEMM: the smallest split whose CTA count fills whole waves of the 148 SMs
 // (>= 93 % of the last wave used), chunks of >= 256, partials capped at 64 M doubles.  1 = no split.
 int splitk_count(int64_t M, int64_t N, int64_t K, bool lower_only = false) {
-    const bool sm = small_cfg(M, N);
-    const int bm = sm ? CfgS::BM : CfgL::BM, bn = sm ? CfgS::BN : CfgL::BN;
-    const int per_sm = sm ? 2 : 1;
+    int bm, bn, per_sm;
+    cfg_dims(pick_cfg(M, N), bm, bn, per_sm);
     int64_t tiles = ((M + bm - 1) / bm) * ((N + bn - 1) / bn);
     if (lower_only) {      // only the tiles on and below the diagonal do work
         tiles = 0;
@@ -409,14 +440,14 @@ int64_t dgemm_splitk_doubles(int64_t M, int64_t N, int64_t K, bool lower_only) {
 cudaError_t dgemm_splitk(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                          int64_t lda, const double* B, int64_t ldb, double* C, int64_t ldc, double* part, bool lower_only) {
     int ns = splitk_count(M, N, K, lower_only);
-    if (ns <= 1 || part == nullptr) return dgemm_klast(st, transa, transb, M, N, K, 0, alpha, A, lda, B, ldb, 0.0, C, ldc, 1, 0, 0, 0, false, lower_only);
+    if (ns <= 1 || part == nullptr) return dgemm_klast(st, transa, transb, M, N, K, 0, alpha, A, lda, B, ldb, 0.0, C, ldc, 1, 0, 0, 0, CFG_AUTO, lower_only);
     // chunk: multiple of BK; the last batch entry takes the ragged tail (klast)
     int64_t chunk = ((K + ns - 1) / ns + kChunkAlign - 1) / kChunkAlign * kChunkAlign;
     int nchunks = (int)((K + chunk - 1) / chunk);
     int64_t tail = K - (int64_t)(nchunks - 1) * chunk;
     const int64_t stepA = transa ? chunk * lda : chunk, stepB = transb ? chunk : chunk * ldb;
     cudaError_t e = dgemm_klast(st, transa, transb, M, N, chunk, tail == chunk ? 0 : tail, 1.0, A, lda, B, ldb, 0.0, part, N, nchunks,
-                                stepA, stepB, M * N, small_cfg(M, N), lower_only);
+                                stepA, stepB, M * N, pick_cfg(M, N), lower_only);
     if (e != cudaSuccess) return e;
     int64_t MN = M * N;
     if (nchunks >= 16 && MN <= (1 << 18)) {
