@@ -274,16 +274,63 @@ struct Stepper {
         return true;
     }
 
+    // orth_chol() (one pass) of two matrices of the same shape: the two Gram matrices on the caller's stream, then the two
+    // factorisation + inversion chains (latency-bound: ~60 small launches each) side by side on two auxiliary streams, then
+    // the decisions and the two Q = mat L^-T products.  All buffers are allocated before the fork; nothing is allocated or
+    // freed while the chains are in flight.  Returns false (nothing kept) unless both operands prove full rank.
+    bool orth_chol_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2]) {
+        SubStreams& ss = sub_streams();
+        if (!ss.ok) {
+            const bool ok0 = orth_chol(m0, Q[0], R[0]), ok1 = orth_chol(m1, Q[1], R[1]);
+            if (ok0 && ok1) return true;
+            if (ok0) drop(Q[0]), drop(R[0]);
+            if (ok1) drop(Q[1]), drop(R[1]);
+            return false;
+        }
+        Scope sc(*this);
+        const int64_t m = m0.d[0], n = m0.d[1];
+        const Tens* mats[2] = {&m0, &m1};
+        Tens G[2], L[2], X[2], T[2]; double* cw[2]; double* res[2];
+        for (int i = 0; i < 2; ++i) {
+            G[i] = mm(true, false, n, n, m, mats[i]->p, n, mats[i]->p, n, true);
+            L[i] = make({n, n}); X[i] = make({n, n}); T[i] = make({(int64_t)tri_inverse_scratch_doubles((int)n)});
+            cw[i] = raw((int64_t)cholesky_work_doubles((int)n)); res[i] = raw(1 + 148 * 8 + 7);
+            ck(fill_zero(st, L[i].p, n * n), "zero"); ck(fill_zero(st, X[i].p, n * n), "zero");
+        }
+        ck(cudaEventRecord(ss.fork, st), "event");
+        for (int i = 0; i < 2; ++i) {
+            cudaStream_t a = ss.s[i];
+            ck(cudaStreamWaitEvent(a, ss.fork, 0), "wait");
+            ck(cholesky(a, (int)n, G[i].p, n, L[i].p, n, 0.0, 1e-14, cw[i]), "cholesky");
+            ck(tri_inverse(a, (int)n, L[i].p, n, cw[i], X[i].p, n, T[i].p), "tri_inverse");
+            ck(dot(a, n * n, X[i].p, X[i].p, res[i]), "dot");
+            ck(cudaEventRecord(ss.join[i], a), "event");
+            ck(cudaStreamWaitEvent(st, ss.join[i], 0), "wait");
+        }
+        bool ok = true;
+        for (int i = 0; i < 2; ++i) {
+            int info = 0;
+            ck(cudaMemcpyAsync(&info, cholesky_info(cw[i], (int)n), sizeof(int), cudaMemcpyDeviceToHost, st), "readback");
+            std::vector<double> d0 = to_host(cholesky_d0(cw[i], (int)n), n);
+            std::vector<double> xn = to_host(res[i], 1);
+            double tr = 0; for (double v : d0) tr += v;
+            if (getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg cholesky qr %lld x %lld] info %d, proven lam_min/lam_max >= %.3e\n", (long long)m, (long long)n, info, 1.0 / (xn[0] * tr));
+            if (info != 0 || !std::isfinite(xn[0]) || !(xn[0] > 0) || !(tr > 0) || !(1.0 / (xn[0] * tr) > kEpsOrthLambda)) ok = false;
+        }
+        if (!ok) return false;
+        for (int i = 0; i < 2; ++i) {
+            Q[i] = mm(false, true, m, n, n, mats[i]->p, n, X[i].p, n);
+            R[i] = perm(view(L[i], {n, n}), {1, 0});
+            keep(Q[i]); keep(R[i]);
+        }
+        return true;
+    }
+
     // orth() of two matrices of the same shape with n > 128 (single pass): the two Gram matrices are decomposed together
     void orth_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2]) {
         const int64_t m = m0.d[0], n = m0.d[1];
         if (n <= 128 || m1.d[0] != m || m1.d[1] != n) { orth(m0, Q[0], R[0]); orth(m1, Q[1], R[1]); return; }
-        if (c.use_subspace) {
-            const bool ok0 = orth_chol(m0, Q[0], R[0]), ok1 = orth_chol(m1, Q[1], R[1]);
-            if (ok0 && ok1) return;
-            if (ok0) drop(Q[0]), drop(R[0]);
-            if (ok1) drop(Q[1]), drop(R[1]);
-        }
+        if (c.use_subspace && orth_chol_pair(m0, m1, Q, R)) return;
         Scope sc(*this);
         const Tens* mats[2] = {&m0, &m1};
         Tens G[2];
