@@ -20,6 +20,10 @@ namespace tatrg {
 namespace {
 constexpr int PB = 64;        // panel width
 constexpr int PP = PB + 1;    // shared-memory pitch
+#ifndef TATRG_POTRF_CW
+#define TATRG_POTRF_CW 16
+#endif
+constexpr int kPotrfCW = TATRG_POTRF_CW;
 
 __global__ void symmetrize_kernel(int n, double* __restrict__ A) {
     const int64_t total = (int64_t)n * n;
@@ -61,27 +65,28 @@ __global__ void diag_shift_kernel(int n, double* __restrict__ A, int64_t lda, do
 // Factorisation, right-looking: step j publishes column j through shared memory (double-buffered: one barrier per step),
 // every thread scales it by 1/sqrt(pivot) and updates its 16 entries.  Inverse, also right-looking: once row k of
 // X = L^-1 is final, every row i > k accumulates l_ik x_k; row k+1 is finished by its own four threads.
-__global__ void __launch_bounds__(256, 1) potrf_block_kernel(int nb, int j0, const double* __restrict__ A, int64_t lda, double* __restrict__ L,
+template <int CW>      // columns per thread: 64 / CW column groups, 64 * (64 / CW) threads
+__global__ void __launch_bounds__(64 * (PB / CW), 1) potrf_block_kernel(int nb, int j0, const double* __restrict__ A, int64_t lda, double* __restrict__ L,
                                                              int64_t ldl, double* __restrict__ Linv, const double* __restrict__ d0,
                                                              double guard_rel, int* __restrict__ info) {
     __shared__ double col[2][PB];        // published column (factorisation) / row of X (inverse)
     __shared__ double Ls[PB * PP];       // the factor, for the inverse
     __shared__ double floor_s[PB];       // pivot floors (global loads kept out of the column loop)
-    const int tid = threadIdx.x, i = tid & 63, g = tid >> 6, c0 = g * 16;
+    const int tid = threadIdx.x, i = tid & 63, g = tid >> 6, c0 = g * CW;
     if (tid < PB) floor_s[tid] = fmax(guard_rel * (tid < nb ? fabs(d0[j0 + tid]) : 1.0), 1e-290);
-    double a[16];
+    double a[CW];
 #pragma unroll
-    for (int cc = 0; cc < 16; ++cc) {
+    for (int cc = 0; cc < CW; ++cc) {
         const int c = c0 + cc;
         a[cc] = (i < nb && c <= i) ? A[(int64_t)(j0 + i) * lda + j0 + c] : ((i == c) ? 1.0 : 0.0);   // identity padding beyond nb
     }
     int flag = 0;
     for (int j = 0; j < PB; ++j) {
-        const int gj = j >> 4, jj = j & 15, buf = j & 1;
+        const int gj = j / CW, jj = j % CW, buf = j & 1;
         if (g == gj) {
             double v = 0;
 #pragma unroll
-            for (int cc = 0; cc < 16; ++cc) if (cc == jj) v = a[cc];
+            for (int cc = 0; cc < CW; ++cc) if (cc == jj) v = a[cc];
             col[buf][i] = v;
         }
         __syncthreads();
@@ -91,7 +96,7 @@ __global__ void __launch_bounds__(256, 1) potrf_block_kernel(int nb, int j0, con
         if (p < floor_p) { flag |= 1; p = floor_p; }
         // warps whose rows all lie above the pivot row, or whose 16 columns all lie left of it, have nothing to update
         // (both conditions are warp-uniform): the serial chain of the 64 columns is issue-bound otherwise
-        if ((i | 31) < j || c0 + 15 < j) continue;
+        if ((i | 31) < j || c0 + CW - 1 < j) continue;
         // l_i l_c = (a_ij / p) a_cj: one DMUL per thread and one DFMA per entry instead of a DMUL + DFMA per entry (the
         // FP64 pipe is what the 64-column chain waits for)
         const double r = rsqrt(p);
@@ -99,7 +104,7 @@ __global__ void __launch_bounds__(256, 1) potrf_block_kernel(int nb, int j0, con
         const double lip = ci * (r * r);
         const double li = (i == j) ? p * r : ci * r;
 #pragma unroll
-        for (int cc = 0; cc < 16; ++cc) {
+        for (int cc = 0; cc < CW; ++cc) {
             const int c = c0 + cc;
             if (c > j) a[cc] -= lip * col[buf][c];
             else if (c == j) a[cc] = li;
@@ -108,7 +113,7 @@ __global__ void __launch_bounds__(256, 1) potrf_block_kernel(int nb, int j0, con
     if (flag && tid == 0) atomicOr(info, flag);
     // factor to shared memory and to L
 #pragma unroll
-    for (int cc = 0; cc < 16; ++cc) {
+    for (int cc = 0; cc < CW; ++cc) {
         const int c = c0 + cc;
         const double v = (c <= i) ? a[cc] : 0.0;
         Ls[i * PP + c] = v;
@@ -116,34 +121,34 @@ __global__ void __launch_bounds__(256, 1) potrf_block_kernel(int nb, int j0, con
     }
     __syncthreads();
     // X = L^-1: x[cc] accumulates sum_{k<i} l_ik x_kc for the thread's 16 columns
-    double x[16];
+    double x[CW];
 #pragma unroll
-    for (int cc = 0; cc < 16; ++cc) x[cc] = 0.0;
+    for (int cc = 0; cc < CW; ++cc) x[cc] = 0.0;
     const double rii = 1.0 / Ls[i * PP + i];
     if (i == 0) {
 #pragma unroll
-        for (int cc = 0; cc < 16; ++cc) { x[cc] = (c0 + cc == 0) ? rii : 0.0; }
+        for (int cc = 0; cc < CW; ++cc) { x[cc] = (c0 + cc == 0) ? rii : 0.0; }
     }
     __shared__ double xr[2][PB];
     for (int k = 0; k < PB; ++k) {
         const int buf = k & 1;
         if (i == k) {
 #pragma unroll
-            for (int cc = 0; cc < 16; ++cc) xr[buf][c0 + cc] = x[cc];      // row k of X is final
+            for (int cc = 0; cc < CW; ++cc) xr[buf][c0 + cc] = x[cc];      // row k of X is final
         }
         __syncthreads();
         if (i > k && c0 <= k + 1) {        // row k of X is zero right of column k: column groups beyond it only need the diagonal
             const double lik = Ls[i * PP + k];
 #pragma unroll
-            for (int cc = 0; cc < 16; ++cc) x[cc] += lik * xr[buf][c0 + cc];
+            for (int cc = 0; cc < CW; ++cc) x[cc] += lik * xr[buf][c0 + cc];
             if (i == k + 1) {       // finish row k+1: x_ic = (delta_ic - sum) / l_ii
 #pragma unroll
-                for (int cc = 0; cc < 16; ++cc) { const int c = c0 + cc; x[cc] = (c > i) ? 0.0 : (((c == i) ? 1.0 : 0.0) - x[cc]) * rii; }
+                for (int cc = 0; cc < CW; ++cc) { const int c = c0 + cc; x[cc] = (c > i) ? 0.0 : (((c == i) ? 1.0 : 0.0) - x[cc]) * rii; }
             }
         }
     }
 #pragma unroll
-    for (int cc = 0; cc < 16; ++cc) {
+    for (int cc = 0; cc < CW; ++cc) {
         const int c = c0 + cc;
         Linv[i * PB + c] = (i < nb && c < nb) ? x[cc] : 0.0;
     }
@@ -179,7 +184,7 @@ cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, 
     diag_shift_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, A, lda, shift, d0); count_launch();
     for (int p = 0; p < np; ++p) {
         const int j0 = p * PB, nb = n - j0 < PB ? n - j0 : PB, m = n - j0 - nb;
-        potrf_block_kernel<<<1, 256, 0, st>>>(nb, j0, A, lda, L, ldl, Linv + (size_t)p * PB * PB, d0, guard_rel, info); count_launch();
+        potrf_block_kernel<kPotrfCW><<<1, 64 * (PB / kPotrfCW), 0, st>>>(nb, j0, A, lda, L, ldl, Linv + (size_t)p * PB * PB, d0, guard_rel, info); count_launch();
         if (m <= 0) break;
         // panel below: L[i, j0:j0+nb] = A[i, j0:j0+nb] Linv^T
         e = dgemm(st, false, true, m, nb, nb, 1.0, A + (int64_t)(j0 + nb) * lda + j0, lda, Linv + (size_t)p * PB * PB, PB, 0.0,

@@ -373,30 +373,19 @@ struct Stepper {
     };
     static int sub_block(int n, int kmax) { int b = 2 * kmax; b = (b + 31) / 32 * 32; return b; }
     static bool sub_applicable(int n, int kmax) { return n > 128 && kmax >= 8 && sub_block(n, kmax) * 2 <= n; }
-    void capdbg(const char* where) {
-        static const bool on = getenv("TATRG_CAP_DEBUG") != nullptr;
-        if (!on) return;
-        cudaStreamCaptureStatus stt = cudaStreamCaptureStatusNone;
-        cudaError_t e = cudaStreamIsCapturing(st, &stt);
-        fprintf(stderr, "[capdbg] %s: status %d err %d\n", where, (int)stt, (int)e);
-    }
     void sub_orth(SubProb& s, int src, double shift) {      // buf[src] = [Z'; W'] -> buf[src^1] = [Z; W], which becomes the basis
         const int64_t rows = s.F ? 2 * (int64_t)s.n : s.n;
         double* X = s.buf[src].p;
         const double* Wp = s.F ? X + (int64_t)s.n * s.b : X;
         mm_into(s.Gm.p, s.b, true, false, s.b, s.b, s.n, X, s.b, Wp, s.b);
-        capdbg("gram");
         ck(cholesky(st, s.b, s.Gm.p, s.b, s.L.p, s.b, shift, 1e-14, s.cw), "cholesky");
-        capdbg("cholesky");
         ck(trsm_right_lt(st, rows, s.b, X, s.b, s.buf[src ^ 1].p, s.b, s.L.p, s.b, s.cw), "trsm");
-        capdbg("trsm");
         s.cur = src ^ 1;
     }
     void sub_apply(SubProb& s, int from) {         // buf[from^1] = [A Z; F A Z] with [Z; W] = buf[from]
         const double* X = s.F ? s.buf[from].p + (int64_t)s.n * s.b : s.buf[from].p;
         double* O = s.buf[from ^ 1].p;
         mm_into(O, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, X, s.b);
-        capdbg("apply");
         if (s.F) mm_into(O + (int64_t)s.n * s.b, s.b, false, false, s.n, s.b, s.n, s.F, s.n, O, s.b);
     }
     void sub_step(SubProb& s, int deg, double shift) {      // deg applications of A, then one orthonormalisation
