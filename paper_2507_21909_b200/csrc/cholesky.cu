@@ -24,6 +24,7 @@ constexpr int PP = PB + 1;    // shared-memory pitch
 #define TATRG_POTRF_CW 16
 #endif
 constexpr int kPotrfCW = TATRG_POTRF_CW;
+constexpr int kPotrfSmem = (2 * PB * PP + 32 * 33 + 4 * PB) * 8;
 
 __global__ void symmetrize_kernel(int n, double* __restrict__ A) {
     const int64_t total = (int64_t)n * n;
@@ -69,9 +70,13 @@ template <int CW>      // columns per thread: 64 / CW column groups, 64 * (64 / 
 __global__ void __launch_bounds__(64 * (PB / CW), 1) potrf_block_kernel(int nb, int j0, const double* __restrict__ A, int64_t lda, double* __restrict__ L,
                                                              int64_t ldl, double* __restrict__ Linv, const double* __restrict__ d0,
                                                              double guard_rel, int* __restrict__ info) {
-    __shared__ double col[2][PB];        // published column (factorisation) / row of X (inverse)
-    __shared__ double Ls[PB * PP];       // the factor, for the inverse
-    __shared__ double floor_s[PB];       // pivot floors (global loads kept out of the column loop)
+    extern __shared__ double sh_potrf[];
+    double* Ls = sh_potrf;                               // the factor, for the inverse
+    double* Xs = Ls + PB * PP;                           // the inverse
+    double* Ts = Xs + PB * PP;                           // 32 x 33 scratch of the doubling levels
+    double (*col)[PB] = reinterpret_cast<double (*)[PB]>(Ts + 32 * 33);     // published column, double-buffered
+    double* floor_s = &col[2][0];                        // pivot floors (global loads kept out of the column loop)
+    double* rdiag_s = floor_s + PB;                      // 1 / l_jj
     const int tid = threadIdx.x, i = tid & 63, g = tid >> 6, c0 = g * CW;
     if (tid < PB) floor_s[tid] = fmax(guard_rel * (tid < nb ? fabs(d0[j0 + tid]) : 1.0), 1e-290);
     double a[CW];
@@ -101,6 +106,7 @@ __global__ void __launch_bounds__(64 * (PB / CW), 1) potrf_block_kernel(int nb, 
             if ((i | 31) < j || c0 + CW - 1 < j) continue;
             // l_i l_c = (a_ij / p) a_cj: one DMUL per thread and one DFMA per entry instead of a DMUL + DFMA per entry
             const double r = rsqrt(p);
+            if (i == j && g == gj) rdiag_s[j] = r;       // 1 / l_jj = 1 / sqrt(p)
             const double ci = (i >= j) ? col[buf][i] : 0.0;
             const double lip = ci * (r * r);
             const double li = (i == j) ? p * r : ci * r;
@@ -122,37 +128,49 @@ __global__ void __launch_bounds__(64 * (PB / CW), 1) potrf_block_kernel(int nb, 
         if (i < nb && c < nb) L[(int64_t)(j0 + i) * ldl + j0 + c] = v;
     }
     __syncthreads();
-    // X = L^-1: x[cc] accumulates sum_{k<i} l_ik x_kc for the thread's 16 columns
-    double x[CW];
+    // X = L^-1 without a serial pass over the 64 rows: the four 16 x 16 diagonal blocks are inverted side by side (one
+    // column per thread, right-looking substitution in registers, no barrier), then two doubling levels
+    // [[X11, 0], [-X22 (L21 X11), X22]] (block size 16, then 32) with all threads: five barriers in total.
+    constexpr int NT = 64 * (PB / CW);
+    for (int e = tid; e < PB * PB; e += NT) Xs[(e >> 6) * PP + (e & 63)] = 0.0;
+    __syncthreads();
+    if (tid < PB) {
+        const int o = tid & ~15, c = tid & 15;         // block origin, column inside the block
+        double x[16];
 #pragma unroll
-    for (int cc = 0; cc < CW; ++cc) x[cc] = 0.0;
-    const double rii = 1.0 / Ls[i * PP + i];
-    if (i == 0) {
+        for (int r = 0; r < 16; ++r) x[r] = (r == c) ? 1.0 : 0.0;
 #pragma unroll
-        for (int cc = 0; cc < CW; ++cc) { x[cc] = (c0 + cc == 0) ? rii : 0.0; }
+        for (int r = 0; r < 16; ++r) {
+            const double xr = (r < c) ? 0.0 : x[r] * rdiag_s[o + r];
+            x[r] = xr;
+#pragma unroll
+            for (int r2 = r + 1; r2 < 16; ++r2) x[r2] -= Ls[(o + r2) * PP + o + r] * xr;
+        }
+#pragma unroll
+        for (int r = 0; r < 16; ++r) Xs[(o + r) * PP + o + c] = x[r];
     }
-    __shared__ double xr[2][PB];
-    for (int k = 0; k < PB; ++k) {
-        const int buf = k & 1;
-        if (i == k) {
-#pragma unroll
-            for (int cc = 0; cc < CW; ++cc) xr[buf][c0 + cc] = x[cc];      // row k of X is final
+    __syncthreads();
+#pragma unroll 1
+    for (int sz = 16; sz < PB; sz *= 2) {
+        const int total = (PB / 2) * sz;               // (64 / 2 sz) pairs of sz x sz outputs
+        for (int e = tid; e < total; e += NT) {        // T = L21 X11
+            const int q = e / (sz * sz), r = e - q * sz * sz, ii = r / sz, c = r - ii * sz, o = 2 * sz * q;
+            double acc = 0.0;
+            for (int k = c; k < sz; ++k) acc += Ls[(o + sz + ii) * PP + o + k] * Xs[(o + k) * PP + o + c];     // X11 is lower triangular
+            Ts[(q * sz + ii) * 33 + c] = acc;
         }
         __syncthreads();
-        if (i > k && c0 <= k + 1) {        // row k of X is zero right of column k: column groups beyond it only need the diagonal
-            const double lik = Ls[i * PP + k];
-#pragma unroll
-            for (int cc = 0; cc < CW; ++cc) x[cc] += lik * xr[buf][c0 + cc];
-            if (i == k + 1) {       // finish row k+1: x_ic = (delta_ic - sum) / l_ii
-#pragma unroll
-                for (int cc = 0; cc < CW; ++cc) { const int c = c0 + cc; x[cc] = (c > i) ? 0.0 : (((c == i) ? 1.0 : 0.0) - x[cc]) * rii; }
-            }
+        for (int e = tid; e < total; e += NT) {        // X21 = -X22 T
+            const int q = e / (sz * sz), r = e - q * sz * sz, ii = r / sz, c = r - ii * sz, o = 2 * sz * q;
+            double acc = 0.0;
+            for (int k = 0; k <= ii; ++k) acc += Xs[(o + sz + ii) * PP + o + sz + k] * Ts[(q * sz + k) * 33 + c];   // X22 too
+            Xs[(o + sz + ii) * PP + o + c] = -acc;
         }
+        __syncthreads();
     }
-#pragma unroll
-    for (int cc = 0; cc < CW; ++cc) {
-        const int c = c0 + cc;
-        Linv[i * PB + c] = (i < nb && c < nb) ? x[cc] : 0.0;
+    for (int e = tid; e < PB * PB; e += NT) {
+        const int r = e >> 6, c = e & 63;
+        Linv[e] = (r < nb && c < nb) ? Xs[r * PP + c] : 0.0;
     }
 }
 
@@ -181,12 +199,18 @@ size_t cholesky_work_doubles(int n) { return (size_t)((n + PB - 1) / PB) * PB * 
 cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, int64_t ldl, double shift, double guard_rel, double* work) {
     const int np = (n + PB - 1) / PB;
     double* Linv = work; double* d0 = work + (size_t)np * PB * PB; int* info = (int*)(d0 + n);
+    static bool cfg = false;
+    if (!cfg) {
+        cudaError_t ea = cudaFuncSetAttribute(potrf_block_kernel<kPotrfCW>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPotrfSmem);
+        if (ea != cudaSuccess) return ea;
+        cfg = true;
+    }
     cudaError_t e = cudaMemsetAsync(info, 0, sizeof(int), st);
     if (e != cudaSuccess) return e;
     diag_shift_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, A, lda, shift, d0); count_launch();
     for (int p = 0; p < np; ++p) {
         const int j0 = p * PB, nb = n - j0 < PB ? n - j0 : PB, m = n - j0 - nb;
-        potrf_block_kernel<kPotrfCW><<<1, 64 * (PB / kPotrfCW), 0, st>>>(nb, j0, A, lda, L, ldl, Linv + (size_t)p * PB * PB, d0, guard_rel, info); count_launch();
+        potrf_block_kernel<kPotrfCW><<<1, 64 * (PB / kPotrfCW), kPotrfSmem, st>>>(nb, j0, A, lda, L, ldl, Linv + (size_t)p * PB * PB, d0, guard_rel, info); count_launch();
         if (m <= 0) break;
         // panel below: L[i, j0:j0+nb] = A[i, j0:j0+nb] Linv^T
         e = dgemm(st, false, true, m, nb, nb, 1.0, A + (int64_t)(j0 + nb) * lda + j0, lda, Linv + (size_t)p * PB * PB, PB, 0.0,
