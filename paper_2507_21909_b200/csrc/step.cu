@@ -434,6 +434,7 @@ struct Stepper {
             Counters* cn = g_counter;
             const long long l0 = cn ? cn->launches : 0, gc0 = cn ? cn->gemm_calls : 0; const double f0 = cn ? cn->gemm_flops : 0;
             cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr;
+            const auto tg0 = std::chrono::steady_clock::now();
             cudaError_t ge = cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal);
             bool ok = ge == cudaSuccess;
             std::string why;
@@ -445,7 +446,7 @@ struct Stepper {
             if (ok) { ge = cudaGraphInstantiate(&exec, graph, 0); ok = ge == cudaSuccess; }
             if (!ok && getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg subspace] graph capture failed: %s %s\n", cudaGetErrorString(ge), why.c_str());
             if (graph) cudaGraphDestroy(graph);
-            if (getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg subspace] graph of %d step(s): %s, %d replays + %d plain steps\n", unit, ok ? "ok" : "FAILED", reps, steps - reps * unit);
+            if (getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg subspace] graph of %d step(s): %s, %d replays + %d plain steps, capture + instantiate %.0f us\n", unit, ok ? "ok" : "FAILED", reps, steps - reps * unit, std::chrono::duration<double, std::micro>(std::chrono::steady_clock::now() - tg0).count());
             if (ok) {
                 for (int r = 0; r < reps && ok; ++r) ok = cudaGraphLaunch(exec, st) == cudaSuccess;
                 c.graveyard.push_back(exec);
