@@ -248,9 +248,11 @@ struct Stepper {
         ck(tri_inverse(st, (int)n, L.p, n, cw, X.p, n, T.p), "tri_inverse");
         ck(dot(st, n * n, X.p, X.p, res), "dot");
         int info = 0;
+        std::vector<double> d0(n), xn(1);              // three read-backs, one synchronisation
         ck(cudaMemcpyAsync(&info, cholesky_info(cw, (int)n), sizeof(int), cudaMemcpyDeviceToHost, st), "readback");
-        std::vector<double> d0 = to_host(cholesky_d0(cw, (int)n), n);
-        std::vector<double> xn = to_host(res, 1);
+        ck(cudaMemcpyAsync(d0.data(), cholesky_d0(cw, (int)n), 8 * n, cudaMemcpyDeviceToHost, st), "readback");
+        ck(cudaMemcpyAsync(xn.data(), res, 8, cudaMemcpyDeviceToHost, st), "readback");
+        ck(cudaStreamSynchronize(st), "sync");
         double tr = 0; for (double v : d0) tr += v;
         if (getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg cholesky qr %lld x %lld] info %d, proven lam_min/lam_max >= %.3e\n", (long long)m, (long long)n, info, 1.0 / (xn[0] * tr));
         if (info != 0 || !std::isfinite(xn[0]) || !(xn[0] > 0) || !(tr > 0)) return false;
@@ -308,14 +310,18 @@ struct Stepper {
             ck(cudaStreamWaitEvent(st, ss.join[i], 0), "wait");
         }
         bool ok = true;
+        int info[2] = {0, 0};
+        std::vector<double> d0[2] = {std::vector<double>(n), std::vector<double>(n)}; double xn[2] = {0, 0};
+        for (int i = 0; i < 2; ++i) {          // six read-backs, one synchronisation
+            ck(cudaMemcpyAsync(&info[i], cholesky_info(cw[i], (int)n), sizeof(int), cudaMemcpyDeviceToHost, st), "readback");
+            ck(cudaMemcpyAsync(d0[i].data(), cholesky_d0(cw[i], (int)n), 8 * n, cudaMemcpyDeviceToHost, st), "readback");
+            ck(cudaMemcpyAsync(&xn[i], res[i], 8, cudaMemcpyDeviceToHost, st), "readback");
+        }
+        ck(cudaStreamSynchronize(st), "sync");
         for (int i = 0; i < 2; ++i) {
-            int info = 0;
-            ck(cudaMemcpyAsync(&info, cholesky_info(cw[i], (int)n), sizeof(int), cudaMemcpyDeviceToHost, st), "readback");
-            std::vector<double> d0 = to_host(cholesky_d0(cw[i], (int)n), n);
-            std::vector<double> xn = to_host(res[i], 1);
-            double tr = 0; for (double v : d0) tr += v;
-            if (getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg cholesky qr %lld x %lld] info %d, proven lam_min/lam_max >= %.3e\n", (long long)m, (long long)n, info, 1.0 / (xn[0] * tr));
-            if (info != 0 || !std::isfinite(xn[0]) || !(xn[0] > 0) || !(tr > 0) || !(1.0 / (xn[0] * tr) > kEpsOrthLambda)) ok = false;
+            double tr = 0; for (double v : d0[i]) tr += v;
+            if (getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg cholesky qr %lld x %lld] info %d, proven lam_min/lam_max >= %.3e\n", (long long)m, (long long)n, info[i], 1.0 / (xn[i] * tr));
+            if (info[i] != 0 || !std::isfinite(xn[i]) || !(xn[i] > 0) || !(tr > 0) || !(1.0 / (xn[i] * tr) > kEpsOrthLambda)) ok = false;
         }
         if (!ok) return false;
         for (int i = 0; i < 2; ++i) {
