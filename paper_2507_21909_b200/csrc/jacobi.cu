@@ -568,26 +568,36 @@ static size_t work_doubles(int N) {
 size_t eigh_work_bytes(int n) { return 8 * work_doubles(padded_n(n)) + 4096; }
 size_t eigh_batched_work_bytes(int nmax, int count) { return 8 * work_doubles(padded_n(nmax)) * (size_t)(count > 0 ? count : 1) + 4096; }
 
-// sorts one matrix' spectrum on the host and gathers its eigenvectors
-static int finish_one(cudaStream_t st, int n, int N, double* lam_u, int* idx, double* Vu, double* lam, double* Vt, std::vector<double>* lam_host,
-                      std::string* err) {
-    std::vector<double> lh(n);
-    if (!check(cudaMemcpyAsync(lh.data(), lam_u, sizeof(double) * n, cudaMemcpyDeviceToHost, st), err, "eigh readback")) return TATRG_ECUDA;
-    if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;
-    std::vector<int> order(n);
-    std::iota(order.begin(), order.end(), 0);
-    for (int i = 0; i < n; ++i) if (!std::isfinite(lh[i])) { if (err) *err = "eigh: non-finite eigenvalue"; return TATRG_ENUMERIC; }
-    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return lh[a] > lh[b]; });
-    if (!check(cudaMemcpyAsync(idx, order.data(), sizeof(int) * n, cudaMemcpyHostToDevice, st), err, "eigh upload")) return TATRG_ECUDA;
-    if (!check(gather_rows_scaled(st, Vt, Vu, idx, nullptr, n, n, N), err, "eigh gather")) return TATRG_ECUDA;
-    if (!check(gather_vec(st, lam, lam_u, idx, n, 1, 1.0), err, "eigh gather")) return TATRG_ECUDA;
-    if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;   // `order` leaves scope
-    if (lam_host) { lam_host->resize(n); for (int i = 0; i < n; ++i) (*lam_host)[i] = lh[order[i]]; }
-    if (getenv("TATRG_EIGH_VERBOSE")) {
-        int c[5] = {0, 0, 0, 0, 0}; const double l0 = lh[order[0]]; const double th[5] = {1e-4, 1e-8, 1e-12, 1e-14, 1e-16};
-        for (int i = 0; i < n; ++i) for (int j = 0; j < 5; ++j) if (lh[i] > th[j] * l0) ++c[j];
-        fprintf(stderr, "[tatrg eigh n=%d] spectrum: >1e-4:%d >1e-8:%d >1e-12:%d >1e-14:%d >1e-16:%d\n", n, c[0], c[1], c[2], c[3], c[4]);
+// sorts the spectra of a batch on the host and gathers the eigenvectors: one synchronisation for all read-backs, one for
+// all uploads / gathers (the index vectors must outlive the copies)
+struct FinishItem { int n; double* lam_u; int* idx; double* Vu; double* lam; double* Vt; std::vector<double>* lam_host; };
+static int finish_batch(cudaStream_t st, int N, const std::vector<FinishItem>& items, std::string* err) {
+    const size_t cnt = items.size();
+    std::vector<std::vector<double>> lh(cnt);
+    for (size_t z = 0; z < cnt; ++z) {
+        lh[z].resize(items[z].n);
+        if (!check(cudaMemcpyAsync(lh[z].data(), items[z].lam_u, sizeof(double) * items[z].n, cudaMemcpyDeviceToHost, st), err, "eigh readback")) return TATRG_ECUDA;
     }
+    if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;
+    std::vector<std::vector<int>> order(cnt);
+    for (size_t z = 0; z < cnt; ++z) {
+        const FinishItem& it = items[z];
+        const int n = it.n;
+        for (int i = 0; i < n; ++i) if (!std::isfinite(lh[z][i])) { if (err) *err = "eigh: non-finite eigenvalue"; return TATRG_ENUMERIC; }
+        order[z].resize(n);
+        std::iota(order[z].begin(), order[z].end(), 0);
+        std::stable_sort(order[z].begin(), order[z].end(), [&](int a, int b) { return lh[z][a] > lh[z][b]; });
+        if (!check(cudaMemcpyAsync(it.idx, order[z].data(), sizeof(int) * n, cudaMemcpyHostToDevice, st), err, "eigh upload")) return TATRG_ECUDA;
+        if (!check(gather_rows_scaled(st, it.Vt, it.Vu, it.idx, nullptr, n, n, N > 0 ? N : n), err, "eigh gather")) return TATRG_ECUDA;
+        if (!check(gather_vec(st, it.lam, it.lam_u, it.idx, n, 1, 1.0), err, "eigh gather")) return TATRG_ECUDA;
+        if (it.lam_host) { it.lam_host->resize(n); for (int i = 0; i < n; ++i) (*it.lam_host)[i] = lh[z][order[z][i]]; }
+        if (getenv("TATRG_EIGH_VERBOSE")) {
+            int c[5] = {0, 0, 0, 0, 0}; const double l0 = lh[z][order[z][0]]; const double th[5] = {1e-4, 1e-8, 1e-12, 1e-14, 1e-16};
+            for (int i = 0; i < n; ++i) for (int j = 0; j < 5; ++j) if (lh[z][i] > th[j] * l0) ++c[j];
+            fprintf(stderr, "[tatrg eigh n=%d] spectrum: >1e-4:%d >1e-8:%d >1e-12:%d >1e-14:%d >1e-16:%d\n", n, c[0], c[1], c[2], c[3], c[4]);
+        }
+    }
+    if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;   // `order` leaves scope
     return TATRG_OK;
 }
 
@@ -642,9 +652,15 @@ int eigh_batched(cudaStream_t st, int count, const EighItem* items, void* work, 
             for (int z = 0; z < bc; ++z) { sb.n[z] = items[z0 + z].n; sb.G[z] = items[z0 + z].G; sb.lam[z] = lam_u(z0 + z); sb.Vt[z] = Vu(z0 + z); }
             eigh_small_kernel<<<bc, 512, kSmallSmem, st>>>(sb); count_launch();
         }
+        // every matrix keeps its own leading dimension n here: one finish per distinct stride
         for (int z = 0; z < count; ++z) {
-            int rc = finish_one(st, items[z].n, items[z].n, lam_u(z), idx(z), Vu(z), items[z].lam, items[z].Vt, items[z].lam_host, err);
+            std::vector<FinishItem> fi{FinishItem{items[z].n, lam_u(z), idx(z), Vu(z), items[z].lam, items[z].Vt, items[z].lam_host}};
+            int z2 = z + 1;
+            for (; z2 < count && items[z2].n == items[z].n; ++z2)
+                fi.push_back(FinishItem{items[z2].n, lam_u(z2), idx(z2), Vu(z2), items[z2].lam, items[z2].Vt, items[z2].lam_host});
+            int rc = finish_batch(st, items[z].n, fi, err);
             if (rc != TATRG_OK) return rc;
+            z = z2 - 1;
         }
         return TATRG_OK;
     }
@@ -701,9 +717,13 @@ int eigh_batched(cudaStream_t st, int count, const EighItem* items, void* work, 
         if (sweep == kMaxBlockSweeps) { if (err) *err = "eigh: block Jacobi did not converge"; return TATRG_ENUMERIC; }
         double* Gfin = Gbuf[t & 1];
         for (int z = 0; z < bc; ++z) { extract_diag_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, Gfin + z * ws, lam_u(z0 + z)); count_launch(); }
-        for (int z = 0; z < bc; ++z) {
-            const EighItem& it = items[z0 + z];
-            int rc = finish_one(st, it.n, N, lam_u(z0 + z), idx(z0 + z), Vu(z0 + z), it.lam, it.Vt, it.lam_host, err);
+        {
+            std::vector<FinishItem> fi;
+            for (int z = 0; z < bc; ++z) {
+                const EighItem& it = items[z0 + z];
+                fi.push_back(FinishItem{it.n, lam_u(z0 + z), idx(z0 + z), Vu(z0 + z), it.lam, it.Vt, it.lam_host});
+            }
+            int rc = finish_batch(st, N, fi, err);
             if (rc != TATRG_OK) return rc;
         }
     }
