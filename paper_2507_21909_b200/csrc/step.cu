@@ -205,8 +205,10 @@ struct Stepper {
     // Orthonormal basis of the numerical column space of mat [m x n]:  mat = Q R, Q [m x r], R [r x n]   (R14).
     // Gram matrix -> eigen-decomposition -> Q = mat V lam^-1/2 (directions with lam <= 1e-12 lam_max dropped), and a
     // second identical pass on Q for narrow matrices (n <= 128), where it is cheap, to restore orthogonality to eps.
-    void orth(const Tens& mat, Tens& Q, Tens& R) {
-        if (c.use_subspace && mat.d[1] >= 8 && mat.d[1] <= 128 && mat.d[0] >= 4 * mat.d[1] && orth_chol(mat, Q, R, 2)) return;
+    // span_only: the caller uses Q only as a basis of the column space that is multiplied by the operator and orthonormalised
+    // again (the intermediate passes of Eq. A.4-A.6): one Cholesky pass (Q^T Q = 1 to cond^2 eps) is enough there.
+    void orth(const Tens& mat, Tens& Q, Tens& R, bool span_only = false) {
+        if (c.use_subspace && mat.d[1] >= 8 && mat.d[1] <= 128 && mat.d[0] >= 4 * mat.d[1] && orth_chol(mat, Q, R, span_only ? 1 : 2)) return;
         Scope sc(*this);
         const int64_t m = mat.d[0], n = mat.d[1];
         Tens G = mm(true, false, n, n, m, mat.p, n, mat.p, n);
@@ -676,7 +678,7 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
         Tens yk = ein("qib,iabm->aqm", RC3, t);                          // Eq. A.4 :356
         drop(t);
         Tens q2, r2;
-        orth(view(yk, {chi * npc, yk.d[2]}), q2, r2);
+        orth(view(yk, {chi * npc, yk.d[2]}), q2, r2, k < c.n_pow);
         drop(yk); drop(r2);
         if (qk.p) drop(qk);
         qk = view(q2, {chi, npc, q2.d[1]});
@@ -687,7 +689,7 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
         keep(qk); keep(yt);
         if (k < c.n_pow) {
             Tens q3, r3;
-            orth(view(yt, {chi * npb, yt.d[2]}), q3, r3);                // Eq. A.6 :365
+            orth(view(yt, {chi * npb, yt.d[2]}), q3, r3, true);          // Eq. A.6 :365
             drop(r3); drop(omega);
             omega = view(q3, {chi, npb, q3.d[1]});
             keep(omega);
