@@ -196,7 +196,8 @@ size_t cholesky_work_doubles(int n) { return (size_t)((n + PB - 1) / PB) * PB * 
 // A [n x n, lda] (lower triangle read, destroyed) -> L [n x n, ldl] lower triangular (strict upper part of the diagonal
 // blocks zeroed; blocks above the diagonal are not touched).  work: cholesky_work_doubles(n) doubles [dev]:
 // [Linv of every panel | d0 | info].  Asynchronous.
-cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, int64_t ldl, double shift, double guard_rel, double* work) {
+cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, int64_t ldl, double shift, double guard_rel, double* work,
+                     bool reset_info) {
     const int np = (n + PB - 1) / PB;
     double* Linv = work; double* d0 = work + (size_t)np * PB * PB; int* info = (int*)(d0 + n);
     static bool cfg = false;
@@ -205,7 +206,8 @@ cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, 
         if (ea != cudaSuccess) return ea;
         cfg = true;
     }
-    cudaError_t e = cudaMemsetAsync(info, 0, sizeof(int), st);
+    cudaError_t e = cudaSuccess;
+    if (reset_info) { e = cudaMemsetAsync(info, 0, sizeof(int), st); count_launch(); }
     if (e != cudaSuccess) return e;
     diag_shift_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, A, lda, shift, d0); count_launch();
     for (int p = 0; p < np; ++p) {

@@ -90,7 +90,9 @@ int svd_rows(cudaStream_t st, int nv, int len, const double* X, double* s, doubl
 cudaError_t symmetrize(cudaStream_t st, int n, double* A);                      // A = (A + A^T) / 2 in place
 cudaError_t mirror_lower(cudaStream_t st, int n, double* A);                    // A[i][j] = A[j][i] for i < j
 size_t cholesky_work_doubles(int n);
-cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, int64_t ldl, double shift, double guard_rel, double* work);
+// reset_info = false accumulates the flags of several factorisations that share `work` (the caller clears them once)
+cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, int64_t ldl, double shift, double guard_rel, double* work,
+                     bool reset_info = true);
 const int* cholesky_info(const double* work, int n);                            // [dev] bit 0: a pivot was raised to the guard, bit 1: non-finite
 cudaError_t trsm_right_lt(cudaStream_t st, int64_t m, int n, double* X, int64_t ldx, double* Q, int64_t ldq, const double* L, int64_t ldl,
                           const double* work);

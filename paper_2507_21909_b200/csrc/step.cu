@@ -386,7 +386,7 @@ struct Stepper {
         double* X = s.buf[src].p;
         const double* Wp = s.F ? X + (int64_t)s.n * s.b : X;
         mm_into(s.Gm.p, s.b, true, false, s.b, s.b, s.n, X, s.b, Wp, s.b);
-        ck(cholesky(st, s.b, s.Gm.p, s.b, s.L.p, s.b, shift, 1e-14, s.cw), "cholesky");
+        ck(cholesky(st, s.b, s.Gm.p, s.b, s.L.p, s.b, shift, 1e-14, s.cw, false), "cholesky");      // flags accumulate over the iteration
         ck(trsm_right_lt(st, rows, s.b, X, s.b, s.buf[src ^ 1].p, s.b, s.L.p, s.b, s.cw), "trsm");
         s.cur = src ^ 1;
     }
@@ -501,6 +501,7 @@ struct Stepper {
             s.Gm = make({s.b, s.b}); s.L = make({s.b, s.b}); s.H = make({s.b, s.b});
             s.cw = raw((int64_t)cholesky_work_doubles(s.b)); s.dg = raw(s.b);
             ck(fill_zero(st, s.L.p, (int64_t)s.b * s.b), "zero");
+            ck(cudaMemsetAsync(const_cast<int*>(cholesky_info(s.cw, s.b)), 0, sizeof(int), st), "memset"); count_launch();
             ck(philox_gauss(st, c.seed, (uint32_t)call, s.sid, 0, (int64_t)s.n * s.b, s.buf[1].p), "philox");
             if (s.F) mm_into(s.buf[1].p + (int64_t)s.n * s.b, s.b, false, false, s.n, s.b, s.n, s.F, s.n, s.buf[1].p, s.b);
             sub_orth(s, 1, kShift);
@@ -511,11 +512,16 @@ struct Stepper {
         auto tA = verbose ? sync_all() : std::chrono::steady_clock::time_point();
         auto estimate = [&](SubProb& s) {
             OnStream on(*this, s);
+            int info = 0;
+            ck(cudaMemcpyAsync(&info, cholesky_info(s.cw, s.b), sizeof(int), cudaMemcpyDeviceToHost, st), "readback");
             s.r = to_host(s.dg, s.b);
+            // a pivot that had to be raised to its guard, or a non-finite one: the block has numerically dependent columns (the
+            // matrix has fewer than b significant directions: unsaturated steps, ordered phase) -> the full decomposition decides
+            if (info != 0) { s.ok = false; return; }
             for (double v : s.r) if (!std::isfinite(v)) { s.ok = false; return; }
             double tail = 0; for (int j = s.b - 4; j < s.b; ++j) tail = std::max(tail, s.r[j]);
             double head = s.r[0]; for (int j = 0; j < s.kmax; ++j) head = std::min(head, s.r[j]);
-            if (!(head > 1e-12 * s.r[0]) || !(tail > 0)) { s.ok = false; return; }     // rank-deficient leading block: full decomposition
+            if (!(head > 1e-12 * s.r[0]) || !(tail > 1e-9 * head)) { s.ok = false; return; }     // rank-deficient block: full decomposition
             // the diagonal of R is that of the last orthonormalisation: r_j ~ lam_j^deg
             const double rho = 1.1 * std::pow(tail / head, 1.0 / s.deg);
             if (!(rho < 0.8)) { s.ok = false; return; }
@@ -551,6 +557,14 @@ struct Stepper {
             double* T = s.buf[s.cur ^ 1].p;
             mm_into(T, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, s.W(), s.b);
             mm_into(s.H.p, s.b, true, false, s.b, s.b, s.n, s.W(), s.b, T, s.b);
+        }
+        for (SubProb& s : ps) {       // the last orthonormalisations must not have met a dependent column either
+            if (!s.ok) continue;
+            OnStream on(*this, s);
+            int info = 0;
+            ck(cudaMemcpyAsync(&info, cholesky_info(s.cw, s.b), sizeof(int), cudaMemcpyDeviceToHost, st), "readback");
+            ck(cudaStreamSynchronize(st), "sync");
+            if (info != 0) s.ok = false;
         }
         if (multi)
             for (size_t i = 0; i < ps.size(); ++i) {

@@ -390,3 +390,22 @@ def test_converged_sketch_mode_is_independent_of_the_random_tensor():
             t.step()
         loose.append(t.lnZ_per_site())
     assert abs(loose[0] - loose[1]) > 1e-9
+
+
+@pytest.mark.parametrize("D,beta,h,steps", [(24, 0.12, 0.0, 8), (16, 0.2, 0.0, 14), (16, 0.1497, 0.05, 14)])
+def test_subspace_path_falls_back_on_rank_deficient_blocks(D, beta, h, steps):
+    """Away from criticality and in the unsaturated first steps the Gram matrices have fewer significant directions than the
+    iteration block (D = 24, beta = 0.12, step 4: rank 64 of a 96-wide block).  The Cholesky guard flags the dependent columns
+    and the full decomposition takes over: the run completes and agrees with TATRG_OPT_SUBSPACE = 0 throughout."""
+    runs = []
+    for sub in (1, 0):
+        t = T.Tatrg(beta, h, D, D, 11)
+        t.set_option(T.OPT_SUBSPACE, sub)
+        out = []
+        for _ in range(steps):
+            t.step()
+            out.append(t.lnZ_per_site())
+        runs.append(out)
+        t.close()
+    for a, b in zip(*runs):
+        assert np.isfinite(a) and abs(a - b) <= 1e-11 * abs(b)
