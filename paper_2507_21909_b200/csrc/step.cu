@@ -282,7 +282,9 @@ struct Stepper {
     // factorisation + inversion chains (latency-bound: ~60 small launches each) side by side on two auxiliary streams, then
     // the decisions and the two Q = mat L^-T products.  All buffers are allocated before the fork; nothing is allocated or
     // freed while the chains are in flight.  Returns false (nothing kept) unless both operands prove full rank.
-    bool orth_chol_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2]) {
+    // Xinv != nullptr: Q = mat L^-T is NOT formed; the caller gets Xinv[i] = L^-1 instead (Q[i].p stays null) and applies it
+    // to whatever multiplies Q (bond_swap: Q only ever appears in products, so two n x n x n GEMMs replace two m x n x n ones).
+    bool orth_chol_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2], Tens* Xinv = nullptr) {
         SubStreams& ss = sub_streams();
         if (!ss.ok) {
             const bool ok0 = orth_chol(m0, Q[0], R[0]), ok1 = orth_chol(m1, Q[1], R[1]);
@@ -327,18 +329,23 @@ struct Stepper {
         }
         if (!ok) return false;
         for (int i = 0; i < 2; ++i) {
-            Q[i] = mm(false, true, m, n, n, mats[i]->p, n, X[i].p, n);
+            if (Xinv) { Xinv[i] = X[i]; keep(X[i]); Q[i] = Tens(); Q[i].p = nullptr; }
+            else { Q[i] = mm(false, true, m, n, n, mats[i]->p, n, X[i].p, n); keep(Q[i]); }
             R[i] = perm(view(L[i], {n, n}), {1, 0});
-            keep(Q[i]); keep(R[i]);
+            keep(R[i]);
         }
         return true;
     }
 
     // orth() of two matrices of the same shape with n > 128 (single pass): the two Gram matrices are decomposed together
-    void orth_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2]) {
+    // Xinv: see orth_chol_pair (set only when the Cholesky path with two streams was taken; else Xinv[i].p stays null and Q is explicit)
+    void orth_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2], Tens* Xinv = nullptr) {
         const int64_t m = m0.d[0], n = m0.d[1];
+        if (Xinv) { Xinv[0].p = nullptr; Xinv[1].p = nullptr; }
         if (n <= 128 || m1.d[0] != m || m1.d[1] != n) { orth(m0, Q[0], R[0]); orth(m1, Q[1], R[1]); return; }
-        if (c.use_subspace && orth_chol_pair(m0, m1, Q, R)) return;
+        if (c.use_subspace && sub_streams().ok && orth_chol_pair(m0, m1, Q, R, Xinv)) return;
+        if (Xinv) { Xinv[0].p = nullptr; Xinv[1].p = nullptr; }
+        if (c.use_subspace && !sub_streams().ok && orth_chol_pair(m0, m1, Q, R)) return;
         Scope sc(*this);
         const Tens* mats[2] = {&m0, &m1};
         Tens G[2];
@@ -655,7 +662,8 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
     Scope sc(*this);
     const int64_t d1 = a.d[0], d2 = a.d[1], d3 = a.d[2], d4 = a.d[3], chi = a.d[4];
     const int64_t F = d1 * d2 * d3 * d4, J = d2 * d3 * d4;
-    Tens QB, RB, QC, RC;
+    Tens QB, RB, QC, RC, XB, XC;      // implicit: QB, QC hold B, C themselves and XB, XC the inverse Cholesky factors
+    bool implicit = false;
     {
         Scope s2(*this);
         // B[i1,j',al] = sum_a' Dt[i1,j',a'] core[al,a'],  C[i1,i',be] = sum_a' A[i1,i',a'] core[a',be]   (core symmetric)
@@ -665,10 +673,21 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
         Tens cc = mm(false, false, F, chi, chi, a.p, chi, core.p, chi);
         Tens cm = perm(view(cc, {d1, J, chi}), {1, 0, 2});             // Eq. A.3 :348  C[(i'),(i1 be)]
         drop(cc);
-        Tens Qs[2], Rs[2];
-        orth_pair(view(bm, {J, d1 * chi}), view(cm, {J, d1 * chi}), Qs, Rs);
-        QB = Qs[0]; RB = Rs[0]; QC = Qs[1]; RC = Rs[1];
-        keep(QB); keep(RB); keep(QC); keep(RC);
+        Tens Qs[2], Rs[2], Xs[2];
+        orth_pair(view(bm, {J, d1 * chi}), view(cm, {J, d1 * chi}), Qs, Rs, Xs);
+        RB = Rs[0]; RC = Rs[1];
+        if (Xs[0].p) {
+            // Cholesky QR: Q^B = B L_B^-T and Q^C = C L_C^-T are never formed.  They only enter through the products
+            // Q^B^T Omega^phys (R12) and Q^C U^bond, Q^B V^bond (Eq. A.10-A.11), where the n x n inverse factor is
+            // applied to the small operand instead (saves two D^3 x D^2 x D^2 products).
+            implicit = true;
+            QB = view(bm, {J, d1 * chi}); QC = view(cm, {J, d1 * chi}); XB = Xs[0]; XC = Xs[1];
+            keep(bm); keep(cm); keep(XB); keep(XC);
+        } else {
+            QB = Qs[0]; QC = Qs[1];
+            keep(QB); keep(QC);
+        }
+        keep(RB); keep(RC);
     }
     if (submark) submark();                                              // end of TATRG_ST_QR
     const int64_t npb = QB.d[1], npc = QC.d[1];
@@ -682,7 +701,10 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
         ck(philox_gauss(st, c.seed, (uint32_t)call, 0, 0, chi * J * l, om.p), "philox");
         Tens omp = perm(om, {1, 0, 2});                                   // [j', be, m]: one wide GEMM instead of chi narrow ones
         drop(om);
-        omega = ein("jp,jbm->bpm", QB, omp);
+        if (implicit) {
+            Tens tmp = ein("jc,jbm->cbm", QB, omp);
+            omega = ein("pc,cBm->Bpm", XB, tmp);
+        } else omega = ein("jp,jbm->bpm", QB, omp);
         keep(omega);
     }
     Tens qk, yt;
@@ -733,8 +755,14 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
     // one GEMM with N = (al, g) each: the batched form has N = g <= D, a quarter of a tile
     Tens ubp = perm(view(ub, {chi, npc, gr}), {1, 0, 2});
     Tens vbp = perm(view(vb, {chi, npb, gr}), {1, 0, 2});
-    x = ein("jq,qag->ajg", QC, ubp);
-    y = ein("jp,pbg->bjg", QB, vbp);
+    if (implicit) {
+        Tens wx = ein("qc,qag->cag", XC, ubp), wy = ein("pc,pbg->cbg", XB, vbp);
+        x = ein("jc,cag->ajg", QC, wx);
+        y = ein("jc,cbg->bjg", QB, wy);
+    } else {
+        x = ein("jq,qag->ajg", QC, ubp);
+        y = ein("jp,pbg->bjg", QB, vbp);
+    }
     x = view(x, {chi, d2, d3, d4, gr});
     y = view(y, {chi, d2, d3, d4, gr});
     sig = raw(gr);
