@@ -411,7 +411,10 @@ struct Stepper {
     }
     // The problems of a stage are independent chains of small launches: each runs on a stream of its own (created once
     // per process), forked from and joined to the caller's stream by events, so that their kernels overlap on the device.
-    struct SubStreams { cudaStream_t s[4]; cudaEvent_t fork, join[4]; bool ok = false; bool tried = false; };
+    // All of them have the greatest priority: while a big contraction of the caller's stream is in flight (run(): the squeezer
+    // chains overlap the Gram matrices and the Xi products), their small CTAs get the next SM slot that frees up.
+    // q: the stream that stands in for the caller's during such an overlapped stage; forkq/joinq its events.
+    struct SubStreams { cudaStream_t s[4], q; cudaEvent_t fork, join[4], forkq, joinq; bool ok = false; bool tried = false; };
     static SubStreams& sub_streams() {      // one set per device; not for concurrent use from several host threads
         static std::map<int, SubStreams> per_device;
         static std::mutex mu;
@@ -421,9 +424,13 @@ struct Stepper {
         SubStreams& ss = per_device[dev];
         if (!ss.tried) {
             ss.tried = true;
+            int lo = 0, hi = 0;
+            cudaDeviceGetStreamPriorityRange(&lo, &hi);          // hi = greatest priority (numerically lowest)
             bool ok = cudaEventCreateWithFlags(&ss.fork, cudaEventDisableTiming) == cudaSuccess;
             for (int i = 0; i < 4 && ok; ++i)
-                ok = cudaStreamCreateWithFlags(&ss.s[i], cudaStreamNonBlocking) == cudaSuccess && cudaEventCreateWithFlags(&ss.join[i], cudaEventDisableTiming) == cudaSuccess;
+                ok = cudaStreamCreateWithPriority(&ss.s[i], cudaStreamNonBlocking, hi) == cudaSuccess && cudaEventCreateWithFlags(&ss.join[i], cudaEventDisableTiming) == cudaSuccess;
+            if (ok) ok = cudaStreamCreateWithPriority(&ss.q, cudaStreamNonBlocking, hi) == cudaSuccess && cudaEventCreateWithFlags(&ss.forkq, cudaEventDisableTiming) == cudaSuccess &&
+                         cudaEventCreateWithFlags(&ss.joinq, cudaEventDisableTiming) == cudaSuccess;
             ss.ok = ok;
         }
         return ss;
@@ -606,7 +613,9 @@ struct Stepper {
     void bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x, Tens& y, double*& sig, int& gr);
     void triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y, const double* sig, Tens U[4], Tens& e, Tens& f, Tens& g, Tens& h);
     void half_grams(const Tens& P, const Tens& Q, const Tens& Iu, const Tens& Jl, Tens th[3]);
-    void squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], Tens Nt[3]);
+    void squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], Tens Nt[3], int dmask = 7);
+    void half_grams4(const Tens& P, const Tens& Q, Tens th[3]);
+    void half_grams23(const Tens& P, const Tens& Q, const Tens& Iu, const Tens& Jl, Tens th[3]);
     void atrg_grams(const Tens& P, const Tens& Q, Tens th[3]);
     Tens atrg_contract(const Tens& P, const Tens& Q, Tens S[3]);
     void run();
@@ -867,14 +876,19 @@ void Stepper::triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y,
 // P[o1,kU,u4,bond] sits on the upper site, Q[bond,kL,l4,o2] on the lower site; Iu[kU,u2,u3], Jl[kL,l2,l3].
 // th[d-2][(u l),(u' l')] for d = 2,3,4, staged so that nothing larger than K^4 appears.
 void Stepper::half_grams(const Tens& P, const Tens& Q, const Tens& Iu, const Tens& Jl, Tens th[3]) {
+    half_grams4(P, Q, th);
+    half_grams23(P, Q, Iu, Jl, th);
+}
+void Stepper::half_grams4(const Tens& P, const Tens& Q, Tens th[3]) {
+    // direction 4: Iu and Jl are isometries and drop out
+    Scope s2(*this);
+    Tens ee = ein("ikua,ikvb->uavb", P, P);
+    Tens ff = ein("akld,bkwd->albw", Q, Q);
+    th[2] = ein("uavb,albw->ulvw", ee, ff);
+    keep(th[2]);
+}
+void Stepper::half_grams23(const Tens& P, const Tens& Q, const Tens& Iu, const Tens& Jl, Tens th[3]) {
     Scope sc(*this);
-    {   // direction 4: Iu and Jl are isometries and drop out
-        Scope s2(*this);
-        Tens ee = ein("ikua,ikvb->uavb", P, P);
-        Tens ff = ein("akld,bkwd->albw", Q, Q);
-        th[2] = ein("uavb,albw->ulvw", ee, ff);
-        keep(th[2]);
-    }
     Tens ef;
     {
         Scope s2(*this);
@@ -891,13 +905,14 @@ void Stepper::half_grams(const Tens& P, const Tens& Q, const Tens& Iu, const Ten
         th[d - 2] = ein("uvxy,lwxy->ulvw", tmp, jj);
         keep(th[d - 2]);
     }
-    for (int i = 0; i < 3; ++i) keep(th[i]);
+    for (int i = 0; i < 2; ++i) keep(th[i]);
 }
 
 // (d) squeezer pairs of the three directions (R6): thf = R1^T R1, thb = R2 R2^T, SVD R1 R2 = U s V^T,
 // M = R2 V s^-1/2, N = R1^T U s^-1/2, gauge-fixed (R10).  Returned as rows: Mt[k,u,l], Nt[k,u,l].
 // The six Gram matrices are eigen-decomposed in one batch, then the three (R1 R2)^T (R1 R2) in another.
-void Stepper::squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], Tens Nt[3]) {
+// dmask: bit d set = direction d + 2 is computed by this call (run() computes direction 4 ahead of the other two).
+void Stepper::squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], Tens Nt[3], int dmask) {
     Scope sc(*this);
     // per direction: s (host, leading values), wt [k x n] = (R2 V)^T, nt [k x n] = (Theta_f R2 V)^T
     std::vector<double> sval[3]; Tens wts[3], nts[3]; int kk[3] = {0, 0, 0}; bool have[3] = {false, false, false};
@@ -907,6 +922,7 @@ void Stepper::squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], T
     {
         std::vector<SubProb> ps; std::vector<int> dirs;
         for (int d = 0; d < 3; ++d) {
+            if (!((dmask >> d) & 1)) continue;
             const int n = du[d] * du[d];
             if (!c.use_subspace || !sub_applicable(n, c.D)) continue;
             ck(symmetrize(st, n, thf[d].p), "symmetrize"); ck(symmetrize(st, n, thb[d].p), "symmetrize");
@@ -942,7 +958,7 @@ void Stepper::squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], T
     // (2) full decompositions for the directions the iteration does not cover (small or rank-deficient problems):
     //     the Gram matrices are eigen-decomposed in one batch, then the (R1 R2)^T (R1 R2) in another.
     std::vector<int> todo;
-    for (int d = 0; d < 3; ++d) if (!have[d]) todo.push_back(d);
+    for (int d = 0; d < 3; ++d) if (((dmask >> d) & 1) && !have[d]) todo.push_back(d);
     if (!todo.empty()) {
         std::vector<EigOut> eo;
         {
@@ -985,9 +1001,10 @@ void Stepper::squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], T
             sval[d] = s; kk[d] = k;
         }
     }
-    for (int d = 0; d < 3; ++d) { drop(thf[d]); drop(thb[d]); }
+    for (int d = 0; d < 3; ++d) if ((dmask >> d) & 1) { drop(thf[d]); drop(thb[d]); }
     // (3) gauge (R10), s^-1/2 scalings
     for (int d = 0; d < 3; ++d) {
+        if (!((dmask >> d) & 1)) continue;
         const int n = du[d] * du[d], dir = d + 2, k = kk[d];
         const std::vector<double>& s = sval[d];
         std::vector<double> sk(s.begin(), s.begin() + k);
@@ -1119,32 +1136,84 @@ void Stepper::run() {
         save("UA", U[0]); save("UX", U[1]); save("UY", U[2]); save("UD", U[3]);
         drop(a); drop(dt); drop(core); drop(x); drop(y);
         mark();
+        const int du[3] = {(int)c.phi.d[1], (int)c.phi.d[2], (int)c.phi.d[3]};
+        Tens thf[3], thb[3], Mt[3], Nt[3];
+        // Overlapped schedule (saturated steps): the squeezers are chains of small launches with host decisions in between
+        // (subspace iteration, Rayleigh-Ritz) that leave the SMs almost idle.  Direction 4 is the only one the Xi products of
+        // Eq. 2.18-2.19 need, so: Gram matrices of direction 4 | squeezer 4 on the auxiliary stream q while the caller's stream
+        // computes the Gram matrices of directions 2, 3 | squeezers 2, 3 on q while the caller's stream computes Xi and Xi' |
+        // Lambda, Phi', Psi'.  Everything the q stage allocates comes from an arena of its own (a block of the workspace taken
+        // before the fork), because the pool's reuse rule is enqueue order on ONE stream.
+        SubStreams& ss = sub_streams();
+        bool overlap = c.use_subspace && ss.ok && getenv("TATRG_NO_OVERLAP") == nullptr;
+        for (int d = 0; d < 3; ++d) overlap = overlap && sub_applicable(du[d] * du[d], c.D);
+        double* arena = nullptr; size_t arena_bytes = 0;
+        if (overlap) {
+            const size_t n = (size_t)std::max(du[0], std::max(du[1], du[2])); const size_t n2 = n * n;
+            arena_bytes = 8 * (64 * n2 * n2 + (2u << 20));
+            // both Xi tensors are alive at once in this schedule; leave the arena's size again as headroom
+            const size_t xi_bytes = 8 * (size_t)(e.d[0] * e.d[1] * f.d[1] * f.d[3]) * (size_t)c.D;
+            if (c.pool.in_use() + 2 * arena_bytes + 3 * xi_bytes <= c.pool.capacity())
+                arena = c.pool.alloc((int64_t)(arena_bytes / 8));   // freed at the end of the step, after the joins
+            if (!arena) overlap = false;
+        }
+        Pool arena_pool;
+        if (arena) arena_pool.reset(arena, arena_bytes);
+        struct ArenaGuard {        // c.pool stands for the arena while the q stage issues work; restored on every exit path
+            tatrg_ctx& c; Pool& other;
+            ArenaGuard(tatrg_ctx& c_, Pool& o) : c(c_), other(o) { std::swap(other, c.pool); }
+            ~ArenaGuard() { std::swap(other, c.pool); }
+        };
+        auto on_q = [&](cudaEvent_t after, int dmask) {      // squeezers of the directions in dmask on stream q, after event `after`
+            ArenaGuard guard(c, arena_pool);
+            Stepper sq(c, ss.q);
+            ck(cudaStreamWaitEvent(ss.q, after, 0), "wait");
+            sq.squeezers(thf, thb, du, Mt, Nt, dmask);
+            for (int d = 0; d < 3; ++d) if ((dmask >> d) & 1) { sq.detach(Mt[d]); sq.detach(Nt[d]); }
+            ck(cudaEventRecord(ss.joinq, ss.q), "event");
+        };
         // (d) squeezer Gram matrices of the upper half (E F I J) and of the sigma-weighted lower half (G sigma, H, K, L)
-        Tens thf[3], thb[3];
-        half_grams(e, f, U[0], U[1], thf);
+        Tens P, Q;
         {
-            Scope s2(*this);
             Tens gs = make({g.d[0], g.d[1], g.d[2], g.d[3]});
             ck(scale_last(st, gs.p, g.p, sig, g.size() / gr, gr, 0), "scale");
-            Tens P = perm(gs, {3, 1, 2, 0});          // [g, kY, j4u, be]
-            Tens Q = perm(h, {3, 1, 2, 0});           // [be, kD, j4l, j1]
-            half_grams(P, Q, U[2], U[3], thb);
-            for (int i = 0; i < 3; ++i) keep(thb[i]);
+            P = perm(gs, {3, 1, 2, 0});          // [g, kY, j4u, be]
+            Q = perm(h, {3, 1, 2, 0});           // [be, kD, j4l, j1]
+            drop(gs);
         }
+        half_grams4(e, f, thf);
+        half_grams4(P, Q, thb);
+        if (overlap) ck(cudaEventRecord(ss.forkq, st), "event");
+        half_grams23(e, f, U[0], U[1], thf);
+        half_grams23(P, Q, U[2], U[3], thb);
+        drop(P); drop(Q);
         mark();
-        Tens Mt[3], Nt[3];
-        {
-            const int du[3] = {(int)c.phi.d[1], (int)c.phi.d[2], (int)c.phi.d[3]};
+        if (overlap) {
+            on_q(ss.forkq, 4);                                          // direction 4 (bit 2)
+            ck(cudaStreamWaitEvent(st, ss.joinq, 0), "wait");
+            ck(cudaEventRecord(ss.forkq, st), "event");                 // after the Gram matrices of directions 2, 3
+        } else {
             squeezers(thf, thb, du, Mt, Nt);
         }
-        save("M2", Mt[0]); save("M3", Mt[1]); save("M4", Mt[2]); save("N2", Nt[0]); save("N3", Nt[1]); save("N4", Nt[2]);
         mark();
-        // (e) Eq. 2.18 :175  Phi'[i1,k2,k3,k4,g]
+        // (e) Eq. 2.18-2.19 :175  Xi[i1,kA,kX,k4,g], Xi'[j1,kD,kY,k4,g]
+        Tens xi, xip;
         {
-            Scope s2(*this);
             Tens fm = ein("zul,axld->uaxzd", Mt[2], f);
-            Tens xi = ein("ikua,uaxzd->ikxzd", e, fm);                  // Xi[i1,kA,kX,k4,g]
+            xi = ein("ikua,uaxzd->ikxzd", e, fm);
             drop(fm);
+            Tens gn = ein("zul,byug->lbyzg", Nt[2], g);
+            xip = ein("jdlb,lbyzg->jdyzg", h, gn);
+            drop(gn);
+        }
+        if (overlap) {
+            on_q(ss.forkq, 3);                                          // directions 2, 3 while Xi, Xi' are computed
+            ck(cudaStreamWaitEvent(st, ss.joinq, 0), "wait");
+            for (int d = 0; d < 3; ++d) { drop(thf[d]); drop(thb[d]); }
+        }
+        save("M2", Mt[0]); save("M3", Mt[1]); save("M4", Mt[2]); save("N2", Nt[0]); save("N3", Nt[1]); save("N4", Nt[2]);
+        {   // Phi'[i1,k2,k3,k4,g]
+            Scope s2(*this);
             Tens im = ein("kuc,zul->kclz", U[0], Mt[0]);
             Tens imm = ein("kclz,ycw->klwzy", im, Mt[1]);
             Tens lam = ein("klwzy,xlw->kxzy", imm, U[1]);               // Lambda[kA,kX,k2,k3]
@@ -1154,20 +1223,18 @@ void Stepper::run() {
             phin = perm(ph, {1, 2, 3, 0, 4});                           // (f) rotate: axis 1 becomes axis 4  (R5)
             keep(phin);
         }
-        {   // Eq. 2.19 :175  Psi'[j1,k2,k3,k4,g]
+        {   // Psi'[j1,k2,k3,k4,g]
             Scope s2(*this);
-            Tens gn = ein("zul,byug->lbyzg", Nt[2], g);
-            Tens xi = ein("jdlb,lbyzg->jdyzg", h, gn);                  // Xi'[j1,kD,kY,k4,g]
-            drop(gn);
             Tens kn = ein("yuc,zul->yclz", U[2], Nt[0]);
             Tens knn = ein("yclz,vcw->ylwzv", kn, Nt[1]);
             Tens lam = ein("ylwzv,dlw->dyzv", knn, U[3]);               // Lambda'[kD,kY,k2,k3]
             drop(kn); drop(knn);
-            Tens ps = ein("Jdyzg,dypq->Jpqzg", xi, lam);
-            drop(xi);
+            Tens ps = ein("Jdyzg,dypq->Jpqzg", xip, lam);
+            drop(xip);
             psin = perm(ps, {1, 2, 3, 0, 4});
             keep(psin);
         }
+        if (arena) c.pool.free(arena);
         mark();
     }
     c.pool.free(c.phi.p); c.pool.free(c.psi.p);
@@ -1199,7 +1266,7 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
     g_counter = nullptr;
     c->last_stream = st;
     c->last_launches = cn.launches;
-    if (rc != TATRG_OK) { c->failed = true; c->lnc.resize(lnc0); return rc; }
+    if (rc != TATRG_OK) { cudaDeviceSynchronize(); c->failed = true; c->lnc.resize(lnc0); return rc; }   // auxiliary streams may still be running
     c->gemm_flops = cn.gemm_flops; c->gemm_calls = cn.gemm_calls; c->perm_calls = cn.permute_calls; c->perm_bytes = cn.permuted_bytes;
     if (c->timing >= 1) {
         cudaError_t e = cudaStreamSynchronize(st);
