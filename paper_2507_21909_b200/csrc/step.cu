@@ -284,7 +284,9 @@ struct Stepper {
     // freed while the chains are in flight.  Returns false (nothing kept) unless both operands prove full rank.
     // Xinv != nullptr: Q = mat L^-T is NOT formed; the caller gets Xinv[i] = L^-1 instead (Q[i].p stays null) and applies it
     // to whatever multiplies Q (bond_swap: Q only ever appears in products, so two n x n x n GEMMs replace two m x n x n ones).
-    bool orth_chol_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2], Tens* Xinv = nullptr) {
+    // meanwhile: work for the caller's stream that does not depend on the factors, issued while the two chains are in flight
+    // (it may allocate: the chains' buffers stay allocated and the chains themselves allocate nothing).
+    bool orth_chol_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2], Tens* Xinv = nullptr, const std::function<void()>* meanwhile = nullptr) {
         SubStreams& ss = sub_streams();
         if (!ss.ok) {
             const bool ok0 = orth_chol(m0, Q[0], R[0]), ok1 = orth_chol(m1, Q[1], R[1]);
@@ -311,8 +313,9 @@ struct Stepper {
             ck(tri_inverse(a, (int)n, L[i].p, n, cw[i], X[i].p, n, T[i].p), "tri_inverse");
             ck(dot(a, n * n, X[i].p, X[i].p, res[i]), "dot");
             ck(cudaEventRecord(ss.join[i], a), "event");
-            ck(cudaStreamWaitEvent(st, ss.join[i], 0), "wait");
         }
+        if (meanwhile && *meanwhile) (*meanwhile)();
+        for (int i = 0; i < 2; ++i) ck(cudaStreamWaitEvent(st, ss.join[i], 0), "wait");
         bool ok = true;
         int info[2] = {0, 0};
         std::vector<double> d0[2] = {std::vector<double>(n), std::vector<double>(n)}; double xn[2] = {0, 0};
@@ -339,11 +342,11 @@ struct Stepper {
 
     // orth() of two matrices of the same shape with n > 128 (single pass): the two Gram matrices are decomposed together
     // Xinv: see orth_chol_pair (set only when the Cholesky path with two streams was taken; else Xinv[i].p stays null and Q is explicit)
-    void orth_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2], Tens* Xinv = nullptr) {
+    void orth_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2], Tens* Xinv = nullptr, const std::function<void()>* meanwhile = nullptr) {
         const int64_t m = m0.d[0], n = m0.d[1];
         if (Xinv) { Xinv[0].p = nullptr; Xinv[1].p = nullptr; }
         if (n <= 128 || m1.d[0] != m || m1.d[1] != n) { orth(m0, Q[0], R[0]); orth(m1, Q[1], R[1]); return; }
-        if (c.use_subspace && sub_streams().ok && orth_chol_pair(m0, m1, Q, R, Xinv)) return;
+        if (c.use_subspace && sub_streams().ok && orth_chol_pair(m0, m1, Q, R, Xinv, meanwhile)) return;
         if (Xinv) { Xinv[0].p = nullptr; Xinv[1].p = nullptr; }
         if (c.use_subspace && !sub_streams().ok && orth_chol_pair(m0, m1, Q, R)) return;
         Scope sc(*this);
@@ -672,6 +675,7 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
     const int64_t d1 = a.d[0], d2 = a.d[1], d3 = a.d[2], d4 = a.d[3], chi = a.d[4];
     const int64_t F = d1 * d2 * d3 * d4, J = d2 * d3 * d4;
     Tens QB, RB, QC, RC, XB, XC;      // implicit: QB, QC hold B, C themselves and XB, XC the inverse Cholesky factors
+    Tens btom;                        // B^T Omega^phys [c, be, m], formed ahead while the Cholesky chains run
     bool implicit = false;
     {
         Scope s2(*this);
@@ -683,7 +687,21 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
         Tens cm = perm(view(cc, {d1, J, chi}), {1, 0, 2});             // Eq. A.3 :348  C[(i'),(i1 be)]
         drop(cc);
         Tens Qs[2], Rs[2], Xs[2];
-        orth_pair(view(bm, {J, d1 * chi}), view(cm, {J, d1 * chi}), Qs, Rs, Xs);
+        // While the two Cholesky chains are in flight the caller's stream draws Omega^phys and forms B^T Omega^phys, the part of
+        // the projection Q^B^T Omega^phys = L_B^-1 (B^T Omega^phys) that needs no factor (full rank presumed: n columns; the
+        // result is discarded when the Cholesky path is rejected).
+        std::function<void()> early = [&]() {
+            const int64_t n = d1 * chi, l0 = std::min<int64_t>(c.Dbond + c.p, chi * n);
+            Tens om = make({chi, J, l0});
+            ck(philox_gauss(st, c.seed, (uint32_t)call, 0, 0, chi * J * l0, om.p), "philox");
+            Tens omp = perm(om, {1, 0, 2});
+            drop(om);
+            btom = ein("jc,jbm->cbm", view(bm, {J, n}), omp);
+            drop(omp);
+            detach(btom);
+        };
+        orth_pair(view(bm, {J, d1 * chi}), view(cm, {J, d1 * chi}), Qs, Rs, Xs, &early);
+        if (btom.p) scopes[scopes.size() - 2].push_back(btom.p);      // into bond_swap's scope
         RB = Rs[0]; RC = Rs[1];
         if (Xs[0].p) {
             // Cholesky QR: Q^B = B L_B^-T and Q^C = C L_C^-T are never formed.  They only enter through the products
@@ -704,7 +722,11 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
     const int64_t l = std::min<int64_t>(c.Dbond + c.p, std::min(chi * npc, chi * npb));     // R3: sketch width (fn 9 :381)
     // Omega drawn in the physical basis (be, j', m) and projected on Q^B  (R11, R12)
     Tens omega;
-    {
+    if (implicit && btom.p && btom.d[2] == l) {
+        omega = ein("pc,cBm->Bpm", XB, btom);
+        drop(btom);
+    } else {
+        if (btom.p) drop(btom);
         Scope s2(*this);
         Tens om = make({chi, J, l});
         ck(philox_gauss(st, c.seed, (uint32_t)call, 0, 0, chi * J * l, om.p), "philox");
