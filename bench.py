@@ -71,7 +71,8 @@ class ClockSampler(threading.Thread):
 
 
 # ---- the oracle on a bounded sample (cpu_baseline leg and --impl reference) -------------------------------------------
-MODEL_FLOPS_PER_STEP = 2.385e12    # 2*M*N*K of every contraction of one saturated D=32 step (counted by the library)
+MODEL_FLOPS_PER_STEP = 2.385e12    # 2*M*N*K of every contraction of one saturated D=32 step as the ORACLE performs it (Q^B, Q^C formed
+                                   # explicitly; the library counted this before it made them implicit, it now counts 2.115e12)
 
 
 def oracle_sample(n_slabs=32, seed=0):
@@ -217,22 +218,32 @@ def run_cuda(args):
     sampler.join(timeout=2)
     # ---- profiling pass (not part of `value`): per-launch CUDA events on the library's stream around every DGEMM / permute ----
     t.set_option(T.OPT_STAGE_TIMING, 2)
-    g_ms = g_fl = p_ms = p_by = l_ms = l_fl = 0.0
-    g_n = p_n = l_n = 0
-    stage = None
     n_prof = max(1, min(args.steps, 3))
-    step_ms_prof = 0.0
-    for _ in range(n_prof):
-        t.step()
-        a, b, c = t.gemm_profile()
-        g_ms, g_fl, g_n = g_ms + a, g_fl + b, g_n + c
-        a, b, c = t.gemm_profile_large()
-        l_ms, l_fl, l_n = l_ms + a, l_fl + b, l_n + c
-        a, b, c = t.permute_profile()
-        p_ms, p_by, p_n = p_ms + a, p_by + b, p_n + c
-        sm = t.stage_ms()
-        stage = sm if stage is None else stage + sm
-        step_ms_prof += float(sm.sum())
+
+    def profile_pass():
+        g_ms = g_fl = p_ms = p_by = l_ms = l_fl = 0.0
+        g_n = p_n = l_n = 0
+        stage = None
+        step_ms_prof = 0.0
+        for _ in range(n_prof):
+            t.step()
+            a, b, c = t.gemm_profile()
+            g_ms, g_fl, g_n = g_ms + a, g_fl + b, g_n + c
+            a, b, c = t.gemm_profile_large()
+            l_ms, l_fl, l_n = l_ms + a, l_fl + b, l_n + c
+            a, b, c = t.permute_profile()
+            p_ms, p_by, p_n = p_ms + a, p_by + b, p_n + c
+            sm = t.stage_ms()
+            stage = sm if stage is None else stage + sm
+            step_ms_prof += float(sm.sum())
+        return g_ms, g_fl, g_n, l_ms, l_fl, l_n, p_ms, p_by, p_n, stage, step_ms_prof
+
+    # in situ: the schedule `value` was timed with (solver chains on auxiliary streams beside the contractions)
+    g_ms, g_fl, g_n, l_ms, l_fl, l_n, p_ms, p_by, p_n, stage, step_ms_prof = profile_pass()
+    # alone: the same kernels with every stage on one stream (TATRG_NO_OVERLAP=1), i.e. without other kernels beside them
+    os.environ["TATRG_NO_OVERLAP"] = "1"
+    _, _, _, la_ms, la_fl, _, pa_ms, pa_by, _, _, _ = profile_pass()
+    del os.environ["TATRG_NO_OVERLAP"]
     t.set_option(T.OPT_STAGE_TIMING, 0)
     dmma = T.dmma_issue_rate(20000, 2)
     # ---- max over ranks ----
@@ -255,16 +266,23 @@ def run_cuda(args):
             "model_tflops": g_fl / n_prof / (ms / args.steps * 1e-3) / 1e12,
             "roofline": {"bound": "tensor", "kernel": "dgemm_kernel (DMMA m8n8k4): the %d contraction launches of a step (>= 1e9 flop each, "
                                                       "%.1f%% of the step's DGEMM flops)" % (l_n // n_prof, 100.0 * l_fl / g_fl),
-                         "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": DGEMM_TRAFFIC,
+                         "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf,
+                         "traffic": DGEMM_TRAFFIC["dram_bytes"], "traffic_detail": DGEMM_TRAFFIC,
                          "all_launches": {"launches_per_step": g_n // n_prof, "achieved": all_tf, "frac": all_tf / peak_tf,
                                           "note": "includes the small products of the Cholesky / subspace-iteration solvers, which "
                                                   "run concurrently on several streams: their event times overlap"},
                          "peak_source": "max(register-resident DMMA issue rate measured in this run, MEASURED_PEAKS.json "
                                         "bf16_tflops_sustained (%s) x nominal FP64:bf16 ratio 45/2250)" % pk["src"],
-                         "dmma_issue_rate_tflops": dmma, "derived_peak_tflops": derived_tf, "time_share_of_step": l_ms / step_ms_prof},
+                         "dmma_issue_rate_tflops": dmma, "derived_peak_tflops": derived_tf, "time_share_of_step": l_ms / step_ms_prof,
+                         "schedule": "in situ (solver chains run on auxiliary streams beside some of these launches)",
+                         "alone": {"achieved": la_fl / (la_ms * 1e-3) / 1e12, "frac": la_fl / (la_ms * 1e-3) / 1e12 / peak_tf,
+                                   "schedule": "TATRG_NO_OVERLAP=1: every stage on one stream, no kernel beside them"}},
             "permute": {"bound": "hbm", "achieved": p_by / (p_ms * 1e-3) / 1e9, "peak": pk["hbm"], "unit": "GB/s",
                         "frac": p_by / (p_ms * 1e-3) / 1e9 / pk["hbm"], "launches_per_step": p_n // n_prof,
-                        "time_share_of_step": p_ms / step_ms_prof},
+                        "time_share_of_step": p_ms / step_ms_prof,
+                        "schedule": "in situ (some permutes share HBM with the solver chains on auxiliary streams)",
+                        "alone": {"achieved": pa_by / (pa_ms * 1e-3) / 1e9, "frac": pa_by / (pa_ms * 1e-3) / 1e9 / pk["hbm"],
+                                  "schedule": "TATRG_NO_OVERLAP=1: every stage on one stream, no kernel beside them"}},
             "stage_ms": {k: round(float(v) / n_prof, 2) for k, v in zip(T.STAGES, stage) if not k.startswith("_")},
         }
         if world == 1:

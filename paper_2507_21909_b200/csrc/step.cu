@@ -615,6 +615,8 @@ struct Stepper {
     void decompose(Tens& a, Tens& dt, Tens& core);
     void bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x, Tens& y, double*& sig, int& gr);
     void triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y, const double* sig, Tens U[4], Tens& e, Tens& f, Tens& g, Tens& h);
+    void triad_grams(const Tens& aa, const Tens& xx, const double* sig, Tens& ga, Tens& gx);
+    void triad_isos(Tens gram[4], const std::vector<int>& which, int64_t d2, int64_t d3, Tens U[4]);
     void half_grams(const Tens& P, const Tens& Q, const Tens& Iu, const Tens& Jl, Tens th[3]);
     void squeezers(Tens thf[3], Tens thb[3], const int du[3], Tens Mt[3], Tens Nt[3], int dmask = 7);
     void half_grams4(const Tens& P, const Tens& Q, Tens th[3]);
@@ -804,85 +806,92 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
 
 // (c) Eq. 2.9 :135 (canonical form :137) and Eq. 2.10-2.17 :147-167.
 // U[0..3] = U^A, U^X, U^Y, U^D stored [k, leg2, leg3]; E[i1,kA,i4,al], F[al,kX,i4,g] (carries sigma), G[be,kY,j4,g], H[j1,kD,j4,be].
+// Gram matrices of one side on the leg pair (2,3): side 0: xx = X, aa = A -> ga = G^A, gx = G^X; side 1: xx = Y, aa = Dt -> G^D, G^Y.
+void Stepper::triad_grams(const Tens& aa, const Tens& xx, const double* sig, Tens& ga, Tens& gx) {
+    Scope s2(*this);
+    const int64_t d1 = aa.d[0], d2 = aa.d[1], d3 = aa.d[2], d4 = aa.d[3], chi = aa.d[4], gr = xx.d[4];
+    const int64_t n = d2 * d3, J = d2 * d3 * d4;
+    Tens xs = make({chi, d2, d3, d4, gr});
+    ck(scale_last(st, xs.p, xx.p, sig, chi * J, gr, 0), "scale");
+    // G^X[(i2 i3),(i2' i3')] = sum_{al,i4,g} Xs Xs
+    Tens xp = perm(xs, {0, 3, 4, 1, 2});
+    gx = mm(true, false, n, n, chi * d4 * gr, xp.p, n, xp.p, n, true);
+    drop(xp);
+    // kappa[al,al'] = sum_{i',g} Xs Xs ;  G^A = sum_{i1,i4,al,al'} A kappa A
+    Tens ka = mm(false, true, chi, chi, J * gr, xs.p, J * gr, xs.p, J * gr);
+    drop(xs);
+    Tens ta = mm(false, false, d1 * J, chi, chi, aa.p, chi, ka.p, chi);
+    Tens ap = perm(aa, {0, 3, 4, 1, 2});
+    Tens tp = perm(view(ta, {d1, d2, d3, d4, chi}), {0, 3, 4, 1, 2});
+    drop(ta);
+    ga = mm(true, false, n, n, d1 * d4 * chi, ap.p, n, tp.p, n, true);      // A kappa A: symmetric because kappa is
+    keep(ga); keep(gx);
+}
+
+// Isometries U[i] (rows: the leading eigenvectors, [k, d2, d3]) of the Gram matrices gram[i], i in `which` (0..3 = A, X, Y, D).
+void Stepper::triad_isos(Tens gram[4], const std::vector<int>& which, int64_t d2, int64_t d3, Tens U[4]) {
+    Scope s2(*this);
+    const int64_t n = d2 * d3;
+    const int kmax = (int)std::min<int64_t>(c.Ktri, n);
+    const double eps_sv = std::sqrt(kEpsLambda);
+    bool have[4] = {false, false, false, false};
+    if (c.use_subspace && sub_applicable((int)n, kmax)) {
+        // top-K eigenvectors by subspace iteration + one b x b Rayleigh-Ritz problem per Gram matrix
+        std::vector<SubProb> ps(which.size());
+        for (size_t j = 0; j < which.size(); ++j) {
+            const int i = which[j];
+            ck(symmetrize(st, (int)n, gram[i].p), "symmetrize");
+            ps[j].Bm = gram[i].p; ps[j].F = nullptr; ps[j].n = (int)n; ps[j].kmax = kmax; ps[j].b = sub_block((int)n, kmax); ps[j].sid = 16 + i;
+        }
+        const bool vb = getenv("TATRG_SUB_VERBOSE") != nullptr;
+        auto now = [&]() { cudaStreamSynchronize(st); return std::chrono::steady_clock::now(); };
+        auto t0 = vb ? now() : std::chrono::steady_clock::time_point();
+        sub_iterate(ps);
+        auto t1 = vb ? now() : t0;
+        std::vector<Tens*> hs; std::vector<int> ns, who;
+        for (size_t j = 0; j < ps.size(); ++j) if (ps[j].ok) { hs.push_back(&ps[j].H); ns.push_back(ps[j].b); who.push_back((int)j); }
+        std::vector<EigOut> er;
+        if (!hs.empty()) eig_batch(hs, ns, er);
+        if (vb) { auto t2 = now(); fprintf(stderr, "[tatrg triad] subspace iterations %.2f ms, Rayleigh-Ritz %.2f ms\n", std::chrono::duration<double, std::milli>(t1 - t0).count(), std::chrono::duration<double, std::milli>(t2 - t1).count()); }
+        for (size_t j = 0; j < who.size(); ++j) {
+            const int pj = who[j], i = which[pj], b = ps[pj].b;
+            std::vector<double> sv(b);
+            for (int t = 0; t < b; ++t) sv[t] = std::sqrt(std::max(er[j].lh[t], 0.0));
+            if (!(sv[kmax] > eps_sv * sv[0])) continue;              // numerical rank <= kmax: the full decomposition decides
+            const int k = select_rank(sv, kmax, eps_sv, c.tau);
+            if (k <= 0) continue;
+            U[i] = mm(false, true, k, n, b, er[j].Vt.p, b, ps[pj].Z(), b);     // rows: Ritz vectors Y_k^T Z^T
+            U[i] = view(U[i], {k, d2, d3});
+            keep(U[i]);
+            have[i] = true;
+        }
+    }
+    std::vector<Tens*> gs; std::vector<int> ns, who;
+    for (int i : which) if (!have[i]) { gs.push_back(&gram[i]); ns.push_back((int)n); who.push_back(i); }
+    std::vector<EigOut> eo;
+    if (!gs.empty()) eig_batch(gs, ns, eo);
+    for (size_t j = 0; j < who.size(); ++j) {
+        const int i = who[j];
+        const std::vector<double>& lh = eo[j].lh;
+        std::vector<double> sv(lh.size());
+        for (size_t t = 0; t < lh.size(); ++t) sv[t] = std::sqrt(std::max(lh[t], 0.0));    // multiplet rule on the singular-value scale
+        const int k = select_rank(sv, kmax, eps_sv, c.tau);
+        if (k <= 0) fail(TATRG_ENUMERIC, "triad: empty isometry");
+        U[i] = make({k, d2, d3});
+        ck(cudaMemcpyAsync(U[i].p, eo[j].Vt.p, 8 * (int64_t)k * n, cudaMemcpyDeviceToDevice, st), "copy"); count_launch();
+        keep(U[i]);
+    }
+}
+
 void Stepper::triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y, const double* sig, Tens U[4], Tens& e, Tens& f,
                     Tens& g, Tens& h) {
     Scope sc(*this);
-    const int64_t d1 = a.d[0], d2 = a.d[1], d3 = a.d[2], d4 = a.d[3], chi = a.d[4], gr = x.d[4];
-    const int64_t n = d2 * d3, J = d2 * d3 * d4;
+    const int64_t gr = x.d[4];
     Tens gram[4];
-    for (int side = 0; side < 2; ++side) {      // side 0: X and A,  side 1: Y and Dt
-        Scope s2(*this);
-        const Tens& xx = side == 0 ? x : y;
-        const Tens& aa = side == 0 ? a : dt;
-        Tens xs = make({chi, d2, d3, d4, gr});
-        ck(scale_last(st, xs.p, xx.p, sig, chi * J, gr, 0), "scale");
-        // G^X[(i2 i3),(i2' i3')] = sum_{al,i4,g} Xs Xs
-        Tens xp = perm(xs, {0, 3, 4, 1, 2});
-        Tens gx = mm(true, false, n, n, chi * d4 * gr, xp.p, n, xp.p, n, true);
-        drop(xp);
-        // kappa[al,al'] = sum_{i',g} Xs Xs ;  G^A = sum_{i1,i4,al,al'} A kappa A
-        Tens ka = mm(false, true, chi, chi, J * gr, xs.p, J * gr, xs.p, J * gr);
-        drop(xs);
-        Tens ta = mm(false, false, d1 * J, chi, chi, aa.p, chi, ka.p, chi);
-        Tens ap = perm(aa, {0, 3, 4, 1, 2});
-        Tens tp = perm(view(ta, {d1, d2, d3, d4, chi}), {0, 3, 4, 1, 2});
-        drop(ta);
-        Tens ga = mm(true, false, n, n, d1 * d4 * chi, ap.p, n, tp.p, n, true);      // A kappa A: symmetric because kappa is
-        gram[side == 0 ? 0 : 3] = ga; gram[side == 0 ? 1 : 2] = gx;
-        keep(ga); keep(gx);
-    }
-    {
-        Scope s2(*this);
-        const int kmax = (int)std::min<int64_t>(c.Ktri, n);
-        const double eps_sv = std::sqrt(kEpsLambda);
-        bool have[4] = {false, false, false, false};
-        if (c.use_subspace && sub_applicable((int)n, kmax)) {
-            // top-K eigenvectors by subspace iteration + one b x b Rayleigh-Ritz problem per Gram matrix
-            std::vector<SubProb> ps(4);
-            for (int i = 0; i < 4; ++i) {
-                ck(symmetrize(st, (int)n, gram[i].p), "symmetrize");
-                ps[i].Bm = gram[i].p; ps[i].F = nullptr; ps[i].n = (int)n; ps[i].kmax = kmax; ps[i].b = sub_block((int)n, kmax); ps[i].sid = 16 + i;
-            }
-            const bool vb = getenv("TATRG_SUB_VERBOSE") != nullptr;
-            auto now = [&]() { cudaStreamSynchronize(st); return std::chrono::steady_clock::now(); };
-            auto t0 = vb ? now() : std::chrono::steady_clock::time_point();
-            sub_iterate(ps);
-            auto t1 = vb ? now() : t0;
-            std::vector<Tens*> hs; std::vector<int> ns, who;
-            for (int i = 0; i < 4; ++i) if (ps[i].ok) { hs.push_back(&ps[i].H); ns.push_back(ps[i].b); who.push_back(i); }
-            std::vector<EigOut> er;
-            if (!hs.empty()) eig_batch(hs, ns, er);
-            if (vb) { auto t2 = now(); fprintf(stderr, "[tatrg triad] subspace iterations %.2f ms, Rayleigh-Ritz %.2f ms\n", std::chrono::duration<double, std::milli>(t1 - t0).count(), std::chrono::duration<double, std::milli>(t2 - t1).count()); }
-            for (size_t j = 0; j < who.size(); ++j) {
-                const int i = who[j], b = ps[i].b;
-                std::vector<double> sv(b);
-                for (int t = 0; t < b; ++t) sv[t] = std::sqrt(std::max(er[j].lh[t], 0.0));
-                if (!(sv[kmax] > eps_sv * sv[0])) continue;              // numerical rank <= kmax: the full decomposition decides
-                const int k = select_rank(sv, kmax, eps_sv, c.tau);
-                if (k <= 0) continue;
-                U[i] = mm(false, true, k, n, b, er[j].Vt.p, b, ps[i].Z(), b);     // rows: Ritz vectors Y_k^T Z^T
-                U[i] = view(U[i], {k, d2, d3});
-                keep(U[i]);
-                have[i] = true;
-            }
-        }
-        std::vector<Tens*> gs; std::vector<int> ns, who;
-        for (int i = 0; i < 4; ++i) if (!have[i]) { gs.push_back(&gram[i]); ns.push_back((int)n); who.push_back(i); }
-        std::vector<EigOut> eo;
-        if (!gs.empty()) eig_batch(gs, ns, eo);
-        for (size_t j = 0; j < who.size(); ++j) {
-            const int i = who[j];
-            const std::vector<double>& lh = eo[j].lh;
-            std::vector<double> sv(lh.size());
-            for (size_t t = 0; t < lh.size(); ++t) sv[t] = std::sqrt(std::max(lh[t], 0.0));    // multiplet rule on the singular-value scale
-            const int k = select_rank(sv, kmax, eps_sv, c.tau);
-            if (k <= 0) fail(TATRG_ENUMERIC, "triad: empty isometry");
-            U[i] = make({k, d2, d3});
-            ck(cudaMemcpyAsync(U[i].p, eo[j].Vt.p, 8 * (int64_t)k * n, cudaMemcpyDeviceToDevice, st), "copy"); count_launch();
-            keep(U[i]);
-        }
-        for (int i = 0; i < 4; ++i) drop(gram[i]);
-    }
+    triad_grams(a, x, sig, gram[0], gram[1]);
+    triad_grams(dt, y, sig, gram[3], gram[2]);
+    triad_isos(gram, {0, 1, 2, 3}, a.d[1], a.d[2], U);
+    for (int i = 0; i < 4; ++i) drop(gram[i]);
     if (submark) submark();                                                // end of TATRG_ST_TRIAD_ISO
     e = ein("mjk,Ijkla->Imla", U[0], a);                                   // Eq. 2.10
     Tens f0 = ein("xjk,Ajklg->Axlg", U[1], x);                             // Eq. 2.11 (sigma goes into F only)
@@ -1150,16 +1159,8 @@ void Stepper::run() {
         drop(dt);
         mark();
     } else {
-        Tens U[4], e, f, g, h;
-        submark = mark;
-        triad(a, dt, x, y, sig, U, e, f, g, h);                         // (c)
-        submark = nullptr;
-        save("E", e); save("F", f); save("G", g); save("H", h);
-        save("UA", U[0]); save("UX", U[1]); save("UY", U[2]); save("UD", U[3]);
-        drop(a); drop(dt); drop(core); drop(x); drop(y);
-        mark();
         const int du[3] = {(int)c.phi.d[1], (int)c.phi.d[2], (int)c.phi.d[3]};
-        Tens thf[3], thb[3], Mt[3], Nt[3];
+        Tens U[4], e, f, g, h, thf[3], thb[3], Mt[3], Nt[3];
         // Overlapped schedule (saturated steps): the squeezers are chains of small launches with host decisions in between
         // (subspace iteration, Rayleigh-Ritz) that leave the SMs almost idle.  Direction 4 is the only one the Xi products of
         // Eq. 2.18-2.19 need, so: Gram matrices of direction 4 | squeezer 4 on the auxiliary stream q while the caller's stream
@@ -1174,7 +1175,8 @@ void Stepper::run() {
             const size_t n = (size_t)std::max(du[0], std::max(du[1], du[2])); const size_t n2 = n * n;
             arena_bytes = 8 * (64 * n2 * n2 + (2u << 20));
             // both Xi tensors are alive at once in this schedule; leave the arena's size again as headroom
-            const size_t xi_bytes = 8 * (size_t)(e.d[0] * e.d[1] * f.d[1] * f.d[3]) * (size_t)c.D;
+            const size_t kt = (size_t)std::min<int64_t>(c.Ktri, a.d[1] * a.d[2]);
+            const size_t xi_bytes = 8 * (size_t)a.d[0] * kt * kt * (size_t)x.d[4] * (size_t)c.D;
             if (c.pool.in_use() + 2 * arena_bytes + 3 * xi_bytes <= c.pool.capacity())
                 arena = c.pool.alloc((int64_t)(arena_bytes / 8));   // freed at the end of the step, after the joins
             if (!arena) overlap = false;
@@ -1186,14 +1188,28 @@ void Stepper::run() {
             ArenaGuard(tatrg_ctx& c_, Pool& o) : c(c_), other(o) { std::swap(other, c.pool); }
             ~ArenaGuard() { std::swap(other, c.pool); }
         };
-        auto on_q = [&](cudaEvent_t after, int dmask) {      // squeezers of the directions in dmask on stream q, after event `after`
+        auto on_stream_q = [&](cudaEvent_t after, const std::function<void(Stepper&)>& body) {   // body on stream q after event `after`; ends with joinq
             ArenaGuard guard(c, arena_pool);
             Stepper sq(c, ss.q);
             ck(cudaStreamWaitEvent(ss.q, after, 0), "wait");
-            sq.squeezers(thf, thb, du, Mt, Nt, dmask);
-            for (int d = 0; d < 3; ++d) if ((dmask >> d) & 1) { sq.detach(Mt[d]); sq.detach(Nt[d]); }
+            body(sq);
             ck(cudaEventRecord(ss.joinq, ss.q), "event");
         };
+        auto on_q = [&](cudaEvent_t after, int dmask) {      // squeezers of the directions in dmask
+            on_stream_q(after, [&](Stepper& sq) {
+                sq.squeezers(thf, thb, du, Mt, Nt, dmask);
+                for (int d = 0; d < 3; ++d) if ((dmask >> d) & 1) { sq.detach(Mt[d]); sq.detach(Nt[d]); }
+            });
+        };
+        // (The triad stage itself is not overlapped: splitting its four subspace iterations into two pairs, the second one hidden
+        // behind E, F and the Gram matrices of the upper half, was measured slower -- a pair of chains takes as long as all four.)
+        submark = mark;
+        triad(a, dt, x, y, sig, U, e, f, g, h);                         // (c)
+        submark = nullptr;
+        mark();
+        save("E", e); save("F", f); save("G", g); save("H", h);
+        save("UA", U[0]); save("UX", U[1]); save("UY", U[2]); save("UD", U[3]);
+        drop(a); drop(dt); drop(core); drop(x); drop(y);
         // (d) squeezer Gram matrices of the upper half (E F I J) and of the sigma-weighted lower half (G sigma, H, K, L)
         Tens P, Q;
         {

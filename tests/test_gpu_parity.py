@@ -409,3 +409,27 @@ def test_subspace_path_falls_back_on_rank_deficient_blocks(D, beta, h, steps):
         t.close()
     for a, b in zip(*runs):
         assert np.isfinite(a) and abs(a - b) <= 1e-11 * abs(b)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("D,steps", [(16, 10), (32, 8)])
+def test_overlapped_schedule_equals_the_serial_one(D, steps, monkeypatch):
+    """Saturated steps run the squeezer chains on an auxiliary stream beside the Gram matrices and the Xi products of
+    Eq. 2.18-2.19 (schedule).  TATRG_NO_OVERLAP=1 issues the same work on one stream: the results
+    are the same numbers (no arithmetic differs, only what runs beside what; the bound leaves room for nothing but that)."""
+    runs = []
+    for serial in (False, True):
+        if serial:
+            monkeypatch.setenv("TATRG_NO_OVERLAP", "1")
+        else:
+            monkeypatch.delenv("TATRG_NO_OVERLAP", raising=False)
+        t = T.Tatrg(0.1497, 0.0, D, D, 5)
+        out = []
+        for _ in range(steps):
+            t.step()
+            out.append((t.lnZ_per_site(), t.singular_values(T.SV_SIGMA, D), t.singular_values(T.SV_S, D)))
+        runs.append(out)
+        t.close()
+    for a, b in zip(*runs):
+        assert abs(a[0] - b[0]) <= 1e-13 * abs(b[0])
+        assert np.abs(a[1] - b[1]).max() <= 1e-12 and np.abs(a[2] - b[2]).max() <= 1e-12
