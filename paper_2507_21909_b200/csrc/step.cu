@@ -1188,18 +1188,13 @@ void Stepper::run() {
             ArenaGuard(tatrg_ctx& c_, Pool& o) : c(c_), other(o) { std::swap(other, c.pool); }
             ~ArenaGuard() { std::swap(other, c.pool); }
         };
-        auto on_stream_q = [&](cudaEvent_t after, const std::function<void(Stepper&)>& body) {   // body on stream q after event `after`; ends with joinq
+        auto on_q = [&](cudaEvent_t after, int dmask) {      // squeezers of the directions in dmask on stream q after event `after`; ends with joinq
             ArenaGuard guard(c, arena_pool);
             Stepper sq(c, ss.q);
             ck(cudaStreamWaitEvent(ss.q, after, 0), "wait");
-            body(sq);
+            sq.squeezers(thf, thb, du, Mt, Nt, dmask);
+            for (int d = 0; d < 3; ++d) if ((dmask >> d) & 1) { sq.detach(Mt[d]); sq.detach(Nt[d]); }
             ck(cudaEventRecord(ss.joinq, ss.q), "event");
-        };
-        auto on_q = [&](cudaEvent_t after, int dmask) {      // squeezers of the directions in dmask
-            on_stream_q(after, [&](Stepper& sq) {
-                sq.squeezers(thf, thb, du, Mt, Nt, dmask);
-                for (int d = 0; d < 3; ++d) if ((dmask >> d) & 1) { sq.detach(Mt[d]); sq.detach(Nt[d]); }
-            });
         };
         // (The triad stage itself is not overlapped: splitting its four subspace iterations into two pairs, the second one hidden
         // behind E, F and the Gram matrices of the upper half, was measured slower -- a pair of chains takes as long as all four.)
