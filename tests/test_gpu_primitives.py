@@ -72,6 +72,28 @@ def test_dgemm_batched_alpha_beta(torch):
     assert np.abs(C.cpu().numpy() - ref).max() <= 8 * EPS * 40 * 25
 
 
+@pytest.mark.parametrize("M,N,K", [(1666, 1538, 70), (2050, 1300, 16), (1280, 1920, 130)])
+@pytest.mark.parametrize("ta,tb", [(False, False), (True, False), (False, True), (True, True)])
+def test_dgemm_multiwave(torch, M, N, K, ta, tb):
+    """More than 148 tiles of 128 x 128 (several waves of CTAs) with 16-byte-aligned operands: ragged last tiles in M and N, K not a
+    multiple of the 16-deep k-step, a K of exactly one k-step (shorter than the cp.async pipeline)."""
+    a = inputs.random_tensor((M, K), 11)
+    b = inputs.random_tensor((K, N), 12)
+    ref = a @ b
+    C = T.dgemm(dev(torch, a.T if ta else a), dev(torch, b.T if tb else b), transa=ta, transb=tb).cpu().numpy()
+    assert np.abs(C - ref).max() <= 8 * EPS * K * np.abs(a).max() * np.abs(b).max()
+
+
+def test_dgemm_multiwave_batched_alpha_beta(torch):
+    a = inputs.random_tensor((3, 1100, 48), 13)
+    b = inputs.random_tensor((3, 48, 1000), 14)
+    c0 = inputs.random_tensor((3, 1100, 1000), 15)
+    C = dev(torch, c0)
+    T.dgemm(dev(torch, a), dev(torch, b), alpha=-1.5, beta=0.25, C=C)
+    ref = -1.5 * np.einsum("bik,bkj->bij", a, b) + 0.25 * c0
+    assert np.abs(C.cpu().numpy() - ref).max() <= 8 * EPS * 48 * np.abs(a).max() * np.abs(b).max() * 2
+
+
 # ---- permute ------------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("shape,perm", [((3, 5, 7, 4, 6), (1, 2, 3, 0, 4)), ((3, 5, 7, 4, 6), (4, 3, 2, 1, 0)), ((33, 65), (1, 0)),
                                         ((2, 2, 2, 2, 2), (1, 2, 3, 0, 4)), ((8, 8, 8, 8, 8), (0, 3, 4, 1, 2)), ((1, 7, 1, 5), (3, 2, 1, 0)),
