@@ -25,6 +25,7 @@ if ROOT not in sys.path:
 
 BETA, H, D, P, N_POW, SEED = 0.1497, 0.0, 32, 32, 2, 42
 PRE_STEPS = 5                      # legs grow 2 -> 4 -> 16 -> 32: saturated from step 6 on
+FULL_RUN_STEPS = 60                # configs[3]: 2^15 per axis
 METRIC = "sec_per_coarse_graining_step_D32"
 UNIT = "s/step"
 WORKLOAD = "configs[3]: 4D Ising beta=0.1497 h=0, Triad-ATRG D=32 p=32 (K=l=64), 2 power iterations, Philox seed 42, saturated steps"
@@ -41,33 +42,63 @@ def peaks():
 
 
 class ClockSampler(threading.Thread):
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    """SM clock and throttle reasons during the timed region (B200_PROFILING.md), read through NVML in-process (a query costs
+    microseconds; spawning nvidia-smi several times inside a 0.4 s timed region perturbs the host-driven launches).  Falls back to
+    nvidia-smi when the NVML binding is missing."""
 
     def __init__(self, index):
         super().__init__(daemon=True)
         self.index, self.samples, self.reasons, self.stop_flag = index, [], set(), False
         self.max_mhz = None
+        self.nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            # LOCAL_RANK indexes CUDA_VISIBLE_DEVICES, NVML indexes the physical devices
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and all(x.strip().isdigit() for x in vis.split(",")) else index
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.nvml = pynvml
+        except Exception:
+            self.nvml = None
 
-    def run(self):
+    def sample_nvml(self):
+        n = self.nvml
+        self.samples.append(float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM)))
+        self.max_mhz = float(n.nvmlDeviceGetMaxClockInfo(self.handle, n.NVML_CLOCK_SM))
+        r = n.nvmlDeviceGetCurrentClocksEventReasons(self.handle) if hasattr(n, "nvmlDeviceGetCurrentClocksEventReasons") \
+            else n.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle)
+        for name, bit in (("hw_slowdown", 0x8), ("hw_thermal_slowdown", 0x40), ("sw_thermal_slowdown", 0x20), ("sw_power_cap", 0x4)):
+            if r & bit:
+                self.reasons.add(name)
+
+    def sample_smi(self):
         q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q, "--format=csv,noheader,nounits"],
+                             capture_output=True, text=True, timeout=5).stdout.strip().split(",")
+        self.samples.append(float(out[0]))
+        self.max_mhz = float(out[1])
+        for n, v in zip(names, out[2:]):
+            if v.strip().lower().startswith("active"):
+                self.reasons.add(n)
+
+    def run(self):
         while not self.stop_flag:
             try:
-                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q, "--format=csv,noheader,nounits"],
-                                     capture_output=True, text=True, timeout=5).stdout.strip().split(",")
-                self.samples.append(float(out[0]))
-                self.max_mhz = float(out[1])
-                for n, v in zip(names, out[2:]):
-                    if v.strip().lower().startswith("active"):
-                        self.reasons.add(n)
+                if self.nvml:
+                    self.sample_nvml()
+                else:
+                    self.sample_smi()
             except Exception:
                 pass
-            time.sleep(0.2)
+            time.sleep(0.05 if self.nvml else 0.2)
 
     def summary(self):
         s = sorted(self.samples)
-        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s), "source": "nvml" if self.nvml else "nvidia-smi"}
 
 
 # ---- the oracle on a bounded sample (cpu_baseline leg and --impl reference) -------------------------------------------
@@ -187,14 +218,17 @@ def run_cuda(args):
     # ---- timed region 1: K steps, state resident in HBM ----
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches = 0
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]      # per-step split of the same region (diagnostic)
     barrier()
     ev0.record()
-    for _ in range(args.steps):
+    for i in range(args.steps):
         t.step()
         launches += t.launches()
+        marks[i].record()
     ev1.record()
     barrier()
     ms = ev0.elapsed_time(ev1)
+    step_ms = [([ev0] + marks)[i].elapsed_time(marks[i]) for i in range(args.steps)]
     lnz = t.lnZ_per_site()
     # ---- timed region 2: end to end through the C ABI with host buffers ----
     n5 = D ** 5
@@ -246,6 +280,20 @@ def run_cuda(args):
     del os.environ["TATRG_NO_OVERLAP"]
     t.set_option(T.OPT_STAGE_TIMING, 0)
     dmma = T.dmma_issue_rate(20000, 2)
+    # ---- the whole run of configs[3] (60 steps from the initial tensor), not part of `value`: total run time (north_star) ----
+    # After the flow has left criticality (step ~20 at this beta) the local tensor is numerically rank-deficient and the
+    # rank-revealing full decompositions replace Cholesky QR / subspace iteration: those steps are slower.
+    t.close()
+    t = T.Tatrg(BETA, H, D, P, SEED + rank, power_iters=N_POW, device="cuda:%d" % local)
+    per_step = []
+    for _ in range(FULL_RUN_STEPS):
+        ev0.record()
+        t.step()
+        ev1.record()
+        ev1.synchronize()
+        per_step.append(ev0.elapsed_time(ev1) * 1e-3)
+    lnz_full = t.lnZ_per_site()
+    sat = sorted(per_step[PRE_STEPS:])
     # ---- max over ranks ----
     ms, ms_e2e = max_over_ranks([ms, ms_e2e], "cuda")
     if rank == 0:
@@ -262,7 +310,7 @@ def run_cuda(args):
             "data": "synthetic", "config": {"workload": WORKLOAD, "parallelism": "replicas" if world > 1 else "single",
                                             "l2": "inputs_exceed_l2 (state 2 x 268 MB, Xi 1.07 GB vs 126 MB L2)", "pre_steps": PRE_STEPS},
             "e2e": {"value": sec_e2e, "unit": UNIT, "h2d_bytes_per_step": 16 * n5, "d2h_bytes_per_step": 16 * n5 + 8 * (1 + D), "steps": k_e2e},
-            "gpu_launches": launches, "lnZ_per_site": lnz, "clocks": sampler.summary(),
+            "gpu_launches": launches, "lnZ_per_site": lnz, "clocks": sampler.summary(), "step_ms": [round(x, 2) for x in step_ms],
             "model_tflops": g_fl / n_prof / (ms / args.steps * 1e-3) / 1e12,
             "roofline": {"bound": "tensor", "kernel": "dgemm_kernel (DMMA m8n8k4): the %d contraction launches of a step (>= 1e9 flop each, "
                                                       "%.1f%% of the step's DGEMM flops)" % (l_n // n_prof, 100.0 * l_fl / g_fl),
@@ -284,6 +332,11 @@ def run_cuda(args):
                         "alone": {"achieved": pa_by / (pa_ms * 1e-3) / 1e9, "frac": pa_by / (pa_ms * 1e-3) / 1e9 / pk["hbm"],
                                   "schedule": "TATRG_NO_OVERLAP=1: every stage on one stream, no kernel beside them"}},
             "stage_ms": {k: round(float(v) / n_prof, 2) for k, v in zip(T.STAGES, stage) if not k.startswith("_")},
+            "full_run": {"steps": FULL_RUN_STEPS, "seconds": sum(per_step), "mean_s_per_step": sum(per_step) / len(per_step),
+                         "median_s_per_step_saturated": sat[len(sat) // 2], "min_s_per_step_saturated": sat[0], "max_s_per_step": max(per_step),
+                         "lnZ_per_site": lnz_full,
+                         "note": "configs[3] from the initial tensor on rank 0's replica; steps after the flow leaves criticality run "
+                                 "rank-revealing full decompositions (numerically rank-deficient tensors) and are slower than `value`"},
         }
         if world == 1:
             v, dt, fl, threads = oracle_sample(32)
