@@ -255,8 +255,8 @@ def run_cuda(args):
     n_prof = max(1, min(args.steps, 3))
 
     def profile_pass():
-        g_ms = g_fl = p_ms = p_by = l_ms = l_fl = 0.0
-        g_n = p_n = l_n = 0
+        g_ms = g_fl = p_ms = p_by = l_ms = l_fl = q_ms = q_by = 0.0
+        g_n = p_n = l_n = q_n = 0
         stage = None
         step_ms_prof = 0.0
         for _ in range(n_prof):
@@ -267,16 +267,18 @@ def run_cuda(args):
             l_ms, l_fl, l_n = l_ms + a, l_fl + b, l_n + c
             a, b, c = t.permute_profile()
             p_ms, p_by, p_n = p_ms + a, p_by + b, p_n + c
+            a, b, c = t.permute_profile_large()
+            q_ms, q_by, q_n = q_ms + a, q_by + b, q_n + c
             sm = t.stage_ms()
             stage = sm if stage is None else stage + sm
             step_ms_prof += float(sm.sum())
-        return g_ms, g_fl, g_n, l_ms, l_fl, l_n, p_ms, p_by, p_n, stage, step_ms_prof
+        return g_ms, g_fl, g_n, l_ms, l_fl, l_n, p_ms, p_by, p_n, stage, step_ms_prof, q_ms, q_by, q_n
 
     # in situ: the schedule `value` was timed with (solver chains on auxiliary streams beside the contractions)
-    g_ms, g_fl, g_n, l_ms, l_fl, l_n, p_ms, p_by, p_n, stage, step_ms_prof = profile_pass()
+    g_ms, g_fl, g_n, l_ms, l_fl, l_n, p_ms, p_by, p_n, stage, step_ms_prof, q_ms, q_by, q_n = profile_pass()
     # alone: the same kernels with every stage on one stream (TATRG_NO_OVERLAP=1), i.e. without other kernels beside them
     os.environ["TATRG_NO_OVERLAP"] = "1"
-    _, _, _, la_ms, la_fl, _, pa_ms, pa_by, _, _, _ = profile_pass()
+    _, _, _, la_ms, la_fl, _, pa_ms, pa_by, _, _, _, qa_ms, qa_by, _ = profile_pass()
     del os.environ["TATRG_NO_OVERLAP"]
     t.set_option(T.OPT_STAGE_TIMING, 0)
     dmma = T.dmma_issue_rate(20000, 2)
@@ -330,7 +332,12 @@ def run_cuda(args):
                         "time_share_of_step": p_ms / step_ms_prof,
                         "schedule": "in situ (some permutes share HBM with the solver chains on auxiliary streams)",
                         "alone": {"achieved": pa_by / (pa_ms * 1e-3) / 1e9, "frac": pa_by / (pa_ms * 1e-3) / 1e9 / pk["hbm"],
-                                  "schedule": "TATRG_NO_OVERLAP=1: every stage on one stream, no kernel beside them"}},
+                                  "schedule": "TATRG_NO_OVERLAP=1: every stage on one stream, no kernel beside them"},
+                        "large": {"what": "the %d permutes of a step that move >= 100 MB (tensors larger than L2: the D^5 operands); the other "
+                                          "launches are L2-resident permutes of ~10 us, where the events around a launch cost as much as the "
+                                          "launch" % (q_n // n_prof),
+                                  "bytes_share": q_by / p_by, "achieved": q_by / (q_ms * 1e-3) / 1e9, "frac": q_by / (q_ms * 1e-3) / 1e9 / pk["hbm"],
+                                  "alone": {"achieved": qa_by / (qa_ms * 1e-3) / 1e9, "frac": qa_by / (qa_ms * 1e-3) / 1e9 / pk["hbm"]}}},
             "stage_ms": {k: round(float(v) / n_prof, 2) for k, v in zip(T.STAGES, stage) if not k.startswith("_")},
             "full_run": {"steps": FULL_RUN_STEPS, "seconds": sum(per_step), "mean_s_per_step": sum(per_step) / len(per_step),
                          "median_s_per_step_saturated": sat[len(sat) // 2], "min_s_per_step_saturated": sat[0], "max_s_per_step": max(per_step),

@@ -109,6 +109,9 @@ int tatrg_gemm_profile(tatrg_handle, double* ms, double* flops, long long* calls
  * A.2-A.11), without the small products inside the Cholesky / subspace-iteration solvers.  Needs STAGE_TIMING=2. */
 int tatrg_gemm_profile_large(tatrg_handle, double* ms, double* flops, long long* calls);
 int tatrg_permute_profile(tatrg_handle, double* ms, double* bytes, long long* calls);
+/* The same restricted to the permutes that move >= 100 MB (read + written): tensors larger than L2, the D^5 operands of the
+ * saturated steps (Eq. A.2-A.3 :345-348 layouts, the leg pair of Eq. 2.9 :135, the axis rotation of Fig. 5(f)).  Needs STAGE_TIMING=2. */
+int tatrg_permute_profile_large(tatrg_handle, double* ms, double* bytes, long long* calls);
 /* high-water mark (bytes) of the workspace since tatrg_create */
 size_t tatrg_workspace_peak(tatrg_handle);
 

@@ -43,6 +43,7 @@ _SIGNATURES = {
     "tatrg_gemm_profile": (_c.c_int, [_c.c_void_p, _dp, _dp, _c.POINTER(_c.c_longlong)]),
     "tatrg_gemm_profile_large": (_c.c_int, [_c.c_void_p, _dp, _dp, _c.POINTER(_c.c_longlong)]),
     "tatrg_permute_profile": (_c.c_int, [_c.c_void_p, _dp, _dp, _c.POINTER(_c.c_longlong)]),
+    "tatrg_permute_profile_large": (_c.c_int, [_c.c_void_p, _dp, _dp, _c.POINTER(_c.c_longlong)]),
     "tatrg_workspace_peak": (_c.c_size_t, [_c.c_void_p]),
     "tatrg_get_tensor": (_c.c_longlong, [_c.c_void_p, _c.c_char_p, _dp, _c.c_longlong, _c.POINTER(_c.c_int),
                                          _c.POINTER(_c.c_longlong)]),
@@ -207,6 +208,11 @@ class Tatrg:
     def permute_profile(self):
         ms, by, n = ctypes.c_double(), ctypes.c_double(), ctypes.c_longlong()
         _check(lib().tatrg_permute_profile(self._h, ctypes.byref(ms), ctypes.byref(by), ctypes.byref(n)), "tatrg_permute_profile")
+        return ms.value, by.value, n.value
+
+    def permute_profile_large(self):
+        ms, by, n = ctypes.c_double(), ctypes.c_double(), ctypes.c_longlong()
+        _check(lib().tatrg_permute_profile_large(self._h, ctypes.byref(ms), ctypes.byref(by), ctypes.byref(n)), "tatrg_permute_profile_large")
         return ms.value, by.value, n.value
 
     def workspace_peak(self):

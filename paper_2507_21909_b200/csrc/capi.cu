@@ -171,6 +171,11 @@ int tatrg_permute_profile(tatrg_handle c, double* ms, double* bytes, long long* 
     if (ms) *ms = c->perm_ms; if (bytes) *bytes = (double)c->perm_bytes; if (calls) *calls = c->perm_calls;
     return TATRG_OK;
 }
+int tatrg_permute_profile_large(tatrg_handle c, double* ms, double* bytes, long long* calls) {
+    if (!c) return TATRG_EINVAL;
+    if (ms) *ms = c->perm_large_ms; if (bytes) *bytes = (double)c->perm_large_bytes; if (calls) *calls = c->perm_large_calls;
+    return TATRG_OK;
+}
 
 long long tatrg_get_tensor(tatrg_handle c, const char* name, double* out_host, long long capacity, int* ndim, long long* dims) {
     if (!c || !name) return TATRG_EINVAL;

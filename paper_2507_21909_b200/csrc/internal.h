@@ -28,6 +28,7 @@ struct Counters {
     // optional device timing of the two kernel families (TATRG_OPT_STAGE_TIMING = 2): events bracket each launch
     bool time_kernels = false;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> gemm_ev, perm_ev;
+    std::vector<long long> perm_ev_bytes;   // algorithmic bytes of the permute timed by perm_ev[i]
     struct GemmShape { int64_t M, N, K; int batch; bool ta, tb; double frac = 1.0; };   // frac < 1: lower-triangular tiles only
     std::vector<GemmShape> gemm_shapes;   // parallel to gemm_ev (time_kernels only)
     std::vector<cudaEvent_t> ev_pool;

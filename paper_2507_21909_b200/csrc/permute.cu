@@ -122,7 +122,7 @@ cudaError_t permute(cudaStream_t st, int nd, const int64_t* dims, const int* per
     if (c) { int64_t t = 1; for (int i = 0; i < nd; ++i) t *= dims[i]; c->permuted_bytes += 16 * t; c->permute_calls += 1; }
     if (c && c->time_kernels) { e0 = c->next_event(); e1 = c->next_event(); cudaEventRecord(e0, st); }
     cudaError_t e = permute_raw(st, nd, dims, perm, in, out);
-    if (e0) { cudaEventRecord(e1, st); c->perm_ev.push_back({e0, e1}); }
+    if (e0) { cudaEventRecord(e1, st); c->perm_ev.push_back({e0, e1}); int64_t t = 1; for (int i = 0; i < nd; ++i) t *= dims[i]; c->perm_ev_bytes.push_back(16 * t); }
     return e;
 }
 static cudaError_t permute_raw(cudaStream_t st, int nd, const int64_t* dims, const int* perm, const double* in, double* out) {

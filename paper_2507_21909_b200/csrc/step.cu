@@ -1282,7 +1282,7 @@ void Stepper::run() {
 int run_step(tatrg_ctx* c, cudaStream_t st) {
     Counters& cn = c->cnt;
     cn.launches = 0; cn.gemm_flops = 0; cn.gemm_calls = 0; cn.permuted_bytes = 0; cn.permute_calls = 0;
-    cn.time_kernels = c->timing >= 2; cn.gemm_ev.clear(); cn.perm_ev.clear(); cn.gemm_shapes.clear(); cn.ev_used = 0;
+    cn.time_kernels = c->timing >= 2; cn.gemm_ev.clear(); cn.perm_ev.clear(); cn.perm_ev_bytes.clear(); cn.gemm_shapes.clear(); cn.ev_used = 0;
     g_counter = &cn;
     for (cudaGraphExec_t g : c->graveyard) cudaGraphExecDestroy(g);    // their launches completed before the previous step's last read-back
     c->graveyard.clear();
@@ -1321,7 +1321,11 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
                         (long long)g.K, g.batch, (int)g.ta, (int)g.tb, ms, 2.0 * g.frac * g.M * g.N * g.K * g.batch / (ms * 1e-3) / 1e12);
             }
         }
-        for (auto& ev : cn.perm_ev) { float ms = 0; cudaEventElapsedTime(&ms, ev.first, ev.second); c->perm_ms += ms; }
+        c->perm_large_ms = 0; c->perm_large_bytes = 0; c->perm_large_calls = 0;
+        for (size_t i = 0; i < cn.perm_ev.size(); ++i) {
+            float ms = 0; cudaEventElapsedTime(&ms, cn.perm_ev[i].first, cn.perm_ev[i].second); c->perm_ms += ms;
+            if (i < cn.perm_ev_bytes.size() && cn.perm_ev_bytes[i] >= kLargePermuteBytes) { c->perm_large_ms += ms; c->perm_large_bytes += cn.perm_ev_bytes[i]; c->perm_large_calls += 1; }
+        }
     }
     return TATRG_OK;
 }

@@ -9,6 +9,7 @@ namespace tatrg {
 // DGEMM launches of at least this many flops are the tensor contractions of the path (Eq. 2.18-2.19, 2.9-2.17, A.2-A.11:
 // >= 4e9 each at D = 32); the products inside the Cholesky / subspace solvers are <= 3e8.
 constexpr double kLargeGemmFlops = 1e9;
+constexpr long long kLargePermuteBytes = 100000000;   // permutes of >= 100 MB read + written: larger than L2 (the D^5 tensors at D = 32)
 
 struct Fail {
     int code; std::string msg;
@@ -39,6 +40,7 @@ struct tatrg_ctx {
     double stage_ms[TATRG_NSTAGES] = {0}, stage_flops[TATRG_NSTAGES] = {0};
     double gemm_ms = 0, gemm_flops = 0, perm_ms = 0; long long gemm_calls = 0, perm_calls = 0, perm_bytes = 0;
     double gemm_large_ms = 0, gemm_large_flops = 0; long long gemm_large_calls = 0;   // launches of >= kLargeGemmFlops
+    double perm_large_ms = 0; long long perm_large_bytes = 0, perm_large_calls = 0;       // permutes of >= kLargePermuteBytes
     long long last_launches = 0;
     tatrg::Counters cnt;
     std::map<std::string, tatrg::Tens> kept;   // tensors of the last step (keep_tensors only)
