@@ -49,6 +49,7 @@ class ClockSampler(threading.Thread):
     def __init__(self, index):
         super().__init__(daemon=True)
         self.index, self.samples, self.reasons, self.stop_flag = index, [], set(), False
+        self.active = False       # the thread polls from before the warm-up on (first NVML queries are slow); samples count only while active
         self.max_mhz = None
         self.nvml = None
         try:
@@ -87,10 +88,14 @@ class ClockSampler(threading.Thread):
     def run(self):
         while not self.stop_flag:
             try:
+                n0, r0 = len(self.samples), set(self.reasons)
                 if self.nvml:
                     self.sample_nvml()
-                else:
+                elif self.active:
                     self.sample_smi()
+                if not self.active:               # outside the timed regions: discard
+                    del self.samples[n0:]
+                    self.reasons = r0
             except Exception:
                 pass
             time.sleep(0.05 if self.nvml else 0.2)
@@ -211,10 +216,11 @@ def run_cuda(args):
     t = T.Tatrg(BETA, H, D, P, SEED + rank, power_iters=N_POW, device="cuda:%d" % local)
     for _ in range(PRE_STEPS):
         t.step()
-    for _ in range(args.warmup):
-        t.step()
     sampler = ClockSampler(local)
     sampler.start()
+    for _ in range(args.warmup):
+        t.step()
+    sampler.active = True
     # ---- timed region 1: K steps, state resident in HBM ----
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches = 0
@@ -248,6 +254,7 @@ def run_cuda(args):
     ev1.record()
     barrier()
     ms_e2e = ev0.elapsed_time(ev1)
+    sampler.active = False
     sampler.stop_flag = True
     sampler.join(timeout=2)
     # ---- profiling pass (not part of `value`): per-launch CUDA events on the library's stream around every DGEMM / permute ----
