@@ -433,3 +433,26 @@ def test_overlapped_schedule_equals_the_serial_one(D, steps, monkeypatch):
     for a, b in zip(*runs):
         assert abs(a[0] - b[0]) <= 1e-13 * abs(b[0])
         assert np.abs(a[1] - b[1]).max() <= 1e-12 and np.abs(a[2] - b[2]).max() <= 1e-12
+
+
+@pytest.mark.gpu
+def test_post_critical_steps_at_d32_agree_with_full_decompositions():
+    """configs[3] beyond criticality: around step 20 the flow leaves the critical surface, the local tensor becomes numerically
+    rank-deficient (s_32 / s_1 ~ 1e-8) and the default path hands the QR pre-reduction, and often the triad isometries, to the
+    rank-revealing full decompositions while the squeezers still run on the auxiliary stream (full_run).
+    Through 28 steps the default path and TATRG_OPT_SUBSPACE = 0 (full decompositions everywhere, one stream) give the same physics."""
+    runs = []
+    for sub in (1, 0):
+        t = T.Tatrg(0.1497, 0.0, 32, 32, 42)
+        t.set_option(T.OPT_SUBSPACE, sub)
+        out = []
+        for _ in range(28):
+            t.step()
+            out.append((t.lnZ_per_site(), t.singular_values(T.SV_S, 32)))
+        runs.append(out)
+        t.close()
+    assert min(len(a[1]) for a in runs[0][19:]) >= 1 and runs[0][-1][1][-1] < 1e-4       # the regime is reached: s_32 / s_1 has collapsed
+    for a, b in zip(*runs):
+        assert np.isfinite(a[0]) and abs(a[0] - b[0]) <= 1e-11 * abs(b[0])
+        n = min(len(a[1]), len(b[1]))
+        assert np.abs(a[1][:n] - b[1][:n]).max() <= 1e-8
