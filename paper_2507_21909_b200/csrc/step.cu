@@ -386,6 +386,7 @@ struct Stepper {
         int cur = 0;                 // the basis [Z; W] lives in buf[cur]
         int done = 0, target = 0, deg = 1;
         bool ok = true;
+        int bcap = 0; bool widen = false, widened = false;     // the block may be doubled once when convergence is too slow
         const double* Z() const { return buf[cur].p; }
         const double* W() const { return F ? buf[cur].p + (int64_t)n * b : buf[cur].p; }
     };
@@ -506,17 +507,18 @@ struct Stepper {
                 SubProb& s = ps[i];
                 s.stream = ss.s[i];
                 ck(cudaStreamWaitEvent(s.stream, ss.fork, 0), "wait");
-                s.part_cap = std::max(dgemm_splitk_doubles(s.b, s.b, s.n), dgemm_splitk_doubles(s.n, s.b, s.n));
+                s.part_cap = std::max(std::max(dgemm_splitk_doubles(s.b, s.b, s.n), dgemm_splitk_doubles(s.n, s.b, s.n)),
+                                      std::max(dgemm_splitk_doubles(2 * s.b, 2 * s.b, s.n), dgemm_splitk_doubles(s.n, 2 * s.b, s.n)));
                 s.part = s.part_cap ? raw(s.part_cap) : nullptr;
                 if (!s.part) s.part_cap = 0;
             }
         }
-        for (SubProb& s : ps) {
+        // A flat stretch of the spectrum between positions kmax and b (rho >= 0.8: seen in the post-critical steps) would need
+        // hundreds of applications; the block is then doubled once (lam_{2b+1} / lam_kmax instead of lam_{b+1} / lam_kmax) and the
+        // iteration restarted, before the full decomposition is considered.  All buffers are sized for the doubled block up front.
+        auto init_problem = [&](SubProb& s) {
             OnStream on(*this, s);
-            const int64_t rows = s.F ? 2 * (int64_t)s.n : s.n;
-            s.buf[0] = make({rows, s.b}); s.buf[1] = make({rows, s.b});
-            s.Gm = make({s.b, s.b}); s.L = make({s.b, s.b}); s.H = make({s.b, s.b});
-            s.cw = raw((int64_t)cholesky_work_doubles(s.b)); s.dg = raw(s.b);
+            s.cur = 0; s.done = 0; s.target = 0; s.deg = 1;
             ck(fill_zero(st, s.L.p, (int64_t)s.b * s.b), "zero");
             ck(cudaMemsetAsync(const_cast<int*>(cholesky_info(s.cw, s.b)), 0, sizeof(int), st), "memset"); count_launch();
             ck(philox_gauss(st, c.seed, (uint32_t)call, s.sid, 0, (int64_t)s.n * s.b, s.buf[1].p), "philox");
@@ -524,6 +526,14 @@ struct Stepper {
             sub_orth(s, 1, kShift);
             for (int i = 0; i < q0; ++i) sub_step(s, 1, kShift);
             ck(extract_diag(st, s.b, s.L.p, s.b, s.dg), "diag");
+        };
+        for (SubProb& s : ps) {
+            const int64_t rows = s.F ? 2 * (int64_t)s.n : s.n;
+            s.bcap = (4 * s.b <= s.n) ? 2 * s.b : s.b;
+            s.buf[0] = make({rows, s.bcap}); s.buf[1] = make({rows, s.bcap});
+            s.Gm = make({s.bcap, s.bcap}); s.L = make({s.bcap, s.bcap}); s.H = make({s.bcap, s.bcap});
+            s.cw = raw((int64_t)cholesky_work_doubles(s.bcap)); s.dg = raw(s.bcap);
+            init_problem(s);
         }
         auto sync_all = [&]() { for (SubProb& s : ps) if (s.stream) cudaStreamSynchronize(s.stream); cudaStreamSynchronize(st); return std::chrono::steady_clock::now(); };
         auto tA = verbose ? sync_all() : std::chrono::steady_clock::time_point();
@@ -541,7 +551,7 @@ struct Stepper {
             if (!(head > 1e-12 * s.r[0]) || !(tail > 1e-9 * head)) { s.ok = false; return; }     // rank-deficient block: full decomposition
             // the diagonal of R is that of the last orthonormalisation: r_j ~ lam_j^deg
             const double rho = 1.1 * std::pow(tail / head, 1.0 / s.deg);
-            if (!(rho < 0.8)) { s.ok = false; return; }
+            if (!(rho < 0.8)) { if (!s.widened && s.bcap > s.b) s.widen = true; else s.ok = false; return; }
             s.target = std::max(s.target, (int)std::ceil(13.0 / std::log10(1.0 / rho)) + 2);
             if (s.target > qmax) s.ok = false;
             const double range = std::pow(s.r[0] / tail, 1.0 / s.deg);
@@ -553,7 +563,17 @@ struct Stepper {
         for (int pass = 0; pass < 3; ++pass) {
             bool more = false;
             // a re-estimate within 1 of the count already done is the noise of the estimator (+-10 % in rho), not missing work
-            for (SubProb& s : ps) if (s.ok) { estimate(s); if (s.ok && s.target > s.done + (pass > 0 ? 1 : 0)) more = true; else if (s.ok) s.target = std::min(s.target, s.done); }
+            for (SubProb& s : ps) if (s.ok) {
+                estimate(s);
+                if (s.widen) {
+                    if (verbose) fprintf(stderr, "[tatrg subspace n=%d b=%d kmax=%d%s] convergence too slow: block doubled to %d, restart\n", s.n, s.b, s.kmax, s.F ? " product" : "", s.bcap);
+                    s.widen = false; s.widened = true; s.b = s.bcap;
+                    init_problem(s);
+                    estimate(s);
+                    if (s.widen) { s.widen = false; s.ok = false; }
+                }
+                if (s.ok && s.target > s.done + (pass > 0 ? 1 : 0)) more = true; else if (s.ok) s.target = std::min(s.target, s.done);
+            }
             if (!more) break;
             for (SubProb& s : ps) {
                 if (!s.ok || s.target <= s.done) continue;
