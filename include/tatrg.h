@@ -38,6 +38,13 @@ enum {
                                   r_bond D + oversample wide (fn 9 :381); the squeezed legs stay at D.  default D (r_bond = 1, :331).
                                   Before the first step only; integer in [D, 4D]; ENOMEM unless the workspace holds
                                   tatrg_workspace_bytes_ilo(D, oversample, value). */
+    TATRG_OPT_OVERLAP = 9,     /* 1 (default): in saturated steps the solver chains (squeezers, Cholesky factorisations) run on the library's
+                                  auxiliary streams beside the contractions of the caller's stream; 0: every stage on the caller's stream,
+                                  one after the other (used by bench.py to time the kernels with nothing beside them).  Same result. */
+    TATRG_OPT_GRAPHS = 10,     /* 1 (default): the repeated steps of the subspace iterations are captured once and replayed as CUDA graphs;
+                                  0: plain launches.  Same result. */
+    TATRG_OPT_VERBOSE = 11,    /* debugging aid, bit mask, default 0: 1 = solver chains report ranks / convergence on stderr, 2 = spectra of
+                                  the full eigen-decompositions, 4 = shape and rate of every DGEMM (with TATRG_OPT_STAGE_TIMING = 2) */
     TATRG_OPT_METHOD = 6       /* 0: Triad-ATRG (default).  1: plain ATRG, Eq. 2.7-2.8 (:104-113): no triad split, squeezers from
                                   Gamma^ATRG, O(D^9) contraction sliced so that no D^7 tensor is stored (fn 6 :205).  Before the first
                                   step only; ENOMEM unless the workspace holds tatrg_workspace_bytes_atrg(D, oversample). */
@@ -102,6 +109,8 @@ void tatrg_destroy(tatrg_handle); /* frees the host struct only */
 int tatrg_stage_ms(tatrg_handle, double* ms);
 int tatrg_stage_flops(tatrg_handle, double* flops);
 long long tatrg_last_step_launches(tatrg_handle);
+/* host <-> device synchronisations inside the last tatrg_step call (read-backs of spectra and flags for the rank decisions) */
+long long tatrg_last_step_host_syncs(tatrg_handle);
 /* device time (ms; needs STAGE_TIMING=2), flops and launches of the DGEMM kernel during the last step; likewise the
  * leg-permutation kernel with its algorithmic bytes (8 B read + 8 B written per element). Any out pointer may be NULL. */
 int tatrg_gemm_profile(tatrg_handle, double* ms, double* flops, long long* calls);

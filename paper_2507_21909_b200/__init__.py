@@ -16,6 +16,7 @@ _lib = None
 
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC, ESTATE = 0, -1, -2, -3, -4, -5
 OPT_POWER_ITERS, OPT_K_TRIAD, OPT_TAU, OPT_STAGE_TIMING, OPT_KEEP_TENSORS, OPT_METHOD, OPT_SUBSPACE, OPT_BOND_RANK = 1, 2, 3, 4, 5, 6, 7, 8
+OPT_OVERLAP, OPT_GRAPHS, OPT_VERBOSE = 9, 10, 11
 METHOD_TRIAD, METHOD_ATRG = 0, 1
 SV_SIGMA, SV_S = 0, 1
 STAGES = ["decompose", "qr", "rsvd", "lift", "triad", "triad_tensors", "squeezer_grams", "squeezers", "contract",
@@ -40,6 +41,7 @@ _SIGNATURES = {
     "tatrg_stage_ms": (_c.c_int, [_c.c_void_p, _dp]),
     "tatrg_stage_flops": (_c.c_int, [_c.c_void_p, _dp]),
     "tatrg_last_step_launches": (_c.c_longlong, [_c.c_void_p]),
+    "tatrg_last_step_host_syncs": (_c.c_longlong, [_c.c_void_p]),
     "tatrg_gemm_profile": (_c.c_int, [_c.c_void_p, _dp, _dp, _c.POINTER(_c.c_longlong)]),
     "tatrg_gemm_profile_large": (_c.c_int, [_c.c_void_p, _dp, _dp, _c.POINTER(_c.c_longlong)]),
     "tatrg_permute_profile": (_c.c_int, [_c.c_void_p, _dp, _dp, _c.POINTER(_c.c_longlong)]),
@@ -194,6 +196,9 @@ class Tatrg:
 
     def launches(self):
         return lib().tatrg_last_step_launches(self._h)
+
+    def host_syncs(self):
+        return lib().tatrg_last_step_host_syncs(self._h)
 
     def gemm_profile(self):
         ms, fl, n = ctypes.c_double(), ctypes.c_double(), ctypes.c_longlong()

@@ -69,6 +69,9 @@ int tatrg_set_option(tatrg_handle c, int key, double value) {
         case TATRG_OPT_STAGE_TIMING: c->timing = (int)value; return TATRG_OK;
         case TATRG_OPT_KEEP_TENSORS: c->keep_tensors = value != 0; return TATRG_OK;
         case TATRG_OPT_SUBSPACE: c->use_subspace = value != 0; return TATRG_OK;
+        case TATRG_OPT_OVERLAP: c->use_overlap = value != 0; return TATRG_OK;
+        case TATRG_OPT_GRAPHS: c->use_graphs = value != 0; return TATRG_OK;
+        case TATRG_OPT_VERBOSE: if (value < 0 || value > 7) return TATRG_EINVAL; c->verbose = (int)value; return TATRG_OK;
         case TATRG_OPT_BOND_RANK: {
             if (c->m > 0) return TATRG_ESTATE;
             if (value != std::floor(value) || value < c->D) return TATRG_EINVAL;
@@ -156,6 +159,7 @@ int tatrg_stage_flops(tatrg_handle c, double* fl) {
     return TATRG_OK;
 }
 long long tatrg_last_step_launches(tatrg_handle c) { return c ? c->last_launches : TATRG_EINVAL; }
+long long tatrg_last_step_host_syncs(tatrg_handle c) { return c ? c->last_host_syncs : TATRG_EINVAL; }
 int tatrg_gemm_profile(tatrg_handle c, double* ms, double* flops, long long* calls) {
     if (!c) return TATRG_EINVAL;
     if (ms) *ms = c->gemm_ms; if (flops) *flops = c->gemm_flops; if (calls) *calls = c->gemm_calls;

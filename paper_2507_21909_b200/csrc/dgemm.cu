@@ -17,6 +17,7 @@
 
 namespace tatrg {
 thread_local Counters* g_counter = nullptr;
+thread_local int g_verbose = 0;
 cudaEvent_t Counters::next_event() {
     if (ev_used == ev_pool.size()) { cudaEvent_t e; cudaEventCreate(&e); ev_pool.push_back(e); }
     return ev_pool[ev_used++];

@@ -25,6 +25,7 @@ struct Counters {
     long long gemm_calls = 0;
     long long permuted_bytes = 0;   // read + write bytes of every leg permutation
     long long permute_calls = 0;
+    long long host_syncs = 0;       // host <-> device synchronisations inside the step (read-backs of spectra / flags)
     // optional device timing of the two kernel families (TATRG_OPT_STAGE_TIMING = 2): events bracket each launch
     bool time_kernels = false;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> gemm_ev, perm_ev;
@@ -37,6 +38,9 @@ struct Counters {
 };
 extern thread_local Counters* g_counter;
 inline void count_launch(int k = 1) { if (g_counter) g_counter->launches += k; }
+inline void count_sync() { if (g_counter) g_counter->host_syncs += 1; }
+// TATRG_OPT_VERBOSE of the handle whose step is being enqueued (debugging aid): bit 0 solver chains, bit 1 eigh, bit 2 per-DGEMM rates
+extern thread_local int g_verbose;
 
 // ---- kernels (each file exposes host launchers only) --------------------------------------------------------
 // dgemm.cu : C[M,N] = alpha*op(A)*op(B) + beta*C on FP64 tensor cores (DMMA m8n8k4)

@@ -578,7 +578,7 @@ static int finish_batch(cudaStream_t st, int N, const std::vector<FinishItem>& i
         lh[z].resize(items[z].n);
         if (!check(cudaMemcpyAsync(lh[z].data(), items[z].lam_u, sizeof(double) * items[z].n, cudaMemcpyDeviceToHost, st), err, "eigh readback")) return TATRG_ECUDA;
     }
-    if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;
+    count_sync(); if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;
     std::vector<std::vector<int>> order(cnt);
     for (size_t z = 0; z < cnt; ++z) {
         const FinishItem& it = items[z];
@@ -591,13 +591,13 @@ static int finish_batch(cudaStream_t st, int N, const std::vector<FinishItem>& i
         if (!check(gather_rows_scaled(st, it.Vt, it.Vu, it.idx, nullptr, n, n, N > 0 ? N : n), err, "eigh gather")) return TATRG_ECUDA;
         if (!check(gather_vec(st, it.lam, it.lam_u, it.idx, n, 1, 1.0), err, "eigh gather")) return TATRG_ECUDA;
         if (it.lam_host) { it.lam_host->resize(n); for (int i = 0; i < n; ++i) (*it.lam_host)[i] = lh[z][order[z][i]]; }
-        if (getenv("TATRG_EIGH_VERBOSE")) {
+        if (g_verbose & 2) {
             int c[5] = {0, 0, 0, 0, 0}; const double l0 = lh[z][order[z][0]]; const double th[5] = {1e-4, 1e-8, 1e-12, 1e-14, 1e-16};
             for (int i = 0; i < n; ++i) for (int j = 0; j < 5; ++j) if (lh[z][i] > th[j] * l0) ++c[j];
             fprintf(stderr, "[tatrg eigh n=%d] spectrum: >1e-4:%d >1e-8:%d >1e-12:%d >1e-14:%d >1e-16:%d\n", n, c[0], c[1], c[2], c[3], c[4]);
         }
     }
-    if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;   // `order` leaves scope
+    count_sync(); if (!check(cudaStreamSynchronize(st), err, "eigh sync")) return TATRG_ECUDA;   // `order` leaves scope
     return TATRG_OK;
 }
 
@@ -664,7 +664,7 @@ int eigh_batched(cudaStream_t st, int count, const EighItem* items, void* work, 
         }
         return TATRG_OK;
     }
-    static const bool verbose = getenv("TATRG_EIGH_VERBOSE") != nullptr;   // debugging aid only
+    const bool verbose = (g_verbose & 2) != 0;   // debugging aid only
     const int nb = N / BW, npair = nb / 2;
     for (int z0 = 0; z0 < count; z0 += kMaxBatch) {
         const int bc = std::min(kMaxBatch, count - z0);
@@ -710,7 +710,7 @@ int eigh_batched(cudaStream_t st, int count, const EighItem* items, void* work, 
             }
             int rot = 0;
             if (!check(cudaMemcpyAsync(&rot, counter, sizeof(int), cudaMemcpyDeviceToHost, ss), err, "eigh readback")) return TATRG_ECUDA;
-            if (!check(cudaStreamSynchronize(ss), err, "eigh sync")) return TATRG_ECUDA;
+            count_sync(); if (!check(cudaStreamSynchronize(ss), err, "eigh sync")) return TATRG_ECUDA;
             if (verbose) fprintf(stderr, "[tatrg eigh batch=%d N=%d] sweep %d rotations %d\n", bc, N, sweep, rot);
             if (rot == 0) break;
         }
@@ -756,7 +756,7 @@ int svd_rows(cudaStream_t st, int nv, int len, const double* X, double* s, doubl
     svd_rows_kernel<<<1, 1024, smem, st>>>(nv, len, X, su, Uu, Vu); count_launch();
     std::vector<double> sh(nv);
     if (!check(cudaMemcpyAsync(sh.data(), su, sizeof(double) * nv, cudaMemcpyDeviceToHost, st), err, "svd readback")) return TATRG_ECUDA;
-    if (!check(cudaStreamSynchronize(st), err, "svd sync")) return TATRG_ECUDA;
+    count_sync(); if (!check(cudaStreamSynchronize(st), err, "svd sync")) return TATRG_ECUDA;
     for (int i = 0; i < nv; ++i) if (!std::isfinite(sh[i])) { if (err) *err = "svd_rows: non-finite singular value"; return TATRG_ENUMERIC; }
     std::vector<int> order(nv);
     std::iota(order.begin(), order.end(), 0);
@@ -765,7 +765,7 @@ int svd_rows(cudaStream_t st, int nv, int len, const double* X, double* s, doubl
     if (!check(gather_rows_scaled(st, Ut, Uu, idx, nullptr, nv, len, len), err, "svd gather")) return TATRG_ECUDA;
     if (!check(gather_rows_scaled(st, Vacc, Vu, idx, nullptr, nv, nv, nv), err, "svd gather")) return TATRG_ECUDA;
     if (!check(gather_vec(st, s, su, idx, nv, 1, 1.0), err, "svd gather")) return TATRG_ECUDA;
-    if (!check(cudaStreamSynchronize(st), err, "svd sync")) return TATRG_ECUDA;
+    count_sync(); if (!check(cudaStreamSynchronize(st), err, "svd sync")) return TATRG_ECUDA;
     if (s_host) { s_host->resize(nv); for (int i = 0; i < nv; ++i) (*s_host)[i] = sh[order[i]]; }
     return TATRG_OK;
 }

@@ -153,8 +153,7 @@ static cudaError_t permute_raw(cudaStream_t st, int nd, const int64_t* dims, con
         a.nd = m - 1;
         for (int i = 0; i < m - 1; ++i) { a.ext[i] = od[i]; a.sin[i] = sin_o[i]; a.sout[i] = sout_o[i]; }
         int64_t inner = od[m - 1], rows = total / inner;
-        static const int variant = getenv("TATRG_PERMUTE_VARIANT") ? atoi(getenv("TATRG_PERMUTE_VARIANT")) : 3;   // A/B aid: bit 0 runs kernel, bit 1 tiled64
-        const bool al16 = (variant & 1) && (((uintptr_t)in | (uintptr_t)out) & 15) == 0;
+        const bool al16 = (((uintptr_t)in | (uintptr_t)out) & 15) == 0;
         if (al16 && inner % 2 == 0 && inner / 2 <= 32 * 1024 && m >= 2) {
             // vectorised: runs over the last outer leg (all input strides are multiples of `inner`, hence even)
             PermArgs b; b.nd = m - 2;
@@ -181,8 +180,7 @@ static cudaError_t permute_raw(cudaStream_t st, int nd, const int64_t* dims, con
     int64_t extA = od[ia], extB = od[ib];
     int64_t outer = total / (extA * extB);
     {
-        static const int variant2 = getenv("TATRG_PERMUTE_VARIANT") ? atoi(getenv("TATRG_PERMUTE_VARIANT")) : 3;
-        bool even = (variant2 & 2) && (extA % 2 == 0) && (extB % 2 == 0) && (sin_o[ib] % 2 == 0) && (sout_o[ia] % 2 == 0) && ((((uintptr_t)in | (uintptr_t)out) & 15) == 0);
+        bool even = (extA % 2 == 0) && (extB % 2 == 0) && (sin_o[ib] % 2 == 0) && (sout_o[ia] % 2 == 0) && ((((uintptr_t)in | (uintptr_t)out) & 15) == 0);
         for (int i = 0; i < a.nd; ++i) even = even && (a.sin[i] % 2 == 0) && (a.sout[i] % 2 == 0);
         if (even && extA >= 64 && extB >= 64) {
             int64_t tA = (extA + 63) / 64, tB = (extB + 63) / 64, nb = tA * tB * outer;

@@ -152,7 +152,7 @@ struct Stepper {
     std::vector<double> to_host(const double* d, int64_t n) {
         std::vector<double> h(n);
         ck(cudaMemcpyAsync(h.data(), d, 8 * n, cudaMemcpyDeviceToHost, st), "readback");
-        ck(cudaStreamSynchronize(st), "sync");
+        ck(cudaStreamSynchronize(st), "sync"); count_sync();
         return h;
     }
     double* to_dev(const std::vector<double>& h) {
@@ -254,9 +254,9 @@ struct Stepper {
         ck(cudaMemcpyAsync(&info, cholesky_info(cw, (int)n), sizeof(int), cudaMemcpyDeviceToHost, st), "readback");
         ck(cudaMemcpyAsync(d0.data(), cholesky_d0(cw, (int)n), 8 * n, cudaMemcpyDeviceToHost, st), "readback");
         ck(cudaMemcpyAsync(xn.data(), res, 8, cudaMemcpyDeviceToHost, st), "readback");
-        ck(cudaStreamSynchronize(st), "sync");
+        ck(cudaStreamSynchronize(st), "sync"); count_sync();
         double tr = 0; for (double v : d0) tr += v;
-        if (getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg cholesky qr %lld x %lld] info %d, proven lam_min/lam_max >= %.3e\n", (long long)m, (long long)n, info, 1.0 / (xn[0] * tr));
+        if (g_verbose & 1) fprintf(stderr, "[tatrg cholesky qr %lld x %lld] info %d, proven lam_min/lam_max >= %.3e\n", (long long)m, (long long)n, info, 1.0 / (xn[0] * tr));
         if (info != 0 || !std::isfinite(xn[0]) || !(xn[0] > 0) || !(tr > 0)) return false;
         if (!(1.0 / (xn[0] * tr) > kEpsOrthLambda)) return false;
         Q = mm(false, true, m, n, n, mat.p, n, X.p, n);
@@ -281,20 +281,16 @@ struct Stepper {
     // orth_chol() (one pass) of two matrices of the same shape: the two Gram matrices on the caller's stream, then the two
     // factorisation + inversion chains (latency-bound: ~60 small launches each) side by side on two auxiliary streams, then
     // the decisions and the two Q = mat L^-T products.  All buffers are allocated before the fork; nothing is allocated or
-    // freed while the chains are in flight.  Returns false (nothing kept) unless both operands prove full rank.
+    // freed while the chains are in flight.  Returns false (nothing kept but the Gram matrices, see Gkeep) unless both operands
+    // prove full rank.
     // Xinv != nullptr: Q = mat L^-T is NOT formed; the caller gets Xinv[i] = L^-1 instead (Q[i].p stays null) and applies it
     // to whatever multiplies Q (bond_swap: Q only ever appears in products, so two n x n x n GEMMs replace two m x n x n ones).
     // meanwhile: work for the caller's stream that does not depend on the factors, issued while the two chains are in flight
     // (it may allocate: the chains' buffers stay allocated and the chains themselves allocate nothing).
+    // Gkeep != nullptr: on failure the two Gram matrices (recomputed: the factorisation destroys them) are NOT needed -- the
+    // caller recomputes them; kept simple on purpose.
     bool orth_chol_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2], Tens* Xinv = nullptr, const std::function<void()>* meanwhile = nullptr) {
         SubStreams& ss = sub_streams();
-        if (!ss.ok) {
-            const bool ok0 = orth_chol(m0, Q[0], R[0]), ok1 = orth_chol(m1, Q[1], R[1]);
-            if (ok0 && ok1) return true;
-            if (ok0) drop(Q[0]), drop(R[0]);
-            if (ok1) drop(Q[1]), drop(R[1]);
-            return false;
-        }
         Scope sc(*this);
         const int64_t m = m0.d[0], n = m0.d[1];
         const Tens* mats[2] = {&m0, &m1};
@@ -305,17 +301,17 @@ struct Stepper {
             cw[i] = raw((int64_t)cholesky_work_doubles((int)n)); res[i] = raw(1 + 148 * 8 + 7);
             ck(fill_zero(st, L[i].p, n * n), "zero"); ck(fill_zero(st, X[i].p, n * n), "zero");
         }
-        ck(cudaEventRecord(ss.fork, st), "event");
+        if (ss.ok) ck(cudaEventRecord(ss.fork, st), "event");
         for (int i = 0; i < 2; ++i) {
-            cudaStream_t a = ss.s[i];
-            ck(cudaStreamWaitEvent(a, ss.fork, 0), "wait");
+            cudaStream_t a = ss.ok ? ss.s[i] : st;
+            if (ss.ok) ck(cudaStreamWaitEvent(a, ss.fork, 0), "wait");
             ck(cholesky(a, (int)n, G[i].p, n, L[i].p, n, 0.0, 1e-14, cw[i]), "cholesky");
             ck(tri_inverse(a, (int)n, L[i].p, n, cw[i], X[i].p, n, T[i].p), "tri_inverse");
             ck(dot(a, n * n, X[i].p, X[i].p, res[i]), "dot");
-            ck(cudaEventRecord(ss.join[i], a), "event");
+            if (ss.ok) ck(cudaEventRecord(ss.join[i], a), "event");
         }
         if (meanwhile && *meanwhile) (*meanwhile)();
-        for (int i = 0; i < 2; ++i) ck(cudaStreamWaitEvent(st, ss.join[i], 0), "wait");
+        if (ss.ok) for (int i = 0; i < 2; ++i) ck(cudaStreamWaitEvent(st, ss.join[i], 0), "wait");
         bool ok = true;
         int info[2] = {0, 0};
         std::vector<double> d0[2] = {std::vector<double>(n), std::vector<double>(n)}; double xn[2] = {0, 0};
@@ -324,10 +320,10 @@ struct Stepper {
             ck(cudaMemcpyAsync(d0[i].data(), cholesky_d0(cw[i], (int)n), 8 * n, cudaMemcpyDeviceToHost, st), "readback");
             ck(cudaMemcpyAsync(&xn[i], res[i], 8, cudaMemcpyDeviceToHost, st), "readback");
         }
-        ck(cudaStreamSynchronize(st), "sync");
+        ck(cudaStreamSynchronize(st), "sync"); count_sync();
         for (int i = 0; i < 2; ++i) {
             double tr = 0; for (double v : d0[i]) tr += v;
-            if (getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg cholesky qr %lld x %lld] info %d, proven lam_min/lam_max >= %.3e\n", (long long)m, (long long)n, info[i], 1.0 / (xn[i] * tr));
+            if (g_verbose & 1) fprintf(stderr, "[tatrg cholesky qr %lld x %lld] info %d, proven lam_min/lam_max >= %.3e\n", (long long)m, (long long)n, info[i], 1.0 / (xn[i] * tr));
             if (info[i] != 0 || !std::isfinite(xn[i]) || !(xn[i] > 0) || !(tr > 0) || !(1.0 / (xn[i] * tr) > kEpsOrthLambda)) ok = false;
         }
         if (!ok) return false;
@@ -340,15 +336,16 @@ struct Stepper {
         return true;
     }
 
-    // orth() of two matrices of the same shape with n > 128 (single pass): the two Gram matrices are decomposed together
-    // Xinv: see orth_chol_pair (set only when the Cholesky path with two streams was taken; else Xinv[i].p stays null and Q is explicit)
+    // orth() of two matrices of the same shape with n > 128 (single pass): Cholesky QR when both prove full rank, else the two
+    // Gram matrices are eigen-decomposed together (rank-revealing: directions with lam <= 1e-12 lam_max dropped, R14).
+    // Xinv != nullptr: Q is NOT formed (Q[i].p stays null); Xinv[i] [r x n] is the factor with Q = mat Xinv^T -- L^-1 of the
+    // Cholesky path, lam^-1/2 V^T of the eigen path -- and R[i] = Q^T mat [r x n] (L^T resp. lam^1/2 V^T).
     void orth_pair(const Tens& m0, const Tens& m1, Tens Q[2], Tens R[2], Tens* Xinv = nullptr, const std::function<void()>* meanwhile = nullptr) {
         const int64_t m = m0.d[0], n = m0.d[1];
         if (Xinv) { Xinv[0].p = nullptr; Xinv[1].p = nullptr; }
         if (n <= 128 || m1.d[0] != m || m1.d[1] != n) { orth(m0, Q[0], R[0]); orth(m1, Q[1], R[1]); return; }
-        if (c.use_subspace && sub_streams().ok && orth_chol_pair(m0, m1, Q, R, Xinv, meanwhile)) return;
-        if (Xinv) { Xinv[0].p = nullptr; Xinv[1].p = nullptr; }
-        if (c.use_subspace && !sub_streams().ok && orth_chol_pair(m0, m1, Q, R)) return;
+        if (c.use_subspace && orth_chol_pair(m0, m1, Q, R, Xinv, meanwhile)) return;
+        const bool implicit = Xinv != nullptr && c.use_subspace;
         Scope sc(*this);
         const Tens* mats[2] = {&m0, &m1};
         Tens G[2];
@@ -360,11 +357,19 @@ struct Stepper {
             if (!(lh[0] > 0)) fail(TATRG_ENUMERIC, "orth: zero matrix");
             int r = 0;
             for (double x : lh) if (x > kEpsOrthLambda * lh[0]) ++r;
-            Q[i] = mm(false, true, m, r, n, mats[i]->p, n, eo[i].Vt.p, n);
-            ck(scale_last(st, Q[i].p, Q[i].p, eo[i].lam, m, r, 2), "scale");
+            if (g_verbose & 1) fprintf(stderr, "[tatrg orth %lld x %lld] eigen-decomposition of the Gram matrix: rank %d\n", (long long)m, (long long)n, r);
+            if (implicit) {
+                Xinv[i] = make({r, n});
+                ck(scale_rows(st, Xinv[i].p, eo[i].Vt.p, eo[i].lam, r, n, 2), "scale");     // lam^-1/2 V^T
+                keep(Xinv[i]); Q[i] = Tens(); Q[i].p = nullptr;
+            } else {
+                Q[i] = mm(false, true, m, r, n, mats[i]->p, n, eo[i].Vt.p, n);
+                ck(scale_last(st, Q[i].p, Q[i].p, eo[i].lam, m, r, 2), "scale");
+                keep(Q[i]);
+            }
             R[i] = make({r, n});
             ck(scale_rows(st, R[i].p, eo[i].Vt.p, eo[i].lam, r, n, 3), "scale");
-            keep(Q[i]); keep(R[i]);
+            keep(R[i]);
         }
     }
 
@@ -450,12 +455,12 @@ struct Stepper {
     // flight are bound by the host's launch rate: one unit (1 step, or 2 when the basis alternates between the two buffers)
     // is captured into a CUDA graph and replayed.  Counters are incremented at capture time only, hence the correction.
     void sub_run(SubProb& s, double shift) {
-        static bool graphs_ok = getenv("TATRG_NO_GRAPHS") == nullptr;
+        static bool graphs_ok = true;      // cleared for the process when stream capture is unavailable
         const int steps = (s.target - s.done + s.deg - 1) / s.deg;
         const int unit = (s.deg % 2 == 0) ? 2 : 1;
         const int reps = steps / unit;
         int left = steps;
-        if (graphs_ok && s.stream && c.timing < 2 && reps >= 3) {      // never the caller's stream: it may be the legacy default stream
+        if (graphs_ok && c.use_graphs && s.stream && c.timing < 2 && reps >= 3) {      // never the caller's stream: it may be the legacy default stream
             const int done0 = s.done, cur0 = s.cur;
             Counters* cn = g_counter;
             const long long l0 = cn ? cn->launches : 0, gc0 = cn ? cn->gemm_calls : 0; const double f0 = cn ? cn->gemm_flops : 0;
@@ -470,9 +475,9 @@ struct Stepper {
                 if (ge != cudaSuccess || !graph) ok = false;
             }
             if (ok) { ge = cudaGraphInstantiate(&exec, graph, 0); ok = ge == cudaSuccess; }
-            if (!ok && getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg subspace] graph capture failed: %s %s\n", cudaGetErrorString(ge), why.c_str());
+            if (!ok && (g_verbose & 1)) fprintf(stderr, "[tatrg subspace] graph capture failed: %s %s\n", cudaGetErrorString(ge), why.c_str());
             if (graph) cudaGraphDestroy(graph);
-            if (getenv("TATRG_SUB_VERBOSE")) fprintf(stderr, "[tatrg subspace] graph of %d step(s): %s, %d replays + %d plain steps, capture + instantiate %.0f us\n", unit, ok ? "ok" : "FAILED", reps, steps - reps * unit, std::chrono::duration<double, std::micro>(std::chrono::steady_clock::now() - tg0).count());
+            if (g_verbose & 1) fprintf(stderr, "[tatrg subspace] graph of %d step(s): %s, %d replays + %d plain steps, capture + instantiate %.0f us\n", unit, ok ? "ok" : "FAILED", reps, steps - reps * unit, std::chrono::duration<double, std::micro>(std::chrono::steady_clock::now() - tg0).count());
             if (ok) {
                 for (int r = 0; r < reps && ok; ++r) ok = cudaGraphLaunch(exec, st) == cudaSuccess;
                 c.graveyard.push_back(exec);
@@ -496,9 +501,9 @@ struct Stepper {
     // scaling) tolerates several applications of A per orthonormalisation, as long as the dynamic range of the block,
     // (r_1 / r_b)^deg, stays below 1e11.
     void sub_iterate(std::vector<SubProb>& ps) {
-        constexpr int q0 = 4, qmax = 96;
+        constexpr int q0 = 4, qmax = 240;
         constexpr double kShift = 1e-13;
-        static const bool verbose = getenv("TATRG_SUB_VERBOSE") != nullptr;   // debugging aid only
+        const bool verbose = (g_verbose & 1) != 0;   // debugging aid only
         SubStreams& ss = sub_streams();
         const bool multi = ss.ok && !ps.empty() && ps.size() <= 4;
         if (multi) {
@@ -513,7 +518,7 @@ struct Stepper {
                 if (!s.part) s.part_cap = 0;
             }
         }
-        // A flat stretch of the spectrum between positions kmax and b (rho >= 0.8: seen in the post-critical steps) would need
+        // A flat stretch of the spectrum between positions kmax and b (rho >= 0.6: seen in the post-critical steps) would need
         // hundreds of applications; the block is then doubled once (lam_{2b+1} / lam_kmax instead of lam_{b+1} / lam_kmax) and the
         // iteration restarted, before the full decomposition is considered.  All buffers are sized for the doubled block up front.
         auto init_problem = [&](SubProb& s) {
@@ -551,7 +556,11 @@ struct Stepper {
             if (!(head > 1e-12 * s.r[0]) || !(tail > 1e-9 * head)) { s.ok = false; return; }     // rank-deficient block: full decomposition
             // the diagonal of R is that of the last orthonormalisation: r_j ~ lam_j^deg
             const double rho = 1.1 * std::pow(tail / head, 1.0 / s.deg);
-            if (!(rho < 0.8)) { if (!s.widened && s.bcap > s.b) s.widen = true; else s.ok = false; return; }
+            // slow convergence (rho >= 0.6: more than 60 applications): the doubled block converges like lam_{2b+1} / lam_kmax and
+            // costs twice as much per application -- taken whenever it is available; without it up to qmax applications are
+            // still far cheaper than the full decomposition (0.1 ms each against 25 ms)
+            if (!(rho < 0.6) && !s.widened && s.bcap > s.b) { s.widen = true; return; }
+            if (!(rho < 0.95)) { s.ok = false; return; }
             s.target = std::max(s.target, (int)std::ceil(13.0 / std::log10(1.0 / rho)) + 2);
             if (s.target > qmax) s.ok = false;
             const double range = std::pow(s.r[0] / tail, 1.0 / s.deg);
@@ -600,7 +609,7 @@ struct Stepper {
             OnStream on(*this, s);
             int info = 0;
             ck(cudaMemcpyAsync(&info, cholesky_info(s.cw, s.b), sizeof(int), cudaMemcpyDeviceToHost, st), "readback");
-            ck(cudaStreamSynchronize(st), "sync");
+            ck(cudaStreamSynchronize(st), "sync"); count_sync();
             if (info != 0) s.ok = false;
         }
         if (multi)
@@ -696,7 +705,7 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
     Scope sc(*this);
     const int64_t d1 = a.d[0], d2 = a.d[1], d3 = a.d[2], d4 = a.d[3], chi = a.d[4];
     const int64_t F = d1 * d2 * d3 * d4, J = d2 * d3 * d4;
-    Tens QB, RB, QC, RC, XB, XC;      // implicit: QB, QC hold B, C themselves and XB, XC the inverse Cholesky factors
+    Tens QB, RB, QC, RC, XB, XC;      // implicit: QB, QC hold B, C themselves and XB, XC the factors with Q = B XB^T, C XC^T
     Tens btom;                        // B^T Omega^phys [c, be, m], formed ahead while the Cholesky chains run
     bool implicit = false;
     {
@@ -710,8 +719,7 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
         drop(cc);
         Tens Qs[2], Rs[2], Xs[2];
         // While the two Cholesky chains are in flight the caller's stream draws Omega^phys and forms B^T Omega^phys, the part of
-        // the projection Q^B^T Omega^phys = L_B^-1 (B^T Omega^phys) that needs no factor (full rank presumed: n columns; the
-        // result is discarded when the Cholesky path is rejected).
+        // the projection Q^B^T Omega^phys = XB (B^T Omega^phys) that needs no factor.
         std::function<void()> early = [&]() {
             const int64_t n = d1 * chi, l0 = std::min<int64_t>(c.Dbond + c.p, chi * n);
             Tens om = make({chi, J, l0});
@@ -726,9 +734,9 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
         if (btom.p) scopes[scopes.size() - 2].push_back(btom.p);      // into bond_swap's scope
         RB = Rs[0]; RC = Rs[1];
         if (Xs[0].p) {
-            // Cholesky QR: Q^B = B L_B^-T and Q^C = C L_C^-T are never formed.  They only enter through the products
-            // Q^B^T Omega^phys (R12) and Q^C U^bond, Q^B V^bond (Eq. A.10-A.11), where the n x n inverse factor is
-            // applied to the small operand instead (saves two D^3 x D^2 x D^2 products).
+            // Q^B = B XB^T and Q^C = C XC^T are never formed (XB = L_B^-1 of the Cholesky QR, or lam^-1/2 V^T of the rank-revealing
+            // eigen-decomposition).  They only enter through the products Q^B^T Omega^phys (R12) and Q^C U^bond, Q^B V^bond
+            // (Eq. A.10-A.11), where the small factor is applied to the small operand instead (saves two D^3 x D^2 x D^2 products).
             implicit = true;
             QB = view(bm, {J, d1 * chi}); QC = view(cm, {J, d1 * chi}); XB = Xs[0]; XC = Xs[1];
             keep(bm); keep(cm); keep(XB); keep(XC);
@@ -739,7 +747,7 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
         keep(RB); keep(RC);
     }
     if (submark) submark();                                              // end of TATRG_ST_QR
-    const int64_t npb = QB.d[1], npc = QC.d[1];
+    const int64_t npb = RB.d[0], npc = RC.d[0];      // ranks of Q^B, Q^C (= QB.d[1], QC.d[1] unless Q is implicit)
     Tens RB3 = view(RB, {npb, d1, chi}), RC3 = view(RC, {npc, d1, chi});
     const int64_t l = std::min<int64_t>(c.Dbond + c.p, std::min(chi * npc, chi * npb));     // R3: sketch width (fn 9 :381)
     // Omega drawn in the physical basis (be, j', m) and projected on Q^B  (R11, R12)
@@ -863,7 +871,7 @@ void Stepper::triad_isos(Tens gram[4], const std::vector<int>& which, int64_t d2
             ck(symmetrize(st, (int)n, gram[i].p), "symmetrize");
             ps[j].Bm = gram[i].p; ps[j].F = nullptr; ps[j].n = (int)n; ps[j].kmax = kmax; ps[j].b = sub_block((int)n, kmax); ps[j].sid = 16 + i;
         }
-        const bool vb = getenv("TATRG_SUB_VERBOSE") != nullptr;
+        const bool vb = (g_verbose & 1) != 0;
         auto now = [&]() { cudaStreamSynchronize(st); return std::chrono::steady_clock::now(); };
         auto t0 = vb ? now() : std::chrono::steady_clock::time_point();
         sub_iterate(ps);
@@ -1188,7 +1196,7 @@ void Stepper::run() {
         // Lambda, Phi', Psi'.  Everything the q stage allocates comes from an arena of its own (a block of the workspace taken
         // before the fork), because the pool's reuse rule is enqueue order on ONE stream.
         SubStreams& ss = sub_streams();
-        bool overlap = c.use_subspace && ss.ok && getenv("TATRG_NO_OVERLAP") == nullptr;
+        bool overlap = c.use_subspace && ss.ok && c.use_overlap;
         for (int d = 0; d < 3; ++d) overlap = overlap && sub_applicable(du[d] * du[d], c.D);
         double* arena = nullptr; size_t arena_bytes = 0;
         if (overlap) {
@@ -1301,9 +1309,10 @@ void Stepper::run() {
 
 int run_step(tatrg_ctx* c, cudaStream_t st) {
     Counters& cn = c->cnt;
-    cn.launches = 0; cn.gemm_flops = 0; cn.gemm_calls = 0; cn.permuted_bytes = 0; cn.permute_calls = 0;
+    cn.launches = 0; cn.gemm_flops = 0; cn.gemm_calls = 0; cn.permuted_bytes = 0; cn.permute_calls = 0; cn.host_syncs = 0;
     cn.time_kernels = c->timing >= 2; cn.gemm_ev.clear(); cn.perm_ev.clear(); cn.perm_ev_bytes.clear(); cn.gemm_shapes.clear(); cn.ev_used = 0;
     g_counter = &cn;
+    g_verbose = c->verbose;
     for (cudaGraphExec_t g : c->graveyard) cudaGraphExecDestroy(g);    // their launches completed before the previous step's last read-back
     c->graveyard.clear();
     int rc = TATRG_OK;
@@ -1317,8 +1326,10 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
         rc = TATRG_ECUDA; c->err = e.what();
     }
     g_counter = nullptr;
+    g_verbose = 0;
     c->last_stream = st;
     c->last_launches = cn.launches;
+    c->last_host_syncs = cn.host_syncs;
     if (rc != TATRG_OK) { cudaDeviceSynchronize(); c->failed = true; c->lnc.resize(lnc0); return rc; }   // auxiliary streams may still be running
     c->gemm_flops = cn.gemm_flops; c->gemm_calls = cn.gemm_calls; c->perm_calls = cn.permute_calls; c->perm_bytes = cn.permuted_bytes;
     if (c->timing >= 1) {
@@ -1326,7 +1337,7 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
         if (e != cudaSuccess) { c->failed = true; c->err = cudaGetErrorString(e); return TATRG_ECUDA; }
         for (int i = 0; i < TATRG_NSTAGES; ++i) { float ms = 0; cudaEventElapsedTime(&ms, c->stage_ev[i], c->stage_ev[i + 1]); c->stage_ms[i] = ms; }
         c->gemm_ms = 0; c->perm_ms = 0;
-        const bool verbose = getenv("TATRG_GEMM_VERBOSE") != nullptr;   // debugging aid: per-launch shapes and rates
+        const bool verbose = (c->verbose & 4) != 0;   // debugging aid: per-launch shapes and rates
         c->gemm_large_ms = 0; c->gemm_large_flops = 0; c->gemm_large_calls = 0;
         for (size_t i = 0; i < cn.gemm_ev.size(); ++i) {
             float ms = 0; cudaEventElapsedTime(&ms, cn.gemm_ev[i].first, cn.gemm_ev[i].second); c->gemm_ms += ms;

@@ -28,6 +28,9 @@ struct tatrg_ctx {
     double tau = tatrg::kTauDefault;
     int timing = 0;
     bool keep_tensors = false;
+    bool use_overlap = true;         // TATRG_OPT_OVERLAP: solver chains beside the contractions (saturated steps)
+    bool use_graphs = true;          // TATRG_OPT_GRAPHS: replay the iteration steps of the solver chains as CUDA graphs
+    int verbose = 0;                 // TATRG_OPT_VERBOSE
     tatrg::Pool pool;
     cudaStream_t last_stream = nullptr;
     tatrg::Tens phi, psi;            // state: Phi[i1,i2,i3,i4,g], Psi[j1,j2,j3,j4,g]
@@ -41,7 +44,7 @@ struct tatrg_ctx {
     double gemm_ms = 0, gemm_flops = 0, perm_ms = 0; long long gemm_calls = 0, perm_calls = 0, perm_bytes = 0;
     double gemm_large_ms = 0, gemm_large_flops = 0; long long gemm_large_calls = 0;   // launches of >= kLargeGemmFlops
     double perm_large_ms = 0; long long perm_large_bytes = 0, perm_large_calls = 0;       // permutes of >= kLargePermuteBytes
-    long long last_launches = 0;
+    long long last_launches = 0, last_host_syncs = 0;
     tatrg::Counters cnt;
     std::map<std::string, tatrg::Tens> kept;   // tensors of the last step (keep_tensors only)
     std::vector<cudaEvent_t> stage_ev;

@@ -1,6 +1,7 @@
 """Writes tests/golden/oracle_<name>.json from the CPU oracle ONLY (never from the CUDA path).
 
     python tests/golden/make_golden.py c1 c2 c3 [c4:12]      (name[:steps])
+    GOLDEN_CKPT=/some/dir python tests/golden/make_golden.py c4:26    (long runs: state saved after each step)
 
 Each file holds, per step: ln Z/V, the bond-swap spectrum sigma/sigma_1 and the T-decomposition spectrum s/s_1
 for one BASELINE.json config (see tests/inputs.py::configs); these take minutes to hours on a CPU, so the GPU
@@ -10,6 +11,8 @@ import json
 import os
 import sys
 import time
+
+import numpy as np
 
 ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 sys.path.insert(0, ROOT)
@@ -32,7 +35,13 @@ if __name__ == "__main__":
             steps = min(steps, int(lim)) if lim else steps
             o = O.TatrgOracle(beta, h, D, p, seed, n_pow=n_pow)
             rec = dict(tag=tag, beta=beta, h=h, D=D, oversample=p, n_pow=n_pow, seed=seed, lnZ=[], sigma=[], s=[], sec=[])
-            for m in range(steps):
+            # optional resume of a multi-hour run: the oracle's whole state is (Phi, Psi, [ln c_m], m) plus what was recorded
+            ckpt = os.environ.get("GOLDEN_CKPT") and os.path.join(os.environ["GOLDEN_CKPT"], "ckpt_%s_%s.npz" % (name, tag))
+            if ckpt and os.path.exists(ckpt):
+                z = np.load(ckpt, allow_pickle=False)
+                o.phi, o.psi, o.lnc, o.m = z["phi"], z["psi"], list(z["lnc"]), int(z["m"])
+                rec = json.loads(str(z["rec"]))
+            for m in range(o.m, steps):
                 t0 = time.time()
                 o.step()
                 rec["lnZ"].append(o.lnZ_per_site())
@@ -41,5 +50,8 @@ if __name__ == "__main__":
                 rec["sec"].append(round(time.time() - t0, 3))
                 print(name, tag, m + 1, rec["lnZ"][-1], rec["sec"][-1], flush=True)
                 json.dump(out | {"runs": out["runs"] + [rec]}, open(os.path.join(os.path.dirname(__file__), "oracle_%s.json" % name), "w"), indent=0)
+                if ckpt:
+                    np.savez(ckpt + ".tmp.npz", phi=o.phi, psi=o.psi, lnc=np.array(o.lnc), m=o.m, rec=json.dumps(rec))
+                    os.replace(ckpt + ".tmp.npz", ckpt)
             out["runs"].append(rec)
         json.dump(out, open(os.path.join(os.path.dirname(__file__), "oracle_%s.json" % name), "w"), indent=0)

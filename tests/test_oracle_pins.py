@@ -47,6 +47,27 @@ def test_gaussian_box_muller_by_hand():
     assert 0 < u1 < 1 and 0 < u2 < 1
 
 
+def test_gaussian_counter_layout_beyond_32_bits():
+    """R11: counter = (e & 0xffffffff, e >> 32, call, stream), key = (seed lo, seed hi).  Random123's third known-answer
+    vector has ctr = (243f6a88, 85a308d3, 13198a2e, 03707344), key = (a4093822, 299f31d0) -> d16cfe09 94fdcceb 5001e420
+    24126ea1, i.e. element e = 0x85a308d3243f6a88 >= 2^32 of call 0x13198a2e, stream 0x03707344, seed 0x299f31d0a4093822.
+    The Gaussian is recomputed by hand from the PUBLISHED integers (not from the oracle's generator)."""
+    x0, x1, x2, x3 = 0xD16CFE09, 0x94FDCCEB, 0x5001E420, 0x24126EA1
+    u1 = ((x0 >> 6) * 2 ** 27 + (x1 >> 5) + 0.5) / 2 ** 53
+    u2 = ((x2 >> 6) * 2 ** 27 + (x3 >> 5) + 0.5) / 2 ** 53
+    z = math.sqrt(-2 * math.log(u1)) * math.cos(2 * math.pi * u2)
+    e = (0x85A308D3 << 32) | 0x243F6A88
+    got = philox.gaussians((0x299F31D0 << 32) | 0xA4093822, 0x13198A2E, 0x03707344, e, 1)[0]
+    assert abs(got - z) < 4e-16 * max(1.0, abs(z))
+    # consecutive elements across the 2^32 boundary: e = 2^32 - 1 -> ctr (ffffffff, 0), e = 2^32 -> ctr (0, 1)
+    zz = philox.gaussians(42, 3, 0, 2 ** 32 - 1, 2)
+    for j, (c0, c1) in enumerate([(0xFFFFFFFF, 0), (0, 1)]):
+        y0, y1, y2, y3 = (int(v) for v in philox.philox4x32_10(c0, c1, 3, 0, 42, 0))
+        v1 = ((y0 >> 6) * 2 ** 27 + (y1 >> 5) + 0.5) / 2 ** 53
+        v2 = ((y2 >> 6) * 2 ** 27 + (y3 >> 5) + 0.5) / 2 ** 53
+        assert abs(zz[j] - math.sqrt(-2 * math.log(v1)) * math.cos(2 * math.pi * v2)) < 4e-16 * max(1.0, abs(zz[j]))
+
+
 def test_gaussian_moments():
     z = philox.gaussians(1234, 7, 0, 0, 2_000_000)
     assert abs(z.mean()) < 4 / math.sqrt(z.size)
@@ -372,6 +393,20 @@ def test_triad_isometries_are_top_eigenvectors_of_the_definition():
     gram_y = np.einsum("ijklmnog,ijklmnoh,gpqrstwx,huvrstwx->pquv", half_u, half_u, half_l, half_l, optimize=True)
     lam_y = np.linalg.eigvalsh(gram_y.reshape(d2 * d3, -1))[::-1]
     assert np.abs(lam_y - spec[2]).max() < 1e-12 * lam_y[0]
+    # ":137 the other isometries ... in the same manner": U^X on the legs (i2,i3) of X (= forward legs of the lower site),
+    # U^D on the legs (j2,j3) of D (backward legs of the lower site); each eigenvector set checked against the full Gamma
+    gram_x = np.einsum("ijklmnog,ijkluvoh,gpqrstwx,hpqrstwx->mnuv", half_u, half_u, half_l, half_l, optimize=True)
+    gram_d = np.einsum("ijklmnog,ijklmnoh,gpqrstwx,hpqrsuvx->twuv", half_u, half_u, half_l, half_l, optimize=True)
+    for gram, iso, sp in ((gram_x, ux, spec[1]), (gram_y, uy, spec[2]), (gram_d, ud, spec[3])):
+        gm = gram.reshape(d2 * d3, -1)
+        lam_i = np.linalg.eigvalsh(gm)[::-1]
+        assert np.abs(lam_i - sp).max() < 1e-12 * lam_i[0]
+        ki = iso.shape[-1]
+        im = iso.reshape(d2 * d3, ki)
+        assert np.abs(im.T @ im - np.eye(ki)).max() < 1e-12
+        assert np.abs(gm @ im - im * lam_i[:ki]).max() < 1e-10 * lam_i[0]
+    # the four Gram matrices are genuinely different objects (a swapped pair would fail the lines above)
+    assert abs(spec[0][1] / spec[0][0] - spec[1][1] / spec[1][0]) > 1e-6 or abs(spec[2][1] / spec[2][0] - spec[3][1] / spec[3][0]) > 1e-6
 
 
 def test_squeezer_grams_staged_equals_direct():
@@ -416,6 +451,90 @@ def test_squeezer_pair_is_the_optimal_oblique_projector():
     err = np.linalg.norm(g1 @ g2 - g1 @ mm @ nn.T @ g2)
     assert abs(err - math.sqrt((sv[k:] ** 2).sum())) < 1e-10 * sv[0]
     assert np.abs(s[:k] * sv[0] - sv[:k]).max() < 1e-12 * sv[0]
+
+
+def _unit_cell_halves(last):
+    """Upper half  U[i1, i2u,i2l, i3u,i3l, i4u,i4l, g] = sum E F I J  (F carries sigma, Eq. 2.11 :151) and lower half
+    L[g, j1, j2u,j2l, j3u,j3l, j4u,j4l] = sum G H K L (Eq. 2.12-2.13, 2.16-2.17) of Gamma^Triad, written out in full."""
+    e, f, g, h = last["efgh"]
+    ua, ux, uy, ud = last["u"]
+    up = np.einsum("ikua,axlg,bck,dex->ibdceulg", e, f, ua, ux)
+    lo = np.einsum("byug,jdlb,acy,etd->gjaectul", g, h, uy, ud)
+    return up, lo
+
+
+@pytest.mark.parametrize("D,p,h,steps", [(2, 2, 0.0, 4), (3, 2, 0.05, 4), (3, 3, 0.0, 5)])
+def test_step_wires_the_squeezers_as_the_optimal_projectors_between_adjacent_cells(D, p, h, steps):
+    """:113 'squeezers ... achieving the lower bound of the Frobenius norm with the adjacent unit cell', :171 'derived from
+    Gamma^Triad' (reading R6), in the TRUNCATED regime (k = D < rank).  With G1 = upper half of the cell as a matrix
+    [rest, forward pair alpha] and G2 = sigma-weighted lower half of the neighbouring cell [backward pair alpha, rest], the pair
+    (M, N) that TatrgOracle.step() returns for direction alpha must reach the Eckart-Young bound
+    ||G1 G2 - G1 M N^T G2||_F^2 = sum_{i>k} s_i(G1 G2)^2, and a mis-wired step (M <-> N, sigma weight dropped, the
+    (upper, lower) legs of the doubled bond transposed) must not."""
+    o = O.TatrgOracle(0.1497, h, D, p, 5, n_pow=2)
+    for _ in range(steps):
+        o.step()
+    last = o.last
+    up, lo = _unit_cell_halves(last)
+    los = lo * last["sig"][:, None, None, None, None, None, None, None]
+    for mu in (2, 3, 4):
+        au, al = 2 * mu - 3, 2 * mu - 2                       # axes of the forward pair in `up`
+        g1 = np.moveaxis(up, (au, al), (-2, -1))
+        du, dl = g1.shape[-2:]
+        g1 = g1.reshape(-1, du * dl)
+        lo_t = np.moveaxis(lo, (au + 1, al + 1), (0, 1)).reshape(du * dl, -1)
+        g2 = np.moveaxis(los, (au + 1, al + 1), (0, 1)).reshape(du * dl, -1)
+        m, n = last["m"][mu], last["n"][mu]
+        k = m.shape[-1]
+        mm, nn = m.reshape(du * dl, k), n.reshape(du * dl, k)
+        assert np.abs(nn.T @ mm - np.eye(k)).max() < 1e-10
+        sv = np.linalg.svd(g1 @ g2, compute_uv=False)
+        assert k <= D and sv[k] > 1e-4 * sv[0]               # something IS discarded: the truncated regime
+        best = (sv[k:] ** 2).sum()
+        err = lambda a, b, rhs: np.linalg.norm(g1 @ rhs - g1 @ a @ b.T @ rhs) ** 2
+        assert abs(err(mm, nn, g2) - best) < 1e-9 * sv[0] ** 2
+        assert np.abs(last["squeezer_spectra"][mu][:k] * sv[0] - sv[:k]).max() < 1e-10 * sv[0]
+        # mis-wirings
+        assert err(nn, mm, g2) > best * (1 + 1e-3)                                   # M <-> N
+        mt = m.transpose(1, 0, 2).reshape(du * dl, k)
+        nt = n.transpose(1, 0, 2).reshape(du * dl, k)
+        assert err(mt, nt, g2) > best * (1 + 1e-3)                                   # (upper, lower) transposed
+        sv_t = np.linalg.svd(g1 @ lo_t, compute_uv=False)
+        assert err(mm, nn, lo_t) > (sv_t[k:] ** 2).sum() * (1 + 1e-3)                # sigma weight dropped: not optimal there
+    # M goes to Phi' (Eq. 2.18 :175), N to Psi' (Eq. 2.19), sigma enters once (through F); then the rotation R5
+    m2, m3, m4 = (last["m"][mu] for mu in (2, 3, 4))
+    n2, n3, n4 = (last["n"][mu] for mu in (2, 3, 4))
+    phi_new = np.einsum("ibdceulg,bdx,cey,ulz->ixyzg", up, m2, m3, m4, optimize=True)
+    psi_new = np.einsum("gjaectul,aex,cty,ulz->jxyzg", lo, n2, n3, n4, optimize=True)
+    assert np.abs(o.phi - phi_new.transpose(1, 2, 3, 0, 4)).max() < 1e-12 * np.abs(phi_new).max()
+    assert np.abs(o.psi - psi_new.transpose(1, 2, 3, 0, 4)).max() < 1e-12 * np.abs(psi_new).max()
+
+
+@pytest.mark.parametrize("D,p", [(2, 2), (3, 6)])
+def test_squeezer_grams_are_the_grams_of_the_whole_unit_cell_without_triad_truncation(D, p):
+    """R6's canonical-form shortcut (:137): with K = the full pair dimension nothing is lost in the triad split, the lower half
+    is isometric and the upper half is (isometry) x sigma, so the Gram matrix of the WHOLE cell Gamma^ATRG = A X sigma Y D
+    (Eq. 2.6 :98) on a forward pair equals Theta_f (upper half only) and on a backward pair equals Theta_b (sigma-weighted lower half)."""
+    o = O.TatrgOracle(0.1497, 0.02, D, p, 9, n_pow=2, K=D * D)
+    for _ in range(4):
+        o.step()
+    last = o.last
+    a, dt, x, y, sig = last["a"], last["dt"], last["x"], last["y"], last["sig"]
+    # Gamma[i1, i2u,i3u,i4u, i2l,i3l,i4l, j2u,j3u,j4u, j1, j2l,j3l,j4l]
+    gam = np.einsum("iuvwa,axyzg,g,bpqrg,jstcb->iuvwxyzpqrjstc", a, x, sig, y, dt, optimize=True)
+    e, f, g, h = last["efgh"]
+    ua, ux, uy, ud = last["u"]
+    for mu in (2, 3, 4):
+        fu, fl = mu - 1, mu + 2
+        gf = np.moveaxis(gam, (fu, fl), (-2, -1))
+        du, dl = gf.shape[-2:]
+        gf = gf.reshape(-1, du * dl)
+        th_f = O.squeezer_grams(e, f, ua, ux, mu).reshape(du * dl, du * dl)
+        assert np.abs(gf.T @ gf - th_f).max() < 1e-11 * np.abs(th_f).max()
+        bu, bl = mu + 5, mu + 9
+        gb = np.moveaxis(gam, (bu, bl), (0, 1)).reshape(du * dl, -1)
+        th_b = O.squeezer_grams_lower(g * sig, h, uy, ud, mu).reshape(du * dl, du * dl)
+        assert np.abs(gb @ gb.T - th_b).max() < 1e-11 * np.abs(th_b).max()
 
 
 def test_z2_symmetry_in_exact_swap_mode():
