@@ -8,8 +8,10 @@
  *
  * Pointers are marked  [dev]  (device memory, FP64 unless stated, 16-byte aligned)  or  [host].
  * The library never frees caller memory and never allocates device memory of its own.  All work of a call is ordered on
- * the caller's stream; the eigen-decompositions additionally use ONE auxiliary high-priority stream and a few events that
- * the library creates on first use (forked from and joined back into the caller's stream inside the call).
+ * the caller's stream.  Inside a call the independent solver chains run on auxiliary streams that the library creates on
+ * first use, once per device, and never destroys: four chain streams and one stage stream (subspace iterations, Cholesky
+ * chains, squeezers) plus one solver stream of the block-Jacobi eigen-decomposition, all non-blocking and of the greatest
+ * priority, with the events that fork them from and join them back into the caller's stream before the call returns.
  */
 #ifndef TATRG_H
 #define TATRG_H
@@ -86,6 +88,8 @@ int tatrg_set_option(tatrg_handle, int key, double value);
  * what is enqueued on it afterwards.  Handles on the same device must not be stepped from several host threads at once.
  * Errors: ECUDA, ENUMERIC (non-finite or non-positive normalisation), ENOMEM, ESTATE (after an earlier failure). */
 int tatrg_step(tatrg_handle, void* cuda_stream);
+/* Streams: consecutive calls may use different streams; a call on a stream other than the previous step's first waits (on the
+ * device) for an event recorded at the end of that step, so the state is never read before it is complete. */
 
 /* ln Z / V of the periodic lattice of V = 2^steps sites: sum_j 2^-j ln c_j + 2^-m ln tTr(T^(m)) (R8).
  * Synchronises the stream of the last step.  NaN on error. */

@@ -9,7 +9,7 @@ Philox4x32-10".  The stream layout is reading R11 of DESIGN.md:
     key     = (seed & 0xffffffff, seed >> 32)
     counter = (e & 0xffffffff, e >> 32, call, stream)     e = element index, call = RG step, stream = 0 Omega / 1 rho
     (x0,x1,x2,x3) = philox4x32_10(counter, key)
-    u1 = ((x0 >> 6) * 2^27 + (x1 >> 5) + 0.5) * 2^-53      in (0,1)
+    u1 = ((x0 >> 6) * 2^27 + (x1 >> 5) + 0.5) * 2^-53      in (0,1]
     u2 = ((x2 >> 6) * 2^27 + (x3 >> 5) + 0.5) * 2^-53
     z  = sqrt(-2 ln u1) * cos(2 pi u2)                     one Gaussian per counter
 
@@ -54,7 +54,8 @@ def philox4x32_10(c0, c1, c2, c3, k0, k1):
 
 
 def uniforms53(x0, x1):
-    """(x0>>6)*2^27 + (x1>>5) is a 53-bit integer; +0.5 keeps the result strictly inside (0,1)."""
+    """(x0>>6)*2^27 + (x1>>5) is a 53-bit integer k; (k + 0.5) 2^-53 lies in (0,1]: never 0 (the logarithm is finite); for
+    k = 2^53 - 1 the sum rounds to 2^53 and u = 1 exactly, which gives z = 0."""
     a = (np.asarray(x0, dtype=np.uint64) >> np.uint64(6)).astype(np.float64)
     b = (np.asarray(x1, dtype=np.uint64) >> np.uint64(5)).astype(np.float64)
     return (a * 134217728.0 + b + 0.5) * (1.0 / 9007199254740992.0)

@@ -110,6 +110,7 @@ int tatrg_x_ratio(tatrg_handle c, void* cuda_stream, double* x_out) {
     if (!c || !x_out) return TATRG_EINVAL;
     if (c->failed) return TATRG_ESTATE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (c->done_ev && st != c->last_stream && cudaStreamWaitEvent(st, c->done_ev, 0) != cudaSuccess) return TATRG_ECUDA;
     const int n = (int)c->phi.d[3];
     Tens a; a.p = c->pool.alloc((int64_t)n * n + 2);
     if (!a.p) return TATRG_ENOMEM;
@@ -144,6 +145,7 @@ void tatrg_destroy(tatrg_handle c) {
     if (!c) return;
     for (auto e : c->stage_ev) cudaEventDestroy(e);
     for (auto e : c->cnt.ev_pool) cudaEventDestroy(e);
+    if (c->done_ev) cudaEventDestroy(c->done_ev);
     if (!c->graveyard.empty()) { cudaStreamSynchronize(c->last_stream); for (auto g : c->graveyard) cudaGraphExecDestroy(g); }
     delete c;
 }

@@ -200,11 +200,10 @@ cudaError_t cholesky(cudaStream_t st, int n, double* A, int64_t lda, double* L, 
                      bool reset_info) {
     const int np = (n + PB - 1) / PB;
     double* Linv = work; double* d0 = work + (size_t)np * PB * PB; int* info = (int*)(d0 + n);
-    static bool cfg = false;
-    if (!cfg) {
+    static unsigned long long cfg = 0;
+    if (first_use_on_device(cfg)) {
         cudaError_t ea = cudaFuncSetAttribute(potrf_block_kernel<kPotrfCW>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPotrfSmem);
         if (ea != cudaSuccess) return ea;
-        cfg = true;
     }
     cudaError_t e = cudaSuccess;
     if (reset_info) { e = cudaMemsetAsync(info, 0, sizeof(int), st); count_launch(); }

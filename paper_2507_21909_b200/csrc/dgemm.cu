@@ -266,11 +266,10 @@ struct Args {
 template <class C_, bool A_KC, bool B_KC, bool AV, bool BV>
 cudaError_t launch(const Args& a) {
     auto kern = dgemm_kernel<C_, A_KC, B_KC, AV, BV>;
-    static bool configured = false;
-    if (!configured) {
+    static unsigned long long configured = 0;
+    if (first_use_on_device(configured)) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C_::SMEM);
         if (e != cudaSuccess) return e;
-        configured = true;
     }
     int64_t tm = (a.M + C_::BM - 1) / C_::BM, tn = (a.N + C_::BN - 1) / C_::BN;
     dim3 grid((unsigned)(tm * tn), 1, (unsigned)a.batch);

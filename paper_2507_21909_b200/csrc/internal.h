@@ -42,6 +42,14 @@ inline void count_sync() { if (g_counter) g_counter->host_syncs += 1; }
 // TATRG_OPT_VERBOSE of the handle whose step is being enqueued (debugging aid): bit 0 solver chains, bit 1 eigh, bit 2 per-DGEMM rates
 extern thread_local int g_verbose;
 
+// cudaFuncSetAttribute (the > 48 KB shared-memory opt-in) is per device: true the first time a launcher runs on the current device
+inline bool first_use_on_device(unsigned long long& seen) {
+    int dev = 0; cudaGetDevice(&dev);
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (seen & bit) return false;
+    seen |= bit; return true;
+}
+
 // ---- kernels (each file exposes host launchers only) --------------------------------------------------------
 // dgemm.cu : C[M,N] = alpha*op(A)*op(B) + beta*C on FP64 tensor cores (DMMA m8n8k4)
 cudaError_t dgemm(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,

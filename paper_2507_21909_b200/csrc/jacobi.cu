@@ -629,12 +629,11 @@ static Aux& aux() {
 // launch latency of a round is paid once for the whole batch.  All matrices are padded to the largest one.
 int eigh_batched(cudaStream_t st, int count, const EighItem* items, void* work, std::string* err) {
     if (count <= 0) return TATRG_OK;
-    static bool cfg = false;
-    if (!cfg) {
+    static unsigned long long cfg = 0;
+    if (first_use_on_device(cfg)) {
         if (!check(cudaFuncSetAttribute(eigh_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmallSmem), err, "eigh attr")) return TATRG_ECUDA;
         if (!check(cudaFuncSetAttribute(blk_solve2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSolve2Smem), err, "eigh attr")) return TATRG_ECUDA;
         if (!check(cudaFuncSetAttribute(blk_apply2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kApplySmem), err, "eigh attr")) return TATRG_ECUDA;
-        cfg = true;
     }
     int nmax = 0;
     for (int i = 0; i < count; ++i) { if (items[i].n <= 0) { if (err) *err = "eigh: empty matrix"; return TATRG_EINVAL; } nmax = std::max(nmax, items[i].n); }
@@ -743,7 +742,9 @@ int svd_rows(cudaStream_t st, int nv, int len, const double* X, double* s, doubl
     if (nv <= 0 || len <= 0) return TATRG_OK;
     size_t smem = 8 * ((size_t)nv * (len + 1) + (size_t)nv * (nv + 1));
     if (smem > 200 * 1024) { if (err) *err = "svd_rows: matrix too large for shared memory"; return TATRG_EINVAL; }
-    static size_t cfg = 0;
+    static size_t cfg_dev[64] = {0};
+    int dev = 0; cudaGetDevice(&dev);
+    size_t& cfg = cfg_dev[dev & 63];
     if (smem > cfg) {
         if (!check(cudaFuncSetAttribute(svd_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err, "svd attr")) return TATRG_ECUDA;
         cfg = smem;

@@ -1317,6 +1317,8 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
     c->graveyard.clear();
     int rc = TATRG_OK;
     const size_t lnc0 = c->lnc.size();
+    // the state (Phi, Psi, trace) and the workspace were last written on last_stream: order a different stream behind it
+    if (c->done_ev && st != c->last_stream && cudaStreamWaitEvent(st, c->done_ev, 0) != cudaSuccess) { c->err = "cannot order the new stream behind the previous step"; return TATRG_ECUDA; }
     try {
         Stepper s(*c, st);
         s.run();
@@ -1328,6 +1330,10 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
     g_counter = nullptr;
     g_verbose = 0;
     c->last_stream = st;
+    if (rc == TATRG_OK) {
+        if (!c->done_ev && cudaEventCreateWithFlags(&c->done_ev, cudaEventDisableTiming) != cudaSuccess) c->done_ev = nullptr;
+        if (c->done_ev) cudaEventRecord(c->done_ev, st);
+    }
     c->last_launches = cn.launches;
     c->last_host_syncs = cn.host_syncs;
     if (rc != TATRG_OK) { cudaDeviceSynchronize(); c->failed = true; c->lnc.resize(lnc0); return rc; }   // auxiliary streams may still be running

@@ -33,6 +33,7 @@ struct tatrg_ctx {
     int verbose = 0;                 // TATRG_OPT_VERBOSE
     tatrg::Pool pool;
     cudaStream_t last_stream = nullptr;
+    cudaEvent_t done_ev = nullptr;   // recorded on last_stream after the last step: a call on another stream waits for it first
     tatrg::Tens phi, psi;            // state: Phi[i1,i2,i3,i4,g], Psi[j1,j2,j3,j4,g]
     double* trace_dev = nullptr;     // 1 + 148*8 doubles
     std::vector<double> lnc;         // ln c_j

@@ -2,6 +2,7 @@
 
     python tests/golden/make_golden.py c1 c2 c3 [c4:12]      (name[:steps])
     GOLDEN_CKPT=/some/dir python tests/golden/make_golden.py c4:26    (long runs: state saved after each step)
+    python tests/golden/make_golden.py --timing                      (oracle_timing.json: what bench.py scales its CPU sample by)
 
 Each file holds, per step: ln Z/V, the bond-swap spectrum sigma/sigma_1 and the T-decomposition spectrum s/s_1
 for one BASELINE.json config (see tests/inputs.py::configs); these take minutes to hours on a CPU, so the GPU
@@ -27,7 +28,38 @@ RUNS = {
     "c4": [("b0.1497", 0.1497, 0.0, 32, 32, 2, 42, 60)],
 }
 
+def timing():
+    """oracle_timing.json: seconds of the oracle's coarse-graining contraction (Eq. 2.18-2.19, contract_half + contract_psi on
+    saturated D = 32 shapes: the bounded sample bench.py times as cpu_baseline) on THIS box, next to the seconds the oracle took
+    for whole saturated steps of configs[3] on the same box (oracle_c4.json `sec`).  Their ratio turns bench.py's timed sample
+    into seconds per step; both numbers are oracle timings, none comes from the CUDA path."""
+    D, K = 32, 64
+    rng = np.random.default_rng(0)
+    e, h = rng.standard_normal((D, K, D, D)), rng.standard_normal((D, K, D, D))
+    f, g = rng.standard_normal((D, K, D, D)), rng.standard_normal((D, K, D, D))
+    i_, j_ = rng.standard_normal((D, D, K)), rng.standard_normal((D, D, K))
+    m2, m3, m4 = (rng.standard_normal((D, D, D)) for _ in range(3))
+    best = None
+    for _ in range(3):
+        t0 = time.time()
+        O.contract_half(e, f, i_, j_, m2, m3, m4)
+        O.contract_psi(g, h, i_, j_, m2, m3, m4)
+        dt = time.time() - t0
+        best = dt if best is None else min(best, dt)
+    here = os.path.dirname(__file__)
+    sec = json.load(open(os.path.join(here, "oracle_c4.json")))["runs"][0]["sec"]
+    sat = sorted(sec[5:])                      # steps 6.. are saturated
+    out = {"generator": "tests/golden/make_golden.py --timing (oracle only)", "cores": os.cpu_count(),
+           "contraction_sample_s": round(best, 3), "saturated_step_s_median": sat[len(sat) // 2], "saturated_steps_recorded": len(sat),
+           "saturated_step_s_all": sat}
+    json.dump(out, open(os.path.join(here, "oracle_timing.json"), "w"), indent=1)
+    print(out)
+
+
 if __name__ == "__main__":
+    if "--timing" in sys.argv:
+        timing()
+        sys.exit(0)
     for arg in sys.argv[1:]:
         name, _, lim = arg.partition(":")
         out = {"generator": "tests/golden/make_golden.py (oracle only)", "runs": []}

@@ -413,26 +413,26 @@ def test_subspace_path_falls_back_on_rank_deficient_blocks(D, beta, h, steps):
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("D,steps", [(16, 10), (32, 8)])
-def test_overlapped_schedule_equals_the_serial_one(D, steps, monkeypatch):
+def test_overlapped_schedule_equals_the_serial_one(D, steps):
     """Saturated steps run the squeezer chains on an auxiliary stream beside the Gram matrices and the Xi products of
-    Eq. 2.18-2.19 (schedule).  TATRG_NO_OVERLAP=1 issues the same work on one stream: the results
-    are the same numbers (no arithmetic differs, only what runs beside what; the bound leaves room for nothing but that)."""
+    Eq. 2.18-2.19 (schedule).  TATRG_OPT_OVERLAP = 0 issues the same work on one stream, TATRG_OPT_GRAPHS = 0
+    launches the iteration steps one by one instead of replaying a captured graph: the results are the same numbers (no arithmetic
+    differs, only what runs beside what; the bound leaves room for nothing but that)."""
     runs = []
-    for serial in (False, True):
-        if serial:
-            monkeypatch.setenv("TATRG_NO_OVERLAP", "1")
-        else:
-            monkeypatch.delenv("TATRG_NO_OVERLAP", raising=False)
+    for overlap, graphs in ((1, 1), (0, 1), (1, 0)):
         t = T.Tatrg(0.1497, 0.0, D, D, 5)
+        t.set_option(T.OPT_OVERLAP, overlap)
+        t.set_option(T.OPT_GRAPHS, graphs)
         out = []
         for _ in range(steps):
             t.step()
             out.append((t.lnZ_per_site(), t.singular_values(T.SV_SIGMA, D), t.singular_values(T.SV_S, D)))
         runs.append(out)
         t.close()
-    for a, b in zip(*runs):
-        assert abs(a[0] - b[0]) <= 1e-13 * abs(b[0])
-        assert np.abs(a[1] - b[1]).max() <= 1e-12 and np.abs(a[2] - b[2]).max() <= 1e-12
+    for other in runs[1:]:
+        for a, b in zip(runs[0], other):
+            assert abs(a[0] - b[0]) <= 1e-13 * abs(b[0])
+            assert np.abs(a[1] - b[1]).max() <= 1e-12 and np.abs(a[2] - b[2]).max() <= 1e-12
 
 
 @pytest.mark.gpu
