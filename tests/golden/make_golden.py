@@ -26,6 +26,9 @@ RUNS = {
            for b, s in zip((0.140, 0.145, 0.1497, 0.155, 0.160), (1, 2, 3, 4, 5))],
     "c3": [("h+1e-3", 0.1497, 1e-3, 16, 16, 2, 7, 48), ("h-1e-3", 0.1497, -1e-3, 16, 16, 2, 7, 48)],
     "c4": [("b0.1497", 0.1497, 0.0, 32, 32, 2, 42, 60)],
+    # configs[4]: only the first steps are affordable (c5:4, c5a:5); the saturated steps are checked slab by slab on the GPU box
+    "c5": [("d48", 0.1497, 0.0, 48, 48, 2, 99, 60)],
+    "c5a": [("atrg_d24", 0.1497, 0.0, 24, 24, 2, 99, 60, {"method": "atrg"})],
 }
 
 def timing():
@@ -63,10 +66,10 @@ if __name__ == "__main__":
     for arg in sys.argv[1:]:
         name, _, lim = arg.partition(":")
         out = {"generator": "tests/golden/make_golden.py (oracle only)", "runs": []}
-        for tag, beta, h, D, p, n_pow, seed, steps in RUNS[name]:
+        for tag, beta, h, D, p, n_pow, seed, steps, *kw in RUNS[name]:
             steps = min(steps, int(lim)) if lim else steps
-            o = O.TatrgOracle(beta, h, D, p, seed, n_pow=n_pow)
-            rec = dict(tag=tag, beta=beta, h=h, D=D, oversample=p, n_pow=n_pow, seed=seed, lnZ=[], sigma=[], s=[], sec=[])
+            o = O.TatrgOracle(beta, h, D, p, seed, n_pow=n_pow, **(kw[0] if kw else {}))
+            rec = dict(tag=tag, beta=beta, h=h, D=D, oversample=p, n_pow=n_pow, seed=seed, lnZ=[], sigma=[], s=[], sec=[], **(kw[0] if kw else {}))
             # optional resume of a multi-hour run: the oracle's whole state is (Phi, Psi, [ln c_m], m) plus what was recorded
             ckpt = os.environ.get("GOLDEN_CKPT") and os.path.join(os.environ["GOLDEN_CKPT"], "ckpt_%s_%s.npz" % (name, tag))
             if ckpt and os.path.exists(ckpt):

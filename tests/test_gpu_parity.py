@@ -257,26 +257,111 @@ def test_d32_stage_properties_and_sampled_contraction():
         assert np.abs(got - slab).max() <= 1e-11 * max(1.0, np.abs(slab).max())
 
 
-def test_config5_d48_runs_and_improves_on_d32():
+def test_config5_d48_against_the_oracle():
     """BASELINE.json configs[4], Triad half (D=48, p=48, K=96, seed 99): the largest size; n = 2304 eigen-problems.
-    No oracle value exists at this size (a saturated oracle step would take hours): properties only --
-    workspace bound, isometry of A, ordered positive spectrum, and ln Z/V above the D=32 value after the same number
-    of steps (the free energy decreases monotonically with D, Fig. 9 :286-288)."""
+    (i) the first steps against the oracle's golden run (tests/golden/oracle_c5.json: the unsaturated steps, which the oracle
+    affords); (ii) at step 6 (saturated: a whole oracle step would take hours) the O(r^2 D^7) contraction of Eq. 2.18-2.19 :175
+    recomputed slab by slab with the oracle's contract_half / contract_psi from the GPU's own triad tensors and squeezers
+    (teacher-forced stage parity at full size), isometries, N^T M = 1; (iii) ln Z/V above the D=32 value after the same number of
+    steps (the free energy decreases monotonically with D, Fig. 9 :286-288)."""
+    from oracle import tatrg_oracle as O
+    path = os.path.join(HERE, "golden", "oracle_c5.json")
+    rec = json.load(open(path))["runs"][0] if os.path.exists(path) else None
     t48 = T.Tatrg(0.1497, 0.0, 48, 48, 99)
-    t48.set_option(T.OPT_KEEP_TENSORS, 1)
     t32 = T.Tatrg(0.1497, 0.0, 32, 32, 99)
-    for _ in range(6):
+    for m in range(6):
+        if m == 5:
+            t48.set_option(T.OPT_KEEP_TENSORS, 1)
         t48.step()
         t32.step()
+        if rec is not None and m < len(rec["lnZ"]):
+            assert abs(t48.lnZ_per_site() - rec["lnZ"][m]) <= TOL_LNZ * abs(rec["lnZ"][m]), m
+            for which, key in ((T.SV_SIGMA, "sigma"), (T.SV_S, "s")):
+                got, ref = np.zeros(48), np.zeros(48)
+                g = t48.singular_values(which, 48)
+                got[:len(g)] = g
+                ref[:len(rec[key][m])] = rec[key][m]
+                assert np.abs(got - ref).max() <= TOL_SV, (m, key)
     assert t48.workspace_peak() <= T.workspace_bytes(48, 48)
     a = t48.get_tensor("A")
     assert a.shape == (48, 48, 48, 48, 48)
     am = a.reshape(-1, 48)
     assert np.abs(am.T @ am - np.eye(48)).max() <= 1e-10
+    del a, am
     sig = t48.singular_values(T.SV_SIGMA, 48)
     assert len(sig) == 48 and np.all(np.diff(sig) <= 0) and sig[-1] > 0
     z48, z32 = t48.lnZ_per_site(), t32.lnZ_per_site()
     assert np.isfinite(z48) and z48 > z32 and z48 - z32 < 5e-3
+    t32.close()
+    tr = lambda m: np.ascontiguousarray(m.transpose(1, 2, 0))             # [k,u,l] -> oracle's [u,l,k]; [k,j,k'] -> [j,k',k]
+    for mu in (2, 3, 4):
+        mg, ng = t48.get_tensor("M%d" % mu), t48.get_tensor("N%d" % mu)
+        assert np.abs(np.einsum("kul,jul->kj", mg, ng) - np.eye(mg.shape[0])).max() <= 1e-8
+    e, f, g, h = (t48.get_tensor(n) for n in "EFGH")
+    ua, ux, uy, ud = (tr(t48.get_tensor(n)) for n in ("UA", "UX", "UY", "UD"))
+    ms = [tr(t48.get_tensor("M%d" % mu)) for mu in (2, 3, 4)]
+    ns = [tr(t48.get_tensor("N%d" % mu)) for mu in (2, 3, 4)]
+    assert e.shape == (48, 96, 48, 48) and ua.shape == (48, 48, 96)
+    rng = np.random.default_rng(1)
+    phi = t48.get_tensor("phi")                                            # [k2,k3,k4,i1,g]
+    i1 = int(rng.integers(0, 48))
+    slab = O.contract_half(e[i1:i1 + 1], f, ua, ux, *ms)[0]                # [k2,k3,k4,g]
+    assert np.abs(phi[:, :, :, i1, :] - slab).max() <= 1e-11 * max(1.0, np.abs(slab).max())
+    del phi
+    psi = t48.get_tensor("psi")
+    j1 = int(rng.integers(0, 48))
+    slab = O.contract_psi(g, h[j1:j1 + 1], uy, ud, *ns)[0]
+    assert np.abs(psi[:, :, :, j1, :] - slab).max() <= 1e-11 * max(1.0, np.abs(slab).max())
+    t48.close()
+
+
+def test_config5_plain_atrg_d24_sliced_contraction_against_the_oracle():
+    """BASELINE.json configs[4], plain-ATRG half (D=24, p=24, seed 99; Eq. 2.7-2.8 :106-109).  The library never stores
+    the D^7 intermediate (fn 6 :205 "memory blocking"): it slices the O(D^9) contraction over the outer leg.  At a saturated step
+    (a whole oracle step is out of reach) 24 fibres of Phi' and 24 of Psi' are recomputed with the oracle's contract_atrg -- ONE
+    einsum, the definition -- from the GPU's own A, X sigma, Y, D and squeezers; plus the first steps against the golden run when
+    tests/golden/oracle_c5a.json exists."""
+    from oracle import tatrg_oracle as O
+    path = os.path.join(HERE, "golden", "oracle_c5a.json")
+    rec = json.load(open(path))["runs"][0] if os.path.exists(path) else None
+    D = 24
+    t = T.Tatrg(0.1497, 0.0, D, D, 99, method=T.METHOD_ATRG)
+    for m in range(6):
+        if m == 5:
+            t.set_option(T.OPT_KEEP_TENSORS, 1)
+        t.step()
+        if rec is not None and m < len(rec["lnZ"]):
+            assert abs(t.lnZ_per_site() - rec["lnZ"][m]) <= TOL_LNZ * abs(rec["lnZ"][m]), m
+            got, ref = np.zeros(D), np.zeros(D)
+            g = t.singular_values(T.SV_SIGMA, D)
+            got[:len(g)] = g
+            ref[:len(rec["sigma"][m])] = rec["sigma"][m]
+            assert np.abs(got - ref).max() <= TOL_SV, m
+    a, x, y, dt, sig = (t.get_tensor(n) for n in ("A", "X", "Y", "Dt", "sigma"))
+    assert a.shape == (D,) * 5 and x.shape[:4] == (D,) * 4
+    tr = lambda m: np.ascontiguousarray(m.transpose(1, 2, 0))             # [k,u,l] -> oracle's [u,l,k]
+    ms = [tr(t.get_tensor("M%d" % mu)) for mu in (2, 3, 4)]
+    ns = [tr(t.get_tensor("N%d" % mu)) for mu in (2, 3, 4)]
+    xs = x * sig
+    phi = t.get_tensor("phi")                                              # [k2,k3,k4,i1,g]
+    rng = np.random.default_rng(2)
+    # sampled outputs, one fibre (all k4 at fixed i1, k2, k3, g) at a time: with every free leg but one cut to a single value
+    # the oracle's one-einsum definition costs O(D^5) per fibre (a whole slab of it would take hours: its einsum path degenerates)
+    scale = np.abs(phi).max()
+    for _ in range(24):
+        i1, k2, k3, gg = (int(v) for v in rng.integers(0, D, size=4))
+        fib = O.contract_atrg(a[i1:i1 + 1], xs[..., gg:gg + 1], ms[0][:, :, k2:k2 + 1], ms[1][:, :, k3:k3 + 1], ms[2])[0, 0, 0, :, 0]   # Eq. 2.7
+        assert np.abs(phi[k2, k3, :, i1, gg] - fib).max() <= 1e-11 * scale
+    # Eq. 2.8: the lower half is Y[be,u2,u3,u4,g] (upper site) . D[j1,l2,l3,l4,be] (lower site) with the squeezers N
+    yp = np.ascontiguousarray(y.transpose(4, 1, 2, 3, 0))                 # [g,u2,u3,u4,be]
+    dp = np.ascontiguousarray(dt.transpose(4, 1, 2, 3, 0))                # [be,l2,l3,l4,j1]
+    psi = t.get_tensor("psi")                                              # [k2,k3,k4,j1,g]
+    scale = np.abs(psi).max()
+    for _ in range(24):
+        j1, k2, k3, gg = (int(v) for v in rng.integers(0, D, size=4))
+        fib = O.contract_atrg(yp[gg:gg + 1], dp[..., j1:j1 + 1], ns[0][:, :, k2:k2 + 1], ns[1][:, :, k3:k3 + 1], ns[2])[0, 0, 0, :, 0]
+        assert np.abs(psi[k2, k3, :, j1, gg] - fib).max() <= 1e-11 * scale
+    t.close()
 
 
 def test_x_ratio_matches_oracle_and_closed_form():
