@@ -193,6 +193,16 @@ int tatrg_gram(void* cuda_stream, long long m, int n, const double* X, double* G
 size_t tatrg_cholqr_work_bytes(int n);
 int tatrg_cholqr(void* cuda_stream, long long m, int n, double* X, double* Q, double* R, void* work);
 
+/* Truncated Cholesky factorisation with diagonal pivoting (the rank-revealing first half of the QR pre-reduction, Eq. A.2-A.3
+ * :345-348, when the operand is numerically rank-deficient; R14):  G [dev] n x n row-major, symmetric positive
+ * semi-definite up to rounding (preserved) = L L^T + S.  L [dev] n x n row-major: rows in the ORIGINAL order, column j belongs
+ * to the j-th pivot (the largest remaining diagonal entry, lowest index on ties); only columns 0..rank-1 are written.  The
+ * factorisation stops as soon as the remaining Schur complement S has tr S <= tol_rel * tr G (S is positive semi-definite, so
+ * ||G - L L^T||_2 <= tr S).  *rank_out, *resid_out [host]: number of pivots taken, tr S / tr G.  One cooperative kernel on 64 CTAs.
+ * work [dev] >= tatrg_pchol_work_bytes(n), 256-byte aligned.  Synchronises.  EINVAL for n < 1 or tol_rel < 0. */
+size_t tatrg_pchol_work_bytes(int n);
+int tatrg_pchol(void* cuda_stream, int n, const double* G, double* L, double tol_rel, void* work, int* rank_out, double* resid_out);
+
 /* result[0] [dev] = sum_i x[i]*y[i]  (the tensor trace tTr of Eq. 2.1 :48 on the factored tensor).
  * result must have room for 1200 doubles (partial sums of the first pass follow result[0]). */
 int tatrg_dot(void* cuda_stream, long long n, const double* x, const double* y, double* result);

@@ -68,6 +68,8 @@ _SIGNATURES = {
                              _c.c_void_p]),
     "tatrg_gram_scratch_bytes": (_c.c_size_t, [_c.c_longlong, _c.c_int]),
     "tatrg_gram": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
+    "tatrg_pchol_work_bytes": (_c.c_size_t, [_c.c_int]),
+    "tatrg_pchol": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_double, _c.c_void_p, _c.POINTER(_c.c_int), _c.POINTER(_c.c_double)]),
     "tatrg_cholqr_work_bytes": (_c.c_size_t, [_c.c_int]),
     "tatrg_cholqr": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
     "tatrg_dot": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
@@ -374,6 +376,18 @@ def cholqr(X):
     work = torch.empty(lib().tatrg_cholqr_work_bytes(n), dtype=torch.uint8, device=X.device)
     _check(lib().tatrg_cholqr(_stream_ptr(), m, n, _p(x), _p(q), _p(r), _p(work)), "tatrg_cholqr")
     return q, r
+
+
+def pchol(G, tol_rel=1e-14):
+    """G = L L^T + S by truncated Cholesky with diagonal pivoting (torch CUDA float64, n x n): (L[:, :rank], rank, tr S / tr G)."""
+    torch = _torch_cuda()
+    n = G.shape[0]
+    g = G.contiguous()
+    L = torch.zeros((n, n), dtype=torch.float64, device=G.device)
+    work = torch.empty(lib().tatrg_pchol_work_bytes(n), dtype=torch.uint8, device=G.device)
+    rank, resid = ctypes.c_int(), ctypes.c_double()
+    _check(lib().tatrg_pchol(_stream_ptr(), n, _p(g), _p(L), tol_rel, _p(work), ctypes.byref(rank), ctypes.byref(resid)), "tatrg_pchol")
+    return L[:, :rank.value], rank.value, resid.value
 
 
 def dot(x, y):

@@ -298,6 +298,18 @@ int tatrg_cholqr(void* stp, long long m, int n, double* X, double* Q, double* R,
     if (e != cudaSuccess) return TATRG_ECUDA;
     return info == 0 ? TATRG_OK : TATRG_ENUMERIC;
 }
+size_t tatrg_pchol_work_bytes(int n) { return n > 0 ? 8 * pchol_work_doubles(n) + 4096 : 0; }
+int tatrg_pchol(void* stp, int n, const double* G, double* L, double tol_rel, void* work, int* rank_out, double* resid_out) {
+    if (n < 1 || !(tol_rel >= 0) || !G || !L || !work || !rank_out || !resid_out) return TATRG_EINVAL;
+    cudaStream_t st = (cudaStream_t)stp;
+    double info[4] = {0, 0, 0, 0};
+    cudaError_t e = pchol(st, n, G, L, n, tol_rel, (double*)work);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(info, pchol_info((const double*)work), sizeof info, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return TATRG_ECUDA;
+    *rank_out = (int)info[0]; *resid_out = info[2] > 0 ? info[1] / info[2] : 0.0;
+    return TATRG_OK;
+}
 int tatrg_dot(void* st, long long n, const double* x, const double* y, double* result) {
     if (n < 0 || !x || !y || !result) return TATRG_EINVAL;
     return dot((cudaStream_t)st, n, x, y, result) == cudaSuccess ? TATRG_OK : TATRG_ECUDA;

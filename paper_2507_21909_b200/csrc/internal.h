@@ -114,6 +114,11 @@ cudaError_t tri_inverse(cudaStream_t st, int n, const double* L, int64_t ldl, co
 const double* cholesky_d0(const double* work, int n);                           // [dev] the n original diagonal entries
 cudaError_t extract_diag(cudaStream_t st, int n, const double* A, int64_t lda, double* d);
 
+// pchol.cu : truncated Cholesky with diagonal pivoting, G = L L^T + S with tr S <= tol_rel tr G (one cooperative kernel)
+size_t pchol_work_doubles(int n);
+cudaError_t pchol(cudaStream_t st, int n, const double* G, double* L, int64_t ldl, double tol_rel, double* work);
+const double* pchol_info(const double* work);                                   // [dev] rank, residual trace, tr G, first pivot
+
 // ---- tensors and the workspace pool -------------------------------------------------------------------------
 struct Tens {
     double* p = nullptr;

@@ -282,7 +282,7 @@ struct Stepper {
     // factorisation + inversion chains (latency-bound: ~60 small launches each) side by side on two auxiliary streams, then
     // the decisions and the two Q = mat L^-T products.  All buffers are allocated before the fork; nothing is allocated or
     // freed while the chains are in flight.  Returns false (nothing kept but the Gram matrices, see Gkeep) unless both operands
-    // prove full rank.
+    // prove full rank.  The proof here is sharper than orth_chol()'s: lam_min >= ||G^-4||_F^(-1/4) instead of 1 / tr G^-1.
     // Xinv != nullptr: Q = mat L^-T is NOT formed; the caller gets Xinv[i] = L^-1 instead (Q[i].p stays null) and applies it
     // to whatever multiplies Q (bond_swap: Q only ever appears in products, so two n x n x n GEMMs replace two m x n x n ones).
     // meanwhile: work for the caller's stream that does not depend on the factors, issued while the two chains are in flight
@@ -294,11 +294,12 @@ struct Stepper {
         Scope sc(*this);
         const int64_t m = m0.d[0], n = m0.d[1];
         const Tens* mats[2] = {&m0, &m1};
-        Tens G[2], L[2], X[2], T[2]; double* cw[2]; double* res[2];
+        Tens G[2], L[2], X[2], T[2], W[2], W2[2]; double* cw[2]; double* res[2];
         for (int i = 0; i < 2; ++i) {
             G[i] = mm(true, false, n, n, m, mats[i]->p, n, mats[i]->p, n, true);
             L[i] = make({n, n}); X[i] = make({n, n}); T[i] = make({(int64_t)tri_inverse_scratch_doubles((int)n)});
             cw[i] = raw((int64_t)cholesky_work_doubles((int)n)); res[i] = raw(1 + 148 * 8 + 7);
+            W[i] = make({n, n}); W2[i] = make({n, n});
             ck(fill_zero(st, L[i].p, n * n), "zero"); ck(fill_zero(st, X[i].p, n * n), "zero");
         }
         if (ss.ok) ck(cudaEventRecord(ss.fork, st), "event");
@@ -307,7 +308,12 @@ struct Stepper {
             if (ss.ok) ck(cudaStreamWaitEvent(a, ss.fork, 0), "wait");
             ck(cholesky(a, (int)n, G[i].p, n, L[i].p, n, 0.0, 1e-14, cw[i]), "cholesky");
             ck(tri_inverse(a, (int)n, L[i].p, n, cw[i], X[i].p, n, T[i].p), "tri_inverse");
-            ck(dot(a, n * n, X[i].p, X[i].p, res[i]), "dot");
+            // ||G^-4||_F = (sum_i lam_i^-8)^1/2 >= lam_min^-4: three n^3 products (0.1 ms each) for a bound on lam_min that is
+            // within (number of eigenvalues near lam_min)^1/8 of it (tr G^-1 = ||L^-1||_F^2 overshoots by that number itself)
+            ck(dgemm(a, true, false, n, n, n, 1.0, X[i].p, n, X[i].p, n, 0.0, W[i].p, n), "dgemm");       // G^-1 = L^-T L^-1
+            ck(dgemm(a, false, false, n, n, n, 1.0, W[i].p, n, W[i].p, n, 0.0, W2[i].p, n), "dgemm");     // G^-2
+            ck(dgemm(a, false, false, n, n, n, 1.0, W2[i].p, n, W2[i].p, n, 0.0, W[i].p, n), "dgemm");    // G^-4
+            ck(dot(a, n * n, W[i].p, W[i].p, res[i]), "dot");
             if (ss.ok) ck(cudaEventRecord(ss.join[i], a), "event");
         }
         if (meanwhile && *meanwhile) (*meanwhile)();
@@ -323,8 +329,9 @@ struct Stepper {
         ck(cudaStreamSynchronize(st), "sync"); count_sync();
         for (int i = 0; i < 2; ++i) {
             double tr = 0; for (double v : d0[i]) tr += v;
-            if (g_verbose & 1) fprintf(stderr, "[tatrg cholesky qr %lld x %lld] info %d, proven lam_min/lam_max >= %.3e\n", (long long)m, (long long)n, info[i], 1.0 / (xn[i] * tr));
-            if (info[i] != 0 || !std::isfinite(xn[i]) || !(xn[i] > 0) || !(tr > 0) || !(1.0 / (xn[i] * tr) > kEpsOrthLambda)) ok = false;
+            const double inv_lmin = std::pow(xn[i], 0.125);        // ||G^-4||_F^(1/4) >= 1 / lam_min
+            if (g_verbose & 1) fprintf(stderr, "[tatrg cholesky qr %lld x %lld] info %d, proven lam_min/lam_max >= %.3e\n", (long long)m, (long long)n, info[i], 1.0 / (inv_lmin * tr));
+            if (info[i] != 0 || !std::isfinite(xn[i]) || !(xn[i] > 0) || !(tr > 0) || !(1.0 / (inv_lmin * tr) > kEpsOrthLambda)) ok = false;
         }
         if (!ok) return false;
         for (int i = 0; i < 2; ++i) {
@@ -332,6 +339,51 @@ struct Stepper {
             else { Q[i] = mm(false, true, m, n, n, mats[i]->p, n, X[i].p, n); keep(Q[i]); }
             R[i] = perm(view(L[i], {n, n}), {1, 0});
             keep(R[i]);
+        }
+        return true;
+    }
+
+    // Rank-revealing path of orth_pair() (R14), Q implicit: the Gram matrices G[i] (preserved) are factored by truncated pivoted
+    // Cholesky, G = L L^T + S with tr S <= 1e-14 tr G (pchol.cu; below the rounding of the DGEMM that formed G and 1 % of the
+    // eigenvalue the rank decision turns on), the r' x r' matrices L^T L -- same non-zero eigenvalues, nearly diagonal --
+    // are eigen-decomposed together (V, lam: 8 Jacobi sweeps instead of 24-32 on G itself, on r' ~ 0.6 n), and with the
+    // eigenvectors U = L V lam^-1/2 of G:  R = lam^1/2 U^T = V^T L^T,  Xinv = lam^-1/2 U^T = lam^-1 R, rows with
+    // lam <= 1e-12 lam_max dropped exactly as in the eigen-decomposition of G itself.
+    bool orth_pchol_pair(Tens G[2], int n, Tens R[2], Tens Xinv[2]) {
+        SubStreams& ss = sub_streams();
+        Scope sc(*this);
+        Tens L[2]; double* pw[2];
+        for (int i = 0; i < 2; ++i) { L[i] = make({n, n}); pw[i] = raw((int64_t)pchol_work_doubles(n)); }
+        if (ss.ok) ck(cudaEventRecord(ss.fork, st), "event");
+        for (int i = 0; i < 2; ++i) {
+            cudaStream_t a = ss.ok ? ss.s[i] : st;
+            if (ss.ok) ck(cudaStreamWaitEvent(a, ss.fork, 0), "wait");
+            ck(pchol(a, n, G[i].p, L[i].p, n, 1e-14, pw[i]), "pchol");
+            if (ss.ok) { ck(cudaEventRecord(ss.join[i], a), "event"); ck(cudaStreamWaitEvent(st, ss.join[i], 0), "wait"); }
+        }
+        double info[2][4];
+        for (int i = 0; i < 2; ++i) ck(cudaMemcpyAsync(info[i], pchol_info(pw[i]), 32, cudaMemcpyDeviceToHost, st), "readback");
+        ck(cudaStreamSynchronize(st), "sync"); count_sync();
+        int rp[2];
+        for (int i = 0; i < 2; ++i) {
+            rp[i] = (int)info[i][0];
+            if (g_verbose & 1) fprintf(stderr, "[tatrg orth %d] pivoted Cholesky: rank %d, residual trace / trace %.2e\n", n, rp[i], info[i][2] > 0 ? info[i][1] / info[i][2] : 0.0);
+            if (rp[i] <= 0 || rp[i] > n || !std::isfinite(info[i][1])) return false;
+        }
+        Tens G1[2];
+        for (int i = 0; i < 2; ++i) G1[i] = mm(true, false, rp[i], rp[i], n, L[i].p, n, L[i].p, n, true);
+        std::vector<EigOut> eo;
+        eig_batch({&G1[0], &G1[1]}, {rp[0], rp[1]}, eo);
+        for (int i = 0; i < 2; ++i) {
+            const std::vector<double>& lh = eo[i].lh;
+            if (!(lh[0] > 0)) fail(TATRG_ENUMERIC, "orth: zero matrix");
+            int r = 0;
+            for (double x : lh) if (x > kEpsOrthLambda * lh[0]) ++r;
+            if (g_verbose & 1) fprintf(stderr, "[tatrg orth %d] eigen-decomposition of L^T L (%d x %d): rank %d\n", n, rp[i], rp[i], r);
+            R[i] = mm(false, true, r, n, rp[i], eo[i].Vt.p, rp[i], L[i].p, n);          // V^T L^T = lam^1/2 U^T
+            Xinv[i] = make({r, n});
+            ck(scale_rows(st, Xinv[i].p, R[i].p, eo[i].lam, r, n, 1), "scale");          // lam^-1/2 U^T
+            keep(R[i]); keep(Xinv[i]);
         }
         return true;
     }
@@ -350,6 +402,7 @@ struct Stepper {
         const Tens* mats[2] = {&m0, &m1};
         Tens G[2];
         for (int i = 0; i < 2; ++i) G[i] = mm(true, false, n, n, m, mats[i]->p, n, mats[i]->p, n, true);
+        if (implicit && orth_pchol_pair(G, (int)n, R, Xinv)) { for (int i = 0; i < 2; ++i) { Q[i] = Tens(); keep(R[i]); keep(Xinv[i]); } return; }
         std::vector<EigOut> eo;
         eig_batch({&G[0], &G[1]}, {(int)n, (int)n}, eo);
         for (int i = 0; i < 2; ++i) {

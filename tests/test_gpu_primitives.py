@@ -228,6 +228,69 @@ def test_cholqr_reports_rank_deficiency(torch):
         T.cholqr(dev(torch, x))
 
 
+def _pivoted_cholesky_by_definition(g, tol_rel):
+    """Greedy definition: always eliminate the largest remaining diagonal entry (lowest index on ties) of the Schur
+    complement, stop when its trace is <= tol_rel tr G.  Returns (pivot order, residual trace / trace)."""
+    s = g.copy()
+    n = len(g)
+    alive = np.ones(n, bool)
+    t0 = np.trace(g)
+    piv = []
+    while True:
+        d = np.where(alive, np.diag(s), -1.0)
+        tr = d[d > 0].sum()
+        k = int(np.argmax(d))
+        if len(piv) == n or not d[k] > 0 or not tr > tol_rel * t0:
+            return piv, tr / t0
+        col = s[:, k] / np.sqrt(d[k])
+        col[~alive] = 0.0
+        s -= np.outer(col, col)
+        alive[k] = False
+        piv.append(k)
+
+
+@pytest.mark.parametrize("n,rank,decades", [(5, 5, 1.0), (64, 64, 3.0), (200, 37, 2.0), (256, 256, 14.0), (513, 300, 20.0), (1024, 1024, 0.5), (1024, 500, 24.0), (1500, 90, 6.0)])
+def test_pivoted_cholesky_is_the_truncated_factorisation(torch, n, rank, decades):
+    """G = L L^T + S with S positive semi-definite and tr S <= tol tr G; the pivots are those of the greedy definition
+    (compared while the remaining diagonal is far above the rounding of the updates); L^T L has the eigenvalues of G."""
+    rng = np.random.default_rng(n + rank)
+    q = np.linalg.qr(rng.standard_normal((n, rank)))[0]
+    lam = 10.0 ** (-decades * np.arange(rank) / max(rank - 1, 1))
+    g = (q * lam) @ q.T
+    g = 0.5 * (g + g.T)
+    tol = 1e-14
+    L, r, resid = T.pchol(dev(torch, g), tol)
+    L = L.cpu().numpy()
+    assert 1 <= r <= min(n, rank + 2) and L.shape == (n, r)
+    s = g - L @ L.T
+    assert np.abs(s).max() <= max(2 * tol * np.trace(g), 64 * EPS * n * np.abs(g).max())
+    assert resid <= tol or r == n
+    assert np.linalg.eigvalsh(s).min() >= -64 * EPS * n * np.abs(g).max()
+    piv, resid_def = _pivoted_cholesky_by_definition(g, tol)
+    # each column of L has its pivot entry as the largest entry: L[k_j, j]^2 is the pivot, |L[i, j]| <= L[k_j, j]
+    mine = [int(np.argmax(np.abs(L[:, j]))) for j in range(r)]
+    safe = sum(1 for j in range(min(r, len(piv))) if L[mine[j], j] ** 2 > 1e-9 * np.abs(g).max())
+    assert mine[:safe] == piv[:safe]
+    assert abs(r - len(piv)) <= max(2, r // 50)
+    # rows that were pivots are zero in later columns (lower triangular in pivot order)
+    for j in range(r):
+        assert np.all(L[mine[:j], j] == 0.0)
+    w = np.sort(np.linalg.eigvalsh(g))[::-1][:r]
+    w1 = np.sort(np.linalg.eigvalsh(L.T @ L))[::-1]
+    assert np.abs(w - w1).max() <= 2 * tol * np.trace(g) + 64 * EPS * n * w[0]
+
+
+def test_pivoted_cholesky_edge_cases(torch):
+    z = np.zeros((17, 17))
+    L, r, resid = T.pchol(dev(torch, z))
+    assert r == 0
+    e = np.eye(3)
+    L, r, resid = T.pchol(dev(torch, e))
+    assert r == 3 and np.array_equal(L.cpu().numpy(), e)           # ties: lowest index first
+    with pytest.raises(T.TatrgError):
+        T.pchol(dev(torch, e), tol_rel=-1.0)
+
+
 @pytest.mark.parametrize("m,n", [(5, 3), (1000, 64), (4096, 256), (33000, 300), (2048, 1024), (777, 513)])
 def test_gram_symmetric_mode_matches_definition(torch, m, n):
     """X^T X with only the lower tiles computed (n >= 256), split along K, mirrored: against the definition, and exactly symmetric."""
