@@ -183,6 +183,16 @@ int tatrg_svd(void* cuda_stream, int nv, int len, const double* X, double* s, do
 size_t tatrg_gram_scratch_bytes(long long m, int n);
 int tatrg_gram(void* cuda_stream, long long m, int n, const double* X, double* G, void* scratch);
 
+/* tatrg_gram for callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): same kernels, same result, but the split-K partial products go to a 16 MiB file-scope __device__ array
+ * inside the library (tatrg_gram_static_max_scratch_bytes(); every GPU that loads the library holds it until exit) instead of
+ * caller scratch.  The call allocates nothing and does not synchronise.  EINVAL, with the reason in err [host, err_cap bytes,
+ * may be NULL], when tatrg_gram_scratch_bytes(m, n) exceeds the array -- use tatrg_gram then.  All calls on a device share the
+ * array: calls whose kernels overlap on the GPU (different streams without ordering) race on it.  Nothing in it has to
+ * start at zero; the previous call's contents are never read. */
+size_t tatrg_gram_static_max_scratch_bytes(void);
+int tatrg_gram_static(void* cuda_stream, long long m, int n, const double* X, double* G, char* err, size_t err_cap);
+
 /* Cholesky QR of a tall matrix (the orthonormalisation of the QR pre-reduction, Eq. A.2-A.3 :345-348, of the RSVD
  * sketches, Eq. A.4-A.6 :352-369, and of the subspace iterations behind Eq. 2.9 :135 and the squeezers :171):
  * X [dev] m x n row-major (m >= n; DESTROYED), Q [dev] m x n with orthonormal columns up to cond(X)^2 eps (one pass),

@@ -68,6 +68,8 @@ _SIGNATURES = {
                              _c.c_void_p]),
     "tatrg_gram_scratch_bytes": (_c.c_size_t, [_c.c_longlong, _c.c_int]),
     "tatrg_gram": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
+    "tatrg_gram_static_max_scratch_bytes": (_c.c_size_t, []),
+    "tatrg_gram_static": (_c.c_int, [_c.c_void_p, _c.c_longlong, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_char_p, _c.c_size_t]),
     "tatrg_pchol_work_bytes": (_c.c_size_t, [_c.c_int]),
     "tatrg_pchol": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_double, _c.c_void_p, _c.POINTER(_c.c_int), _c.POINTER(_c.c_double)]),
     "tatrg_cholqr_work_bytes": (_c.c_size_t, [_c.c_int]),
@@ -363,6 +365,20 @@ def gram(X):
     nb = lib().tatrg_gram_scratch_bytes(m, n)
     scratch = torch.empty(max(nb, 8), dtype=torch.uint8, device=X.device)
     _check(lib().tatrg_gram(_stream_ptr(), m, n, _p(x), _p(g), _p(scratch)), "tatrg_gram")
+    return g
+
+
+def gram_static(X, out=None):
+    """X^T X like gram(), through tatrg_gram_static: no device allocation inside the call (split-K scratch in the library's
+    16 MiB static array).  `out` (n x n, float64, CUDA) lets the caller provide the result buffer too."""
+    torch = _torch_cuda()
+    m, n = X.shape
+    x = X.contiguous()
+    g = out if out is not None else torch.empty((n, n), dtype=torch.float64, device=X.device)
+    err = ctypes.create_string_buffer(512)
+    rc = lib().tatrg_gram_static(_stream_ptr(), m, n, _p(x), _p(g), err, 512)
+    if rc < 0:
+        raise TatrgError("tatrg_gram_static failed with status %d: %s" % (rc, err.value.decode()))
     return g
 
 
