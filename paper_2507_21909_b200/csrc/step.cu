@@ -349,7 +349,7 @@ struct Stepper {
     // are eigen-decomposed together (V, lam: 8 Jacobi sweeps instead of 24-32 on G itself, on r' ~ 0.6 n), and with the
     // eigenvectors U = L V lam^-1/2 of G:  R = lam^1/2 U^T = V^T L^T,  Xinv = lam^-1/2 U^T = lam^-1 R, rows with
     // lam <= 1e-12 lam_max dropped exactly as in the eigen-decomposition of G itself.
-    bool orth_pchol_pair(Tens G[2], int n, Tens R[2], Tens Xinv[2]) {
+    bool orth_pchol_pair(Tens G[2], int n, Tens R[2], Tens Xinv[2], const std::function<void()>* meanwhile, bool* full_rank) {
         SubStreams& ss = sub_streams();
         Scope sc(*this);
         Tens L[2]; double* pw[2];
@@ -359,21 +359,26 @@ struct Stepper {
             cudaStream_t a = ss.ok ? ss.s[i] : st;
             if (ss.ok) ck(cudaStreamWaitEvent(a, ss.fork, 0), "wait");
             ck(pchol(a, n, G[i].p, L[i].p, n, 1e-14, pw[i]), "pchol");
-            if (ss.ok) { ck(cudaEventRecord(ss.join[i], a), "event"); ck(cudaStreamWaitEvent(st, ss.join[i], 0), "wait"); }
+            if (ss.ok) ck(cudaEventRecord(ss.join[i], a), "event");
         }
+        if (meanwhile && *meanwhile) (*meanwhile)();
+        if (ss.ok) for (int i = 0; i < 2; ++i) ck(cudaStreamWaitEvent(st, ss.join[i], 0), "wait");
         double info[2][4];
         for (int i = 0; i < 2; ++i) ck(cudaMemcpyAsync(info[i], pchol_info(pw[i]), 32, cudaMemcpyDeviceToHost, st), "readback");
         ck(cudaStreamSynchronize(st), "sync"); count_sync();
+        const auto tv0 = std::chrono::steady_clock::now();
         int rp[2];
         for (int i = 0; i < 2; ++i) {
             rp[i] = (int)info[i][0];
             if (g_verbose & 1) fprintf(stderr, "[tatrg orth %d] pivoted Cholesky: rank %d, residual trace / trace %.2e\n", n, rp[i], info[i][2] > 0 ? info[i][1] / info[i][2] : 0.0);
             if (rp[i] <= 0 || rp[i] > n || !std::isfinite(info[i][1])) return false;
         }
+        *full_rank = true;
         Tens G1[2];
         for (int i = 0; i < 2; ++i) G1[i] = mm(true, false, rp[i], rp[i], n, L[i].p, n, L[i].p, n, true);
         std::vector<EigOut> eo;
         eig_batch({&G1[0], &G1[1]}, {rp[0], rp[1]}, eo);
+        if (g_verbose & 1) fprintf(stderr, "[tatrg orth %d] L^T L + eigen-decomposition: %.2f ms\n", n, std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - tv0).count());
         for (int i = 0; i < 2; ++i) {
             const std::vector<double>& lh = eo[i].lh;
             if (!(lh[0] > 0)) fail(TATRG_ENUMERIC, "orth: zero matrix");
@@ -384,6 +389,7 @@ struct Stepper {
             Xinv[i] = make({r, n});
             ck(scale_rows(st, Xinv[i].p, R[i].p, eo[i].lam, r, n, 1), "scale");          // lam^-1/2 U^T
             keep(R[i]); keep(Xinv[i]);
+            if (r < n) *full_rank = false;
         }
         return true;
     }
@@ -396,13 +402,26 @@ struct Stepper {
         const int64_t m = m0.d[0], n = m0.d[1];
         if (Xinv) { Xinv[0].p = nullptr; Xinv[1].p = nullptr; }
         if (n <= 128 || m1.d[0] != m || m1.d[1] != n) { orth(m0, Q[0], R[0]); orth(m1, Q[1], R[1]); return; }
-        if (c.use_subspace && orth_chol_pair(m0, m1, Q, R, Xinv, meanwhile)) return;
         const bool implicit = Xinv != nullptr && c.use_subspace;
+        // `meanwhile` runs once, beside whichever factorisation comes first.  After a step whose operands were numerically
+        // rank-deficient (every step once the flow has left criticality) the Cholesky attempt is skipped: its outcome is known, it
+        // costs 5 ms and destroys the Gram matrices; the first full-rank result of the rank-revealing path clears the hint.
+        bool ran = false;
+        std::function<void()> once = [&]() { if (!ran && meanwhile && *meanwhile) { ran = true; (*meanwhile)(); } };
+        if (c.use_subspace && !(implicit && c.qr_deficient_hint) && orth_chol_pair(m0, m1, Q, R, Xinv, &once)) { c.qr_deficient_hint = false; return; }
         Scope sc(*this);
         const Tens* mats[2] = {&m0, &m1};
         Tens G[2];
         for (int i = 0; i < 2; ++i) G[i] = mm(true, false, n, n, m, mats[i]->p, n, mats[i]->p, n, true);
-        if (implicit && orth_pchol_pair(G, (int)n, R, Xinv)) { for (int i = 0; i < 2; ++i) { Q[i] = Tens(); keep(R[i]); keep(Xinv[i]); } return; }
+        if (implicit) {
+            bool full = false;
+            if (orth_pchol_pair(G, (int)n, R, Xinv, &once, &full)) {
+                c.qr_deficient_hint = !full;
+                for (int i = 0; i < 2; ++i) { Q[i] = Tens(); keep(R[i]); keep(Xinv[i]); }
+                return;
+            }
+        }
+        once();
         std::vector<EigOut> eo;
         eig_batch({&G[0], &G[1]}, {(int)n, (int)n}, eo);
         for (int i = 0; i < 2; ++i) {
