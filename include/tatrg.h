@@ -47,6 +47,10 @@ enum {
                                   0: plain launches.  Same result. */
     TATRG_OPT_VERBOSE = 11,    /* debugging aid, bit mask, default 0: 1 = solver chains report ranks / convergence on stderr, 2 = spectra of
                                   the full eigen-decompositions, 4 = shape and rate of every DGEMM (with TATRG_OPT_STAGE_TIMING = 2) */
+    TATRG_OPT_DGEMM_TMA = 12,  /* 1 (default): contractions whose output takes the 128 x 128 tile and whose operands meet the tensor-map rules
+                                  (16-byte aligned bases, even leading dimensions and batch strides) run the TMA-fed kernel (dgemm_tma.cu:
+                                  producer warp, cp.async.bulk.tensor into a 128B-swizzled 6-stage mbarrier ring); 0: the cp.async kernel
+                                  everywhere.  Same products up to the order of nothing: both accumulate k in the same order. */
     TATRG_OPT_METHOD = 6       /* 0: Triad-ATRG (default).  1: plain ATRG, Eq. 2.7-2.8 (:104-113): no triad split, squeezers from
                                   Gamma^ATRG, O(D^9) contraction sliced so that no D^7 tensor is stored (fn 6 :205).  Before the first
                                   step only; ENOMEM unless the workspace holds tatrg_workspace_bytes_atrg(D, oversample). */
@@ -145,6 +149,12 @@ int tatrg_set_state(tatrg_handle, const double* phi_host, const double* psi_host
 int tatrg_dgemm(void* cuda_stream, int transa, int transb, long long M, long long N, long long K, double alpha,
                 const double* A, long long lda, const double* B, long long ldb, double beta, double* C, long long ldc,
                 int batch, long long strideA, long long strideB, long long strideC);
+/* The same product through a named kernel variant (tests, profiling): 0 = cp.async-fed tiles (all four tile configurations),
+ * 1 = the TMA-fed 128 x 128 x 16 tile whatever the shape.  EINVAL for variant 1 when the operands do not meet the tensor-map
+ * rules (16-byte aligned A, B; even lda, ldb, sA, sB; extents below 2^31; batch <= 65535) or an extent is 0. */
+int tatrg_dgemm_variant(void* cuda_stream, int variant, int transa, int transb, long long M, long long N, long long K, double alpha,
+                        const double* A, long long lda, const double* B, long long ldb, double beta, double* C, long long ldc,
+                        int batch, long long sA, long long sB, long long sC);
 
 /* out = in with legs permuted: out leg i is in leg perm[i]; dims[ndim] are the extents of `in` (row-major). */
 int tatrg_permute(void* cuda_stream, int ndim, const long long* dims, const int* perm, const double* in, double* out);

@@ -16,7 +16,7 @@ _lib = None
 
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC, ESTATE = 0, -1, -2, -3, -4, -5
 OPT_POWER_ITERS, OPT_K_TRIAD, OPT_TAU, OPT_STAGE_TIMING, OPT_KEEP_TENSORS, OPT_METHOD, OPT_SUBSPACE, OPT_BOND_RANK = 1, 2, 3, 4, 5, 6, 7, 8
-OPT_OVERLAP, OPT_GRAPHS, OPT_VERBOSE = 9, 10, 11
+OPT_OVERLAP, OPT_GRAPHS, OPT_VERBOSE, OPT_DGEMM_TMA = 9, 10, 11, 12
 METHOD_TRIAD, METHOD_ATRG = 0, 1
 SV_SIGMA, SV_S = 0, 1
 STAGES = ["decompose", "qr", "rsvd", "lift", "triad", "triad_tensors", "squeezer_grams", "squeezers", "contract",
@@ -53,6 +53,9 @@ _SIGNATURES = {
     "tatrg_dgemm": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_int, _c.c_longlong, _c.c_longlong, _c.c_longlong, _c.c_double,
                                _c.c_void_p, _c.c_longlong, _c.c_void_p, _c.c_longlong, _c.c_double, _c.c_void_p,
                                _c.c_longlong, _c.c_int, _c.c_longlong, _c.c_longlong, _c.c_longlong]),
+    "tatrg_dgemm_variant": (_c.c_int, [_c.c_void_p, _c.c_int, _c.c_int, _c.c_int, _c.c_longlong, _c.c_longlong, _c.c_longlong, _c.c_double,
+                            _c.c_void_p, _c.c_longlong, _c.c_void_p, _c.c_longlong, _c.c_double, _c.c_void_p, _c.c_longlong,
+                            _c.c_int, _c.c_longlong, _c.c_longlong, _c.c_longlong]),
     "tatrg_permute": (_c.c_int, [_c.c_void_p, _c.c_int, _c.POINTER(_c.c_longlong), _c.POINTER(_c.c_int), _c.c_void_p,
                                  _c.c_void_p]),
     "tatrg_contract": (_c.c_int, [_c.c_void_p, _c.c_char_p, _c.c_void_p, _c.POINTER(_c.c_longlong), _c.c_void_p,
@@ -274,8 +277,9 @@ def _p(t):
     return ctypes.c_void_p(t.data_ptr())
 
 
-def dgemm(A, B, transa=False, transb=False, alpha=1.0, beta=0.0, C=None):
-    """C = alpha*op(A)@op(B) + beta*C for 2-D or batched 3-D row-major tensors."""
+def dgemm(A, B, transa=False, transb=False, alpha=1.0, beta=0.0, C=None, variant=None):
+    """C = alpha*op(A)@op(B) + beta*C for 2-D or batched 3-D row-major tensors.  variant: None = the library's choice,
+    0 = cp.async-fed kernels, 1 = the TMA-fed 128 x 128 tile (tatrg_dgemm_variant)."""
     torch = _torch_cuda()
     batched = A.dim() == 3
     a2, b2 = A.shape[-2:], B.shape[-2:]
@@ -284,9 +288,12 @@ def dgemm(A, B, transa=False, transb=False, alpha=1.0, beta=0.0, C=None):
     nb = A.shape[0] if batched else 1
     if C is None:
         C = torch.empty((nb, M, N) if batched else (M, N), dtype=torch.float64, device=A.device)
-    _check(lib().tatrg_dgemm(_stream_ptr(), int(transa), int(transb), M, N, K, alpha, _p(A), a2[1], _p(B), b2[1], beta, _p(C), N,
-                             nb, a2[0] * a2[1] if batched else 0, b2[0] * b2[1] if batched else 0, M * N if batched else 0),
-           "tatrg_dgemm")
+    rest = (int(transa), int(transb), M, N, K, alpha, _p(A), a2[1], _p(B), b2[1], beta, _p(C), N,
+            nb, a2[0] * a2[1] if batched else 0, b2[0] * b2[1] if batched else 0, M * N if batched else 0)
+    if variant is None:
+        _check(lib().tatrg_dgemm(_stream_ptr(), *rest), "tatrg_dgemm")
+    else:
+        _check(lib().tatrg_dgemm_variant(_stream_ptr(), int(variant), *rest), "tatrg_dgemm_variant")
     return C
 
 

@@ -13,7 +13,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libtatrg.so")
-SOURCES = ["dgemm.cu", "permute.cu", "elementwise.cu", "philox.cu", "jacobi.cu", "cholesky.cu", "pchol.cu", "contract.cu", "step.cu", "capi.cu", "noalloc.cu", "dmma_peak.cu"]
+SOURCES = ["dgemm.cu", "dgemm_tma.cu", "permute.cu", "elementwise.cu", "philox.cu", "jacobi.cu", "cholesky.cu", "pchol.cu", "contract.cu", "step.cu", "capi.cu", "noalloc.cu", "dmma_peak.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "--expt-relaxed-constexpr"]

@@ -72,6 +72,7 @@ int tatrg_set_option(tatrg_handle c, int key, double value) {
         case TATRG_OPT_OVERLAP: c->use_overlap = value != 0; return TATRG_OK;
         case TATRG_OPT_GRAPHS: c->use_graphs = value != 0; return TATRG_OK;
         case TATRG_OPT_VERBOSE: if (value < 0 || value > 7) return TATRG_EINVAL; c->verbose = (int)value; return TATRG_OK;
+        case TATRG_OPT_DGEMM_TMA: c->dgemm_tma = value != 0; return TATRG_OK;
         case TATRG_OPT_BOND_RANK: {
             if (c->m > 0) return TATRG_ESTATE;
             if (value != std::floor(value) || value < c->D) return TATRG_EINVAL;
@@ -221,6 +222,20 @@ int tatrg_dgemm(void* st, int transa, int transb, long long M, long long N, long
                 const double* B, long long ldb, double beta, double* C, long long ldc, int batch, long long sA, long long sB, long long sC) {
     if (M < 0 || N < 0 || K < 0 || batch < 1 || (!A && M * K > 0) || (!B && N * K > 0) || !C) return TATRG_EINVAL;
     cudaError_t e = dgemm((cudaStream_t)st, transa != 0, transb != 0, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+    return e == cudaSuccess ? TATRG_OK : TATRG_ECUDA;
+}
+
+int tatrg_dgemm_variant(void* st, int variant, int transa, int transb, long long M, long long N, long long K, double alpha, const double* A, long long lda,
+                        const double* B, long long ldb, double beta, double* C, long long ldc, int batch, long long sA, long long sB, long long sC) {
+    if (M < 1 || N < 1 || K < 1 || batch < 1 || !A || !B || !C || (variant != 0 && variant != 1)) return TATRG_EINVAL;
+    if (variant == 1) {
+        cudaError_t e = dgemm_tma((cudaStream_t)st, transa == 0, transb != 0, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC, false);
+        return e == cudaSuccess ? TATRG_OK : (e == cudaErrorNotSupported ? TATRG_EINVAL : TATRG_ECUDA);
+    }
+    const int saved = g_dgemm_tma;
+    g_dgemm_tma = 0;
+    cudaError_t e = dgemm((cudaStream_t)st, transa != 0, transb != 0, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, batch, sA, sB, sC);
+    g_dgemm_tma = saved;
     return e == cudaSuccess ? TATRG_OK : TATRG_ECUDA;
 }
 

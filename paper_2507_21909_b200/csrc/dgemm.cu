@@ -18,6 +18,7 @@
 namespace tatrg {
 thread_local Counters* g_counter = nullptr;
 thread_local int g_verbose = 0;
+thread_local int g_dgemm_tma = 1;
 cudaEvent_t Counters::next_event() {
     if (ev_used == ev_pool.size()) { cudaEvent_t e; cudaEventCreate(&e); ev_pool.push_back(e); }
     return ev_pool[ev_used++];
@@ -320,7 +321,13 @@ cudaError_t dgemm_raw(bool transa, bool transb, const Args& a) {
     };
     const bool kodd = (a.K % 2 != 0) || (a.Klast % 2 != 0);
     const bool av = v16(a.A, a.lda, a_kc ? (kodd ? 1 : 2) : a.M, a.sA), bv = v16(a.B, a.ldb, b_kc ? (kodd ? 1 : 2) : a.N, a.sB);
-    switch (a.force_cfg != CFG_AUTO ? a.force_cfg : pick_cfg(a.M, a.N, a.batch)) {
+    const int cfg = a.force_cfg != CFG_AUTO ? a.force_cfg : pick_cfg(a.M, a.N, a.batch);
+    // the 128 x 128 tile fed by TMA (dgemm_tma.cu) whenever the operands meet the tensor-map alignment rules
+    if (cfg == CFG_L && g_dgemm_tma && a.Klast == 0) {
+        cudaError_t e = dgemm_tma(a.st, a_kc, b_kc, a.M, a.N, a.K, a.alpha, a.A, a.lda, a.B, a.ldb, a.beta, a.C, a.ldc, a.batch, a.sA, a.sB, a.sC, a.lower_only);
+        if (e != cudaErrorNotSupported) return e;
+    }
+    switch (cfg) {
         case CFG_L: return pick_order<CfgL>(a_kc, b_kc, av, bv, a);
         case CFG_S: return pick_order<CfgS>(a_kc, b_kc, av, bv, a);
         case CFG_T: return pick_order<CfgT>(a_kc, b_kc, av, bv, a);

@@ -62,6 +62,13 @@ int64_t dgemm_splitk_doubles(int64_t M, int64_t N, int64_t K, bool lower_only = 
 cudaError_t dgemm_splitk(cudaStream_t st, bool transa, bool transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                          int64_t lda, const double* B, int64_t ldb, double* C, int64_t ldc, double* part, bool lower_only = false);
 
+// dgemm_tma.cu : the 128 x 128 x 16 tile fed by TMA (tensor maps, mbarrier ring, producer warp).  a_kc: A stored [M][K]; b_kc: B stored
+// [N][K].  cudaErrorNotSupported when the operands do not meet the tensor-map alignment rules (dgemm_tma_applicable).
+bool dgemm_tma_applicable(int64_t M, int64_t N, int64_t K, const double* A, int64_t lda, const double* B, int64_t ldb, int batch, int64_t sA, int64_t sB);
+cudaError_t dgemm_tma(cudaStream_t st, bool a_kc, bool b_kc, int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda, const double* B,
+                      int64_t ldb, double beta, double* C, int64_t ldc, int batch, int64_t sA, int64_t sB, int64_t sC, bool lower_only);
+extern thread_local int g_dgemm_tma;      // TATRG_OPT_DGEMM_TMA of the handle whose step is being enqueued (dgemm.cu)
+
 // permute.cu
 cudaError_t permute(cudaStream_t st, int nd, const int64_t* dims, const int* perm, const double* in, double* out);
 

@@ -1385,6 +1385,8 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
     cn.time_kernels = c->timing >= 2; cn.gemm_ev.clear(); cn.perm_ev.clear(); cn.perm_ev_bytes.clear(); cn.gemm_shapes.clear(); cn.ev_used = 0;
     g_counter = &cn;
     g_verbose = c->verbose;
+    const int tma_saved = g_dgemm_tma;
+    g_dgemm_tma = c->dgemm_tma;
     for (cudaGraphExec_t g : c->graveyard) cudaGraphExecDestroy(g);    // their launches completed before the previous step's last read-back
     c->graveyard.clear();
     int rc = TATRG_OK;
@@ -1401,6 +1403,7 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
     }
     g_counter = nullptr;
     g_verbose = 0;
+    g_dgemm_tma = tma_saved;
     c->last_stream = st;
     if (rc == TATRG_OK) {
         if (!c->done_ev && cudaEventCreateWithFlags(&c->done_ev, cudaEventDisableTiming) != cudaSuccess) c->done_ev = nullptr;

@@ -94,6 +94,54 @@ def test_dgemm_multiwave_batched_alpha_beta(torch):
     assert np.abs(C.cpu().numpy() - ref).max() <= 8 * EPS * 48 * np.abs(a).max() * np.abs(b).max() * 2
 
 
+@pytest.mark.parametrize("M,N,K", [(128, 128, 16), (1, 1, 1), (130, 70, 33), (1666, 1538, 70), (2050, 1300, 16), (1280, 1920, 131), (300, 260, 1000)])
+@pytest.mark.parametrize("ta,tb", [(False, False), (True, False), (False, True), (True, True)])
+def test_dgemm_tma_variant_matches_definition(torch, M, N, K, ta, tb):
+    """The TMA-fed 128 x 128 x 16 tile (tensor maps with zero fill instead of predicates, 128B-swizzled tiles, permuted atom rows):
+    all four storage orders, ragged M, N, K (K odd, K shorter than one k-step, K longer than the 6-stage ring), several waves."""
+    ld_a = (M if ta else K) + ((M if ta else K) & 1)            # tensor maps need even leading dimensions
+    ld_b = (K if tb else N) + ((K if tb else N) & 1)
+    a = inputs.random_tensor((M, K), 21)
+    b = inputs.random_tensor((K, N), 22)
+    A = torch.zeros((K if ta else M, ld_a), dtype=torch.float64, device="cuda")
+    B = torch.zeros((N if tb else K, ld_b), dtype=torch.float64, device="cuda")
+    A[:, :(M if ta else K)] = dev(torch, a.T if ta else a)
+    B[:, :(K if tb else N)] = dev(torch, b.T if tb else b)
+    C = torch.full((M, N), float("nan"), dtype=torch.float64, device="cuda")
+    import ctypes
+    rc = T.lib().tatrg_dgemm_variant(ctypes.c_void_p(torch.cuda.current_stream().cuda_stream), 1, int(ta), int(tb), M, N, K, 1.0,
+                                     ctypes.c_void_p(A.data_ptr()), ld_a, ctypes.c_void_p(B.data_ptr()), ld_b, 0.0, ctypes.c_void_p(C.data_ptr()), N, 1, 0, 0, 0)
+    assert rc == T.OK
+    assert np.abs(C.cpu().numpy() - a @ b).max() <= 8 * EPS * K * np.abs(a).max() * np.abs(b).max()
+
+
+def test_dgemm_tma_variant_batched_broadcast_alpha_beta(torch):
+    a = inputs.random_tensor((3, 1100, 48), 13)
+    b = inputs.random_tensor((3, 48, 1000), 14)
+    c0 = inputs.random_tensor((3, 1100, 1000), 15)
+    C = dev(torch, c0)
+    T.dgemm(dev(torch, a), dev(torch, b), alpha=-1.5, beta=0.25, C=C, variant=1)
+    ref = -1.5 * np.einsum("bik,bkj->bij", a, b) + 0.25 * c0
+    assert np.abs(C.cpu().numpy() - ref).max() <= 8 * EPS * 48 * np.abs(a).max() * np.abs(b).max() * 2
+    # broadcast B (batch stride 0), transposed A
+    import ctypes
+    at = dev(torch, np.ascontiguousarray(np.transpose(a, (0, 2, 1))))
+    b0 = dev(torch, b[0])
+    out = torch.empty((3, 1100, 1000), dtype=torch.float64, device="cuda")
+    rc = T.lib().tatrg_dgemm_variant(ctypes.c_void_p(torch.cuda.current_stream().cuda_stream), 1, 1, 0, 1100, 1000, 48, 1.0, ctypes.c_void_p(at.data_ptr()), 1100,
+                                     ctypes.c_void_p(b0.data_ptr()), 1000, 0.0, ctypes.c_void_p(out.data_ptr()), 1000, 3, 48 * 1100, 0, 1100 * 1000)
+    assert rc == T.OK
+    assert np.abs(out.cpu().numpy() - np.einsum("bik,kj->bij", a, b[0])).max() <= 8 * EPS * 48 * np.abs(a).max() * np.abs(b).max()
+
+
+def test_dgemm_tma_variant_rejects_what_tensor_maps_cannot_address(torch):
+    a = torch.zeros((64, 33), dtype=torch.float64, device="cuda")      # odd leading dimension
+    b = torch.zeros((33, 64), dtype=torch.float64, device="cuda")
+    with pytest.raises(T.TatrgError):
+        T.dgemm(a, b, variant=1)
+    assert T.dgemm(a, b, variant=0).shape == (64, 64)
+
+
 # ---- permute ------------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("shape,perm", [((3, 5, 7, 4, 6), (1, 2, 3, 0, 4)), ((3, 5, 7, 4, 6), (4, 3, 2, 1, 0)), ((33, 65), (1, 0)),
                                         ((2, 2, 2, 2, 2), (1, 2, 3, 0, 4)), ((8, 8, 8, 8, 8), (0, 3, 4, 1, 2)), ((1, 7, 1, 5), (3, 2, 1, 0)),
