@@ -215,9 +215,11 @@ def decompose(phi, psi, D, seed, step, tau=TAU_MULTIPLET):
 # --------------------------------------------------------------------------------------------------------
 # (a2-a4) bond swapping, Eq. 2.5 :90 and App. A :329-394
 # --------------------------------------------------------------------------------------------------------
-def bond_swap(a, dt, core, D, oversample, n_pow, seed, step, tau=TAU_MULTIPLET, exact=False):
+def bond_swap(a, dt, core, D, oversample, n_pow, seed, step, tau=TAU_MULTIPLET, exact=False, lift=True):
     """sum_i1 B[i1,j',al] C[i1,i',be] ~ sum_g X[al,i',g] sig[g] Y[be,j',g]  (Eq. 2.5 / A.1).
-    B[i1,j2,j3,j4,al] = sum_a' Dt[i1,j2,j3,j4,a'] c[al,a'],  C[i1,i2,i3,i4,be] = sum_a' A[i1,..,a'] c[a',be]."""
+    B[i1,j2,j3,j4,al] = sum_a' Dt[i1,j2,j3,j4,a'] c[al,a'],  C[i1,i2,i3,i4,be] = sum_a' A[i1,..,a'] c[a',be].
+    lift=False stops at Eq. A.9 :379 and returns (U^bond[al,q,g], V^bond[be,p,g], Q^C[i',q], Q^B[j',p], sig, sig_all): the
+    form in which the ILO method keeps the swapped bond (:394 "the tensors X and Y are not explicitly constructed")."""
     b = _es("ijklc,ac->ijkla", dt, core)
     c = _es("ijklc,cb->ijklb", a, core)
     chi1, chi_a = b.shape[0], b.shape[4]
@@ -254,6 +256,8 @@ def bond_swap(a, dt, core, D, oversample, n_pow, seed, step, tau=TAU_MULTIPLET, 
         vbond = vb.reshape(chi_a, npb, -1)
     sig_all = sig / sig[0]
     g = select_rank(sig, D, EPS_SV, tau)
+    if not lift:
+        return ubond[:, :, :g], vbond[:, :, :g], QC, QB, sig[:g], sig_all
     x = _es("aqg,jklq->ajklg", ubond[:, :, :g], QC)         # Eq. A.10 :389
     y = _es("bpg,jklp->bjklg", vbond[:, :, :g], QB)         # Eq. A.11 :392
     return x, y, sig[:g], sig_all
@@ -298,6 +302,47 @@ def triad_tensors(a, dt, x, y, sig, ua, ux, uy, ud):
     g = _es("bjklg,jkm->bmlg", y, uy)               # Eq. 2.12  G[be,kY,j4,g]
     h = _es("ijklb,jkm->imlb", dt, ud)              # Eq. 2.13  H[j1,kD,j4,be]
     return e, f, g, h                                     # Eq. 2.14-2.17: I,J,K,L = ua,ux,uy,ud
+
+
+# --------------------------------------------------------------------------------------------------------
+# (a5-a6) without X and Y, PAPER.md :394 / :201 (ILO Triad-ATRG)
+# --------------------------------------------------------------------------------------------------------
+def triad_isometries_implicit(a, dt, ubond, vbond, qc, qb, sig, K, tau=TAU_MULTIPLET):
+    """Eq. 2.9 with Eq. A.10-A.11 substituted, X = U^bond Q^C and Y = V^bond Q^B never formed (:394 "we work directly with
+    U^bond, sigma and V^*bond to create isometries of the triad representation"; :201 "QR decomposition is applied before
+    the bond-swapping step ..., which allows us to avoid constructing large intermediate tensors X and Y").
+      G^X[(i2 i3),(i2' i3')] = sum_{i4} sum_{q q'} Q^C[i2 i3 i4, q] w^C[q,q'] Q^C[i2' i3' i4, q'],
+      w^C[q,q'] = sum_{al,g} sig_g^2 U^bond[al,q,g] U^bond[al,q',g]
+      kappa^A[al,al'] = sum_{q,g} sig_g^2 U^bond[al,q,g] U^bond[al',q,g]      (Q^C^T Q^C = 1, Eq. A.3 :348)
+    and the same with V^bond, Q^B for G^Y, kappa^D.  Nothing larger than Q^C, Q^B (chi^3 x r_bond D^2) appears."""
+    us, vs = ubond * sig, vbond * sig
+    d2, d3 = qc.shape[0], qc.shape[1]
+    wc = _es("aqg,arg->qr", us, us)
+    gx = _es("jklq,qr,mnlr->jkmn", qc, wc, qc)
+    ka = _es("aqg,bqg->ab", us, us)
+    ga = _es("ijkla,ab,imnlb->jkmn", a, ka, a)
+    wb = _es("bpg,brg->pr", vs, vs)
+    gy = _es("jklp,pr,mnlr->jkmn", qb, wb, qb)
+    kd = _es("apg,bpg->ab", vs, vs)
+    gd = _es("ijkla,ab,imnlb->jkmn", dt, kd, dt)
+    out, spectra = [], []
+    for gram in (ga, gx, gy, gd):
+        vec, lam = _top_eigvecs(gram.reshape(d2 * d3, d2 * d3), K, tau)
+        out.append(vec.reshape(d2, d3, -1))
+        spectra.append(lam)
+    return out, spectra
+
+
+def triad_tensors_implicit(a, dt, ubond, vbond, qc, qb, sig, ua, ux, uy, ud):
+    """Eq. 2.10-2.13 with Eq. A.10-A.11 substituted: the isometry meets Q^C (Q^B) first, a chi4 x K x r_bond D^2 object, and
+    U^bond (V^bond) afterwards, so F and G come out without X and Y (:394)."""
+    e = _es("ijkla,jkm->imla", a, ua)               # Eq. 2.10
+    pc = _es("jklq,jkm->mlq", qc, ux)               # sum_{i2,i3} Q^C[i2,i3,i4,q] U^X[i2,i3,kX]
+    f = _es("aqg,mlq->amlg", ubond, pc) * sig       # Eq. 2.11 with A.10: F[al,kX,i4,g]
+    pb = _es("jklp,jkm->mlp", qb, uy)
+    g = _es("bpg,mlp->bmlg", vbond, pb)             # Eq. 2.12 with A.11: G[be,kY,j4,g]
+    h = _es("ijklb,jkm->imlb", dt, ud)              # Eq. 2.13
+    return e, f, g, h
 
 
 # --------------------------------------------------------------------------------------------------------
@@ -377,7 +422,7 @@ class TatrgOracle:
     """State = (Phi, Psi, [ln c_m], step counter).  step() = Fig. 5 (a)-(f) :193."""
 
     def __init__(self, beta, h, D, oversample, seed, n_pow=2, K=None, tau=TAU_MULTIPLET, exact_swap=False, method="triad",
-                 bond_rank=None):
+                 bond_rank=None, implicit_xy=False):
         self.beta, self.h, self.D, self.p, self.seed = beta, h, D, oversample, seed
         self.method = method                                   # "triad" (Eq. 2.9-2.19) or "atrg" (Eq. 2.7-2.8)
         # ILO Triad-ATRG (PAPER.md section 2.3 :183-209, App. A :331-394): the bond swap keeps r_bond D values (the sum over gamma in
@@ -385,6 +430,11 @@ class TatrgOracle:
         # beta in Eq. (2.4) are also overspanned"); the RSVD sketch is r_bond D + p wide (fn 9 :381).  bond_rank = r_bond D; the
         # squeezed legs stay at D.  bond_rank = D is the Triad-ATRG of section 2.2.
         self.bond_rank = bond_rank if bond_rank is not None else D
+        # implicit_xy: the triad isometries and F, G straight from U^bond, sigma, V^bond, Q^C, Q^B (:394, :201); X and Y never exist.
+        # The same numbers as the explicit route up to rounding (pinned in tests/test_oracle_pins.py).
+        self.implicit_xy = implicit_xy
+        if implicit_xy and method != "triad":
+            raise ValueError("implicit_xy belongs to the triad representation (plain ATRG contracts X and Y themselves, Eq. 2.7-2.8)")
         self.n_pow, self.tau, self.exact_swap = n_pow, tau, exact_swap
         self.K = K if K is not None else D + oversample        # R3: triad internal-line dimension rD = D + p
         self.phi, self.psi = init_tensor(beta, h)
@@ -395,12 +445,20 @@ class TatrgOracle:
     def step(self):
         D, tau, call = self.D, self.tau, self.m + 1
         a, dt, core, s_all, lnc = decompose(self.phi, self.psi, self.bond_rank, self.seed, call, tau)          # (a)
-        x, y, sig, sig_all = bond_swap(a, dt, core, self.bond_rank, self.p, self.n_pow, self.seed, call, tau,
-                                       exact=self.exact_swap)                                        # (b)
+        if self.implicit_xy:
+            ub, vb, qc, qb, sig, sig_all = bond_swap(a, dt, core, self.bond_rank, self.p, self.n_pow, self.seed, call, tau,
+                                                     exact=self.exact_swap, lift=False)              # (b) up to Eq. A.9
+            x = y = None
+            (ua, ux, uy, ud), tri_spec = triad_isometries_implicit(a, dt, ub, vb, qc, qb, sig, self.K, tau)   # (c), :394
+            e, f, g, h = triad_tensors_implicit(a, dt, ub, vb, qc, qb, sig, ua, ux, uy, ud)
+        else:
+            x, y, sig, sig_all = bond_swap(a, dt, core, self.bond_rank, self.p, self.n_pow, self.seed, call, tau,
+                                           exact=self.exact_swap)                                    # (b)
         if self.method == "atrg":
             return self._finish_atrg(a, dt, core, s_all, lnc, x, y, sig, sig_all, call)
-        (ua, ux, uy, ud), tri_spec = triad_isometries(a, dt, x, y, sig, self.K, tau)               # (c)
-        e, f, g, h = triad_tensors(a, dt, x, y, sig, ua, ux, uy, ud)
+        if not self.implicit_xy:
+            (ua, ux, uy, ud), tri_spec = triad_isometries(a, dt, x, y, sig, self.K, tau)           # (c)
+            e, f, g, h = triad_tensors(a, dt, x, y, sig, ua, ux, uy, ud)
         ms, ns, sq_spec = {}, {}, {}
         for mu in (2, 3, 4):                                                                        # (d)
             th_f = squeezer_grams(e, f, ua, ux, mu)

@@ -2,6 +2,8 @@
 
     python tests/golden/make_golden.py c1 c2 c3 [c4:12]      (name[:steps])
     GOLDEN_CKPT=/some/dir python tests/golden/make_golden.py c4:26    (long runs: state saved after each step)
+    GOLDEN_OUT=/some/dir ...                                         (write there instead of tests/golden/: a run restarted from
+                                                                      step 0 must not shorten the committed file while it grows)
     python tests/golden/make_golden.py --timing                      (oracle_timing.json: what bench.py scales its CPU sample by)
 
 Each file holds, per step: ln Z/V, the bond-swap spectrum sigma/sigma_1 and the T-decomposition spectrum s/s_1
@@ -63,6 +65,7 @@ if __name__ == "__main__":
     if "--timing" in sys.argv:
         timing()
         sys.exit(0)
+    outdir = os.environ.get("GOLDEN_OUT") or os.path.dirname(__file__)
     for arg in sys.argv[1:]:
         name, _, lim = arg.partition(":")
         out = {"generator": "tests/golden/make_golden.py (oracle only)", "runs": []}
@@ -84,9 +87,9 @@ if __name__ == "__main__":
                 rec["s"].append([float(x) for x in o.last["s"][:D]])
                 rec["sec"].append(round(time.time() - t0, 3))
                 print(name, tag, m + 1, rec["lnZ"][-1], rec["sec"][-1], flush=True)
-                json.dump(out | {"runs": out["runs"] + [rec]}, open(os.path.join(os.path.dirname(__file__), "oracle_%s.json" % name), "w"), indent=0)
+                json.dump(out | {"runs": out["runs"] + [rec]}, open(os.path.join(outdir, "oracle_%s.json" % name), "w"), indent=0)
                 if ckpt:
                     np.savez(ckpt + ".tmp.npz", phi=o.phi, psi=o.psi, lnc=np.array(o.lnc), m=o.m, rec=json.dumps(rec))
                     os.replace(ckpt + ".tmp.npz", ckpt)
             out["runs"].append(rec)
-        json.dump(out, open(os.path.join(os.path.dirname(__file__), "oracle_%s.json" % name), "w"), indent=0)
+        json.dump(out, open(os.path.join(outdir, "oracle_%s.json" % name), "w"), indent=0)

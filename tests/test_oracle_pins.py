@@ -706,3 +706,88 @@ def test_ilo_first_steps_stay_exact(beta, h):
     assert abs(o.lnZ_per_site() - enumerate_lnz_per_site((2, 1, 1, 1), beta, h)) < 2e-14
     o.step()
     assert abs(o.lnZ_per_site() - enumerate_lnz_per_site((2, 2, 1, 1), beta, h)) < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------ ILO without X, Y (:394, :201)
+def _swap_factors(D=3, Db=6, steps=4, seed=5):
+    """An overspanned state after `steps` ILO steps and the factors of its next bond swap, stopped at Eq. A.9."""
+    o = O.TatrgOracle(0.1497, 0.0, D, D, seed, n_pow=2, bond_rank=Db)
+    for _ in range(steps):
+        o.step()
+    a, dt, core, s, _ = O.decompose(o.phi, o.psi, Db, seed, steps + 1)
+    ub, vb, qc, qb, sig, sig_all = O.bond_swap(a, dt, core, Db, D, 2, seed, steps + 1, lift=False)
+    x, y, sig2, _ = O.bond_swap(a, dt, core, Db, D, 2, seed, steps + 1)
+    return a, dt, ub, vb, qc, qb, sig, x, y, sig2
+
+
+def test_implicit_factors_are_the_lift_of_eq_A10_A11():
+    """lift=False returns exactly the operands of Eq. A.10-A.11 :389-392: contracting them gives the X, Y of the explicit route,
+    Q^C and Q^B are isometries (Eq. A.2-A.3 :345-348), and U^bond, V^bond are isometries on (al q) resp. (be p) (Eq. A.9 :379)."""
+    a, dt, ub, vb, qc, qb, sig, x, y, sig2 = _swap_factors()
+    assert np.array_equal(sig, sig2)
+    assert np.abs(np.einsum("aqg,jklq->ajklg", ub, qc) - x).max() < 1e-14
+    assert np.abs(np.einsum("bpg,jklp->bjklg", vb, qb) - y).max() < 1e-14
+    for q in (qc, qb):
+        m = q.reshape(-1, q.shape[-1])
+        assert np.abs(m.T @ m - np.eye(m.shape[1])).max() < 1e-13
+    for u in (ub, vb):
+        m = u.reshape(-1, u.shape[-1])
+        assert np.abs(m.T @ m - np.eye(m.shape[1])).max() < 1e-12
+
+
+def test_implicit_triad_grams_equal_the_definition_on_explicit_x_y():
+    """:394 'we work directly with U^bond, sigma, and V^*bond to create isometries of the triad representation': the four Gram
+    matrices of Eq. 2.9 :135 formed without X, Y have the spectra of the ones formed from X, Y (all D^2 eigenvalues, not only the
+    kept ones), and the projectors U U^T on the kept subspaces agree wherever the cut does not fall inside a multiplet."""
+    a, dt, ub, vb, qc, qb, sig, x, y, _ = _swap_factors()
+    K = 6
+    iso_i, spec_i = O.triad_isometries_implicit(a, dt, ub, vb, qc, qb, sig, K)
+    iso_e, spec_e = O.triad_isometries(a, dt, x, y, sig, K)
+    for li, le in zip(spec_i, spec_e):
+        assert np.abs(li - le).max() <= 1e-12 * le[0]
+    for ui, ue, lam in zip(iso_i, iso_e, spec_e):
+        assert ui.shape == ue.shape
+        k = ui.shape[-1]
+        if k < len(lam) and lam[k - 1] - lam[k] < 1e-6 * lam[0]:
+            continue
+        pi, pe = ui.reshape(-1, k), ue.reshape(-1, k)
+        assert np.abs(pi @ pi.T - pe @ pe.T).max() < 1e-8
+    # the definition itself, written out on the explicit X (not through triad_isometries): G^X and kappa^A of Eq. 2.9 / :137
+    xs = x * sig
+    gx_def = np.einsum("ajklg,amnlg->jkmn", xs, xs).reshape(9, 9)
+    lam_def = np.sort(np.linalg.eigvalsh(gx_def))[::-1]
+    assert np.abs(lam_def - spec_i[1]).max() <= 1e-12 * lam_def[0]
+    # a wrong weight (sigma instead of sigma^2) or a dropped Q^C would not survive this: change sigma and the spectrum must move
+    _, spec_w = O.triad_isometries_implicit(a, dt, ub, vb, qc, qb, np.sqrt(sig), K)
+    assert np.abs(spec_w[1] - lam_def).max() > 1e-3 * lam_def[0]
+
+
+def test_implicit_triad_tensors_equal_eq_2_11_2_12_on_explicit_x_y():
+    """F and G of Eq. 2.11-2.12 :151-155 from (U^bond, Q^C), (V^bond, Q^B) equal those from X, Y for the same isometries; E, H do
+    not involve the swapped bond."""
+    a, dt, ub, vb, qc, qb, sig, x, y, _ = _swap_factors(D=3, Db=6, steps=5, seed=9)
+    (ua, ux, uy, ud), _ = O.triad_isometries(a, dt, x, y, sig, 6)
+    e0, f0, g0, h0 = O.triad_tensors(a, dt, x, y, sig, ua, ux, uy, ud)
+    e1, f1, g1, h1 = O.triad_tensors_implicit(a, dt, ub, vb, qc, qb, sig, ua, ux, uy, ud)
+    assert np.array_equal(e0, e1) and np.array_equal(h0, h1)
+    assert f1.shape == f0.shape and g1.shape == g0.shape
+    assert np.abs(f1 - f0).max() < 1e-13 and np.abs(g1 - g0).max() < 1e-13
+
+
+@pytest.mark.parametrize("D,Db,p,n_pow", [(3, 6, 3, 2), (4, 8, 4, 1), (4, 4, 4, 1)])
+def test_implicit_run_equals_explicit_run(D, Db, p, n_pow):
+    """The whole ILO run without X, Y gives the explicit route's ln Z/V and spectra step by step (rounding order only differs);
+    X and Y are never stored.  (4, 4) is the plain Triad-ATRG of section 2.2: the implicit form does not need r_bond > 1."""
+    o0 = O.TatrgOracle(0.1497, 0.0, D, p, 7, n_pow=n_pow, bond_rank=Db)
+    o1 = O.TatrgOracle(0.1497, 0.0, D, p, 7, n_pow=n_pow, bond_rank=Db, implicit_xy=True)
+    for m in range(8):
+        o0.step(); o1.step()
+        assert o1.last["x"] is None and o1.last["y"] is None
+        assert abs(o0.lnZ_per_site() - o1.lnZ_per_site()) <= 1e-12 * abs(o0.lnZ_per_site()), m
+        assert np.abs(o0.last["sigma"] - o1.last["sigma"]).max() <= 1e-10
+        assert np.abs(o0.last["s"] - o1.last["s"]).max() <= 1e-10
+
+
+def test_implicit_xy_is_a_triad_feature():
+    with pytest.raises(ValueError):
+        O.TatrgOracle(0.1497, 0.0, 3, 3, 1, method="atrg", implicit_xy=True)
