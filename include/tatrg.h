@@ -51,6 +51,12 @@ enum {
                                   (16-byte aligned bases, even leading dimensions and batch strides) run the TMA-fed kernel (dgemm_tma.cu:
                                   producer warp, cp.async.bulk.tensor into a 128B-swizzled 6-stage mbarrier ring); 0: the cp.async kernel
                                   everywhere.  Same products up to the order of nothing: both accumulate k in the same order. */
+    TATRG_OPT_IMPLICIT_XY = 13,/* 1 (default): the tensors X, Y of Eq. A.10-A.11 (:389-392) are never formed: the Gram matrices of Eq. 2.9 (:135)
+                                  and F, G of Eq. 2.11-2.12 come straight from U^bond, sigma, V^bond and the QR factors of Eq. A.2-A.3
+                                  (PAPER.md :394 "the tensors X and Y are not explicitly constructed", :201), which removes the two
+                                  O(r_bond^2 D^5) tensors and two D^3 x D^2 x D^2 r_bond^3 products per step; 0: X, Y formed as the
+                                  equations are printed.  Same result up to rounding order.  Triad method only (plain ATRG contracts
+                                  X and Y themselves).  With TATRG_OPT_KEEP_TENSORS = 1, X and Y are still formed, for tatrg_get_tensor only. */
     TATRG_OPT_METHOD = 6       /* 0: Triad-ATRG (default).  1: plain ATRG, Eq. 2.7-2.8 (:104-113): no triad split, squeezers from
                                   Gamma^ATRG, O(D^9) contraction sliced so that no D^7 tensor is stored (fn 6 :205).  Before the first
                                   step only; ENOMEM unless the workspace holds tatrg_workspace_bytes_atrg(D, oversample). */

@@ -714,7 +714,13 @@ struct Stepper {
     }
 
     void decompose(Tens& a, Tens& dt, Tens& core);
-    void bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x, Tens& y, double*& sig, int& gr);
+    // The swapped bond in factored form, Eq. A.9 :379 before Eq. A.10-A.11 :389-392 (side 0: X from C, side 1: Y from B):
+    //   X[al,i',g] = sum_c Qm[0][i',c] w[0][c,al,g],  u[0][q,al,g] = U^bond (an isometry on (q al)): Qm is Q^C itself (then w = u) or,
+    //   after the Cholesky QR, the operand C with w = L_C^-T U^bond.  PAPER.md :394: "the tensors X and Y are not explicitly constructed".
+    struct Lift { Tens Qm[2], w[2], u[2]; bool on = false; };
+    void bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x, Tens& y, double*& sig, int& gr, Lift* lf = nullptr);
+    void triad_implicit(const Tens& a, const Tens& dt, const Lift& lf, const double* sig, Tens U[4], Tens& e, Tens& f, Tens& g, Tens& h);
+    void triad_grams_implicit(const Tens& aa, const Tens& Qm, const Tens& w, const Tens& u, const double* sig, int64_t d4, Tens& ga, Tens& gx);
     void triad(const Tens& a, const Tens& dt, const Tens& x, const Tens& y, const double* sig, Tens U[4], Tens& e, Tens& f, Tens& g, Tens& h);
     void triad_grams(const Tens& aa, const Tens& xx, const double* sig, Tens& ga, Tens& gx);
     void triad_isos(Tens gram[4], const std::vector<int>& which, int64_t d2, int64_t d3, Tens U[4]);
@@ -773,7 +779,7 @@ void Stepper::decompose(Tens& a, Tens& dt, Tens& core) {
 }
 
 // (b) Eq. 2.5 :90, App. A :329-394 -- sum_i1 B C ~ X sigma Y by randomized SVD of the never-formed core S.
-void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x, Tens& y, double*& sig, int& gr) {
+void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x, Tens& y, double*& sig, int& gr, Lift* lf) {
     Scope sc(*this);
     const int64_t d1 = a.d[0], d2 = a.d[1], d3 = a.d[2], d4 = a.d[3], chi = a.d[4];
     const int64_t F = d1 * d2 * d3 * d4, J = d2 * d3 * d4;
@@ -888,20 +894,94 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
     // one GEMM with N = (al, g) each: the batched form has N = g <= D, a quarter of a tile
     Tens ubp = perm(view(ub, {chi, npc, gr}), {1, 0, 2});
     Tens vbp = perm(view(vb, {chi, npb, gr}), {1, 0, 2});
-    if (implicit) {
-        Tens wx = ein("qc,qag->cag", XC, ubp), wy = ein("pc,pbg->cbg", XB, vbp);
-        x = ein("jc,cag->ajg", QC, wx);
-        y = ein("jc,cbg->bjg", QB, wy);
-    } else {
-        x = ein("jq,qag->ajg", QC, ubp);
-        y = ein("jp,pbg->bjg", QB, vbp);
+    Tens wx, wy;
+    if (implicit) { wx = ein("qc,qag->cag", XC, ubp); wy = ein("pc,pbg->cbg", XB, vbp); }
+    const bool factored = lf && c.method == 0 && c.implicit_xy;
+    if (!factored || c.keep_tensors) {          // keep_tensors: X, Y are formed for tatrg_get_tensor only, the path below does not read them
+        if (implicit) {
+            x = ein("jc,cag->ajg", QC, wx);
+            y = ein("jc,cbg->bjg", QB, wy);
+        } else {
+            x = ein("jq,qag->ajg", QC, ubp);
+            y = ein("jp,pbg->bjg", QB, vbp);
+        }
+        x = view(x, {chi, d2, d3, d4, gr});
+        y = view(y, {chi, d2, d3, d4, gr});
+        keep(x); keep(y);
     }
-    x = view(x, {chi, d2, d3, d4, gr});
-    y = view(y, {chi, d2, d3, d4, gr});
+    if (factored) {
+        // :394 "we work directly with U^bond, sigma, and V^*bond to create isometries of the triad representation": hand the factors on
+        lf->on = true;
+        lf->Qm[0] = QC; lf->Qm[1] = QB;
+        lf->u[0] = ubp; lf->u[1] = vbp;
+        lf->w[0] = implicit ? wx : ubp; lf->w[1] = implicit ? wy : vbp;
+        keep(QC); keep(QB); keep(ubp); keep(vbp);
+        if (implicit) { keep(wx); keep(wy); }
+    }
     sig = raw(gr);
     ck(cudaMemcpyAsync(sig, s, 8 * gr, cudaMemcpyDeviceToDevice, st), "copy"); count_launch();
-    keep(x); keep(y);
     { Tens t; t.p = sig; keep(t); }
+}
+
+// (c) without X and Y (PAPER.md :394, :201).  With X[al,i',g] = sum_c Qm[i',c] w[c,al,g] (see Lift):
+//   G^X[(i2 i3),(i2' i3')] = sum_{i4} sum_{c c'} Qm[(i2 i3 i4),c] W[c,c'] Qm[(i2' i3' i4),c'],  W = sum_{al,g} sig_g^2 w w^T
+//   kappa^A[al,al'] = sum_{q,g} sig_g^2 U^bond[q,al,g] U^bond[q,al',g]        (Q^C^T Q^C = 1, Eq. A.3 :348)
+// The two big products read Qm as [(i2 i3 i4), c] and as [(i2 i3), (i4 c)]: the same memory, no permute, nothing of size D^5 r_bond^2.
+void Stepper::triad_grams_implicit(const Tens& aa, const Tens& Qm, const Tens& w, const Tens& u, const double* sig, int64_t d4, Tens& ga,
+                                   Tens& gx) {
+    Scope s2(*this);
+    const int64_t d1 = aa.d[0], d2 = aa.d[1], d3 = aa.d[2], chi = aa.d[4], gr = w.d[2], nc = Qm.d[1];
+    const int64_t n = d2 * d3, J = n * d4;
+    {
+        Tens ws = make({nc, chi, gr});
+        ck(scale_last(st, ws.p, w.p, sig, nc * chi, gr, 0), "scale");
+        Tens wm = mm(false, true, nc, nc, chi * gr, ws.p, chi * gr, ws.p, chi * gr, true);
+        drop(ws);
+        Tens t1 = mm(false, false, J, nc, nc, Qm.p, nc, wm.p, nc);
+        drop(wm);
+        gx = mm(false, true, n, n, d4 * nc, t1.p, d4 * nc, Qm.p, d4 * nc, true);
+        drop(t1);
+    }
+    Tens us = make({u.d[0], chi, gr});
+    ck(scale_last(st, us.p, u.p, sig, u.d[0] * chi, gr, 0), "scale");
+    Tens ka = ein("qag,qbg->ab", us, us);
+    drop(us);
+    Tens ta = mm(false, false, d1 * J, chi, chi, aa.p, chi, ka.p, chi);
+    Tens ap = perm(aa, {0, 3, 4, 1, 2});
+    Tens tp = perm(view(ta, {d1, d2, d3, d4, chi}), {0, 3, 4, 1, 2});
+    drop(ta);
+    ga = mm(true, false, n, n, d1 * d4 * chi, ap.p, n, tp.p, n, true);
+    keep(ga); keep(gx);
+}
+
+void Stepper::triad_implicit(const Tens& a, const Tens& dt, const Lift& lf, const double* sig, Tens U[4], Tens& e, Tens& f, Tens& g,
+                             Tens& h) {
+    Scope sc(*this);
+    const int64_t d2 = a.d[1], d3 = a.d[2], d4 = a.d[3], n = d2 * d3, gr = lf.w[0].d[2];
+    Tens gram[4];
+    triad_grams_implicit(a, lf.Qm[0], lf.w[0], lf.u[0], sig, d4, gram[0], gram[1]);
+    triad_grams_implicit(dt, lf.Qm[1], lf.w[1], lf.u[1], sig, d4, gram[3], gram[2]);
+    triad_isos(gram, {0, 1, 2, 3}, d2, d3, U);
+    for (int i = 0; i < 4; ++i) drop(gram[i]);
+    if (submark) submark();                                                // end of TATRG_ST_TRIAD_ISO
+    e = ein("mjk,Ijkla->Imla", U[0], a);                                   // Eq. 2.10
+    {   // Eq. 2.11 with Eq. A.10: the isometry meets Q^C first (K x d4 x nc), U^bond sigma afterwards
+        const int64_t nc = lf.Qm[0].d[1], k1 = U[1].d[0], chi = lf.w[0].d[1];
+        Tens pc = mm(false, false, k1, d4 * nc, n, U[1].p, n, lf.Qm[0].p, d4 * nc);
+        Tens ws = make({nc, chi, gr});
+        ck(scale_last(st, ws.p, lf.w[0].p, sig, nc * chi, gr, 0), "scale");
+        f = ein("xlc,cag->axlg", view(pc, {k1, d4, nc}), ws);
+        drop(pc); drop(ws);
+    }
+    {   // Eq. 2.12 with Eq. A.11 (no sigma: it went into F)
+        const int64_t nc = lf.Qm[1].d[1], k2 = U[2].d[0];
+        Tens pb = mm(false, false, k2, d4 * nc, n, U[2].p, n, lf.Qm[1].p, d4 * nc);
+        g = ein("ylc,cbg->bylg", view(pb, {k2, d4, nc}), lf.w[1]);
+        drop(pb);
+    }
+    h = ein("djk,Jjklb->Jdlb", U[3], dt);                                  // Eq. 2.13
+    for (int i = 0; i < 4; ++i) keep(U[i]);
+    keep(e); keep(f); keep(g); keep(h);
 }
 
 // (c) Eq. 2.9 :135 (canonical form :137) and Eq. 2.10-2.17 :147-167.
@@ -1214,10 +1294,13 @@ void Stepper::run() {
     mark();
     // (b) the QR / RSVD / lift stages are timed together under TATRG_ST_QR..LIFT: QR and RSVD flops are attributed by bond_swap
     Tens x, y; double* sig; int gr;
+    Lift lf;
     submark = mark;
-    bond_swap(a, dt, core, x, y, sig, gr);
+    bond_swap(a, dt, core, x, y, sig, gr, &lf);
     submark = nullptr;
-    save("X", x); save("Y", y); { Tens s; s.p = sig; s.nd = 1; s.d[0] = gr; save("sigma", s); }
+    if (x.p) { save("X", x); save("Y", y); }
+    { Tens s; s.p = sig; s.nd = 1; s.d[0] = gr; save("sigma", s); }
+    if (lf.on && x.p) { drop(x); drop(y); }                  // formed for inspection only (TATRG_OPT_KEEP_TENSORS)
     mark();
     Tens phin, psin;
     if (c.method == 1) {
@@ -1276,7 +1359,7 @@ void Stepper::run() {
             arena_bytes = 8 * (64 * n2 * n2 + (2u << 20));
             // both Xi tensors are alive at once in this schedule; leave the arena's size again as headroom
             const size_t kt = (size_t)std::min<int64_t>(c.Ktri, a.d[1] * a.d[2]);
-            const size_t xi_bytes = 8 * (size_t)a.d[0] * kt * kt * (size_t)x.d[4] * (size_t)c.D;
+            const size_t xi_bytes = 8 * (size_t)a.d[0] * kt * kt * (size_t)gr * (size_t)c.D;
             if (c.pool.in_use() + 2 * arena_bytes + 3 * xi_bytes <= c.pool.capacity())
                 arena = c.pool.alloc((int64_t)(arena_bytes / 8));   // freed at the end of the step, after the joins
             if (!arena) overlap = false;
@@ -1299,12 +1382,16 @@ void Stepper::run() {
         // (The triad stage itself is not overlapped: splitting its four subspace iterations into two pairs, the second one hidden
         // behind E, F and the Gram matrices of the upper half, was measured slower -- a pair of chains takes as long as all four.)
         submark = mark;
-        triad(a, dt, x, y, sig, U, e, f, g, h);                         // (c)
+        if (lf.on) {
+            triad_implicit(a, dt, lf, sig, U, e, f, g, h);              // (c) straight from U^bond, sigma, V^bond (:394)
+            for (int i = 0; i < 2; ++i) { if (lf.w[i].p != lf.u[i].p) drop(lf.w[i]); drop(lf.u[i]); drop(lf.Qm[i]); }
+        } else triad(a, dt, x, y, sig, U, e, f, g, h);                  // (c)
         submark = nullptr;
         mark();
         save("E", e); save("F", f); save("G", g); save("H", h);
         save("UA", U[0]); save("UX", U[1]); save("UY", U[2]); save("UD", U[3]);
-        drop(a); drop(dt); drop(core); drop(x); drop(y);
+        drop(a); drop(dt); drop(core);
+        if (x.p) { drop(x); drop(y); }
         // (d) squeezer Gram matrices of the upper half (E F I J) and of the sigma-weighted lower half (G sigma, H, K, L)
         Tens P, Q;
         {
@@ -1437,6 +1524,8 @@ int run_step(tatrg_ctx* c, cudaStream_t st) {
         for (size_t i = 0; i < cn.perm_ev.size(); ++i) {
             float ms = 0; cudaEventElapsedTime(&ms, cn.perm_ev[i].first, cn.perm_ev[i].second); c->perm_ms += ms;
             if (i < cn.perm_ev_bytes.size() && cn.perm_ev_bytes[i] >= kLargePermuteBytes) { c->perm_large_ms += ms; c->perm_large_bytes += cn.perm_ev_bytes[i]; c->perm_large_calls += 1; }
+            if (verbose && i < cn.perm_ev_bytes.size())
+                fprintf(stderr, "[tatrg perm] %lld bytes  %.4f ms  %.0f GB/s\n", cn.perm_ev_bytes[i], ms, cn.perm_ev_bytes[i] / (ms * 1e-3) / 1e9);
         }
     }
     return TATRG_OK;

@@ -170,13 +170,17 @@ def _proj(x, nlast=1):
     return m @ m.T
 
 
+@pytest.mark.parametrize("implicit", [1, 0])
 @pytest.mark.parametrize("D,p,n_pow,presteps", [(4, 4, 1, 3), (6, 6, 2, 4)])
-def test_stagewise_teacher_forced(D, p, n_pow, presteps):
+def test_stagewise_teacher_forced(D, p, n_pow, presteps, implicit):
+    """implicit = 1 (default): the path takes the triad Gram matrices and F, G from U^bond, sigma, V^bond (:394); X and Y are formed for
+    this inspection only.  implicit = 0: X, Y formed and used as Eq. 2.9-2.12 print them.  Both against the same oracle step."""
     from oracle import tatrg_oracle as O
     beta, h, seed = 0.1497, 0.0, 21
     o = O.TatrgOracle(beta, h, D, p, seed, n_pow=n_pow)
     t = T.Tatrg(beta, h, D, p, seed, power_iters=n_pow)
     t.set_option(T.OPT_KEEP_TENSORS, 1)
+    t.set_option(T.OPT_IMPLICIT_XY, implicit)
     for _ in range(presteps):
         o.step()
         t.step()
@@ -204,6 +208,15 @@ def test_stagewise_teacher_forced(D, p, n_pow, presteps):
         po = uo.reshape(-1, uo.shape[-1]) @ uo.reshape(-1, uo.shape[-1]).T
         assert ug.shape[0] == uo.shape[-1], name
         assert np.abs(pg - po).max() <= 1e-9, name
+    # (c') triad tensors (Eq. 2.10-2.13): invariant under the basis of the kept subspace (internal line summed) and under the signs of
+    #      the swapped bond gamma (summed as well for F, G; E, H carry only physical legs and the canonically gauged alpha / beta)
+    eo, fo, go, ho = L["efgh"]
+    for name, ref in (("F", fo), ("G", go), ("E", eo), ("H", ho)):
+        got = t.get_tensor(name)
+        assert got.shape == ref.shape, name
+        spec = "axlg,bxmg->albm" if name in ("F", "G") else "axlg,bxmh->algbmh"
+        gg, rr = np.einsum(spec, got, got), np.einsum(spec, ref, ref)
+        assert np.abs(gg - rr).max() <= 1e-9 * np.abs(rr).max(), name
     # (d) squeezers: canonical gauge makes M, N comparable up to nothing
     for mu in (2, 3, 4):
         mg, ng = t.get_tensor("M%d" % mu), t.get_tensor("N%d" % mu)        # [k, u, l]
@@ -428,6 +441,51 @@ def test_ilo_triad_atrg_matches_oracle(D, bond_rank, p, n_pow, steps):
             assert np.abs(got[:k] - ref[:k]).max() <= TOL_SV, (m, key)
     assert t.get_tensor("phi").shape == o.phi.shape == (D, D, D, D, bond_rank)
     assert t.get_tensor("X").shape == (bond_rank, D, D, D, bond_rank)
+
+
+@pytest.mark.parametrize("implicit", [1, 0])
+@pytest.mark.parametrize("D,bond_rank,p,n_pow,steps", [(3, 6, 3, 2, 8), (4, 8, 4, 1, 8), (4, 12, 4, 2, 6), (6, 9, 6, 2, 6), (5, 5, 5, 2, 8)])
+def test_ilo_without_x_y_matches_oracle(D, bond_rank, p, n_pow, steps, implicit):
+    """SURVEY NEXT-2 as the paper states it (PAPER.md :394 "the tensors X and Y are not explicitly constructed. Instead, we work directly
+    with U^bond, sigma, and V^*bond to create isometries of the triad representation", :201): TATRG_OPT_IMPLICIT_XY = 1 against the
+    oracle's implicit route, = 0 against its explicit one (the two oracle routes are pinned to each other in test_oracle_pins.py).
+    Without TATRG_OPT_KEEP_TENSORS no X, Y exist on the device in the implicit setting.  (5, 5) is r_bond = 1."""
+    from oracle import tatrg_oracle as O
+    beta, seed = 0.1497, 23
+    t = T.Tatrg(beta, 0.0, D, p, seed, power_iters=n_pow, bond_rank=bond_rank)
+    t.set_option(T.OPT_IMPLICIT_XY, implicit)
+    o = O.TatrgOracle(beta, 0.0, D, p, seed, n_pow=n_pow, bond_rank=bond_rank, implicit_xy=bool(implicit))
+    for m in range(steps):
+        t.step()
+        o.step()
+        lo = o.lnZ_per_site()
+        assert abs(t.lnZ_per_site() - lo) <= TOL_LNZ * abs(lo), m
+        for which, key in ((T.SV_SIGMA, "sigma"), (T.SV_S, "s")):
+            got, ref = t.singular_values(which, bond_rank), o.last[key][:bond_rank]
+            k = min(len(got), len(ref))
+            assert np.abs(got[:k] - ref[:k]).max() <= TOL_SV, (m, key)
+    assert t.get_tensor("phi").shape == o.phi.shape == (D, D, D, D, bond_rank)
+    with pytest.raises(Exception):
+        t.get_tensor("X")                      # nothing kept: X was never formed (implicit) or not retained (explicit)
+
+
+def test_ilo_without_x_y_at_d16_equals_the_explicit_route():
+    """r_bond = 2 at D = 16, a size the oracle does not reach in seconds: the run without X, Y agrees with the run that forms them
+    (rounding order only), both stay inside the workspace bound, and no X is left on the device."""
+    D, p, rb = 16, 16, 32
+    lnz, sig = {}, {}
+    for implicit in (1, 0):
+        t = T.Tatrg(0.1497, 0.0, D, p, 7, bond_rank=rb)
+        t.set_option(T.OPT_IMPLICIT_XY, implicit)
+        for _ in range(9):
+            t.step()
+        assert t.workspace_peak() <= T.lib().tatrg_workspace_bytes_ilo(D, p, rb)
+        lnz[implicit], sig[implicit] = t.lnZ_per_site(), t.singular_values(T.SV_SIGMA, rb)
+        with pytest.raises(Exception):
+            t.get_tensor("X")
+        t.close()
+    assert abs(lnz[1] - lnz[0]) <= 1e-11 * abs(lnz[0])
+    assert np.abs(sig[1] - sig[0]).max() <= 1e-10
 
 
 def test_ilo_at_d16_runs_and_differs_from_plain():
