@@ -46,7 +46,8 @@ enum {
     TATRG_OPT_GRAPHS = 10,     /* 1 (default): the repeated steps of the subspace iterations are captured once and replayed as CUDA graphs;
                                   0: plain launches.  Same result. */
     TATRG_OPT_VERBOSE = 11,    /* debugging aid, bit mask, default 0: 1 = solver chains report ranks / convergence on stderr, 2 = spectra of
-                                  the full eigen-decompositions, 4 = shape and rate of every DGEMM (with TATRG_OPT_STAGE_TIMING = 2) */
+                                  the full eigen-decompositions, 4 = shape and rate of every DGEMM and permute (with TATRG_OPT_STAGE_TIMING = 2), 8 = the
+                                  contractions that needed a permuted copy of an operand or of their result */
     TATRG_OPT_DGEMM_TMA = 12,  /* 1 (default): contractions whose output takes the 128 x 128 tile and whose operands meet the tensor-map rules
                                   (16-byte aligned bases, even leading dimensions and batch strides) run the TMA-fed kernel (dgemm_tma.cu:
                                   producer warp, cp.async.bulk.tensor into a 128B-swizzled 6-stage mbarrier ring); 0: the cp.async kernel

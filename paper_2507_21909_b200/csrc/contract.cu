@@ -10,6 +10,7 @@
 #include "internal.h"
 #include <algorithm>
 #include <cstring>
+#include <cstdio>
 
 namespace tatrg {
 
@@ -176,6 +177,9 @@ int contract(cudaStream_t st, const char* spec, const Tens& A0, const Tens& B0, 
         c.cost = (c.la.ok ? 0 : szA) + (c.lb.ok ? 0 : szB) + (c.lc.ok ? 0 : szC);
         if (best.cost < 0 || c.cost < best.cost) best = c;
     }
+    if ((g_verbose & 8) && best.cost > 0)      // debugging aid: contractions that need a permuted copy of an operand or of the result
+        fprintf(stderr, "[tatrg contract] %s copies:%s%s%s  A %lld B %lld C %lld doubles\n", spec, best.la.ok ? "" : " A", best.lb.ok ? "" : " B",
+                best.lc.ok ? "" : " C", (long long)szA, (long long)szB, (long long)szC);
     std::vector<double*> temps;
     auto fail = [&](int code, const std::string& msg) { for (double* t : temps) pool.free(t); if (err) *err = msg; return code; };
     // operands

@@ -90,6 +90,8 @@ cudaError_t gauge_blocks(cudaStream_t st, const double* cfull, int ldc, const in
 // philox.cu
 cudaError_t philox_raw(cudaStream_t st, uint64_t seed, uint32_t call, uint32_t stream, uint64_t start, int64_t count, uint32_t* raw);
 cudaError_t philox_gauss(cudaStream_t st, uint64_t seed, uint32_t call, uint32_t stream, uint64_t start, int64_t count, double* z);
+// element (a, b, c) of the tensor [na][nb][nc] drawn with counter (a nb + b) nc + c and stored at [b][a][c]
+cudaError_t philox_gauss_swap01(cudaStream_t st, uint64_t seed, uint32_t call, uint32_t stream, int64_t na, int64_t nb, int64_t nc, double* z);
 cudaError_t philox_rho(cudaStream_t st, uint64_t seed, uint32_t call, uint32_t stream, int64_t rows, int ncols, double* out);
 
 // jacobi.cu.  All decompositions return vectors as ROWS.

@@ -789,21 +789,16 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
     {
         Scope s2(*this);
         // B[i1,j',al] = sum_a' Dt[i1,j',a'] core[al,a'],  C[i1,i',be] = sum_a' A[i1,i',a'] core[a',be]   (core symmetric)
-        Tens b = mm(false, true, F, chi, chi, dt.p, chi, core.p, chi);
-        Tens bm = perm(view(b, {d1, J, chi}), {1, 0, 2});              // Eq. A.2 :345  B[(j'),(i1 al)]
-        drop(b);
-        Tens cc = mm(false, false, F, chi, chi, a.p, chi, core.p, chi);
-        Tens cm = perm(view(cc, {d1, J, chi}), {1, 0, 2});             // Eq. A.3 :348  C[(i'),(i1 be)]
-        drop(cc);
+        // written straight into the layout of Eq. A.2-A.3 (rows j', columns (i1 al)): i1 is the batch of the product, ldc = d1 chi
+        Tens bm = ein("Ijc,ac->jIa", view(dt, {d1, J, chi}), core);    // Eq. A.2 :345  B[(j'),(i1 al)]
+        Tens cm = ein("Ijc,cb->jIb", view(a, {d1, J, chi}), core);     // Eq. A.3 :348  C[(i'),(i1 be)]
         Tens Qs[2], Rs[2], Xs[2];
         // While the two Cholesky chains are in flight the caller's stream draws Omega^phys and forms B^T Omega^phys, the part of
         // the projection Q^B^T Omega^phys = XB (B^T Omega^phys) that needs no factor.
         std::function<void()> early = [&]() {
             const int64_t n = d1 * chi, l0 = std::min<int64_t>(c.Dbond + c.p, chi * n);
-            Tens om = make({chi, J, l0});
-            ck(philox_gauss(st, c.seed, (uint32_t)call, 0, 0, chi * J * l0, om.p), "philox");
-            Tens omp = perm(om, {1, 0, 2});
-            drop(om);
+            Tens omp = make({J, chi, l0});                             // drawn as (be, j', m), stored [j', be, m]
+            ck(philox_gauss_swap01(st, c.seed, (uint32_t)call, 0, chi, J, l0, omp.p), "philox");
             btom = ein("jc,jbm->cbm", view(bm, {J, n}), omp);
             drop(omp);
             detach(btom);
@@ -836,10 +831,8 @@ void Stepper::bond_swap(const Tens& a, const Tens& dt, const Tens& core, Tens& x
     } else {
         if (btom.p) drop(btom);
         Scope s2(*this);
-        Tens om = make({chi, J, l});
-        ck(philox_gauss(st, c.seed, (uint32_t)call, 0, 0, chi * J * l, om.p), "philox");
-        Tens omp = perm(om, {1, 0, 2});                                   // [j', be, m]: one wide GEMM instead of chi narrow ones
-        drop(om);
+        Tens omp = make({J, chi, l});                                     // [j', be, m]: one wide GEMM instead of chi narrow ones
+        ck(philox_gauss_swap01(st, c.seed, (uint32_t)call, 0, chi, J, l, omp.p), "philox");
         if (implicit) {
             Tens tmp = ein("jc,jbm->cbm", QB, omp);
             omega = ein("pc,cBm->Bpm", XB, tmp);
@@ -1434,10 +1427,12 @@ void Stepper::run() {
         save("M2", Mt[0]); save("M3", Mt[1]); save("M4", Mt[2]); save("N2", Nt[0]); save("N3", Nt[1]); save("N4", Nt[2]);
         {   // Phi'[i1,k2,k3,k4,g]
             Scope s2(*this);
-            Tens im = ein("kuc,zul->kclz", U[0], Mt[0]);
-            Tens imm = ein("kclz,ycw->klwzy", im, Mt[1]);
-            Tens lam = ein("klwzy,xlw->kxzy", imm, U[1]);               // Lambda[kA,kX,k2,k3]
-            drop(im); drop(imm);
+            // Lambda[kA,kX,k2,k3] = sum_{u,c,l,w} I[kA,u,c] M2[k2,u,l] M3[k3,c,w] J[kX,l,w]: each isometry meets one squeezer first
+            // (two K D^3 tensors), then one K^2 D^2 x D^2 product -- no K D^4 intermediate
+            Tens im = ein("kuc,zul->kzcl", U[0], Mt[0]);                // sum over the upper leg 2
+            Tens jm = ein("xlw,ycw->xycl", U[1], Mt[1]);                // sum over the lower leg 3
+            Tens lam = ein("kzcl,xycl->kxzy", im, jm);
+            drop(im); drop(jm);
             Tens ph = ein("Ikxzd,kxpq->Ipqzd", xi, lam);
             drop(xi);
             phin = perm(ph, {1, 2, 3, 0, 4});                           // (f) rotate: axis 1 becomes axis 4  (R5)
@@ -1445,10 +1440,10 @@ void Stepper::run() {
         }
         {   // Psi'[j1,k2,k3,k4,g]
             Scope s2(*this);
-            Tens kn = ein("yuc,zul->yclz", U[2], Nt[0]);
-            Tens knn = ein("yclz,vcw->ylwzv", kn, Nt[1]);
-            Tens lam = ein("ylwzv,dlw->dyzv", knn, U[3]);               // Lambda'[kD,kY,k2,k3]
-            drop(kn); drop(knn);
+            Tens kn = ein("yuc,zul->yzcl", U[2], Nt[0]);
+            Tens ln = ein("dlw,vcw->dvcl", U[3], Nt[1]);
+            Tens lam = ein("yzcl,dvcl->dyzv", kn, ln);                  // Lambda'[kD,kY,k2,k3]
+            drop(kn); drop(ln);
             Tens ps = ein("Jdyzg,dypq->Jpqzg", xip, lam);
             drop(xip);
             psin = perm(ps, {1, 2, 3, 0, 4});
