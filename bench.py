@@ -234,8 +234,8 @@ def aggregate_seconds_per_step(ms_max, steps, world):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant DGEMM launch (Xi = E (M4 F), Eq. 2.18: M=2048, N=65536, K=1024)
 # from the ncu --set full capture named in `source`; its algorithmic bytes are 8 (MK + KN + MN) = 1.63e9
-DGEMM_TRAFFIC = {"launch": "M=2048 N=65536 K=1024 (grid 8192)", "dram_bytes": 1.602e9, "algorithmic_bytes": 1.627e9,
-                 "source": "profiles/dgemm_r01_ncu_full.txt"}
+DGEMM_TRAFFIC = {"launch": "M=2048 N=65536 K=1024 (grid 8192), dgemm_tma_kernel", "dram_bytes": 1.605e9, "algorithmic_bytes": 1.627e9,
+                 "source": "profiles/dgemm_tma_r02_ncu_full.txt (launch 12: dram__bytes_read.sum 567.7 MB + dram__bytes_write.sum 1.037 GB)"}
 
 
 # ---- the CUDA path ---------------------------------------------------------------------------------------------------
@@ -425,7 +425,7 @@ def run_cuda(args):
             "step_ms": {str(s): round(x, 2) for s, x in zip(steps_abs, step_ms)},
             "model_tflops": prof.g[1] / prof.steps / (ms / args.steps * 1e-3) / 1e12,
             "host_syncs_per_step": prof.syncs / prof.steps, "launches_per_step": prof.launches / prof.steps,
-            "roofline": {"bound": "tensor", "kernel": "dgemm_kernel (DMMA m8n8k4): the %d contraction launches of a step (>= 1e9 flop each, "
+            "roofline": {"bound": "tensor", "kernel": "dgemm_tma_kernel / dgemm_kernel (DMMA m8n8k4, TMA-fed 128x128x16 tile): the %d contraction launches of a step (>= 1e9 flop each, "
                                                       "%.1f%% of the step's DGEMM flops), steps %d-%d" % (main["launches_per_step"], 100.0 * prof.l[1] / prof.g[1], steps_abs[0], steps_abs[n_first - 1]),
                          "achieved": main["achieved"], "peak": peak_tf, "unit": "TFLOP/s", "frac": main["frac"],
                          "traffic": DGEMM_TRAFFIC["dram_bytes"], "traffic_detail": DGEMM_TRAFFIC,
@@ -442,6 +442,10 @@ def run_cuda(args):
                                    "schedule": "TATRG_OPT_OVERLAP = 0: every stage on one stream, no kernel beside them"}},
             "permute": dict(perm_block(prof), bound="hbm", peak=pk["hbm"], unit="GB/s",
                             schedule="in situ (some permutes share HBM with the solver chains on auxiliary streams)",
+                            note="achieved = ALL permute launches of a step (bytes / sum of the per-launch CUDA-event times); `large` = the launches "
+                                 "that move >= 100 MB (D^5 tensors, larger than the 126 MB L2: the HBM-bound class); the rest are L2-resident copies of "
+                                 "<= 67 MB whose event-timed duration is a launch floor (6-20 us each).  Round 2 removed 11 of the 19 large permutes "
+                                 "of a step (16.1 -> 7.8 GB permuted per step), which lowers this aggregate while the step gets faster",
                             alone={k: v for k, v in perm_block(alone).items() if k in ("achieved", "frac", "large")},
                             by_regime={"critical": perm_block(prof_c), "post_critical": perm_block(prof_p)}),
             "stage_ms": stage_block(prof),

@@ -68,6 +68,14 @@ struct Stepper {
         scopes.back().push_back(p);
         return p;
     }
+    // optional scratch (split-K partials, the overlap arena): null when the workspace has no room; registered in the current scope so
+    // that an exception between here and release() cannot leave the block live in the caller's workspace
+    double* scratch(int64_t n) {
+        double* p = n > 0 ? c.pool.alloc(n) : nullptr;
+        if (p) scopes.back().push_back(p);
+        return p;
+    }
+    void release(double* p) { if (p) { Tens t; t.p = p; drop(t); } }
     Tens make(std::initializer_list<int64_t> dims) {
         Tens t; t.nd = 0; for (int64_t d : dims) t.d[t.nd++] = d;
         t.p = raw(t.size());
@@ -129,9 +137,9 @@ struct Stepper {
         Tens C = make({M, N});
         const bool lower = sym && M == N && M >= 256;
         int64_t need = dgemm_splitk_doubles(M, N, K, lower);
-        double* part = need ? c.pool.alloc(need) : nullptr;
+        double* part = scratch(need);
         ck(dgemm_splitk(st, ta, tb, M, N, K, 1.0, A, lda, B, ldb, C.p, N, part, lower), "dgemm");
-        if (part) c.pool.free(part);
+        release(part);
         if (lower) ck(mirror_lower(st, (int)M, C.p), "mirror");
         return C;
     }
@@ -145,9 +153,9 @@ struct Stepper {
             ck(dgemm_splitk(st, ta, tb, M, N, K, 1.0, A, lda, B, ldb, C, ldc, need <= part_cap ? part_fixed : nullptr), "dgemm");
             return;
         }
-        double* part = need ? c.pool.alloc(need) : nullptr;
+        double* part = scratch(need);
         ck(dgemm_splitk(st, ta, tb, M, N, K, 1.0, A, lda, B, ldb, C, ldc, part), "dgemm");
-        if (part) c.pool.free(part);
+        release(part);
     }
     std::vector<double> to_host(const double* d, int64_t n) {
         std::vector<double> h(n);
@@ -1354,7 +1362,7 @@ void Stepper::run() {
             const size_t kt = (size_t)std::min<int64_t>(c.Ktri, a.d[1] * a.d[2]);
             const size_t xi_bytes = 8 * (size_t)a.d[0] * kt * kt * (size_t)gr * (size_t)c.D;
             if (c.pool.in_use() + 2 * arena_bytes + 3 * xi_bytes <= c.pool.capacity())
-                arena = c.pool.alloc((int64_t)(arena_bytes / 8));   // freed at the end of the step, after the joins
+                arena = scratch((int64_t)(arena_bytes / 8));        // released at the end of the step, after the joins (or by the unwinding scope)
             if (!arena) overlap = false;
         }
         Pool arena_pool;
@@ -1449,7 +1457,7 @@ void Stepper::run() {
             psin = perm(ps, {1, 2, 3, 0, 4});
             keep(psin);
         }
-        if (arena) c.pool.free(arena);
+        release(arena);
         mark();
     }
     c.pool.free(c.phi.p); c.pool.free(c.psi.p);
