@@ -16,7 +16,7 @@ _lib = None
 
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC, ESTATE = 0, -1, -2, -3, -4, -5
 OPT_POWER_ITERS, OPT_K_TRIAD, OPT_TAU, OPT_STAGE_TIMING, OPT_KEEP_TENSORS, OPT_METHOD, OPT_SUBSPACE, OPT_BOND_RANK = 1, 2, 3, 4, 5, 6, 7, 8
-OPT_OVERLAP, OPT_GRAPHS, OPT_VERBOSE, OPT_DGEMM_TMA, OPT_IMPLICIT_XY = 9, 10, 11, 12, 13
+OPT_OVERLAP, OPT_GRAPHS, OPT_VERBOSE, OPT_DGEMM_TMA, OPT_IMPLICIT_XY, OPT_CHEBYSHEV = 9, 10, 11, 12, 13, 14
 METHOD_TRIAD, METHOD_ATRG = 0, 1
 SV_SIGMA, SV_S = 0, 1
 STAGES = ["decompose", "qr", "rsvd", "lift", "triad", "triad_tensors", "squeezer_grams", "squeezers", "contract",

@@ -74,6 +74,7 @@ int tatrg_set_option(tatrg_handle c, int key, double value) {
         case TATRG_OPT_VERBOSE: if (value < 0 || value > 15) return TATRG_EINVAL; c->verbose = (int)value; return TATRG_OK;
         case TATRG_OPT_DGEMM_TMA: c->dgemm_tma = value != 0; return TATRG_OK;
         case TATRG_OPT_IMPLICIT_XY: c->implicit_xy = value != 0; return TATRG_OK;
+        case TATRG_OPT_CHEBYSHEV: c->use_cheb = value != 0; return TATRG_OK;
         case TATRG_OPT_BOND_RANK: {
             if (c->m > 0) return TATRG_ESTATE;
             if (value != std::floor(value) || value < c->D) return TATRG_EINVAL;

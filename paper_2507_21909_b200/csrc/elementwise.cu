@@ -19,6 +19,14 @@ __global__ void scale_last_kernel(double* out, const double* in, const double* v
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x)
         out[e] = in[e] * fmode(vec[e % cols], mode);
 }
+// out = a x + b y + c z (z may be null; out may alias any input): the three-term recurrence of the Chebyshev-filtered subspace iteration
+__global__ void lincomb3_kernel(double* out, double a, const double* x, double b, const double* y, double c, const double* z, int64_t total) {
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+        double v = a * x[e] + b * y[e];
+        if (z) v += c * z[e];
+        out[e] = v;
+    }
+}
 __global__ void scale_rows_kernel(double* out, const double* in, const double* vec, int64_t total, int64_t cols, int mode) {
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x)
         out[e] = in[e] * fmode(vec[e / cols], mode);
@@ -122,6 +130,11 @@ inline unsigned nblocks(int64_t total) { int64_t b = (total + 255) / 256; if (b 
 cudaError_t scale_last(cudaStream_t st, double* out, const double* in, const double* vec, int64_t rows, int64_t cols, int mode) {
     if (rows * cols == 0) return cudaSuccess;
     scale_last_kernel<<<nblocks(rows * cols), 256, 0, st>>>(out, in, vec, rows * cols, cols, mode); count_launch();
+    return cudaGetLastError();
+}
+cudaError_t lincomb3(cudaStream_t st, double* out, double a, const double* x, double b, const double* y, double c, const double* z, int64_t n) {
+    if (n == 0) return cudaSuccess;
+    lincomb3_kernel<<<nblocks(n), 256, 0, st>>>(out, a, x, b, y, c, z, n); count_launch();
     return cudaGetLastError();
 }
 cudaError_t scale_rows(cudaStream_t st, double* out, const double* in, const double* vec, int64_t rows, int64_t cols, int mode) {

@@ -76,6 +76,7 @@ cudaError_t permute(cudaStream_t st, int nd, const int64_t* dims, const int* per
 cudaError_t scale_last(cudaStream_t st, double* out, const double* in, const double* vec, int64_t rows, int64_t cols,
                        int mode);  // out[r,c] = in[r,c] * f(vec[c]); mode 0: v, 1: 1/v, 2: 1/sqrt(v), 3: sqrt(v), 4: v^-3/2
 cudaError_t scale_rows(cudaStream_t st, double* out, const double* in, const double* vec, int64_t rows, int64_t cols, int mode);
+cudaError_t lincomb3(cudaStream_t st, double* out, double a, const double* x, double b, const double* y, double c, const double* z, int64_t n);   // out = a x + b y + c z (z may be null)
 cudaError_t gather_rows_scaled(cudaStream_t st, double* out, const double* in, const int* idx, const double* scale, int64_t nrows,
                                int64_t cols, int64_t ld_in);  // out[r,:] = scale[r]*in[idx[r], 0:cols]
 cudaError_t gather_vec(cudaStream_t st, double* out, const double* in, const int* idx, int64_t n, int64_t stride_in, double mul);

@@ -470,6 +470,10 @@ struct Stepper {
         cudaStream_t stream = nullptr; double* part = nullptr; int64_t part_cap = 0;
         int cur = 0;                 // the basis [Z; W] lives in buf[cur]
         int done = 0, target = 0, deg = 1;
+        int rdeg = 1;                // degree of the plain step whose Cholesky factor is in L: its diagonal is ~ lam_j^rdeg
+        // Chebyshev-filtered cycles (symmetric problems): p_deg(A) Z with p_deg the Chebyshev polynomial of the interval [0, cheb_hi]
+        // that holds the unwanted eigenvalues; one cycle is worth `gain` plain applications (done_f counts in that unit)
+        bool cheb = false; double cheb_hi = 0, gain = 0, done_f = 0; Tens tmp[2];
         bool ok = true;
         int bcap = 0; bool widen = false, widened = false;     // the block may be doubled once when convergence is too slow
         const double* Z() const { return buf[cur].p; }
@@ -496,7 +500,33 @@ struct Stepper {
         int a = s.cur;
         for (int i = 0; i < deg; ++i) { sub_apply(s, a); a ^= 1; }
         sub_orth(s, a, shift);
-        s.done += deg;
+        s.done_f += deg; s.done = (int)s.done_f; s.rdeg = deg;
+    }
+    // One Chebyshev-filtered cycle of a symmetric problem: Z <- orthonormalise(T_deg(t) Z), t = (2 / hi) A - 1, which maps the unwanted
+    // eigenvalues [0, hi] into [-1, 1] (|T_deg| <= 1 there) and amplifies lam_k > hi by cosh(deg acosh(2 lam_k / hi - 1)):
+    // the same subspace as plain orthogonal iteration in 2-3 times fewer applications (three-term recurrence
+    // Y_{j+1} = 2 t Y_j - Y_{j-1}, Y_0 = Z, Y_1 = t Z).  The basis stays in buf[cur]; tmp[0] holds A Y_j, tmp[1] the odd iterates.
+    void sub_step_cheb(SubProb& s, int deg, double shift) {
+        const int64_t nb = (int64_t)s.n * s.b;
+        double* Z = s.buf[s.cur].p; double* Y2 = s.buf[s.cur ^ 1].p; double* G = s.tmp[0].p; double* Y1 = s.tmp[1].p;
+        const double a = 2.0 / s.cheb_hi;
+        mm_into(G, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, Z, s.b);
+        ck(lincomb3(st, Y1, a, G, -1.0, Z, 0.0, nullptr, nb), "lincomb");                     // Y1 = t Z
+        double* src = Y1;
+        if (deg >= 2) {
+            mm_into(G, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, Y1, s.b);
+            ck(lincomb3(st, Y2, 2 * a, G, -2.0, Y1, -1.0, Z, nb), "lincomb");                 // Y2 = 2 t Y1 - Z
+            src = Y2;
+        }
+        if (deg >= 3) {
+            mm_into(G, s.b, false, false, s.n, s.b, s.n, s.Bm, s.n, Y2, s.b);
+            ck(lincomb3(st, Y1, 2 * a, G, -2.0, Y2, -1.0, Y1, nb), "lincomb");                // Y3 = 2 t Y2 - Y1 (in place of Y1)
+            src = Y1;
+        }
+        mm_into(s.Gm.p, s.b, true, false, s.b, s.b, s.n, src, s.b, src, s.b);
+        ck(cholesky(st, s.b, s.Gm.p, s.b, s.L.p, s.b, shift, 1e-14, s.cw, false), "cholesky");
+        ck(trsm_right_lt(st, s.n, s.b, src, s.b, Z, s.b, s.L.p, s.b, s.cw), "trsm");           // Z is free: every iterate has been formed
+        s.done_f += s.gain; s.done = (int)s.done_f; s.rdeg = 0;
     }
     // The problems of a stage are independent chains of small launches: each runs on a stream of its own (created once
     // per process), forked from and joined to the caller's stream by events, so that their kernels overlap on the device.
@@ -536,12 +566,16 @@ struct Stepper {
     // is captured into a CUDA graph and replayed.  Counters are incremented at capture time only, hence the correction.
     void sub_run(SubProb& s, double shift) {
         static bool graphs_ok = true;      // cleared for the process when stream capture is unavailable
-        const int steps = (s.target - s.done + s.deg - 1) / s.deg;
-        const int unit = (s.deg % 2 == 0) ? 2 : 1;
+        const bool cheb = s.cheb;
+        const double per = cheb ? s.gain : (double)s.deg;        // plain applications a cycle is worth
+        // Chebyshev cycles are followed by ONE plain step, whose Cholesky diagonal estimates the eigenvalues again (estimate())
+        const int steps = cheb ? std::max(0, (int)std::ceil((s.target - s.done_f - 1.0) / per)) : (s.target - s.done + s.deg - 1) / s.deg;
+        const int unit = cheb ? 1 : ((s.deg % 2 == 0) ? 2 : 1);
         const int reps = steps / unit;
+        auto cycle = [&]() { if (cheb) sub_step_cheb(s, s.deg, shift); else sub_step(s, s.deg, shift); };
         int left = steps;
         if (graphs_ok && c.use_graphs && s.stream && c.timing < 2 && reps >= 3) {      // never the caller's stream: it may be the legacy default stream
-            const int done0 = s.done, cur0 = s.cur;
+            const double done0 = s.done_f; const int cur0 = s.cur;
             Counters* cn = g_counter;
             const long long l0 = cn ? cn->launches : 0, gc0 = cn ? cn->gemm_calls : 0; const double f0 = cn ? cn->gemm_flops : 0;
             cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr;
@@ -550,7 +584,7 @@ struct Stepper {
             bool ok = ge == cudaSuccess;
             std::string why;
             if (ok) {
-                try { for (int u = 0; u < unit; ++u) sub_step(s, s.deg, shift); } catch (const Fail& f) { ok = false; why = f.msg; } catch (...) { ok = false; }
+                try { for (int u = 0; u < unit; ++u) cycle(); } catch (const Fail& f) { ok = false; why = f.msg; } catch (...) { ok = false; }
                 ge = cudaStreamEndCapture(st, &graph);
                 if (ge != cudaSuccess || !graph) ok = false;
             }
@@ -563,16 +597,17 @@ struct Stepper {
                 c.graveyard.push_back(exec);
                 if (!ok) fail(TATRG_ECUDA, "graph launch failed");
                 if (cn) { cn->launches += (cn->launches - l0) * (reps - 1); cn->gemm_calls += (cn->gemm_calls - gc0) * (reps - 1); cn->gemm_flops += (cn->gemm_flops - f0) * (reps - 1); }
-                s.done = done0 + reps * unit * s.deg; s.cur = cur0;
+                s.done_f = done0 + reps * unit * per; s.done = (int)s.done_f; s.cur = cur0;
                 left = steps - reps * unit;
             } else {        // capture unavailable: nothing was executed; plain launches from the saved state
                 cudaGetLastError();
                 graphs_ok = false;
                 if (cn) { cn->launches = l0; cn->gemm_calls = gc0; cn->gemm_flops = f0; }
-                s.done = done0; s.cur = cur0;
+                s.done_f = done0; s.done = (int)s.done_f; s.cur = cur0;
             }
         }
-        for (int i = 0; i < left; ++i) sub_step(s, s.deg, shift);
+        for (int i = 0; i < left; ++i) cycle();
+        if (cheb) sub_step(s, 1, shift);
     }
     // Runs the iterations of all problems (interleaved so that the host reads the convergence estimates of all of them
     // with one synchronisation per phase) and leaves in every s.H the b x b Rayleigh-Ritz matrix.  Problems that cannot
@@ -603,7 +638,7 @@ struct Stepper {
         // iteration restarted, before the full decomposition is considered.  All buffers are sized for the doubled block up front.
         auto init_problem = [&](SubProb& s) {
             OnStream on(*this, s);
-            s.cur = 0; s.done = 0; s.target = 0; s.deg = 1;
+            s.cur = 0; s.done = 0; s.done_f = 0; s.target = 0; s.deg = 1; s.rdeg = 1; s.cheb = false;
             ck(fill_zero(st, s.L.p, (int64_t)s.b * s.b), "zero");
             ck(cudaMemsetAsync(const_cast<int*>(cholesky_info(s.cw, s.b)), 0, sizeof(int), st), "memset"); count_launch();
             ck(philox_gauss(st, c.seed, (uint32_t)call, s.sid, 0, (int64_t)s.n * s.b, s.buf[1].p), "philox");
@@ -618,6 +653,7 @@ struct Stepper {
             s.buf[0] = make({rows, s.bcap}); s.buf[1] = make({rows, s.bcap});
             s.Gm = make({s.bcap, s.bcap}); s.L = make({s.bcap, s.bcap}); s.H = make({s.bcap, s.bcap});
             s.cw = raw((int64_t)cholesky_work_doubles(s.bcap)); s.dg = raw(s.bcap);
+            if (c.use_cheb && !s.F) { s.tmp[0] = make({(int64_t)s.n, s.bcap}); s.tmp[1] = make({(int64_t)s.n, s.bcap}); }
             init_problem(s);
         }
         auto sync_all = [&]() { for (SubProb& s : ps) if (s.stream) cudaStreamSynchronize(s.stream); cudaStreamSynchronize(st); return std::chrono::steady_clock::now(); };
@@ -635,7 +671,8 @@ struct Stepper {
             double head = s.r[0]; for (int j = 0; j < s.kmax; ++j) head = std::min(head, s.r[j]);
             if (!(head > 1e-12 * s.r[0]) || !(tail > 1e-9 * head)) { s.ok = false; return; }     // rank-deficient block: full decomposition
             // the diagonal of R is that of the last orthonormalisation: r_j ~ lam_j^deg
-            const double rho = 1.1 * std::pow(tail / head, 1.0 / s.deg);
+            const int rd = std::max(1, s.rdeg);
+            const double rho = 1.1 * std::pow(tail / head, 1.0 / rd);
             // slow convergence (rho >= 0.6: more than 60 applications): the doubled block converges like lam_{2b+1} / lam_kmax and
             // costs twice as much per application -- taken whenever it is available; without it up to qmax applications are
             // still far cheaper than the full decomposition (0.1 ms each against 25 ms)
@@ -643,10 +680,23 @@ struct Stepper {
             if (!(rho < 0.95)) { s.ok = false; return; }
             s.target = std::max(s.target, (int)std::ceil(13.0 / std::log10(1.0 / rho)) + 2);
             if (s.target > qmax) s.ok = false;
-            const double range = std::pow(s.r[0] / tail, 1.0 / s.deg);
+            const double range = std::pow(s.r[0] / tail, 1.0 / rd);
             int deg = 1;
             while (deg < 3 && std::pow(range, deg + 1) <= 1e11) ++deg;
-            if (verbose) fprintf(stderr, "[tatrg subspace n=%d b=%d kmax=%d%s] after %d iterations: rho %.3f -> %d iterations, %d per orthonormalisation\n", s.n, s.b, s.kmax, s.F ? " product" : "", s.done, rho, s.target, deg);
+            s.cheb = false;
+            if (c.use_cheb && !s.F && s.tmp[0].p) {
+                // unwanted eigenvalues in [0, 1.1 lam_tail]: x_k = 2 lam_k / hi - 1 = 2 / rho - 1 for the slowest wanted one; the dynamic
+                // range of a cycle is T_deg(x_1) (the block must stay numerically independent between orthonormalisations)
+                const double x1 = 2.0 * range / 1.1 - 1.0, xk = 2.0 / rho - 1.0;
+                auto T = [](int d, double x) { return std::cosh(d * std::acosh(x)); };
+                if (xk > 1.02 && T(1, x1) <= 1e11) {
+                    int d = 1;
+                    while (d < 3 && T(d + 1, x1) <= 1e11) ++d;
+                    const double gain = std::log10(T(d, xk)) / std::log10(1.0 / rho);
+                    if (gain > 1.15 * deg) { s.cheb = true; s.gain = gain; s.cheb_hi = 1.1 * std::pow(tail, 1.0 / rd); deg = d; }
+                }
+            }
+            if (verbose) fprintf(stderr, "[tatrg subspace n=%d b=%d kmax=%d%s] after %d iterations: rho %.3f -> %d iterations, %d per orthonormalisation%s\n", s.n, s.b, s.kmax, s.F ? " product" : "", s.done, rho, s.target, deg, s.cheb ? " (Chebyshev)" : "");
             s.deg = deg;
         };
         for (int pass = 0; pass < 3; ++pass) {

@@ -32,6 +32,7 @@ struct tatrg_ctx {
     bool use_graphs = true;          // TATRG_OPT_GRAPHS: replay the iteration steps of the solver chains as CUDA graphs
     int verbose = 0;                 // TATRG_OPT_VERBOSE
     int dgemm_tma = 1;               // TATRG_OPT_DGEMM_TMA
+    bool use_cheb = true;            // TATRG_OPT_CHEBYSHEV: Chebyshev-filtered cycles in the subspace iterations of the symmetric (triad) problems
     bool implicit_xy = true;         // TATRG_OPT_IMPLICIT_XY: triad isometries and F, G from U^bond, sigma, V^bond; X, Y never formed (:394)
     bool qr_deficient_hint = false;  // the last QR pre-reduction met numerically rank-deficient operands: the next one goes straight to the rank-revealing path
     tatrg::Pool pool;

@@ -83,6 +83,43 @@ def test_config4_first_steps_at_full_size(subspace):
     assert w[0] <= TOL_LNZ and w[1] <= TOL_SV and w[2] <= TOL_SV, w
 
 
+@pytest.mark.parametrize("idx", range(2))
+def test_config3_field_with_plain_orthogonal_iteration(idx):
+    """configs[2] once more with TATRG_OPT_CHEBYSHEV = 0: plain powers of the Gram matrix per orthonormalisation instead of the
+    Chebyshev-filtered cycles the default path takes (which test_config3_field covers); same oracle, same tolerance."""
+    rec = golden("c3")[idx]
+    t = T.Tatrg(rec["beta"], rec["h"], rec["D"], rec["oversample"], rec["seed"], power_iters=rec["n_pow"])
+    t.set_option(T.OPT_CHEBYSHEV, 0)
+    for m in range(len(rec["lnZ"])):
+        t.step()
+        assert abs(t.lnZ_per_site() - rec["lnZ"][m]) <= TOL_LNZ * abs(rec["lnZ"][m]), m
+        got = t.singular_values(T.SV_SIGMA, rec["D"])
+        ref = np.zeros(rec["D"]); ref[:len(rec["sigma"][m])] = rec["sigma"][m]
+        g = np.zeros(rec["D"]); g[:len(got)] = got
+        assert np.abs(g - ref).max() <= TOL_SV, m
+    t.close()
+
+
+def test_chebyshev_and_plain_iterations_agree_at_d32():
+    """TATRG_OPT_CHEBYSHEV 1 / 0 at D = 32 through 24 steps (critical and post-critical regime, block widening included): the filtered
+    iteration converges to the same isometries (ln Z/V to 1e-12, spectra to 1e-10) in fewer launches."""
+    runs = []
+    for cheb in (1, 0):
+        t = T.Tatrg(0.1497, 0.0, 32, 32, 42)
+        t.set_option(T.OPT_CHEBYSHEV, cheb)
+        out, launches = [], 0
+        for _ in range(24):
+            t.step()
+            launches += t.launches()
+            out.append((t.lnZ_per_site(), t.singular_values(T.SV_SIGMA, 32), t.singular_values(T.SV_S, 32)))
+        runs.append((out, launches))
+        t.close()
+    for a, b in zip(runs[0][0], runs[1][0]):
+        assert abs(a[0] - b[0]) <= 1e-12 * abs(b[0])
+        assert np.abs(a[1] - b[1]).max() <= 1e-10 and np.abs(a[2] - b[2]).max() <= 1e-10
+    assert runs[0][1] < runs[1][1]
+
+
 def test_subspace_and_full_decompositions_agree_at_d32():
     """The two ways of getting the triad isometries / squeezers / QR factors (TATRG_OPT_SUBSPACE 1 / 0) give the same
     physics over 10 steps at D = 32, well inside the parity tolerance, and the iteration is the faster one."""
