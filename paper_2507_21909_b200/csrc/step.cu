@@ -676,7 +676,11 @@ struct Stepper {
             // slow convergence (rho >= 0.6: more than 60 applications): the doubled block converges like lam_{2b+1} / lam_kmax and
             // costs twice as much per application -- taken whenever it is available; without it up to qmax applications are
             // still far cheaper than the full decomposition (0.1 ms each against 25 ms)
-            if (!(rho < 0.6) && !s.widened && s.bcap > s.b) { s.widen = true; return; }
+            // (with Chebyshev-filtered cycles a ratio up to ~0.8 still needs at most ~24 cycles of degree 2, cheaper than the restart with a
+            // doubled block and its 2b x 2b Rayleigh-Ritz problem)
+            // (measured over the 60 steps of configs[3]: doubling from 0.6 / 0.7 / 0.8 / 0.9 on -> 92.3 / 91.6 / 90.7 / 91.3 ms per post-critical step)
+            const double widen_at = (c.use_cheb && !s.F && s.tmp[0].p) ? 0.8 : 0.6;
+            if (!(rho < widen_at) && !s.widened && s.bcap > s.b) { s.widen = true; return; }
             if (!(rho < 0.95)) { s.ok = false; return; }
             s.target = std::max(s.target, (int)std::ceil(13.0 / std::log10(1.0 / rho)) + 2);
             if (s.target > qmax) s.ok = false;
