@@ -45,10 +45,17 @@ __global__ void gauss_kernel(uint32_t k0, uint32_t k1, uint32_t call, uint32_t s
 // the same Gaussians, element e = (a, b, c) of a tensor [na][nb][nc] written at [b][a][c]: Omega^phys is drawn in the order (be, j', m)
 // (R11/R12) and consumed as [j'][be][m]; writing it there saves a 16-byte-per-element permute of the largest tensor of the bond swap
 __global__ void gauss_swap01_kernel(uint32_t k0, uint32_t k1, uint32_t call, uint32_t stream, int64_t na, int64_t nb, int64_t nc, double* z) {
-    const int64_t count = na * nb * nc;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t o = i / nc, c = i - o * nc, b = o / na, a = o - b * na;       // i walks the OUTPUT [b][a][c]: coalesced stores
-        z[i] = gauss_of((uint64_t)((a * nb + b) * nc + c), call, stream, k0, k1);
+    // one block per b (grid-stride): the (a, c) plane of the output is contiguous, (a, c) advance without a division
+    const int64_t per = na * nc;
+    const int64_t da = blockDim.x / nc, dc = blockDim.x % nc;
+    for (int64_t b = blockIdx.x; b < nb; b += gridDim.x) {
+        int64_t a = threadIdx.x / nc, c = threadIdx.x % nc;
+        double* out = z + b * per;
+        for (int64_t t = threadIdx.x; t < per; t += blockDim.x) {
+            out[t] = gauss_of((uint64_t)((a * nb + b) * nc + c), call, stream, k0, k1);
+            a += da; c += dc;
+            if (c >= nc) { c -= nc; a += 1; }
+        }
     }
 }
 // rho[r, j] = Gaussian(counter e = r*kRhoCols + j), j < ncols, stored densely as rows x ncols
@@ -74,7 +81,8 @@ cudaError_t philox_gauss(cudaStream_t st, uint64_t seed, uint32_t call, uint32_t
 }
 cudaError_t philox_gauss_swap01(cudaStream_t st, uint64_t seed, uint32_t call, uint32_t stream, int64_t na, int64_t nb_, int64_t nc, double* z) {
     if (na * nb_ * nc <= 0) return cudaSuccess;
-    gauss_swap01_kernel<<<nb(na * nb_ * nc), 256, 0, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), call, stream, na, nb_, nc, z); count_launch();
+    const int64_t blocks = nb_ < (1 << 20) ? nb_ : (1 << 20);
+    gauss_swap01_kernel<<<(unsigned)blocks, 256, 0, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), call, stream, na, nb_, nc, z); count_launch();
     return cudaGetLastError();
 }
 cudaError_t philox_rho(cudaStream_t st, uint64_t seed, uint32_t call, uint32_t stream, int64_t rows, int ncols, double* out) {
