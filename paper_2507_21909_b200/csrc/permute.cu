@@ -160,6 +160,9 @@ static cudaError_t permute_raw(cudaStream_t st, int nd, const int64_t* dims, con
             for (int i = 0; i < m - 2; ++i) { b.ext[i] = od[i]; b.sin[i] = sin_o[i]; b.sout[i] = sout_o[i]; }
             const int64_t ext_last = od[m - 2], nruns = rows / ext_last;
             int64_t chunk_rows = 1024 / (inner / 2); if (chunk_rows < 1) chunk_rows = 1;      // ~16 KB per warp visit
+            // small (L2-resident) tensors: shorter visits until every SM has 16 warps to hide the latency with (a 8 MB tensor at 16 KB
+            // per visit is 512 visits = 64 CTAs: 10 us, latency-bound)
+            while (chunk_rows > 1 && nruns * ((ext_last + chunk_rows - 1) / chunk_rows) < 148 * 16) chunk_rows = (chunk_rows + 1) / 2;
             const int64_t chunks = (ext_last + chunk_rows - 1) / chunk_rows;
             int64_t nb = (nruns * chunks + 7) / 8; if (nb > 148 * 64) nb = 148 * 64;
             permute_runs_kernel<<<(unsigned)nb, 256, 0, st>>>(b, ext_last, sin_o[m - 2], inner, nruns, chunk_rows, chunks, in, out);
