@@ -28,7 +28,8 @@ RUNS = {
            for b, s in zip((0.140, 0.145, 0.1497, 0.155, 0.160), (1, 2, 3, 4, 5))],
     "c3": [("h+1e-3", 0.1497, 1e-3, 16, 16, 2, 7, 48), ("h-1e-3", 0.1497, -1e-3, 16, 16, 2, 7, 48)],
     "c4": [("b0.1497", 0.1497, 0.0, 32, 32, 2, 42, 60)],
-    # configs[4]: only the first steps are affordable (c5:4, c5a:5); the saturated steps are checked slab by slab on the GPU box
+    # configs[4]: only the first steps are affordable (c5:3, c5a:3 -- step 4 of either takes hours: n = 2304 Jacobi problems resp. the one-einsum
+    # O(D^9) definition at D = 24); the saturated steps are checked slab by slab / fibre by fibre on the GPU box
     "c5": [("d48", 0.1497, 0.0, 48, 48, 2, 99, 60)],
     "c5a": [("atrg_d24", 0.1497, 0.0, 24, 24, 2, 99, 60, {"method": "atrg"})],
 }
