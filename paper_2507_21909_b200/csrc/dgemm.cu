@@ -41,6 +41,8 @@ struct Cfg {
 using CfgL = Cfg<128, 128, 2, 4, 16, 4>;     // BK = 32 with 3 stages (221 KB) measured no faster
 using CfgS = Cfg<64, 64, 2, 2, 16, 4>;
 using CfgT = Cfg<128, 32, 4, 1, 16, 4>;      // tall and skinny: C = A G with G = D x D (M = D^4): HBM-bound, no padded DMMAs along N
+using CfgT2 = Cfg<128, 32, 4, 1, 16, 2>;     // the same for K <= 32 (two k-steps: two stages are all it can use): 51 KB, four CTAs per SM
+using CfgS2 = Cfg<64, 64, 2, 2, 16, 2>;      // wide outputs with K <= 32 (M4 F, N4 G of Eq. 2.18-2.19): written once, HBM-bound; many small CTAs in flight
 using CfgU = Cfg<32, 32, 2, 2, 16, 4>;       // 32 x 32 outputs (Gram matrices of D^4 x D operands, batched over K-chunks)
 enum { CFG_AUTO = -1, CFG_L = 0, CFG_S = 1, CFG_T = 2, CFG_U = 3 };
 
@@ -162,7 +164,7 @@ struct TileLoader {
 };
 
 template <class C_, bool A_KC, bool B_KC, bool AV16, bool BV16>
-__global__ void __launch_bounds__(C_::NT, C_::NT == 256 ? 1 : 2)
+__global__ void __launch_bounds__(C_::NT, C_::NT == 256 ? 1 : (C_::STAGES == 2 ? 4 : 2))
 dgemm_kernel(int64_t M, int64_t N, int64_t Kall, int64_t Klast, double alpha, const double* __restrict__ A, int64_t lda,
              const double* __restrict__ B, int64_t ldb, double beta, double* __restrict__ C, int64_t ldc, int64_t sA,
              int64_t sB, int64_t sC, int tiles_m, int lower_only) {
@@ -322,6 +324,8 @@ cudaError_t dgemm_raw(bool transa, bool transb, const Args& a) {
     const bool kodd = (a.K % 2 != 0) || (a.Klast % 2 != 0);
     const bool av = v16(a.A, a.lda, a_kc ? (kodd ? 1 : 2) : a.M, a.sA), bv = v16(a.B, a.ldb, b_kc ? (kodd ? 1 : 2) : a.N, a.sB);
     const int cfg = a.force_cfg != CFG_AUTO ? a.force_cfg : pick_cfg(a.M, a.N, a.batch);
+    if ((cfg == CFG_L || cfg == CFG_S) && a.K <= 2 * CfgS2::BK && a.Klast == 0 && a.force_cfg == CFG_AUTO && !a.lower_only && a.M * a.N >= (1 << 22))
+        return pick_order<CfgS2>(a_kc, b_kc, av, bv, a);
     // the 128 x 128 tile fed by TMA (dgemm_tma.cu) whenever the operands meet the tensor-map alignment rules
     if (cfg == CFG_L && g_dgemm_tma && a.Klast == 0) {
         cudaError_t e = dgemm_tma(a.st, a_kc, b_kc, a.M, a.N, a.K, a.alpha, a.A, a.lda, a.B, a.ldb, a.beta, a.C, a.ldc, a.batch, a.sA, a.sB, a.sC, a.lower_only);
@@ -330,7 +334,7 @@ cudaError_t dgemm_raw(bool transa, bool transb, const Args& a) {
     switch (cfg) {
         case CFG_L: return pick_order<CfgL>(a_kc, b_kc, av, bv, a);
         case CFG_S: return pick_order<CfgS>(a_kc, b_kc, av, bv, a);
-        case CFG_T: return pick_order<CfgT>(a_kc, b_kc, av, bv, a);
+        case CFG_T: return (a.K <= 2 * CfgT2::BK && a.Klast == 0) ? pick_order<CfgT2>(a_kc, b_kc, av, bv, a) : pick_order<CfgT>(a_kc, b_kc, av, bv, a);
         default: return pick_order<CfgU>(a_kc, b_kc, av, bv, a);
     }
 }
