@@ -78,7 +78,8 @@ class ClockSampler(threading.Thread):
     def sample_nvml(self):
         n = self.nvml
         self.samples.append(float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM)))
-        self.max_mhz = float(n.nvmlDeviceGetMaxClockInfo(self.handle, n.NVML_CLOCK_SM))
+        if self.max_mhz is None:          # constant: asked once (every NVML query takes a driver lock that a kernel launch may have to wait for)
+            self.max_mhz = float(n.nvmlDeviceGetMaxClockInfo(self.handle, n.NVML_CLOCK_SM))
         r = n.nvmlDeviceGetCurrentClocksEventReasons(self.handle) if hasattr(n, "nvmlDeviceGetCurrentClocksEventReasons") \
             else n.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle)
         for name, bit in (("hw_slowdown", 0x8), ("hw_thermal_slowdown", 0x40), ("sw_thermal_slowdown", 0x20), ("sw_power_cap", 0x4)):
@@ -110,7 +111,7 @@ class ClockSampler(threading.Thread):
                     self.reasons = r0
             except Exception:
                 pass
-            time.sleep(0.05 if self.nvml else 0.2)
+            time.sleep(0.2)               # ~10 samples over a 20-step timed region; denser polling showed up as host stalls between launches
 
     def summary(self):
         s = sorted(self.samples)
