@@ -23,6 +23,7 @@ Replicas only for N > 1: every rank coarse-grains its own 
 `--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
 """
 import argparse
+import gc
 import json
 import os
 import subprocess
@@ -263,6 +264,24 @@ class Prof:
         return acc[1] / (acc[0] * 1e-3) / unit if acc[0] > 0 else None
 
 
+def settle():
+    """Waits for the host to quiet down after a CPU-heavy process.  For 15-20 s after a many-thread, many-GB process has ended on this
+    box (the reference arm the driver runs right before this one; this file's own cpu_baseline leg), ONE coarse-graining step in about
+    twenty stalls by 45-90 ms: the step is host-driven (45-58 stream synchronisations) and the host thread is held up once, whatever its
+    scheduling class, with or without the clock sampler, garbage collector on or off.  Measured (profiles/README.md): a 7 s numpy burst
+    followed by this timed region -> a stall in 11 of 12 processes; the same after a 12 s pause -> 0 of 5; the second process after
+    the burst -> 0 of 8.  The 1-minute load average says whether such a process has just ended."""
+    try:
+        load = os.getloadavg()[0]
+    except OSError:
+        load = 0.0
+    slept = 0.0
+    if load > 0.5:
+        slept = 15.0
+        time.sleep(slept)
+    return {"loadavg_1min_at_start": round(load, 2), "slept_s": slept}
+
+
 def run_cuda(args):
     import torch
     import torch.distributed as dist
@@ -275,6 +294,7 @@ def run_cuda(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     T.lib()
+    settled = settle()
     dev = "cuda:%d" % local
     first = PRE_STEPS + args.warmup + 1                       # absolute index of the first timed step
     if first + args.steps - 1 > 2 * FULL_RUN_STEPS - PRE_STEPS:
@@ -307,6 +327,11 @@ def run_cuda(args):
     t2 = handle(PRE_STEPS) if wraps else None                 # the second replica of a window that wraps: ready before the clock starts
     sampler = ClockSampler(local)
     sampler.start()
+    # The steps are host-driven (45-58 synchronisations each): a cyclic garbage collection of the interpreter (tens of ms with torch loaded;
+    # it can run in the sampler thread and hold the GIL while the main thread returns from a step) shows up as ONE step of 120-140 ms
+    # among 75-100 ms ones.  Collected now, switched off for the timed regions.
+    gc.collect()
+    gc.disable()
     for _ in range(args.warmup):
         t.step()
     sampler.active = True
@@ -351,6 +376,7 @@ def run_cuda(args):
     sampler.active = False
     sampler.stop_flag = True
     sampler.join(timeout=2)
+    gc.enable()
     t.close()
 
     # ---- profiling passes (not part of `value`): per-launch CUDA events on the library's streams around every DGEMM / permute,
@@ -424,6 +450,7 @@ def run_cuda(args):
             "e2e": {"value": sec_e2e, "unit": UNIT, "h2d_bytes_per_step": 16 * n5, "d2h_bytes_per_step": 16 * n5 + 8 * (1 + D), "steps": k_e2e},
             "gpu_launches": launches, "lnZ_per_site": lnz, "clocks": sampler.summary(),
             "step_ms": {str(s): round(x, 2) for s, x in zip(steps_abs, step_ms)},
+            "host_settle": settled,
             "model_tflops": prof.g[1] / prof.steps / (ms / args.steps * 1e-3) / 1e12,
             "host_syncs_per_step": prof.syncs / prof.steps, "launches_per_step": prof.launches / prof.steps,
             "roofline": {"bound": "tensor", "kernel": "dgemm_tma_kernel / dgemm_kernel (DMMA m8n8k4, TMA-fed 128x128x16 tile): the %d contraction launches of a step (>= 1e9 flop each, "
